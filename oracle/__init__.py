@@ -1,0 +1,187 @@
+"""CPU oracle for the DF-JK hot path -- TEST INFRASTRUCTURE ONLY.
+
+Thin ctypes binding over ``oracle/dfjk_oracle.c`` (plain C loops, FP64, OpenMP).
+Only ``tests/``, ``__graft_entry__.smoke()`` and the ``cpu_baseline`` /
+``--impl reference`` legs of ``bench.py`` may import this package.  It imports
+nothing from ``paper_2506_06661_b200`` and the product never imports it.
+
+Definitions and citations live in the C file header (Eq. 1-3,
+PAPER.md:96/126-131 ``get_jk``; BASELINE.json north_star for the J/K formulas).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from typing import Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "dfjk_oracle.c")
+_LIB = os.path.join(_HERE, "liboracle_dfjk.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with gcc (no fast-math, no reassociation)."""
+    if (not force and os.path.exists(_LIB)
+            and os.path.getmtime(_LIB) >= os.path.getmtime(_SRC)):
+        return _LIB
+    cmd = ["gcc", "-O2", "-fopenmp", "-shared", "-fPIC", "-Wall",
+           "-o", _LIB, _SRC, "-lm"]
+    subprocess.run(cmd, check=True)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        build()
+        lib = ctypes.CDLL(_LIB)
+        pp = ctypes.POINTER(ctypes.c_void_p)
+        lib.oracle_num_threads.restype = ctypes.c_int
+        lib.oracle_jk_slab.restype = ctypes.c_int
+        lib.oracle_jk_slab.argtypes = [
+            ctypes.c_int64, ctypes.c_int64, ctypes.c_void_p, ctypes.c_int,
+            pp, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, pp,
+            ctypes.c_void_p]
+        lib.oracle_bruteforce_jk.restype = ctypes.c_int
+        lib.oracle_bruteforce_jk.argtypes = [
+            ctypes.c_int64, ctypes.c_int64, ctypes.c_void_p, ctypes.c_int,
+            pp, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, pp,
+            ctypes.c_void_p]
+        lib.oracle_kv_slab.restype = ctypes.c_int
+        lib.oracle_kv_slab.argtypes = [
+            ctypes.c_int64, ctypes.c_int64, ctypes.c_void_p, ctypes.c_int,
+            pp, ctypes.c_void_p, ctypes.c_int64, ctypes.c_void_p, pp]
+        _lib = lib
+    return _lib
+
+
+def num_threads() -> int:
+    return int(_load().oracle_num_threads())
+
+
+def _f64c(a) -> np.ndarray:
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _ptr_array(arrs: Sequence[Optional[np.ndarray]]):
+    out = (ctypes.c_void_p * len(arrs))()
+    for i, a in enumerate(arrs):
+        out[i] = None if a is None else a.ctypes.data
+    return out
+
+
+def _check_inputs(Bp, nao, Cs):
+    npair = nao * (nao + 1) // 2
+    if Bp.ndim != 2 or Bp.shape[1] != npair:
+        raise ValueError(f"Bp must be [rows][{npair}], got {Bp.shape}")
+    for C in Cs:
+        if C.ndim != 2 or C.shape[0] != nao or C.shape[1] < 1:
+            raise ValueError("each C must be nao x nocc with nocc >= 1")
+
+
+class JKAccumulator:
+    """Feed packed-B slabs, get J and K_s (oracle_jk_slab; P outermost).
+
+    ``Cs`` is a list of nao x nocc_s arrays, ``w`` their density weights
+    (restricted: one set, w=[2.0]; unrestricted: two sets, w=[1.0, 1.0]).
+    """
+
+    def __init__(self, nao: int, Cs: Sequence[np.ndarray], w: Sequence[float],
+                 with_j: bool = True, with_k: bool = True):
+        self.nao = int(nao)
+        self.Cs = [_f64c(C) for C in Cs]
+        self.w = _f64c(np.asarray(w, dtype=np.float64))
+        if len(self.w) != len(self.Cs):
+            raise ValueError("one weight per orbital set")
+        self.nocc = np.asarray([C.shape[1] for C in self.Cs], dtype=np.int64)
+        self.J = np.zeros((nao, nao)) if with_j else None
+        self.K = [np.zeros((nao, nao)) for _ in self.Cs] if with_k else None
+        self.d = []
+
+    def add_slab(self, Bp_slab: np.ndarray) -> None:
+        Bp_slab = _f64c(Bp_slab)
+        _check_inputs(Bp_slab, self.nao, self.Cs)
+        nrows = Bp_slab.shape[0]
+        d = np.zeros(nrows)
+        Cp = _ptr_array(self.Cs)
+        Kp = _ptr_array(self.K) if self.K is not None else None
+        rc = _load().oracle_jk_slab(
+            nrows, self.nao, Bp_slab.ctypes.data, len(self.Cs), Cp,
+            self.nocc.ctypes.data, self.w.ctypes.data,
+            None if self.J is None else self.J.ctypes.data, Kp, d.ctypes.data)
+        if rc != 0:
+            raise RuntimeError(f"oracle_jk_slab failed: {rc}")
+        self.d.append(d)
+
+    def d_vector(self) -> np.ndarray:
+        return np.concatenate(self.d) if self.d else np.zeros(0)
+
+
+def get_jk(Bp: np.ndarray, nao: int, Cs: Sequence[np.ndarray], w: Sequence[float],
+           with_j: bool = True, with_k: bool = True):
+    """Whole-tensor convenience: returns (J, [K_s], d)."""
+    acc = JKAccumulator(nao, Cs, w, with_j, with_k)
+    acc.add_slab(Bp)
+    return acc.J, acc.K, acc.d_vector()
+
+
+def get_jk_restricted(Bp: np.ndarray, nao: int, C_occ: np.ndarray):
+    """D = 2 C C^T (BASELINE.json north_star): returns (J, K)."""
+    J, K, _ = get_jk(Bp, nao, [C_occ], [2.0])
+    return J, K[0]
+
+
+def get_jk_unrestricted(Bp: np.ndarray, nao: int, C_a: np.ndarray, C_b: np.ndarray):
+    """D_s = C_s C_s^T, J = J[D_a + D_b] (reading R7): returns (J, K_a, K_b)."""
+    J, K, _ = get_jk(Bp, nao, [C_a, C_b], [1.0, 1.0])
+    return J, K[0], K[1]
+
+
+def bruteforce_jk(Bp: np.ndarray, nao: int, Cs: Sequence[np.ndarray],
+                  w: Sequence[float]):
+    """Explicit 4-index tensor (Eq. 1 materialised), tiny inputs only.
+
+    Returns (J, [K_s], diag) with diag[m][n] = (mn|mn)_DF (Eq. 7's second term).
+    """
+    Bp = _f64c(Bp)
+    Cs = [_f64c(C) for C in Cs]
+    _check_inputs(Bp, nao, Cs)
+    wv = _f64c(np.asarray(w, dtype=np.float64))
+    nocc = np.asarray([C.shape[1] for C in Cs], dtype=np.int64)
+    J = np.zeros((nao, nao))
+    K = [np.zeros((nao, nao)) for _ in Cs]
+    diag = np.zeros((nao, nao))
+    rc = _load().oracle_bruteforce_jk(
+        Bp.shape[0], nao, Bp.ctypes.data, len(Cs), _ptr_array(Cs),
+        nocc.ctypes.data, wv.ctypes.data, J.ctypes.data, _ptr_array(K),
+        diag.ctypes.data)
+    if rc != 0:
+        raise RuntimeError(f"oracle_bruteforce_jk failed: {rc}")
+    return J, K, diag
+
+
+class KVAccumulator:
+    """K_s @ V from the definition, slab by slab (oracle_kv_slab)."""
+
+    def __init__(self, nao: int, Cs: Sequence[np.ndarray], V: np.ndarray):
+        self.nao = int(nao)
+        self.Cs = [_f64c(C) for C in Cs]
+        self.nocc = np.asarray([C.shape[1] for C in self.Cs], dtype=np.int64)
+        self.V = _f64c(V)            # [nvec][nao]
+        if self.V.ndim != 2 or self.V.shape[1] != nao:
+            raise ValueError("V must be [nvec][nao]")
+        self.KV = [np.zeros_like(self.V) for _ in self.Cs]
+
+    def add_slab(self, Bp_slab: np.ndarray) -> None:
+        Bp_slab = _f64c(Bp_slab)
+        _check_inputs(Bp_slab, self.nao, self.Cs)
+        rc = _load().oracle_kv_slab(
+            Bp_slab.shape[0], self.nao, Bp_slab.ctypes.data, len(self.Cs),
+            _ptr_array(self.Cs), self.nocc.ctypes.data, self.V.shape[0],
+            self.V.ctypes.data, _ptr_array(self.KV))
+        if rc != 0:
+            raise RuntimeError(f"oracle_kv_slab failed: {rc}")

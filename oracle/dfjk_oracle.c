@@ -1,0 +1,358 @@
+/*
+ * dfjk_oracle.c -- CPU ORACLE for the density-fitted Coulomb/exchange build.
+ *
+ * TEST INFRASTRUCTURE ONLY.  Only tests/, __graft_entry__.smoke() and the
+ * cpu_baseline / --impl reference legs of bench.py may load this library.
+ * It shares no code, header, table or helper with the CUDA path under
+ * paper_2506_06661_b200/ and neither side includes the other.
+ *
+ * What it computes (the plain definition, nothing clever):
+ *
+ *   PAPER.md:346-351 (Sec. IV.C.2, Eq. 1):  (mu nu|kappa lambda) ~= sum_P T_{P,mu nu} T_{P,kappa lambda}
+ *   PAPER.md:353-356 (Eq. 2-3): T is the Cholesky-whitened 3-centre tensor; it is
+ *       symmetric in (mu,nu) and stored packed (aosym='s2'; lower
+ *       triangle via tril_indices).  T is called B here.
+ *   PAPER.md:96, 126-131 (Sec. II.C / III):  jmat, kmat = get_jk(mol, dm)
+ *
+ *   With Eq. 1 inserted into the textbook J_mn = sum_ls (mn|ls) D_ls and
+ *   K_mn = sum_ls (ml|ns) D_ls (BASELINE.json north_star states them in this form):
+ *
+ *       D        = sum_s w_s C_s C_s^T                (restricted: one set, w = 2)
+ *       d_P      = sum_mu sum_nu B(P,mu,nu) D[mu][nu]             FULL square
+ *       J[mu][nu]= sum_P d_P B(P,mu,nu)                           FULL square
+ *       X_P[mu][i] = sum_nu B(P,mu,nu) C_s[nu][i]
+ *       K_s[mu][nu]= sum_P sum_i X_P[mu][i] X_P[nu][i]            FULL square, NO factor 2
+ *                                                       (reading R1)
+ *   B(P,mu,nu) := Bp[P][a(a+1)/2 + b],  a = max(mu,nu), b = min(mu,nu)
+ *                                                       (readings R3, R4)
+ *
+ * Deliberately NOT done here (the CUDA path does all of these, so a shared slip
+ * cannot cancel): off-diagonal doubling of D, packed dot products, lower-triangle
+ * only updates, tiling, chunking of X, mirrored output.
+ *
+ * P is the outermost loop and every output is ACCUMULATED, so B may be fed in
+ * slabs of rows (51 GB / 96 GB tensors never have to fit in host memory): the
+ * caller zeroes J, K_s once and calls oracle_jk_slab() per slab.
+ *
+ * d_P is summed two-level (row sums, then the sum of row sums) in binary64; a
+ * single running total over 1e6 terms drifts to ~1e-13 (reading R9).
+ *
+ * Parity pins (tests/test_oracle_pins.py): brute force over the explicit 4-index
+ * tensor built by oracle_bruteforce_jk() below (itself a different formula:
+ * Eq. 1 materialised, then the textbook J/K contractions), closed forms,
+ * invariants, single-element probes, numpy library reductions.  No function in
+ * this file is "parity unpinned".
+ *
+ * Build: gcc -O2 -fopenmp -shared -fPIC (no -ffast-math; no reassociation).
+ */
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define ORACLE_OK      0
+#define ORACLE_EINVAL -1
+#define ORACLE_ENOMEM -2
+
+int oracle_num_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+/* B(P,mu,nu) of one packed row: Bp_row[a(a+1)/2+b], a=max, b=min (reading R3). */
+static inline double b_elem(const double *Bp_row, int64_t mu, int64_t nu)
+{
+    int64_t a = mu > nu ? mu : nu;
+    int64_t b = mu > nu ? nu : mu;
+    return Bp_row[a * (a + 1) / 2 + b];
+}
+
+/*
+ * oracle_jk_slab: accumulate the contribution of `nrows` rows of packed B
+ * (Bp_slab[r][npair], r = 0..nrows-1) into J and K_s.
+ *
+ *   nao            number of orbital basis functions
+ *   nset           number of orbital sets (1 restricted, 2 unrestricted, any >= 1)
+ *   C[s]           nao x nocc[s], row-major (C[s][mu*nocc[s]+i])
+ *   w[s]           density weight of set s (D = sum_s w_s C_s C_s^T)
+ *   J              nao x nao row-major, accumulated (may be NULL)
+ *   K[s]           nao x nao row-major, accumulated (K may be NULL, or K[s] NULL)
+ *   d_out          nrows doubles, d_P of each slab row (may be NULL)
+ */
+int oracle_jk_slab(int64_t nrows, int64_t nao, const double *Bp_slab,
+                   int nset, const double *const *C, const int64_t *nocc,
+                   const double *w, double *J, double *const *K, double *d_out)
+{
+    if (nrows < 0 || nao < 1 || nset < 1 || !Bp_slab || !C || !nocc || !w)
+        return ORACLE_EINVAL;
+    for (int s = 0; s < nset; ++s)
+        if (!C[s] || nocc[s] < 1)
+            return ORACLE_EINVAL;
+    const int64_t npair = nao * (nao + 1) / 2;
+    int64_t nocc_max = 0;
+    for (int s = 0; s < nset; ++s)
+        if (nocc[s] > nocc_max) nocc_max = nocc[s];
+
+    double *D = (double *)malloc(sizeof(double) * nao * nao);
+    double *Bf = (double *)malloc(sizeof(double) * nao * nao);
+    double *Xt = (double *)malloc(sizeof(double) * nocc_max * nao);
+    double *X = (double *)malloc(sizeof(double) * nocc_max * nao);
+    double *rowsum = (double *)malloc(sizeof(double) * nao);
+    if (!D || !Bf || !Xt || !X || !rowsum) {
+        free(D); free(Bf); free(Xt); free(X); free(rowsum);
+        return ORACLE_ENOMEM;
+    }
+
+    /* D[mu][nu] = sum_s w_s sum_i C_s[mu][i] C_s[nu][i] */
+#pragma omp parallel for schedule(static)
+    for (int64_t mu = 0; mu < nao; ++mu)
+        for (int64_t nu = 0; nu < nao; ++nu) {
+            double acc = 0.0;
+            for (int s = 0; s < nset; ++s) {
+                const double *Cs = C[s];
+                const int64_t no = nocc[s];
+                double t = 0.0;
+                for (int64_t i = 0; i < no; ++i)
+                    t += Cs[mu * no + i] * Cs[nu * no + i];
+                acc += w[s] * t;
+            }
+            D[mu * nao + nu] = acc;
+        }
+
+    for (int64_t r = 0; r < nrows; ++r) {
+        const double *Bp_row = Bp_slab + r * npair;
+
+        /* unpack B_P to the full square by max/min */
+#pragma omp parallel for schedule(static)
+        for (int64_t mu = 0; mu < nao; ++mu)
+            for (int64_t nu = 0; nu < nao; ++nu)
+                Bf[mu * nao + nu] = b_elem(Bp_row, mu, nu);
+
+        /* d_P = sum_mu ( sum_nu B(P,mu,nu) D[mu][nu] ) */
+#pragma omp parallel for schedule(static)
+        for (int64_t mu = 0; mu < nao; ++mu) {
+            double t = 0.0;
+            for (int64_t nu = 0; nu < nao; ++nu)
+                t += Bf[mu * nao + nu] * D[mu * nao + nu];
+            rowsum[mu] = t;
+        }
+        double dP = 0.0;
+        for (int64_t mu = 0; mu < nao; ++mu)
+            dP += rowsum[mu];
+        if (d_out) d_out[r] = dP;
+
+        /* J += d_P * B_P */
+        if (J) {
+#pragma omp parallel for schedule(static)
+            for (int64_t mu = 0; mu < nao; ++mu)
+                for (int64_t nu = 0; nu < nao; ++nu)
+                    J[mu * nao + nu] += dP * Bf[mu * nao + nu];
+        }
+
+        if (K) {
+            for (int s = 0; s < nset; ++s) {
+                if (!K[s]) continue;
+                const double *Cs = C[s];
+                const int64_t no = nocc[s];
+                double *Ks = K[s];
+                /* X_P[mu][i] = sum_nu B(P,mu,nu) C_s[nu][i]  (i innermost: axpy
+                 * form, so the compiler vectorises without reassociation);
+                 * kept transposed, Xt[i][mu], for the update below */
+#pragma omp parallel for schedule(static)
+                for (int64_t mu = 0; mu < nao; ++mu) {
+                    double *xrow = X + mu * no;
+                    for (int64_t i = 0; i < no; ++i) xrow[i] = 0.0;
+                    for (int64_t nu = 0; nu < nao; ++nu) {
+                        const double b = Bf[mu * nao + nu];
+                        const double *crow = Cs + nu * no;
+                        for (int64_t i = 0; i < no; ++i)
+                            xrow[i] += b * crow[i];
+                    }
+                    for (int64_t i = 0; i < no; ++i)
+                        Xt[i * nao + mu] = xrow[i];
+                }
+                /* K_s[mu][nu] += sum_i Xt[i][mu] Xt[i][nu], all mu, nu */
+#pragma omp parallel for schedule(static)
+                for (int64_t mu = 0; mu < nao; ++mu) {
+                    double *Krow = Ks + mu * nao;
+                    for (int64_t i = 0; i < no; ++i) {
+                        const double xm = Xt[i * nao + mu];
+                        const double *Xi = Xt + i * nao;
+                        for (int64_t nu = 0; nu < nao; ++nu)
+                            Krow[nu] += xm * Xi[nu];
+                    }
+                }
+            }
+        }
+    }
+    free(D); free(Bf); free(Xt); free(X); free(rowsum);
+    return ORACLE_OK;
+}
+
+/*
+ * oracle_bruteforce_jk: the definition with Eq. 1 MATERIALISED.
+ * Tiny inputs only (nao^4 doubles are allocated).
+ *
+ *   eri[m][n][l][s] = sum_P B(P,m,n) B(P,l,s)                     (Eq. 1)
+ *   D               = sum_s w_s C_s C_s^T
+ *   J[m][n]         = sum_{l,s} eri[m][n][l][s] D[l][s]            (textbook Coulomb)
+ *   K_s[m][n]       = sum_{l,s} eri[m][l][n][s] (C_s C_s^T)[l][s]  (textbook exchange,
+ *                     per-set density WITHOUT weight: reading R1/R7)
+ *   diag[m][n]      = eri[m][n][m][n]  (Eq. 7's DF diagonal), optional
+ *
+ * Outputs are OVERWRITTEN.  This is the pin for oracle_jk_slab, never the other
+ * way round; the two share only b_elem().
+ */
+int oracle_bruteforce_jk(int64_t naux, int64_t nao, const double *Bp,
+                         int nset, const double *const *C, const int64_t *nocc,
+                         const double *w, double *J, double *const *K, double *diag)
+{
+    if (naux < 1 || nao < 1 || nao > 40 || nset < 1 || !Bp || !C || !nocc || !w)
+        return ORACLE_EINVAL;
+    const int64_t npair = nao * (nao + 1) / 2;
+    const int64_t n2 = nao * nao, n3 = n2 * nao, n4 = n3 * nao;
+    double *eri = (double *)calloc((size_t)n4, sizeof(double));
+    double *Ds = (double *)malloc(sizeof(double) * n2);
+    if (!eri || !Ds) { free(eri); free(Ds); return ORACLE_ENOMEM; }
+
+    for (int64_t m = 0; m < nao; ++m)
+        for (int64_t n = 0; n < nao; ++n)
+            for (int64_t l = 0; l < nao; ++l)
+                for (int64_t s = 0; s < nao; ++s) {
+                    double acc = 0.0;
+                    for (int64_t P = 0; P < naux; ++P)
+                        acc += b_elem(Bp + P * npair, m, n) * b_elem(Bp + P * npair, l, s);
+                    eri[m * n3 + n * n2 + l * nao + s] = acc;
+                }
+
+    if (diag)
+        for (int64_t m = 0; m < nao; ++m)
+            for (int64_t n = 0; n < nao; ++n)
+                diag[m * nao + n] = eri[m * n3 + n * n2 + m * nao + n];
+
+    if (J)
+        for (int64_t i = 0; i < n2; ++i) J[i] = 0.0;
+
+    for (int set = 0; set < nset; ++set) {
+        const double *Cs = C[set];
+        const int64_t no = nocc[set];
+        for (int64_t l = 0; l < nao; ++l)
+            for (int64_t s = 0; s < nao; ++s) {
+                double t = 0.0;
+                for (int64_t i = 0; i < no; ++i)
+                    t += Cs[l * no + i] * Cs[s * no + i];
+                Ds[l * nao + s] = t;
+            }
+        if (J)
+            for (int64_t m = 0; m < nao; ++m)
+                for (int64_t n = 0; n < nao; ++n) {
+                    double acc = 0.0;
+                    for (int64_t l = 0; l < nao; ++l)
+                        for (int64_t s = 0; s < nao; ++s)
+                            acc += eri[m * n3 + n * n2 + l * nao + s] * Ds[l * nao + s];
+                    J[m * nao + n] += w[set] * acc;
+                }
+        if (K && K[set])
+            for (int64_t m = 0; m < nao; ++m)
+                for (int64_t n = 0; n < nao; ++n) {
+                    double acc = 0.0;
+                    for (int64_t l = 0; l < nao; ++l)
+                        for (int64_t s = 0; s < nao; ++s)
+                            acc += eri[m * n3 + l * n2 + n * nao + s] * Ds[l * nao + s];
+                    K[set][m * nao + n] = acc;
+                }
+    }
+    free(eri); free(Ds);
+    return ORACLE_OK;
+}
+
+/*
+ * oracle_kv_slab: matrix-vector form of the K definition, for sizes where the
+ * full-square K update is too slow on a CPU (cfg 4-5).
+ *
+ *   (K_s v)[mu] = sum_P sum_nu B(P,mu,nu) u_P[nu],
+ *        u_P    = C_s ( C_s^T ( B_P v ) )          with  (B_P v)[l] = sum_s' B(P,l,s') v[s']
+ *
+ * which is K_s = sum_P B_P C_s C_s^T B_P (the K of the header, X_P X_P^T expanded)
+ * applied to v, evaluated right-to-left so no nao x nao product is formed.
+ * V holds nvec vectors, V[k*nao + mu]; KV[s][k*nao + mu] is ACCUMULATED over slabs.
+ */
+int oracle_kv_slab(int64_t nrows, int64_t nao, const double *Bp_slab,
+                   int nset, const double *const *C, const int64_t *nocc,
+                   int64_t nvec, const double *V, double *const *KV)
+{
+    if (nrows < 0 || nao < 1 || nset < 1 || nvec < 1 || !Bp_slab || !C || !nocc || !V || !KV)
+        return ORACLE_EINVAL;
+    const int64_t npair = nao * (nao + 1) / 2;
+    int64_t nocc_max = 0;
+    for (int s = 0; s < nset; ++s)
+        if (nocc[s] > nocc_max) nocc_max = nocc[s];
+    int rc = ORACLE_OK;
+
+#pragma omp parallel
+    {
+        double *t = (double *)malloc(sizeof(double) * nao);
+        double *u = (double *)malloc(sizeof(double) * nao);
+        double *y = (double *)malloc(sizeof(double) * nocc_max);
+        double *acc = (double *)calloc((size_t)(nset * nvec * nao), sizeof(double));
+        if (!t || !u || !y || !acc) {
+#pragma omp critical
+            rc = ORACLE_ENOMEM;
+        } else {
+#pragma omp for schedule(dynamic, 1)
+            for (int64_t r = 0; r < nrows; ++r) {
+                const double *Bp_row = Bp_slab + r * npair;
+                for (int64_t k = 0; k < nvec; ++k) {
+                    const double *v = V + k * nao;
+                    /* t = B_P v */
+                    for (int64_t l = 0; l < nao; ++l) {
+                        double a = 0.0;
+                        for (int64_t s2 = 0; s2 < nao; ++s2)
+                            a += b_elem(Bp_row, l, s2) * v[s2];
+                        t[l] = a;
+                    }
+                    for (int s = 0; s < nset; ++s) {
+                        const double *Cs = C[s];
+                        const int64_t no = nocc[s];
+                        /* y = C_s^T t ; u = C_s y */
+                        for (int64_t i = 0; i < no; ++i) {
+                            double a = 0.0;
+                            for (int64_t l = 0; l < nao; ++l)
+                                a += Cs[l * no + i] * t[l];
+                            y[i] = a;
+                        }
+                        for (int64_t l = 0; l < nao; ++l) {
+                            double a = 0.0;
+                            for (int64_t i = 0; i < no; ++i)
+                                a += Cs[l * no + i] * y[i];
+                            u[l] = a;
+                        }
+                        /* acc += B_P u */
+                        double *out = acc + (s * nvec + k) * nao;
+                        for (int64_t m = 0; m < nao; ++m) {
+                            double a = 0.0;
+                            for (int64_t n = 0; n < nao; ++n)
+                                a += b_elem(Bp_row, m, n) * u[n];
+                            out[m] += a;
+                        }
+                    }
+                }
+            }
+#pragma omp critical
+            {
+                for (int s = 0; s < nset; ++s)
+                    if (KV[s])
+                        for (int64_t i = 0; i < nvec * nao; ++i)
+                            KV[s][i] += acc[s * nvec * nao + i];
+            }
+        }
+        free(t); free(u); free(y); free(acc);
+    }
+    return rc;
+}
