@@ -1,0 +1,144 @@
+/*
+ * dfjk.h -- C ABI of the B200-native density-fitted Coulomb/exchange build.
+ *
+ * The operation (what the paper calls  jmat, kmat = get_jk(mol, dm),
+ * PAPER.md:96 and PAPER.md:126-131, Sec. II.C / III) with the two-electron
+ * integrals density-fitted (Sec. IV.C.2, Eq. 1-3):
+ *
+ *     (mu nu|kappa lambda) ~= sum_P T_{P,mu nu} T_{P,kappa lambda}            Eq. 1
+ *
+ * T is the Cholesky-whitened 3-centre tensor (Eq. 2-3); it is called B here and
+ * is symmetric in (mu,nu), stored as a packed lower triangle (aosym='s2',
+ * PAPER.md:669; tril order PAPER.md:726).  Inserting Eq. 1 into the textbook
+ * J_mn = sum_ls (mn|ls) D_ls and K_mn = sum_ls (ml|ns) D_ls gives what this
+ * library computes (BASELINE.json north_star):
+ *
+ *     D     = sum_s w_s C_s C_s^T         restricted: one set, w = 2  (D = 2 C C^T)
+ *                                         unrestricted: two sets, w = 1 each
+ *     d_P   = sum_{mu,nu} B_P[mu,nu] D[mu,nu]
+ *     J     = sum_P d_P B_P
+ *     X_P   = B_P C_s
+ *     K_s   = sum_P X_P X_P^T             NO factor 2  (reading R1)
+ *
+ * Conventions common to every entry point
+ *   - All arithmetic is IEEE binary64.  All arrays are C order (row-major),
+ *     contiguous, with 64-bit element offsets.
+ *   - "DEVICE" pointers live on the CUDA device that was current when
+ *     dfjk_create() ran; "HOST" pointers are ordinary host memory (pinned memory
+ *     makes the copies asynchronous, pageable memory is accepted).
+ *   - Return value: 0 (DFJK_OK) on success, a negative DFJK_E* code on failure;
+ *     dfjk_last_error() then returns a thread-local message.  No exception and
+ *     no signal crosses this boundary.  There is NO CPU fallback: without a
+ *     CUDA device every compute entry point fails with DFJK_ECUDA.
+ *   - The device entry points only ENQUEUE work on `stream` (a cudaStream_t
+ *     passed as void*; NULL = the legacy default stream).  They never
+ *     synchronise the host and never allocate.  Outputs are valid once the
+ *     stream reaches that point.  Calls on one handle share its workspace and
+ *     must therefore be stream-ordered with respect to each other.
+ */
+#ifndef DFJK_H
+#define DFJK_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define DFJK_OK       0
+#define DFJK_EINVAL  -1   /* bad argument: null pointer, size out of range, misaligned B */
+#define DFJK_ENOMEM  -2   /* device or host allocation failed */
+#define DFJK_ECUDA   -3   /* CUDA runtime / launch error (text in dfjk_last_error) */
+
+typedef struct dfjk_handle dfjk_handle;
+
+/*
+ * dfjk_create -- bind a resident DF tensor and allocate the fixed workspace.
+ *
+ *   naux      number of auxiliary functions P (rows of B), >= 1
+ *   nao       number of orbital basis functions, >= 1;  npair = nao*(nao+1)/2
+ *   B_packed  DEVICE, naux*npair doubles:  B_packed[P*npair + mu*(mu+1)/2 + nu], mu >= nu
+ *             (Eq. 1's T_{P,mu nu}; row-major lower triangle, R3/R4).
+ *             BORROWED: never copied, never written, must stay valid and unchanged
+ *             until dfjk_destroy (it is up to 96 GB).  Must be 16-byte aligned.
+ *
+ * Returns the handle, or NULL on failure (dfjk_last_error says why).
+ * Workspace (a few hundred MB at most, independent of naux*npair) is allocated
+ * here with cudaMalloc and freed by dfjk_destroy; get_jk never allocates.
+ */
+dfjk_handle *dfjk_create(int64_t naux, int64_t nao, const double *B_packed);
+
+/*
+ * dfjk_get_jk -- restricted build, D = 2 C_occ C_occ^T  (north_star).
+ *
+ *   C_occ   DEVICE, nao x nocc, C_occ[mu*nocc + i];  1 <= nocc <= nao.  Need not be
+ *           orthonormal (R8).  Read only.
+ *   J       DEVICE, nao x nao, OVERWRITTEN, both triangles written.  NULL skips J.
+ *   K       DEVICE, nao x nao, OVERWRITTEN, both triangles written.  NULL skips K.
+ *           J == NULL and K == NULL together is DFJK_EINVAL.
+ *   stream  cudaStream_t
+ */
+int dfjk_get_jk(dfjk_handle *h, const double *C_occ, int64_t nocc,
+                double *J, double *K, void *stream);
+
+/*
+ * dfjk_get_jk_u -- unrestricted (two-spin) build (UKS usage PAPER.md:172-180;
+ * BASELINE.json config 5; R7):  D_s = C_s C_s^T (weight 1),
+ *     J   = J[D_a + D_b]     formed in ONE pair of passes over B
+ *     K_s = sum_P (B_P C_s)(B_P C_s)^T,  s = a, b   (B is unpacked once for both)
+ *   C_a (nao x nocc_a), C_b (nao x nocc_b): DEVICE, as C_occ above.
+ *   J, K_a, K_b: DEVICE nao x nao, overwritten; any may be NULL, not all three.
+ */
+int dfjk_get_jk_u(dfjk_handle *h, const double *C_a, int64_t nocc_a,
+                  const double *C_b, int64_t nocc_b,
+                  double *J, double *K_a, double *K_b, void *stream);
+
+/*
+ * dfjk_get_jk_host -- the same restricted build for a caller whose orbitals and
+ * results live in HOST memory (the end-to-end call bench.py times):
+ * copies C_occ host->device, runs dfjk_get_jk on an internal stream, copies J and
+ * K device->host and SYNCHRONISES before returning.  B stays resident on the device.
+ *   C_occ_host  HOST nao x nocc;  J_host, K_host  HOST nao x nao (either may be NULL).
+ */
+int dfjk_get_jk_host(dfjk_handle *h, const double *C_occ_host, int64_t nocc,
+                     double *J_host, double *K_host);
+
+/*
+ * dfjk_get_d -- debug/inspection getter: copies the naux fitting coefficients
+ * d_P of the most recent J build on this handle into d_out (DEVICE, naux doubles),
+ * enqueued on `stream`.  DFJK_EINVAL if no J has been built yet.
+ */
+int dfjk_get_d(dfjk_handle *h, double *d_out, void *stream);
+
+/*
+ * dfjk_set_option -- tuning knobs, for benchmarks and tests only.  Unknown names
+ * return DFJK_EINVAL.  Known names:
+ *   "k_chunk"   number of auxiliary rows whose half-transformed X stays in the
+ *               L2-sized workspace between the K1 and K2 kernels (0 = automatic)
+ *   "k_splits"  number of partial-K accumulators the SYRK is split over (0 = automatic)
+ *   "j_fused"   1 = J in one HBM pass (row groups kept in L2 between the dot and
+ *               the axpy), 0 = two plain streaming passes (default)
+ */
+int dfjk_set_option(dfjk_handle *h, const char *name, int64_t value);
+
+/*
+ * dfjk_workspace_bytes -- bytes of device workspace owned by the handle.
+ */
+int64_t dfjk_workspace_bytes(const dfjk_handle *h);
+
+/*
+ * dfjk_destroy -- frees the workspace; never frees B.  NULL is a no-op.  Returns 0.
+ * The caller must make sure no enqueued work still uses the handle.
+ */
+int dfjk_destroy(dfjk_handle *h);
+
+/* dfjk_last_error -- thread-local text of the last failure ("" if none). */
+const char *dfjk_last_error(void);
+
+/* dfjk_version -- "major.minor.patch" of the library. */
+const char *dfjk_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DFJK_H */

@@ -1,0 +1,205 @@
+"""dfjk -- B200-native density-fitted Coulomb/exchange build (``get_jk``).
+
+Thin ctypes binding over ``libdfjk.so`` (C ABI in ``include/dfjk.h``; kernels in
+``csrc/``).  Argument marshalling only: every step of the path runs in the
+library's sm_100a kernels.  PyTorch is used for device memory and streams.
+
+There is NO CPU fallback: if the shared library is missing or no CUDA device is
+present, the calls raise.  This package never imports ``oracle``.
+
+Paper: ``jmat, kmat = get_jk(mol, dm)`` with the integrals
+density-fitted (Eq. 1-3).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from typing import Optional, Tuple
+
+__all__ = ["build", "lib", "DFJK", "DFJKError", "SYMBOLS", "LIB_PATH", "HEADER_PATH"]
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libdfjk.so")
+CSRC = os.path.join(_HERE, "csrc")
+HEADER_PATH = os.path.join(os.path.dirname(_HERE), "include", "dfjk.h")
+
+# every symbol include/dfjk.h declares
+SYMBOLS = (
+    "dfjk_create", "dfjk_get_jk", "dfjk_get_jk_u", "dfjk_get_jk_host", "dfjk_get_d",
+    "dfjk_set_option", "dfjk_workspace_bytes", "dfjk_destroy", "dfjk_last_error",
+    "dfjk_version",
+)
+
+_lib = None
+
+
+class DFJKError(RuntimeError):
+    """A dfjk_* call returned a negative code."""
+
+
+def build(force: bool = False) -> str:
+    """Compile ``libdfjk.so`` in-tree with nvcc for sm_100a (see csrc/Makefile)."""
+    if force:
+        subprocess.run(["make", "-C", CSRC, "clean"], check=True, stdout=subprocess.DEVNULL)
+    subprocess.run(["make", "-C", CSRC, "-j8"], check=True, stdout=subprocess.DEVNULL)
+    return LIB_PATH
+
+
+def lib() -> ctypes.CDLL:
+    """Load the C-ABI library (raises if it has not been built)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise DFJKError(f"{LIB_PATH} is missing: run paper_2506_06661_b200.build() "
+                        "(or __graft_entry__.build()); there is no CPU fallback")
+    L = ctypes.CDLL(LIB_PATH)
+    vp, i64, ci = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int
+    L.dfjk_create.restype = vp
+    L.dfjk_create.argtypes = [i64, i64, vp]
+    L.dfjk_get_jk.restype = ci
+    L.dfjk_get_jk.argtypes = [vp, vp, i64, vp, vp, vp]
+    L.dfjk_get_jk_u.restype = ci
+    L.dfjk_get_jk_u.argtypes = [vp, vp, i64, vp, i64, vp, vp, vp, vp]
+    L.dfjk_get_jk_host.restype = ci
+    L.dfjk_get_jk_host.argtypes = [vp, vp, i64, vp, vp]
+    L.dfjk_get_d.restype = ci
+    L.dfjk_get_d.argtypes = [vp, vp, vp]
+    L.dfjk_set_option.restype = ci
+    L.dfjk_set_option.argtypes = [vp, ctypes.c_char_p, i64]
+    L.dfjk_workspace_bytes.restype = i64
+    L.dfjk_workspace_bytes.argtypes = [vp]
+    L.dfjk_destroy.restype = ci
+    L.dfjk_destroy.argtypes = [vp]
+    L.dfjk_last_error.restype = ctypes.c_char_p
+    L.dfjk_last_error.argtypes = []
+    L.dfjk_version.restype = ctypes.c_char_p
+    L.dfjk_version.argtypes = []
+    _lib = L
+    return L
+
+
+def _check(rc: int, what: str) -> None:
+    if rc != 0:
+        raise DFJKError(f"{what} failed ({rc}): {lib().dfjk_last_error().decode()}")
+
+
+def _dev_f64(t, name: str, numel: Optional[int] = None):
+    import torch
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64
+            and t.is_contiguous()):
+        raise ValueError(f"{name} must be a contiguous CUDA float64 tensor")
+    if numel is not None and t.numel() != numel:
+        raise ValueError(f"{name} has {t.numel()} elements, expected {numel}")
+    return t.data_ptr()
+
+
+class DFJK:
+    """Handle on a device-resident packed DF tensor ``B[naux][nao(nao+1)/2]``.
+
+    ``B`` is borrowed (never copied; up to 96 GB) and must outlive the handle.
+    """
+
+    def __init__(self, B_packed, nao: int):
+        import torch
+        self._h = None
+        if not (isinstance(B_packed, torch.Tensor) and B_packed.is_cuda):
+            raise ValueError("B_packed must be a CUDA tensor (there is no CPU path)")
+        nao = int(nao)
+        npair = nao * (nao + 1) // 2
+        if B_packed.dim() != 2 or B_packed.shape[1] != npair:
+            raise ValueError(f"B_packed must be [naux][{npair}]")
+        ptr = _dev_f64(B_packed, "B_packed")
+        self.B = B_packed                      # keep the borrowed tensor alive
+        self.nao, self.naux, self.npair = nao, int(B_packed.shape[0]), npair
+        self.device = B_packed.device
+        with torch.cuda.device(self.device):
+            self._h = lib().dfjk_create(self.naux, nao, ptr)
+        if not self._h:
+            raise DFJKError("dfjk_create failed: " + lib().dfjk_last_error().decode())
+
+    # -- restricted: D = 2 C C^T
+    def get_jk(self, C_occ, with_j: bool = True, with_k: bool = True, out_j=None, out_k=None,
+               stream=None) -> Tuple[Optional["torch.Tensor"], Optional["torch.Tensor"]]:
+        import torch
+        if C_occ.dim() != 2 or C_occ.shape[0] != self.nao:
+            raise ValueError("C_occ must be nao x nocc")
+        cp = _dev_f64(C_occ, "C_occ")
+        n2 = self.nao * self.nao
+        J = (out_j if out_j is not None else torch.empty(self.nao, self.nao, dtype=torch.float64,
+                                                         device=self.device)) if with_j else None
+        K = (out_k if out_k is not None else torch.empty(self.nao, self.nao, dtype=torch.float64,
+                                                         device=self.device)) if with_k else None
+        jp = _dev_f64(J, "J", n2) if with_j else None
+        kp = _dev_f64(K, "K", n2) if with_k else None
+        with torch.cuda.device(self.device):
+            st = (stream or torch.cuda.current_stream(self.device)).cuda_stream
+            _check(lib().dfjk_get_jk(self._h, cp, int(C_occ.shape[1]), jp, kp, st), "dfjk_get_jk")
+        return J, K
+
+    # -- unrestricted: D_s = C_s C_s^T, J = J[D_a + D_b]
+    def get_jk_u(self, C_a, C_b, with_j: bool = True, with_k: bool = True, stream=None):
+        import torch
+        for C in (C_a, C_b):
+            if C.dim() != 2 or C.shape[0] != self.nao:
+                raise ValueError("C_a, C_b must be nao x nocc")
+        ap, bp = _dev_f64(C_a, "C_a"), _dev_f64(C_b, "C_b")
+        mk = lambda: torch.empty(self.nao, self.nao, dtype=torch.float64, device=self.device)
+        J = mk() if with_j else None
+        Ka, Kb = (mk(), mk()) if with_k else (None, None)
+        with torch.cuda.device(self.device):
+            st = (stream or torch.cuda.current_stream(self.device)).cuda_stream
+            _check(lib().dfjk_get_jk_u(self._h, ap, int(C_a.shape[1]), bp, int(C_b.shape[1]),
+                                       J.data_ptr() if with_j else None,
+                                       Ka.data_ptr() if with_k else None,
+                                       Kb.data_ptr() if with_k else None, st), "dfjk_get_jk_u")
+        return J, Ka, Kb
+
+    # -- host buffers in, host buffers out (B stays resident); synchronous
+    def get_jk_host(self, C_occ_host, J_host=None, K_host=None):
+        import torch
+        for t, name in ((C_occ_host, "C_occ_host"), (J_host, "J_host"), (K_host, "K_host")):
+            if t is not None and not (isinstance(t, torch.Tensor) and not t.is_cuda
+                                      and t.dtype == torch.float64 and t.is_contiguous()):
+                raise ValueError(f"{name} must be a contiguous CPU float64 tensor")
+        if C_occ_host.dim() != 2 or C_occ_host.shape[0] != self.nao:
+            raise ValueError("C_occ_host must be nao x nocc")
+        for t in (J_host, K_host):
+            if t is not None and t.numel() != self.nao * self.nao:
+                raise ValueError("J_host / K_host must be nao x nao")
+        with torch.cuda.device(self.device):
+            _check(lib().dfjk_get_jk_host(self._h, C_occ_host.data_ptr(), int(C_occ_host.shape[1]),
+                                          J_host.data_ptr() if J_host is not None else None,
+                                          K_host.data_ptr() if K_host is not None else None),
+                   "dfjk_get_jk_host")
+        return J_host, K_host
+
+    def get_d(self, stream=None):
+        """Fitting coefficients d_P of the most recent J build (debug getter)."""
+        import torch
+        d = torch.empty(self.naux, dtype=torch.float64, device=self.device)
+        with torch.cuda.device(self.device):
+            st = (stream or torch.cuda.current_stream(self.device)).cuda_stream
+            _check(lib().dfjk_get_d(self._h, d.data_ptr(), st), "dfjk_get_d")
+        return d
+
+    def set_option(self, name: str, value: int) -> None:
+        _check(lib().dfjk_set_option(self._h, name.encode(), int(value)), "dfjk_set_option")
+
+    @property
+    def workspace_bytes(self) -> int:
+        return int(lib().dfjk_workspace_bytes(self._h))
+
+    def close(self) -> None:
+        if self._h:
+            import torch
+            torch.cuda.synchronize(self.device)
+            lib().dfjk_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

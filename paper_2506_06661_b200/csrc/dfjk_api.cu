@@ -1,0 +1,306 @@
+/*
+ * dfjk_api.cu -- the C ABI of include/dfjk.h: handle, argument checks, workspace,
+ * and the launch sequence of one get_jk call.  Every step of the path runs in the
+ * kernels of j_kernels.cu / k1_half_transform.cu / k2_syrk.cu; there is no CPU
+ * fallback (a missing device is DFJK_ECUDA).
+ *
+ *   get_jk = K0 pack C -> [J0 Dt -> J1 dot -> J1b reduce -> J2 axpy -> J3 unpack]
+ *                      -> [for P-chunks: K1 half transform -> K2 SYRK (per set)] -> K3 finish
+ */
+#include "../../include/dfjk.h"
+#include "dfjk_internal.h"
+
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+int fail(int code, const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof g_err, fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define DFJK_CUDA_TRY(expr)                                                              \
+    do {                                                                                 \
+        cudaError_t e_ = (expr);                                                         \
+        if (e_ != cudaSuccess)                                                           \
+            return fail(DFJK_ECUDA, "%s: %s", #expr, cudaGetErrorString(e_));            \
+    } while (0)
+
+int64_t round_up(int64_t x, int64_t m) { return (x + m - 1) / m * m; }
+
+}  // namespace
+
+struct dfjk_handle {
+    int64_t naux, nao, npair;
+    const double *B;
+    int device, sm_count;
+    int64_t l2_bytes;
+    /* workspace (device) */
+    double *Ccat;        /* nao x ldc_max */
+    int64_t ldc_max;
+    double *Dt;          /* npair */
+    double *d_part;      /* nchunk x naux */
+    double *d;           /* naux */
+    double *Jp_part;     /* j2_groups x npair */
+    double *X;           /* x_doubles */
+    double *Kpart;       /* 2 x nsplit_alloc x nao x nao */
+    int64_t nchunk, j2_groups, x_doubles;
+    int nsplit_alloc;
+    int64_t ws_bytes;
+    /* options */
+    int64_t opt_k_chunk, opt_k_splits, opt_j_fused;
+    bool have_d;
+    /* host-call resources (lazy) */
+    cudaStream_t host_stream;
+    double *hostC, *hostJ, *hostK;
+};
+
+namespace {
+
+void free_all(dfjk_handle *h)
+{
+    cudaFree(h->Ccat); cudaFree(h->Dt); cudaFree(h->d_part); cudaFree(h->d);
+    cudaFree(h->Jp_part); cudaFree(h->X); cudaFree(h->Kpart);
+    cudaFree(h->hostC); cudaFree(h->hostJ); cudaFree(h->hostK);
+    if (h->host_stream) cudaStreamDestroy(h->host_stream);
+}
+
+/* split count that fills the SMs best: work items = ntile * s, one CTA per SM */
+int choose_splits(int ntile, int sm_count, int max_splits)
+{
+    int best = 1;
+    double best_eff = 0.0;
+    for (int s = 1; s <= max_splits; ++s) {
+        const int items = ntile * s;
+        const int waves = (items + sm_count - 1) / sm_count;
+        const double eff = (double)items / ((double)waves * sm_count);
+        if (eff > best_eff + 0.02) { best_eff = eff; best = s; }
+    }
+    return best;
+}
+
+int alloc_ws(dfjk_handle *h, double **p, int64_t ndoubles)
+{
+    const cudaError_t e = cudaMalloc((void **)p, (size_t)ndoubles * sizeof(double));
+    if (e != cudaSuccess) {
+        *p = nullptr;
+        return fail(DFJK_ENOMEM, "cudaMalloc of %lld bytes: %s", (long long)(ndoubles * 8),
+                    cudaGetErrorString(e));
+    }
+    h->ws_bytes += ndoubles * 8;
+    return DFJK_OK;
+}
+
+}  // namespace
+
+extern "C" const char *dfjk_last_error(void) { return g_err; }
+extern "C" const char *dfjk_version(void) { return "0.1.0"; }
+
+extern "C" dfjk_handle *dfjk_create(int64_t naux, int64_t nao, const double *B_packed)
+{
+    g_err[0] = 0;
+    if (naux < 1 || nao < 1) { fail(DFJK_EINVAL, "dfjk_create: naux and nao must be >= 1"); return nullptr; }
+    if (nao > 46340) { fail(DFJK_EINVAL, "dfjk_create: nao too large"); return nullptr; }
+    if (!B_packed) { fail(DFJK_EINVAL, "dfjk_create: B_packed is NULL"); return nullptr; }
+    if (((uintptr_t)B_packed & 15) != 0) { fail(DFJK_EINVAL, "dfjk_create: B_packed must be 16-byte aligned"); return nullptr; }
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) { fail(DFJK_ECUDA, "cudaGetDevice: %s (no CUDA device, no CPU fallback)", cudaGetErrorString(e)); return nullptr; }
+    cudaPointerAttributes pa;
+    e = cudaPointerGetAttributes(&pa, B_packed);
+    if (e != cudaSuccess || (pa.type != cudaMemoryTypeDevice && pa.type != cudaMemoryTypeManaged)) {
+        cudaGetLastError();
+        fail(DFJK_EINVAL, "dfjk_create: B_packed is not a device pointer");
+        return nullptr;
+    }
+    dfjk_handle *h = new (std::nothrow) dfjk_handle();
+    if (!h) { fail(DFJK_ENOMEM, "dfjk_create: host allocation failed"); return nullptr; }
+    memset(h, 0, sizeof *h);
+    h->naux = naux; h->nao = nao; h->npair = nao * (nao + 1) / 2; h->B = B_packed; h->device = dev;
+    int v = 0;
+    cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev); h->sm_count = v > 0 ? v : 148;
+    cudaDeviceGetAttribute(&v, cudaDevAttrL2CacheSize, dev); h->l2_bytes = v;
+
+    h->ldc_max = 2 * round_up(nao, 8);
+    h->nchunk = dfjk::j1_num_chunks(h->npair);
+    h->j2_groups = dfjk::j2_num_groups(naux, h->npair, h->sm_count);
+    /* X chunk: ~96 MB (three quarters of L2), but at least two rows at the widest ldc */
+    int64_t xd = (96LL << 20) / 8;
+    if (xd < 2 * nao * h->ldc_max) xd = 2 * nao * h->ldc_max;
+    if (xd > naux * nao * h->ldc_max) xd = naux * nao * h->ldc_max;
+    h->x_doubles = xd;
+    const int nb = (int)((nao + 127) / 128);
+    h->nsplit_alloc = choose_splits(nb * (nb + 1) / 2, h->sm_count, 16);
+
+    int rc = DFJK_OK;
+    if (rc == DFJK_OK) rc = alloc_ws(h, &h->Ccat, nao * h->ldc_max);
+    if (rc == DFJK_OK) rc = alloc_ws(h, &h->Dt, h->npair);
+    if (rc == DFJK_OK) rc = alloc_ws(h, &h->d_part, h->nchunk * naux);
+    if (rc == DFJK_OK) rc = alloc_ws(h, &h->d, naux);
+    if (rc == DFJK_OK) rc = alloc_ws(h, &h->Jp_part, h->j2_groups * h->npair);
+    if (rc == DFJK_OK) rc = alloc_ws(h, &h->X, h->x_doubles);
+    if (rc == DFJK_OK) rc = alloc_ws(h, &h->Kpart, 2LL * h->nsplit_alloc * nao * nao);
+    if (rc != DFJK_OK) { free_all(h); delete h; return nullptr; }
+    return h;
+}
+
+extern "C" int dfjk_destroy(dfjk_handle *h)
+{
+    if (!h) return DFJK_OK;
+    free_all(h);
+    delete h;
+    return DFJK_OK;
+}
+
+extern "C" int64_t dfjk_workspace_bytes(const dfjk_handle *h) { return h ? h->ws_bytes : 0; }
+
+extern "C" int dfjk_set_option(dfjk_handle *h, const char *name, int64_t value)
+{
+    if (!h || !name) return fail(DFJK_EINVAL, "dfjk_set_option: NULL argument");
+    if (value < 0) return fail(DFJK_EINVAL, "dfjk_set_option: negative value");
+    if (!strcmp(name, "k_chunk")) { h->opt_k_chunk = value; return DFJK_OK; }
+    if (!strcmp(name, "k_splits")) {
+        if (value > h->nsplit_alloc) return fail(DFJK_EINVAL, "k_splits > %d allocated", h->nsplit_alloc);
+        h->opt_k_splits = value; return DFJK_OK;
+    }
+    if (!strcmp(name, "j_fused")) {
+        if (value != 0) return fail(DFJK_EINVAL, "j_fused=1 is not available in this build");
+        h->opt_j_fused = value; return DFJK_OK;
+    }
+    return fail(DFJK_EINVAL, "dfjk_set_option: unknown option '%s'", name);
+}
+
+/* ------------------------------------------------------------------ one build */
+namespace {
+
+int get_jk_impl(dfjk_handle *h, int nset, const double *const *C, const int64_t *nocc64,
+                const double *w, double *J, double *const *K, cudaStream_t st, const char *who)
+{
+    g_err[0] = 0;
+    if (!h) return fail(DFJK_EINVAL, "%s: NULL handle", who);
+    bool any_k = false;
+    for (int s = 0; s < nset; ++s) {
+        if (!C[s]) return fail(DFJK_EINVAL, "%s: orbital pointer %d is NULL", who, s);
+        if (nocc64[s] < 1 || nocc64[s] > h->nao)
+            return fail(DFJK_EINVAL, "%s: nocc[%d]=%lld outside [1, nao=%lld]", who, s,
+                        (long long)nocc64[s], (long long)h->nao);
+        any_k = any_k || K[s] != nullptr;
+    }
+    if (!J && !any_k) return fail(DFJK_EINVAL, "%s: no output requested", who);
+    int dev = -1;
+    DFJK_CUDA_TRY(cudaGetDevice(&dev));
+    if (dev != h->device) return fail(DFJK_EINVAL, "%s: handle belongs to device %d, current is %d", who, h->device, dev);
+
+    const int64_t nao = h->nao, naux = h->naux, npair = h->npair;
+    int nocc[4], col0[4];
+    int64_t ldc = 0;
+    for (int s = 0; s < nset; ++s) {
+        nocc[s] = (int)nocc64[s];
+        col0[s] = (int)ldc;
+        ldc += round_up(nocc64[s], 8);
+    }
+    /* K0: zero-padded concatenation [C_0 | C_1], each set padded to a multiple of 8 columns */
+    dfjk::launch_k0_pack_c(C, nocc, col0, nset, nao, ldc, h->Ccat, st);
+
+    if (J) {
+        dfjk::launch_j0_build_dt(h->Ccat, ldc, nao, nset, col0, nocc, w, h->Dt, st);
+        dfjk::launch_j1_dot(h->B, naux, npair, h->Dt, h->d_part, h->sm_count, st);
+        dfjk::launch_j1_reduce(h->d_part, h->nchunk, naux, h->d, st);
+        dfjk::launch_j2_axpy(h->B, naux, npair, h->d, h->Jp_part, h->j2_groups, st);
+        dfjk::launch_j3_unpack(h->Jp_part, h->j2_groups, npair, nao, J, st);
+        h->have_d = true;
+    }
+
+    if (any_k) {
+        int64_t pc = h->x_doubles / (nao * ldc);
+        if (h->opt_k_chunk > 0 && h->opt_k_chunk < pc) pc = h->opt_k_chunk;
+        if (pc > naux) pc = naux;
+        if (pc > 1) pc -= pc & 1;                      /* even: k groups pair up across P */
+        if (pc < 1) return fail(DFJK_ENOMEM, "%s: X workspace too small", who);
+        const int64_t xpitch = pc * ldc;
+        const int nsplit = h->opt_k_splits > 0 ? (int)h->opt_k_splits : h->nsplit_alloc;
+        int chunk = 0;
+        for (int64_t P0 = 0; P0 < naux; P0 += pc, ++chunk) {
+            const int64_t np = (P0 + pc <= naux) ? pc : naux - P0;
+            dfjk::launch_k1_half_transform(h->B, nao, npair, P0, np, h->Ccat, ldc, h->X, xpitch, st);
+            for (int s = 0; s < nset; ++s)
+                if (K[s])
+                    dfjk::launch_k2_syrk_lower(h->X, xpitch, nao, np, ldc, col0[s], nocc[s],
+                                               h->Kpart + (int64_t)s * h->nsplit_alloc * nao * nao,
+                                               nsplit, chunk > 0, st);
+        }
+        for (int s = 0; s < nset; ++s)
+            if (K[s])
+                dfjk::launch_k3_finish(h->Kpart + (int64_t)s * h->nsplit_alloc * nao * nao, nsplit,
+                                       nao, K[s], st);
+    }
+    DFJK_CUDA_TRY(cudaGetLastError());
+    return DFJK_OK;
+}
+
+}  // namespace
+
+extern "C" int dfjk_get_jk(dfjk_handle *h, const double *C_occ, int64_t nocc, double *J, double *K,
+                           void *stream)
+{
+    const double *C[1] = {C_occ};
+    const int64_t no[1] = {nocc};
+    const double w[1] = {2.0};
+    double *Ks[1] = {K};
+    return get_jk_impl(h, 1, C, no, w, J, Ks, (cudaStream_t)stream, "dfjk_get_jk");
+}
+
+extern "C" int dfjk_get_jk_u(dfjk_handle *h, const double *C_a, int64_t nocc_a, const double *C_b,
+                             int64_t nocc_b, double *J, double *K_a, double *K_b, void *stream)
+{
+    const double *C[2] = {C_a, C_b};
+    const int64_t no[2] = {nocc_a, nocc_b};
+    const double w[2] = {1.0, 1.0};
+    double *Ks[2] = {K_a, K_b};
+    return get_jk_impl(h, 2, C, no, w, J, Ks, (cudaStream_t)stream, "dfjk_get_jk_u");
+}
+
+extern "C" int dfjk_get_d(dfjk_handle *h, double *d_out, void *stream)
+{
+    g_err[0] = 0;
+    if (!h || !d_out) return fail(DFJK_EINVAL, "dfjk_get_d: NULL argument");
+    if (!h->have_d) return fail(DFJK_EINVAL, "dfjk_get_d: no J has been built on this handle");
+    DFJK_CUDA_TRY(cudaMemcpyAsync(d_out, h->d, (size_t)h->naux * 8, cudaMemcpyDeviceToDevice,
+                                  (cudaStream_t)stream));
+    return DFJK_OK;
+}
+
+extern "C" int dfjk_get_jk_host(dfjk_handle *h, const double *C_occ_host, int64_t nocc,
+                                double *J_host, double *K_host)
+{
+    g_err[0] = 0;
+    if (!h) return fail(DFJK_EINVAL, "dfjk_get_jk_host: NULL handle");
+    if (!C_occ_host) return fail(DFJK_EINVAL, "dfjk_get_jk_host: C_occ_host is NULL");
+    if (nocc < 1 || nocc > h->nao) return fail(DFJK_EINVAL, "dfjk_get_jk_host: nocc outside [1, nao]");
+    if (!J_host && !K_host) return fail(DFJK_EINVAL, "dfjk_get_jk_host: no output requested");
+    const int64_t n2 = h->nao * h->nao;
+    if (!h->host_stream) {
+        /* first host call: staging buffers for C, J, K (kept until destroy) */
+        DFJK_CUDA_TRY(cudaStreamCreateWithFlags(&h->host_stream, cudaStreamNonBlocking));
+        if (alloc_ws(h, &h->hostC, n2) || alloc_ws(h, &h->hostJ, n2) || alloc_ws(h, &h->hostK, n2))
+            return DFJK_ENOMEM;
+    }
+    cudaStream_t st = h->host_stream;
+    DFJK_CUDA_TRY(cudaMemcpyAsync(h->hostC, C_occ_host, (size_t)h->nao * nocc * 8, cudaMemcpyHostToDevice, st));
+    const int rc = dfjk_get_jk(h, h->hostC, nocc, J_host ? h->hostJ : nullptr,
+                               K_host ? h->hostK : nullptr, st);
+    if (rc != DFJK_OK) return rc;
+    if (J_host) DFJK_CUDA_TRY(cudaMemcpyAsync(J_host, h->hostJ, (size_t)n2 * 8, cudaMemcpyDeviceToHost, st));
+    if (K_host) DFJK_CUDA_TRY(cudaMemcpyAsync(K_host, h->hostK, (size_t)n2 * 8, cudaMemcpyDeviceToHost, st));
+    DFJK_CUDA_TRY(cudaStreamSynchronize(st));
+    return DFJK_OK;
+}

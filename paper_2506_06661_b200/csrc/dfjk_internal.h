@@ -1,0 +1,66 @@
+/*
+ * dfjk_internal.h -- launcher prototypes shared by the translation units of
+ * libdfjk.so (CUDA path only; nothing here is used by, or uses, oracle/).
+ *
+ * Notation follows include/dfjk.h: B packed [naux][npair], C [nao][nocc],
+ * Dt = D-tilde (packed density with doubled off-diagonals), d[naux],
+ * X = half-transformed tensor, K lower tiles.
+ */
+#ifndef DFJK_INTERNAL_H
+#define DFJK_INTERNAL_H
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace dfjk {
+
+/* ---------------------------------------------------------------- J path */
+
+/* J0: Dt[mu(mu+1)/2+nu] = (2 - delta_mu,nu) * sum_s w_s sum_i C_s[mu,i] C_s[nu,i].
+ * Ccat is the zero-padded concatenation built by k0_pack_c: Ccat[nao][ldc], set s
+ * occupying columns [col0[s], col0[s]+nocc[s]). */
+void launch_j0_build_dt(const double *Ccat, int64_t ldc, int64_t nao,
+                        int nset, const int *col0, const int *nocc, const double *w,
+                        double *Dt, cudaStream_t st);
+
+/* J1: d_part[c][P] = sum_{pair in chunk c} B[P][pair] Dt[pair];  nchunk = j1_num_chunks(npair). */
+int64_t j1_num_chunks(int64_t npair);
+void launch_j1_dot(const double *B, int64_t naux, int64_t npair, const double *Dt,
+                   double *d_part, int sm_count, cudaStream_t st);
+/* J1b: d[P] = sum_c d_part[c][P] (fixed order: deterministic). */
+void launch_j1_reduce(const double *d_part, int64_t nchunk, int64_t naux, double *d,
+                      cudaStream_t st);
+
+/* J2: Jp_part[g][pair] = sum_{P in row group g} d[P] B[P][pair];  ngroup = j2_num_groups(...). */
+int64_t j2_num_groups(int64_t naux, int64_t npair, int sm_count);
+void launch_j2_axpy(const double *B, int64_t naux, int64_t npair, const double *d,
+                    double *Jp_part, int64_t ngroup, cudaStream_t st);
+
+/* J3: J[mu][nu] = J[nu][mu] = sum_g Jp_part[g][mu(mu+1)/2+nu]. */
+void launch_j3_unpack(const double *Jp_part, int64_t ngroup, int64_t npair, int64_t nao,
+                      double *J, cudaStream_t st);
+
+/* ---------------------------------------------------------------- K path */
+
+/* K0: Ccat[nao][ldc] = [C_0 | C_1 | ... | 0-pad], ldc multiple of 8. */
+void launch_k0_pack_c(const double *const *C, const int *nocc, const int *col0, int nset,
+                      int64_t nao, int64_t ldc, double *Ccat, cudaStream_t st);
+
+/* K1: for P in [P0, P0+np):  X[mu][(P-P0)*ldc + i] = sum_nu B_P(mu,nu) Ccat[nu][i]
+ * X has row pitch xpitch doubles (>= np*ldc). */
+void launch_k1_half_transform(const double *B, int64_t nao, int64_t npair,
+                              int64_t P0, int64_t np, const double *Ccat, int64_t ldc,
+                              double *X, int64_t xpitch, cudaStream_t st);
+
+/* K2: Kpart[split][mu][nu] (+)= sum_{k in split's share of [kbeg,kend)} X[mu][k] X[nu][k]
+ * for mu-tile >= nu-tile (lower tiles, full 128x128 tiles).  For np auxiliary rows of
+ * pitch ldc, set s uses columns p*ldc + [col0, col0+ncol).  accumulate = 0 overwrites. */
+void launch_k2_syrk_lower(const double *X, int64_t xpitch, int64_t nao,
+                          int64_t np, int64_t ldc, int64_t col0, int64_t ncol,
+                          double *Kpart, int nsplit, int accumulate, cudaStream_t st);
+
+/* K3: K[mu][nu] = K[nu][mu] = sum_split Kpart[split][mu][nu], mu >= nu. */
+void launch_k3_finish(const double *Kpart, int nsplit, int64_t nao, double *K, cudaStream_t st);
+
+}  // namespace dfjk
+#endif

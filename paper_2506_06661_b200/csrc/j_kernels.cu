@@ -1,0 +1,315 @@
+/*
+ * j_kernels.cu -- the Coulomb half of DF get_jk (include/dfjk.h), sm_100a.
+ *
+ *     Dt[pair]  = (2 - delta) * D[mu][nu]              J0   (tiny)
+ *     d_P       = sum_pair B[P][pair] Dt[pair]         J1   streams |B| bytes   HBM-bound
+ *     Jp[pair]  = sum_P d_P B[P][pair]                 J2   streams |B| bytes   HBM-bound
+ *     J         = unpack(Jp), both triangles           J3   (tiny)
+ *
+ * J1/J2 are pure streaming kernels (0.25 flop/byte): what matters is bytes in
+ * flight per SM (>= ~40 KB by Little's law), 128-bit coalesced loads that bypass
+ * L1 and are marked evict-first in L2, Dt/d/Jp staying on chip, and reductions
+ * that never serialise.  Packed rows start at P*npair doubles, which is only
+ * 8-byte aligned when npair is odd: all vector loads are issued on the 16-byte
+ * grid of the FLAT array and the (at most two) straddling elements per row
+ * segment are handled by scalar loads.
+ */
+#include "dfjk_internal.h"
+
+namespace dfjk {
+
+namespace {
+
+__device__ __forceinline__ double2 ldg_stream2(const double *p)
+{
+    /* read-once data: non-coherent path, streaming (evict-first) policy */
+    return __ldcs(reinterpret_cast<const double2 *>(p));
+}
+__device__ __forceinline__ double ldg_stream1(const double *p) { return __ldcs(p); }
+
+/* ------------------------------------------------------------------ J0 */
+struct SetDesc {
+    int nset;
+    int col0[4];
+    int nocc[4];
+    double w[4];
+};
+
+constexpr int J0_T = 32;
+
+__global__ void __launch_bounds__(256)
+j0_build_dt_kernel(const double *__restrict__ Ccat, int64_t ldc, int64_t nao, SetDesc sd,
+                   double *__restrict__ Dt)
+{
+    const int bi = blockIdx.y, bj = blockIdx.x;
+    if (bj > bi) return;
+    __shared__ double Cm[J0_T][J0_T + 1];
+    __shared__ double Cn[J0_T][J0_T + 1];
+    __shared__ double wcol[J0_T];
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;   /* ty 0..7 */
+    const int64_t mu0 = (int64_t)bi * J0_T, nu0 = (int64_t)bj * J0_T;
+    double acc[4] = {0.0, 0.0, 0.0, 0.0};
+    for (int64_t c0 = 0; c0 < ldc; c0 += J0_T) {
+        if (threadIdx.x < J0_T) {
+            const int64_t c = c0 + threadIdx.x;
+            double wv = 0.0;
+            for (int s = 0; s < sd.nset; ++s)
+                if (c >= sd.col0[s] && c < sd.col0[s] + sd.nocc[s]) wv = sd.w[s];
+            wcol[threadIdx.x] = wv;
+        }
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            const int row = ty + 8 * r;
+            const int64_t c = c0 + tx;
+            const int64_t mu = mu0 + row, nu = nu0 + row;
+            Cm[row][tx] = (mu < nao && c < ldc) ? Ccat[mu * ldc + c] : 0.0;
+            Cn[row][tx] = (nu < nao && c < ldc) ? Ccat[nu * ldc + c] : 0.0;
+        }
+        __syncthreads();
+#pragma unroll 8
+        for (int c = 0; c < J0_T; ++c) {
+            const double wn = wcol[c] * Cn[tx][c];
+#pragma unroll
+            for (int r = 0; r < 4; ++r) acc[r] += Cm[ty + 8 * r][c] * wn;
+        }
+        __syncthreads();
+    }
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+        const int64_t mu = mu0 + ty + 8 * r, nu = nu0 + tx;
+        if (mu < nao && nu <= mu)
+            Dt[mu * (mu + 1) / 2 + nu] = (mu == nu ? 1.0 : 2.0) * acc[r];
+    }
+}
+
+/* ------------------------------------------------------------------ J1 */
+constexpr int J1_CH = 4096;          /* columns (pairs) per chunk; Dt chunk = 32 KB of smem */
+constexpr int J1_WARPS = 8;
+constexpr int J1_UNROLL = 8;         /* 128-bit loads in flight per lane */
+
+__global__ void __launch_bounds__(J1_WARPS * 32)
+j1_dot_kernel(const double *__restrict__ B, int64_t naux, int64_t npair,
+              const double *__restrict__ Dt, double *__restrict__ d_part)
+{
+    /* sDt[k] = Dt[c0 - 1 + k], k = 0 .. CH+1 (zero outside [c0, c1)) */
+    __shared__ double sDt[J1_CH + 2];
+    const int64_t chunk = blockIdx.x;
+    const int64_t c0 = chunk * J1_CH;
+    const int64_t c1 = (c0 + J1_CH < npair) ? c0 + J1_CH : npair;
+    for (int k = threadIdx.x; k < J1_CH + 2; k += blockDim.x) {
+        const int64_t col = c0 - 1 + k;
+        sDt[k] = (col >= c0 && col < c1) ? Dt[col] : 0.0;
+    }
+    __syncthreads();
+
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int64_t row_stride = (int64_t)gridDim.y * J1_WARPS;
+    for (int64_t P = (int64_t)blockIdx.y * J1_WARPS + warp; P < naux; P += row_stride) {
+        const int64_t base = P * npair;
+        const int64_t f0 = base + c0, f1 = base + c1;       /* flat range of this segment */
+        const int64_t fa = (f0 + 1) & ~(int64_t)1;          /* first 16-B aligned element */
+        const int64_t fb = f1 & ~(int64_t)1;                /* end of aligned body */
+        double acc0 = 0.0, acc1 = 0.0;
+        if (fa <= fb) {
+            /* head / tail scalars */
+            if (lane == 0 && f0 < fa) acc0 += ldg_stream1(B + f0) * sDt[1];
+            if (lane == 1 && fb < f1) acc1 += ldg_stream1(B + fb) * sDt[fb - f0 + 1];
+            const int64_t nvec = (fb - fa) >> 1;
+            const double *bp = B + fa;
+            const double *sp = sDt + (fa - f0 + 1);
+            int64_t v = lane;
+            for (; v + 32 * (J1_UNROLL - 1) < nvec; v += 32 * J1_UNROLL) {
+                double2 b[J1_UNROLL];
+#pragma unroll
+                for (int u = 0; u < J1_UNROLL; ++u) b[u] = ldg_stream2(bp + 2 * (v + 32 * u));
+#pragma unroll
+                for (int u = 0; u < J1_UNROLL; ++u) {
+                    const int64_t k = 2 * (v + 32 * u);
+                    acc0 += b[u].x * sp[k];
+                    acc1 += b[u].y * sp[k + 1];
+                }
+            }
+            for (; v < nvec; v += 32) {
+                const double2 b = ldg_stream2(bp + 2 * v);
+                acc0 += b.x * sp[2 * v];
+                acc1 += b.y * sp[2 * v + 1];
+            }
+        } else {
+            /* segment of a single element straddling the 16-B grid */
+            if (lane == 0) acc0 += ldg_stream1(B + f0) * sDt[1];
+        }
+        double acc = acc0 + acc1;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+        if (lane == 0) d_part[chunk * naux + P] = acc;
+    }
+}
+
+__global__ void j1_reduce_kernel(const double *__restrict__ d_part, int64_t nchunk, int64_t naux,
+                                 double *__restrict__ d)
+{
+    const int64_t P = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (P >= naux) return;
+    double acc = 0.0;
+    for (int64_t c = 0; c < nchunk; ++c) acc += d_part[c * naux + P];
+    d[P] = acc;
+}
+
+/* ------------------------------------------------------------------ J2 */
+constexpr int J2_THREADS = 256;
+constexpr int J2_UNROLL = 8;
+
+__global__ void __launch_bounds__(J2_THREADS)
+j2_axpy_kernel(const double *__restrict__ B, int64_t naux, int64_t npair,
+               const double *__restrict__ d, double *__restrict__ Jp_part, int64_t ngroup)
+{
+    const int64_t g = blockIdx.y;
+    /* all rows of group g (P = g + t*ngroup, ngroup even) share the parity of P*npair */
+    const int64_t s = (g * npair) & 1;
+    const int64_t vv = (int64_t)blockIdx.x * J2_THREADS + threadIdx.x;
+    const int64_t colx = 2 * vv - s, coly = colx + 1;       /* columns this thread owns */
+    const bool okx = colx >= 0 && colx < npair;
+    const bool oky = coly < npair;                          /* coly >= 0 always */
+    if (!okx && !oky) return;
+    double ax = 0.0, ay = 0.0;
+    if (okx && oky) {
+        const double *bp = B + colx;                        /* + P*npair is 16-B aligned */
+        int64_t P = g;
+        for (; P + (J2_UNROLL - 1) * ngroup < naux; P += J2_UNROLL * ngroup) {
+            double2 b[J2_UNROLL];
+            double dv[J2_UNROLL];
+#pragma unroll
+            for (int u = 0; u < J2_UNROLL; ++u) {
+                b[u] = ldg_stream2(bp + (P + u * ngroup) * npair);
+                dv[u] = __ldg(d + P + u * ngroup);
+            }
+#pragma unroll
+            for (int u = 0; u < J2_UNROLL; ++u) {
+                ax += dv[u] * b[u].x;
+                ay += dv[u] * b[u].y;
+            }
+        }
+        for (; P < naux; P += ngroup) {
+            const double2 b = ldg_stream2(bp + P * npair);
+            const double dv = __ldg(d + P);
+            ax += dv * b.x;
+            ay += dv * b.y;
+        }
+    } else {
+        const int64_t col = okx ? colx : coly;
+        double a = 0.0;
+        for (int64_t P = g; P < naux; P += ngroup) a += __ldg(d + P) * ldg_stream1(B + P * npair + col);
+        if (okx) ax = a; else ay = a;
+    }
+    double *out = Jp_part + g * npair;
+    if (okx) out[colx] = ax;
+    if (oky) out[coly] = ay;
+}
+
+/* ------------------------------------------------------------------ J3 */
+constexpr int J3_T = 32;
+
+__global__ void __launch_bounds__(256)
+j3_unpack_kernel(const double *__restrict__ Jp_part, int64_t ngroup, int64_t npair, int64_t nao,
+                 double *__restrict__ J)
+{
+    const int bi = blockIdx.y, bj = blockIdx.x;
+    if (bj > bi) return;
+    __shared__ double t[J3_T][J3_T + 1];
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    const int64_t mu0 = (int64_t)bi * J3_T, nu0 = (int64_t)bj * J3_T;
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+        const int row = ty + 8 * r;
+        const int64_t mu = mu0 + row, nu = nu0 + tx;
+        double v = 0.0;
+        if (mu < nao && nu <= mu) {
+            const int64_t pair = mu * (mu + 1) / 2 + nu;
+            for (int64_t g = 0; g < ngroup; ++g) v += Jp_part[g * npair + pair];
+        }
+        t[row][tx] = v;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+        const int row = ty + 8 * r;
+        const int64_t mu = mu0 + row, nu = nu0 + tx;
+        if (mu < nao && nu < nao) {
+            const double v = (bi == bj && tx > row) ? t[tx][row] : t[row][tx];
+            J[mu * nao + nu] = v;
+        }
+        if (bi != bj) {
+            /* mirrored tile: J[nu0+row][mu0+tx] = t[tx][row] */
+            const int64_t a = nu0 + row, b = mu0 + tx;
+            if (a < nao && b < nao) J[a * nao + b] = t[tx][row];
+        }
+    }
+}
+
+}  // namespace
+
+/* ------------------------------------------------------------------ launchers */
+void launch_j0_build_dt(const double *Ccat, int64_t ldc, int64_t nao, int nset, const int *col0,
+                        const int *nocc, const double *w, double *Dt, cudaStream_t st)
+{
+    SetDesc sd;
+    sd.nset = nset;
+    for (int s = 0; s < 4; ++s) {
+        sd.col0[s] = s < nset ? col0[s] : 0;
+        sd.nocc[s] = s < nset ? nocc[s] : 0;
+        sd.w[s] = s < nset ? w[s] : 0.0;
+    }
+    const unsigned nb = (unsigned)((nao + J0_T - 1) / J0_T);
+    j0_build_dt_kernel<<<dim3(nb, nb), 256, 0, st>>>(Ccat, ldc, nao, sd, Dt);
+}
+
+int64_t j1_num_chunks(int64_t npair) { return (npair + J1_CH - 1) / J1_CH; }
+
+void launch_j1_dot(const double *B, int64_t naux, int64_t npair, const double *Dt, double *d_part,
+                   int sm_count, cudaStream_t st)
+{
+    const int64_t nchunk = j1_num_chunks(npair);
+    int64_t rg = (16LL * sm_count + nchunk - 1) / nchunk;   /* aim at >= 16 CTAs per SM in total */
+    const int64_t rg_max = (naux + J1_WARPS - 1) / J1_WARPS;
+    if (rg > rg_max) rg = rg_max;
+    if (rg < 1) rg = 1;
+    if (rg > 65535) rg = 65535;
+    j1_dot_kernel<<<dim3((unsigned)nchunk, (unsigned)rg), J1_WARPS * 32, 0, st>>>(B, naux, npair, Dt,
+                                                                                  d_part);
+}
+
+void launch_j1_reduce(const double *d_part, int64_t nchunk, int64_t naux, double *d, cudaStream_t st)
+{
+    j1_reduce_kernel<<<(unsigned)((naux + 127) / 128), 128, 0, st>>>(d_part, nchunk, naux, d);
+}
+
+int64_t j2_num_groups(int64_t naux, int64_t npair, int sm_count)
+{
+    const int64_t nbx = (npair + 1) / 2 / J2_THREADS + 1;
+    int64_t g = (16LL * sm_count + nbx - 1) / nbx;
+    if (g < 2) g = 2;
+    g += g & 1;                               /* even: one 16-B alignment class per group */
+    int64_t gmax = naux / 8;                  /* keep >= 8 rows per group when possible */
+    gmax -= gmax & 1;
+    if (gmax < 2) gmax = 2;
+    if (g > gmax) g = gmax;
+    return g;
+}
+
+void launch_j2_axpy(const double *B, int64_t naux, int64_t npair, const double *d, double *Jp_part,
+                    int64_t ngroup, cudaStream_t st)
+{
+    const int64_t nvec = (npair + 1) / 2 + 1;               /* one spare vector for shifted rows */
+    const unsigned nbx = (unsigned)((nvec + J2_THREADS - 1) / J2_THREADS);
+    j2_axpy_kernel<<<dim3(nbx, (unsigned)ngroup), J2_THREADS, 0, st>>>(B, naux, npair, d, Jp_part,
+                                                                       ngroup);
+}
+
+void launch_j3_unpack(const double *Jp_part, int64_t ngroup, int64_t npair, int64_t nao, double *J,
+                      cudaStream_t st)
+{
+    const unsigned nb = (unsigned)((nao + J3_T - 1) / J3_T);
+    j3_unpack_kernel<<<dim3(nb, nb), 256, 0, st>>>(Jp_part, ngroup, npair, nao, J);
+}
+
+}  // namespace dfjk

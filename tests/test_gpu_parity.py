@@ -1,0 +1,219 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element.
+
+Bar (BASELINE.json north_star): relative Frobenius error <= 1e-11 for J and every K, FP64,
+on the full matrices.  Sizes here are ones the oracle finishes in seconds but that span
+several 128-row tiles, several 16-column k-chunks, several 4096-pair J chunks and ragged tails.
+"""
+import numpy as np
+import pytest
+
+import dfjk_inputs as gi
+import oracle
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-11
+
+
+def relerr(a, b):
+    nb = np.linalg.norm(b)
+    return np.linalg.norm(np.asarray(a) - np.asarray(b)) / (nb if nb > 0 else 1.0)
+
+
+@pytest.fixture(scope="module")
+def dfjk():
+    import paper_2506_06661_b200 as pkg
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    pkg.lib()                      # fails loudly if libdfjk.so is missing
+    return pkg
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def run_restricted(pkg, Bp, nao, C, **opts):
+    Bd = dev(Bp)
+    h = pkg.DFJK(Bd, nao)
+    for k, v in opts.items():
+        h.set_option(k, v)
+    J, K = h.get_jk(dev(C))
+    d = h.get_d()
+    torch.cuda.synchronize()
+    out = J.cpu().numpy(), K.cpu().numpy(), d.cpu().numpy()
+    h.close()
+    return out
+
+
+def rand_case(nao, naux, noccs, seed, orthonormal=True):
+    cfg = gi.custom_config(nao, naux, noccs, seed=seed)
+    Bp = gi.fill_B_host(cfg)
+    Cs = [gi.random_orbitals(nao, n, seed + 11 * i, orthonormal) for i, n in enumerate(noccs)]
+    return Bp, Cs
+
+
+@pytest.mark.parametrize("cfg_id", [1, 2])
+def test_baseline_configs_all_calls(dfjk, cfg_id):
+    cfg = gi.CONFIGS[cfg_id]
+    Bp = gi.fill_B_host(cfg)
+    Bd = dev(Bp)
+    h = dfjk.DFJK(Bd, cfg.nao)
+    for call in range(min(cfg.calls, 3)):
+        C = gi.orbitals(cfg, call)[0]
+        J, K = h.get_jk(dev(C))
+        d = h.get_d()
+        torch.cuda.synchronize()
+        Jo, Ko, do = oracle.get_jk(Bp, cfg.nao, [C], [2.0])
+        assert relerr(d.cpu().numpy(), do) <= TOL
+        assert relerr(J.cpu().numpy(), Jo) <= TOL
+        assert relerr(K.cpu().numpy(), Ko[0]) <= TOL
+    h.close()
+
+
+@pytest.mark.parametrize("nao,naux,nocc", [
+    (1, 1, 1),          # npair = 1
+    (2, 3, 1),
+    (5, 7, 5),          # nocc = nao
+    (17, 9, 7),
+    (33, 5, 8),
+    (64, 16, 9),
+    (129, 10, 3),       # one row past a 128 tile; odd npair
+    (130, 12, 17),      # npair odd (nao mod 4 == 2)
+    (200, 21, 140),     # nocc > 136: two N tiles in K1
+    (257, 6, 31),
+    (300, 40, 300),     # nocc = nao, three N tiles
+])
+def test_ragged_shapes(dfjk, nao, naux, nocc):
+    Bp, (C,) = rand_case(nao, naux, (nocc,), seed=nao + naux)
+    J, K, d = run_restricted(dfjk, Bp, nao, C)
+    Jo, Ko, do = oracle.get_jk(Bp, nao, [C], [2.0])
+    assert relerr(d, do) <= TOL
+    assert relerr(J, Jo) <= TOL
+    assert relerr(K, Ko[0]) <= TOL
+    assert np.array_equal(J, J.T) and np.array_equal(K, K.T)   # mirrored, bit for bit
+
+
+def test_non_orthonormal_orbitals(dfjk):
+    Bp, (C,) = rand_case(150, 30, (20,), seed=5, orthonormal=False)
+    J, K, _ = run_restricted(dfjk, Bp, 150, C)
+    Jo, Ko, _ = oracle.get_jk(Bp, 150, [C], [2.0])
+    assert relerr(J, Jo) <= TOL and relerr(K, Ko[0]) <= TOL
+
+
+@pytest.mark.parametrize("opts", [dict(k_chunk=1), dict(k_chunk=3), dict(k_chunk=4, k_splits=1),
+                                  dict(k_chunk=7, k_splits=2)])
+def test_chunk_and_split_options(dfjk, opts):
+    Bp, (C,) = rand_case(260, 23, (13,), seed=3)
+    J, K, _ = run_restricted(dfjk, Bp, 260, C, **opts)
+    Jo, Ko, _ = oracle.get_jk(Bp, 260, [C], [2.0])
+    assert relerr(J, Jo) <= TOL and relerr(K, Ko[0]) <= TOL
+
+
+def test_unrestricted(dfjk):
+    nao, naux = 210, 33
+    Bp, (Ca, Cb) = rand_case(nao, naux, (19, 14), seed=8)
+    h = dfjk.DFJK(dev(Bp), nao)
+    J, Ka, Kb = h.get_jk_u(dev(Ca), dev(Cb))
+    torch.cuda.synchronize()
+    Jo, Kao, Kbo = oracle.get_jk_unrestricted(Bp, nao, Ca, Cb)
+    assert relerr(J.cpu().numpy(), Jo) <= TOL
+    assert relerr(Ka.cpu().numpy(), Kao) <= TOL
+    assert relerr(Kb.cpu().numpy(), Kbo) <= TOL
+    h.close()
+
+
+def test_j_only_k_only_and_repeatability(dfjk):
+    nao = 190
+    Bp, (C,) = rand_case(nao, 25, (11,), seed=2)
+    h = dfjk.DFJK(dev(Bp), nao)
+    Cd = dev(C)
+    J1, K1 = h.get_jk(Cd)
+    J2, none_k = h.get_jk(Cd, with_k=False)
+    none_j, K2 = h.get_jk(Cd, with_j=False)
+    torch.cuda.synchronize()
+    assert none_k is None and none_j is None
+    # deterministic reductions: repeat calls are bitwise identical
+    assert torch.equal(J1, J2) and torch.equal(K1, K2)
+    # outputs are overwritten, not accumulated
+    Jpre = torch.full((nao, nao), 7.0, dtype=torch.float64, device="cuda")
+    Kpre = torch.full((nao, nao), -3.0, dtype=torch.float64, device="cuda")
+    h.get_jk(Cd, out_j=Jpre, out_k=Kpre)
+    torch.cuda.synchronize()
+    assert torch.equal(Jpre, J1) and torch.equal(Kpre, K1)
+    h.close()
+
+
+def test_side_stream(dfjk):
+    nao = 100
+    Bp, (C,) = rand_case(nao, 12, (6,), seed=4)
+    h = dfjk.DFJK(dev(Bp), nao)
+    Cd = dev(C)
+    torch.cuda.synchronize()
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        J, K = h.get_jk(Cd)
+    s.synchronize()
+    Jo, Ko, _ = oracle.get_jk(Bp, nao, [C], [2.0])
+    assert relerr(J.cpu().numpy(), Jo) <= TOL and relerr(K.cpu().numpy(), Ko[0]) <= TOL
+    h.close()
+
+
+def test_host_entry_point(dfjk):
+    nao = 140
+    Bp, (C,) = rand_case(nao, 18, (9,), seed=6)
+    h = dfjk.DFJK(dev(Bp), nao)
+    Ch = torch.from_numpy(C).pin_memory()
+    Jh = torch.empty(nao, nao, dtype=torch.float64).pin_memory()
+    Kh = torch.empty(nao, nao, dtype=torch.float64).pin_memory()
+    h.get_jk_host(Ch, Jh, Kh)
+    Jo, Ko, _ = oracle.get_jk(Bp, nao, [C], [2.0])
+    assert relerr(Jh.numpy(), Jo) <= TOL and relerr(Kh.numpy(), Ko[0]) <= TOL
+    # pageable memory is accepted too
+    Jp = torch.empty(nao, nao, dtype=torch.float64)
+    h.get_jk_host(torch.from_numpy(C), Jp, None)
+    assert relerr(Jp.numpy(), Jo) <= TOL
+    h.close()
+
+
+def test_single_element_probe_on_gpu(dfjk):
+    """One non-zero packed entry lights exactly the entries the definition predicts."""
+    nao, naux = 37, 3
+    C = gi.random_orbitals(nao, 4, 99, orthonormal=False)
+    G = C @ C.T
+    for (mu, nu) in [(0, 0), (36, 0), (36, 36), (20, 7), (17, 16)]:
+        Bp = np.zeros((naux, nao * (nao + 1) // 2))
+        Bp[2, mu * (mu + 1) // 2 + nu] = 1.5
+        E = np.zeros((nao, nao)); E[mu, nu] = E[nu, mu] = 1.5
+        J, K, d = run_restricted(dfjk, Bp, nao, C)
+        assert d[0] == 0.0 and d[1] == 0.0
+        assert abs(d[2] - 2.0 * (E * G).sum()) <= 1e-13 * max(1.0, abs(d[2]))
+        assert relerr(J, 2.0 * (E * G).sum() * E) <= 1e-13
+        assert relerr(K, E @ G @ E) <= 1e-13
+
+
+def test_error_paths(dfjk):
+    L = dfjk.lib()
+    nao = 8
+    Bp, (C,) = rand_case(nao, 4, (3,), seed=1)
+    Bd, Cd = dev(Bp), dev(C)
+    out = torch.empty(nao, nao, dtype=torch.float64, device="cuda")
+    assert not L.dfjk_create(0, nao, Bd.data_ptr()) and b"naux" in L.dfjk_last_error()
+    assert not L.dfjk_create(4, 0, Bd.data_ptr())
+    assert not L.dfjk_create(4, nao, None)
+    assert not L.dfjk_create(4, nao, Bd.data_ptr() + 8) and b"aligned" in L.dfjk_last_error()
+    hostbuf = np.zeros(4 * 36)
+    assert not L.dfjk_create(4, nao, hostbuf.ctypes.data)
+    h = L.dfjk_create(4, nao, Bd.data_ptr())
+    assert h
+    assert L.dfjk_get_jk(h, Cd.data_ptr(), 0, out.data_ptr(), None, None) == -1
+    assert L.dfjk_get_jk(h, Cd.data_ptr(), nao + 1, out.data_ptr(), None, None) == -1
+    assert L.dfjk_get_jk(h, None, 3, out.data_ptr(), None, None) == -1
+    assert L.dfjk_get_jk(h, Cd.data_ptr(), 3, None, None, None) == -1
+    assert L.dfjk_get_jk(None, Cd.data_ptr(), 3, out.data_ptr(), None, None) == -1
+    assert L.dfjk_get_d(h, out.data_ptr(), None) == -1          # no J built yet
+    assert L.dfjk_set_option(h, b"nonsense", 1) == -1
+    assert L.dfjk_get_jk(h, Cd.data_ptr(), 3, out.data_ptr(), None, None) == 0
+    assert L.dfjk_last_error() == b""
+    torch.cuda.synchronize()
+    assert L.dfjk_destroy(h) == 0 and L.dfjk_destroy(None) == 0
