@@ -1,0 +1,340 @@
+#!/usr/bin/env python
+"""bench.py -- DF get_jk throughput on B200 (BASELINE.json metric), one JSON line.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path: one ``dfjk_get_jk`` (J and K, SURVEY.md
+section 8a rows J0-J3, K0-K3) for one fresh C_occ of the config's call schedule, B
+resident in HBM.  Default workload = BASELINE.json configs[3] (nao=1600, naux=5000,
+nocc=130: the config the metric's roofline target is quoted on; 51 GB fits one GPU).
+
+  value      algorithmic GFLOP/s of the whole job (all ranks), inputs resident in HBM
+  e2e        the same through dfjk_get_jk_host: C_occ from pinned HOST memory, J and K
+             back to pinned HOST memory inside the timed region (B stays resident:
+             it is the handle's state, built once per geometry like the paper's with_df)
+  roofline   dominant kernel (K1 half transform, 2/3 of the flops): DMMA on the FP64 pipe
+  cpu_baseline  the oracle on this box's host cores, on a bounded row-slab sample
+
+Multi-GPU (--gpus N under torchrun): the path does not shard (north_star: one GPU, no
+collectives) => N independent replicas, weak scaling, no data-path collective.
+``--impl reference`` times the CPU oracle as it stands (rank 0 only).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import dfjk_inputs as gi  # noqa: E402
+
+FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12     # 37.2: SMs x FMA/clk/SM x 2 x max clock
+HBM_FALLBACK_GBS = 6650.0
+
+
+def flops_j(cfg):
+    return 4.0 * cfg.naux * cfg.npair
+
+
+def flops_k1(cfg):
+    return 2.0 * cfg.naux * cfg.nao ** 2 * sum(cfg.nocc)
+
+
+def flops_k2(cfg):
+    return 1.0 * cfg.naux * cfg.nao * (cfg.nao + 1) * sum(cfg.nocc)
+
+
+def flops_step(cfg):
+    return flops_j(cfg) + flops_k1(cfg) + flops_k2(cfg)
+
+
+def measured_peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return json.load(f), "measured"
+    except Exception:
+        return {"hbm_gbs": HBM_FALLBACK_GBS}, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                 "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        self.thread.join(timeout=2)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+                for n, v in zip(names, r[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(n)
+            except Exception:
+                pass
+        return {"sm_mhz": float(np.median(sm)) if sm else None,
+                "sm_max_mhz": max(mx) if mx else None, "samples": len(sm),
+                "reasons": sorted(reasons)}
+
+
+def oracle_sample(cfg, rows, call=0):
+    """Time the oracle (as it stands) on `rows` rows of the config's B. Returns seconds, threads."""
+    import oracle
+    Bp = gi.fill_B_host(cfg, 0, rows)
+    Cs = gi.orbitals(cfg, call)
+    acc = oracle.JKAccumulator(cfg.nao, Cs, cfg.weights)
+    acc.add_slab(Bp[:1])                       # touch the code path / page in
+    acc = oracle.JKAccumulator(cfg.nao, Cs, cfg.weights)
+    t0 = time.perf_counter()
+    acc.add_slab(Bp)
+    return time.perf_counter() - t0, oracle.num_threads()
+
+
+def size_sample(cfg, target_s):
+    """Grow the row-slab until the oracle takes about target_s seconds (or all rows)."""
+    rows = min(4, cfg.naux)
+    while True:
+        t, threads = oracle_sample(cfg, rows)
+        if t >= target_s / 3 or rows >= cfg.naux:
+            return rows, t, threads
+        rows = int(min(cfg.naux, max(2 * rows, 0.8 * rows * target_s / max(t, 1e-6))))
+
+
+def run_reference(args, cfg):
+    """--impl reference: the CPU oracle on this box's host cores, bounded sample per step."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    per_row = flops_step(cfg) / cfg.naux
+    # size the per-step sample from one pilot row-slab: aim at ~5 s per step
+    rows, _, threads = size_sample(cfg, 5.0)
+    Bp = gi.fill_B_host(cfg, 0, rows)
+    times = []
+    for step in range(args.warmup + args.steps):
+        Cs = gi.orbitals(cfg, 0)
+        acc = oracle.JKAccumulator(cfg.nao, Cs, cfg.weights)
+        t0 = time.perf_counter()
+        acc.add_slab(Bp)
+        dt = time.perf_counter() - t0
+        if step >= args.warmup:
+            times.append(dt)
+    t = float(np.mean(times))
+    val = per_row * rows / t / 1e9
+    sample = f"{rows} of {cfg.naux} auxiliary rows of cfg {cfg.index} per step (J and K, full nao)"
+    print(json.dumps({
+        "impl": "reference", "metric": "df_get_jk_gflops_fp64", "value": val, "unit": "GFLOP/s",
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": t * 1e3 * cfg.naux / rows, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": workload_config(cfg, args),
+        "cpu_baseline": {"value": val, "unit": "GFLOP/s", "cores": threads, "kind": "oracle",
+                         "sample": sample},
+        "e2e": {"value": val, "unit": "GFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "note": "ms_per_step is the sample time scaled to all naux rows; flops are the algorithmic "
+                "count (4 naux npair + 3 naux nao^2 nocc), the oracle itself does the full-square work",
+    }))
+
+
+def workload_config(cfg, args):
+    return {"workload": f"BASELINE.json configs[{cfg.index - 1}] '{cfg.name}': nao={cfg.nao} "
+                        f"naux={cfg.naux} nocc={'+'.join(map(str, cfg.nocc))} seed={cfg.seed}",
+            "nao": cfg.nao, "naux": cfg.naux, "nocc": list(cfg.nocc),
+            "b_bytes": cfg.b_bytes, "calls_per_step": 1,
+            "l2": "inputs larger than L2: every step streams the packed B "
+                  f"({cfg.b_bytes / 1e9:.1f} GB) three times" if cfg.b_bytes > (1 << 30) else
+                  "L2 flushed between steps (256 MB write)",
+            "parallelism": f"replicas x{args.gpus}" if args.gpus > 1 else "single GPU"}
+
+
+def run_ours(args, cfg):
+    import torch
+    import paper_2506_06661_b200 as pkg
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product has no CPU fallback)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    pkg.lib()
+    unrestricted = len(cfg.nocc) == 2
+    B = torch.empty(cfg.naux, cfg.npair, dtype=torch.float64, device=dev)
+    gi.fill_B_device(cfg, B)
+    h = pkg.DFJK(B, cfg.nao)
+    ncalls = args.warmup + args.steps
+    Cs_host = list(gi.orbital_sequence(cfg, ncalls))          # [call][set] numpy, host
+    Cs_dev = [[torch.from_numpy(C).to(dev) for C in sets] for sets in Cs_host]
+    flush = None if cfg.b_bytes > (1 << 30) else torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+
+    def step(sets):
+        if unrestricted:
+            return h.get_jk_u(sets[0], sets[1])
+        return h.get_jk(sets[0])
+
+    for k in range(args.warmup):
+        step(Cs_dev[k])
+    h.set_option("time_kernels", 1)
+    launches0 = h.launch_count
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+          for _ in range(args.steps)]
+    sampler = ClockSampler(local)
+    barrier()
+    sampler.start()
+    for k in range(args.steps):
+        if flush is not None:
+            flush.fill_(k & 0xFF)
+        ev[k][0].record()
+        out = step(Cs_dev[args.warmup + k])
+        ev[k][1].record()
+    barrier()
+    clocks = sampler.stop()
+    launches = h.launch_count - launches0
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    total_ms = float(sum(step_ms))
+    kt = {name: h.kernel_time(name) for name in pkg.KERNELS}
+    h.set_option("time_kernels", 0)
+    if dist is not None:
+        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+
+    # ---- end to end through the host entry point (restricted configs)
+    e2e = None
+    if not unrestricted:
+        nocc = cfg.nocc[0]
+        Ch = [torch.from_numpy(s[0]).pin_memory() for s in Cs_host]
+        Jh = torch.empty(cfg.nao, cfg.nao, dtype=torch.float64).pin_memory()
+        Kh = torch.empty(cfg.nao, cfg.nao, dtype=torch.float64).pin_memory()
+        h.get_jk_host(Ch[0], Jh, Kh)
+        barrier()
+        t0 = time.perf_counter()
+        for k in range(args.steps):
+            h.get_jk_host(Ch[args.warmup + k], Jh, Kh)
+        e2e_s = time.perf_counter() - t0
+        if dist is not None:
+            t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            e2e_s = float(t.item())
+        e2e = {"value": world * flops_step(cfg) * args.steps / e2e_s / 1e9, "unit": "GFLOP/s",
+               "ms_per_step": e2e_s * 1e3 / args.steps,
+               "h2d_bytes_per_step": cfg.nao * nocc * 8, "d2h_bytes_per_step": 2 * cfg.nao * cfg.nao * 8,
+               "api": "dfjk_get_jk_host (pinned host C_occ in, pinned host J and K out; B resident)"}
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    peaks, peak_src = measured_peaks()
+    ms_per_step = total_ms / args.steps
+    value = world * flops_step(cfg) * args.steps / (total_ms * 1e-3) / 1e9
+    k1_ms, k1_n = kt["K1"]
+    k2_ms, k2_n = kt["K2"]
+    j_ms = sum(kt[n][0] for n in ("J0", "J1", "J1R", "J2", "J3")) / args.steps
+    k_ms = sum(kt[n][0] for n in ("K1", "K2", "K3")) / args.steps
+    traffic = None
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            traffic = json.load(f).get(f"cfg{cfg.index}", {}).get("k1_dram_bytes_per_launch")
+    except Exception:
+        pass
+    k1_tflops = flops_k1(cfg) * args.steps / (k1_ms * 1e-3) / 1e12 if k1_ms > 0 else 0.0
+    roofline = {"kernel": "k1_half_transform_kernel (X_P = B_P C, DMMA.8x8x4 on the FP64 pipe)",
+                "bound": "alu", "achieved": k1_tflops, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
+                "frac": k1_tflops / FP64_PEAK_TFLOPS, "traffic": traffic,
+                "peak_source": "148 SM x 64 FP64 FMA/clk x 2 x 1.965 GHz (DESIGN.md; DMMA microbenchmark "
+                               "reaches 37.07); sm_100a has no tcgen05 FP64 kind",
+                "launches": k1_n, "avg_launch_ms": k1_ms / max(k1_n, 1),
+                "flops_per_launch": flops_k1(cfg) * args.steps / max(k1_n, 1)}
+    hbm = float(peaks.get("hbm_gbs", HBM_FALLBACK_GBS))
+    j_stream_ms = (kt["J1"][0] + kt["J2"][0]) / args.steps
+    k2_tflops = flops_k2(cfg) * args.steps / (k2_ms * 1e-3) / 1e12 if k2_ms > 0 else 0.0
+    out = {
+        "metric": "df_get_jk_gflops_fp64", "value": value, "unit": "GFLOP/s", "n_gpus": world,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "config": workload_config(cfg, args), "clocks": clocks,
+        "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
+        "j": {"ms": j_ms, "stream_ms": j_stream_ms, "bytes": 2 * cfg.b_bytes,
+              "gbs": 2 * cfg.b_bytes / (j_stream_ms * 1e-3) / 1e9 if j_stream_ms > 0 else None,
+              "hbm_peak_gbs": hbm, "peak_source": peak_src,
+              "frac": 2 * cfg.b_bytes / (j_stream_ms * 1e-3) / 1e9 / hbm if j_stream_ms > 0 else None},
+        "k": {"ms": k_ms, "tflops": (flops_k1(cfg) + flops_k2(cfg)) / (k_ms * 1e-3) / 1e12 if k_ms > 0 else None,
+              "frac_fp64_peak": (flops_k1(cfg) + flops_k2(cfg)) / (k_ms * 1e-3) / 1e12 / FP64_PEAK_TFLOPS if k_ms > 0 else None,
+              "k1_ms": k1_ms / args.steps, "k2_ms": k2_ms / args.steps, "k2_tflops": k2_tflops},
+        "step_ms": step_ms,
+    }
+    if world == 1:
+        rows, t, threads = size_sample(cfg, 15.0)
+        out["cpu_baseline"] = {
+            "value": flops_step(cfg) / cfg.naux * rows / t / 1e9, "unit": "GFLOP/s", "cores": threads,
+            "kind": "oracle", "seconds": t,
+            "sample": f"{rows} of {cfg.naux} auxiliary rows of cfg {cfg.index}, J and K, one call "
+                      "(algorithmic flop count; the oracle does the full-square work)"}
+    print(json.dumps(out))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=4, choices=sorted(gi.CONFIGS))
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        print("bench.py: warning: fewer than 3 warm-up steps", file=sys.stderr)
+    cfg = gi.CONFIGS[args.config]
+    if args.impl == "reference":
+        run_reference(args, cfg)
+    else:
+        run_ours(args, cfg)
+
+
+if __name__ == "__main__":
+    main()

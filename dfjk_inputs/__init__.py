@@ -212,6 +212,20 @@ def orbitals(cfg: Config, call: int = 0) -> List[np.ndarray]:
     return out
 
 
+def orbital_sequence(cfg: Config, ncalls: int):
+    """Yield the per-call orbital blocks of calls 0..ncalls-1 (same values as ``orbitals``,
+    computed incrementally; continues the schedule past ``cfg.calls``)."""
+    if cfg.schedule != "rotate":
+        for call in range(ncalls):
+            yield orbitals(cfg, call)
+        return
+    cur = orbitals(cfg, 0)
+    yield cur
+    for k in range(1, ncalls):
+        cur = [_orth(_expm_apply(cfg, k, s, C)) for s, C in enumerate(cur)]
+        yield cur
+
+
 def random_orbitals(nao: int, nocc: int, seed: int, orthonormal: bool = True) -> np.ndarray:
     """A free-standing nao x nocc block for tests (optionally NOT orthonormal, reading R8)."""
     M = normals(seed, STREAM_C, nao * nocc).reshape(nao, nocc)

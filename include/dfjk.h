@@ -116,10 +116,37 @@ int dfjk_get_d(dfjk_handle *h, double *d_out, void *stream);
  *   "k_chunk"   number of auxiliary rows whose half-transformed X stays in the
  *               L2-sized workspace between the K1 and K2 kernels (0 = automatic)
  *   "k_splits"  number of partial-K accumulators the SYRK is split over (0 = automatic)
+ *   "time_kernels"  1 = bracket every kernel launch with CUDA events on the call's stream
+ *               (read back with dfjk_kernel_time); setting it (to 0 or 1) clears the record
  *   "j_fused"   1 = J in one HBM pass (row groups kept in L2 between the dot and
  *               the axpy), 0 = two plain streaming passes (default)
  */
 int dfjk_set_option(dfjk_handle *h, const char *name, int64_t value);
+
+/* kernel ids for dfjk_kernel_time (one per step of the path) */
+#define DFJK_KERNEL_K0   0   /* pack / zero-pad C_occ */
+#define DFJK_KERNEL_J0   1   /* build D-tilde */
+#define DFJK_KERNEL_J1   2   /* d_P = <B_P, D-tilde>       (streams B) */
+#define DFJK_KERNEL_J1R  3   /* reduce d partials */
+#define DFJK_KERNEL_J2   4   /* Jp = sum_P d_P B_P         (streams B) */
+#define DFJK_KERNEL_J3   5   /* unpack Jp -> J */
+#define DFJK_KERNEL_K1   6   /* X_P = B_P C                (DMMA) */
+#define DFJK_KERNEL_K2   7   /* K_lower += X X^T           (DMMA) */
+#define DFJK_KERNEL_K3   8   /* reduce splits, mirror */
+#define DFJK_KERNEL_COUNT 9
+
+/*
+ * dfjk_launch_count -- number of kernels this handle has launched since dfjk_create.
+ */
+int64_t dfjk_launch_count(const dfjk_handle *h);
+
+/*
+ * dfjk_kernel_time -- with option "time_kernels" = 1: total device time (ms, CUDA events
+ * on the launching stream) and number of launches of kernel `kernel` (DFJK_KERNEL_*)
+ * recorded since the option was last set.  Waits for the recorded events (HOST pointers
+ * ms_total, count).  At most 16384 launches are recorded.
+ */
+int dfjk_kernel_time(dfjk_handle *h, int kernel, double *ms_total, int64_t *count);
 
 /*
  * dfjk_workspace_bytes -- bytes of device workspace owned by the handle.

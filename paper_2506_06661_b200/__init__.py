@@ -17,7 +17,7 @@ import os
 import subprocess
 from typing import Optional, Tuple
 
-__all__ = ["build", "lib", "DFJK", "DFJKError", "SYMBOLS", "LIB_PATH", "HEADER_PATH"]
+__all__ = ["build", "lib", "DFJK", "DFJKError", "SYMBOLS", "KERNELS", "LIB_PATH", "HEADER_PATH"]
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libdfjk.so")
@@ -28,8 +28,11 @@ HEADER_PATH = os.path.join(os.path.dirname(_HERE), "include", "dfjk.h")
 SYMBOLS = (
     "dfjk_create", "dfjk_get_jk", "dfjk_get_jk_u", "dfjk_get_jk_host", "dfjk_get_d",
     "dfjk_set_option", "dfjk_workspace_bytes", "dfjk_destroy", "dfjk_last_error",
-    "dfjk_version",
+    "dfjk_version", "dfjk_launch_count", "dfjk_kernel_time",
 )
+
+# DFJK_KERNEL_* ids of include/dfjk.h
+KERNELS = {"K0": 0, "J0": 1, "J1": 2, "J1R": 3, "J2": 4, "J3": 5, "K1": 6, "K2": 7, "K3": 8}
 
 _lib = None
 
@@ -76,6 +79,10 @@ def lib() -> ctypes.CDLL:
     L.dfjk_last_error.argtypes = []
     L.dfjk_version.restype = ctypes.c_char_p
     L.dfjk_version.argtypes = []
+    L.dfjk_launch_count.restype = i64
+    L.dfjk_launch_count.argtypes = [vp]
+    L.dfjk_kernel_time.restype = ci
+    L.dfjk_kernel_time.argtypes = [vp, ci, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(i64)]
     _lib = L
     return L
 
@@ -186,6 +193,17 @@ class DFJK:
 
     def set_option(self, name: str, value: int) -> None:
         _check(lib().dfjk_set_option(self._h, name.encode(), int(value)), "dfjk_set_option")
+
+    @property
+    def launch_count(self) -> int:
+        return int(lib().dfjk_launch_count(self._h))
+
+    def kernel_time(self, kernel: str) -> Tuple[float, int]:
+        """(total ms, launches) of one kernel since ``set_option("time_kernels", 1)``."""
+        ms, n = ctypes.c_double(0.0), ctypes.c_int64(0)
+        _check(lib().dfjk_kernel_time(self._h, KERNELS[kernel], ctypes.byref(ms), ctypes.byref(n)),
+               "dfjk_kernel_time")
+        return ms.value, n.value
 
     @property
     def workspace_bytes(self) -> int:

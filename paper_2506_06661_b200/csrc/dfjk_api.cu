@@ -59,6 +59,12 @@ struct dfjk_handle {
     /* options */
     int64_t opt_k_chunk, opt_k_splits, opt_j_fused;
     bool have_d;
+    /* instrumentation: launch counter and optional per-kernel CUDA-event timing */
+    int64_t launches;
+    int64_t opt_time_kernels;
+    cudaEvent_t *ev;     /* pairs: ev[2*i], ev[2*i+1] */
+    int *ev_kind;        /* which kernel pair i brackets (DFJK_KERNEL_*) */
+    int ev_cap, ev_used;
     /* host-call resources (lazy) */
     cudaStream_t host_stream;
     double *hostC, *hostJ, *hostK;
@@ -72,7 +78,25 @@ void free_all(dfjk_handle *h)
     cudaFree(h->Jp_part); cudaFree(h->X); cudaFree(h->Kpart);
     cudaFree(h->hostC); cudaFree(h->hostJ); cudaFree(h->hostK);
     if (h->host_stream) cudaStreamDestroy(h->host_stream);
+    for (int i = 0; i < 2 * h->ev_cap; ++i) cudaEventDestroy(h->ev[i]);
+    delete[] h->ev;
+    delete[] h->ev_kind;
 }
+
+/* bracket one kernel launch with events when "time_kernels" is on */
+struct Timed {
+    dfjk_handle *h; cudaStream_t st; int slot;
+    Timed(dfjk_handle *h_, int kind, cudaStream_t st_) : h(h_), st(st_), slot(-1)
+    {
+        ++h->launches;
+        if (h->opt_time_kernels && h->ev_used < h->ev_cap) {
+            slot = h->ev_used++;
+            h->ev_kind[slot] = kind;
+            cudaEventRecord(h->ev[2 * slot], st);
+        }
+    }
+    ~Timed() { if (slot >= 0) cudaEventRecord(h->ev[2 * slot + 1], st); }
+};
 
 /* split count that fills the SMs best: work items = ntile * s, one CTA per SM */
 int choose_splits(int ntile, int sm_count, int max_splits)
@@ -172,6 +196,17 @@ extern "C" int dfjk_set_option(dfjk_handle *h, const char *name, int64_t value)
         if (value > h->nsplit_alloc) return fail(DFJK_EINVAL, "k_splits > %d allocated", h->nsplit_alloc);
         h->opt_k_splits = value; return DFJK_OK;
     }
+    if (!strcmp(name, "time_kernels")) {
+        if (value && !h->ev) {
+            const int cap = 16384;
+            h->ev = new (std::nothrow) cudaEvent_t[2 * cap];
+            h->ev_kind = new (std::nothrow) int[cap];
+            if (!h->ev || !h->ev_kind) return fail(DFJK_ENOMEM, "time_kernels: host allocation failed");
+            for (int i = 0; i < 2 * cap; ++i) DFJK_CUDA_TRY(cudaEventCreate(&h->ev[i]));
+            h->ev_cap = cap;
+        }
+        h->opt_time_kernels = value; h->ev_used = 0; return DFJK_OK;
+    }
     if (!strcmp(name, "j_fused")) {
         if (value != 0) return fail(DFJK_EINVAL, "j_fused=1 is not available in this build");
         h->opt_j_fused = value; return DFJK_OK;
@@ -209,14 +244,14 @@ int get_jk_impl(dfjk_handle *h, int nset, const double *const *C, const int64_t 
         ldc += round_up(nocc64[s], 8);
     }
     /* K0: zero-padded concatenation [C_0 | C_1], each set padded to a multiple of 8 columns */
-    dfjk::launch_k0_pack_c(C, nocc, col0, nset, nao, ldc, h->Ccat, st);
+    { Timed t_(h, DFJK_KERNEL_K0, st); dfjk::launch_k0_pack_c(C, nocc, col0, nset, nao, ldc, h->Ccat, st); }
 
     if (J) {
-        dfjk::launch_j0_build_dt(h->Ccat, ldc, nao, nset, col0, nocc, w, h->Dt, st);
-        dfjk::launch_j1_dot(h->B, naux, npair, h->Dt, h->d_part, h->sm_count, st);
-        dfjk::launch_j1_reduce(h->d_part, h->nchunk, naux, h->d, st);
-        dfjk::launch_j2_axpy(h->B, naux, npair, h->d, h->Jp_part, h->j2_groups, st);
-        dfjk::launch_j3_unpack(h->Jp_part, h->j2_groups, npair, nao, J, st);
+        { Timed t_(h, DFJK_KERNEL_J0, st); dfjk::launch_j0_build_dt(h->Ccat, ldc, nao, nset, col0, nocc, w, h->Dt, st); }
+        { Timed t_(h, DFJK_KERNEL_J1, st); dfjk::launch_j1_dot(h->B, naux, npair, h->Dt, h->d_part, h->sm_count, st); }
+        { Timed t_(h, DFJK_KERNEL_J1R, st); dfjk::launch_j1_reduce(h->d_part, h->nchunk, naux, h->d, st); }
+        { Timed t_(h, DFJK_KERNEL_J2, st); dfjk::launch_j2_axpy(h->B, naux, npair, h->d, h->Jp_part, h->j2_groups, st); }
+        { Timed t_(h, DFJK_KERNEL_J3, st); dfjk::launch_j3_unpack(h->Jp_part, h->j2_groups, npair, nao, J, st); }
         h->have_d = true;
     }
 
@@ -231,17 +266,21 @@ int get_jk_impl(dfjk_handle *h, int nset, const double *const *C, const int64_t 
         int chunk = 0;
         for (int64_t P0 = 0; P0 < naux; P0 += pc, ++chunk) {
             const int64_t np = (P0 + pc <= naux) ? pc : naux - P0;
-            dfjk::launch_k1_half_transform(h->B, nao, npair, P0, np, h->Ccat, ldc, h->X, xpitch, st);
+            { Timed t_(h, DFJK_KERNEL_K1, st); dfjk::launch_k1_half_transform(h->B, nao, npair, P0, np, h->Ccat, ldc, h->X, xpitch, st); }
             for (int s = 0; s < nset; ++s)
-                if (K[s])
+                if (K[s]) {
+                    Timed t_(h, DFJK_KERNEL_K2, st);
                     dfjk::launch_k2_syrk_lower(h->X, xpitch, nao, np, ldc, col0[s], nocc[s],
                                                h->Kpart + (int64_t)s * h->nsplit_alloc * nao * nao,
                                                nsplit, chunk > 0, st);
+                }
         }
         for (int s = 0; s < nset; ++s)
-            if (K[s])
+            if (K[s]) {
+                Timed t_(h, DFJK_KERNEL_K3, st);
                 dfjk::launch_k3_finish(h->Kpart + (int64_t)s * h->nsplit_alloc * nao * nao, nsplit,
                                        nao, K[s], st);
+            }
     }
     DFJK_CUDA_TRY(cudaGetLastError());
     return DFJK_OK;
@@ -302,5 +341,27 @@ extern "C" int dfjk_get_jk_host(dfjk_handle *h, const double *C_occ_host, int64_
     if (J_host) DFJK_CUDA_TRY(cudaMemcpyAsync(J_host, h->hostJ, (size_t)n2 * 8, cudaMemcpyDeviceToHost, st));
     if (K_host) DFJK_CUDA_TRY(cudaMemcpyAsync(K_host, h->hostK, (size_t)n2 * 8, cudaMemcpyDeviceToHost, st));
     DFJK_CUDA_TRY(cudaStreamSynchronize(st));
+    return DFJK_OK;
+}
+
+extern "C" int64_t dfjk_launch_count(const dfjk_handle *h) { return h ? h->launches : 0; }
+
+extern "C" int dfjk_kernel_time(dfjk_handle *h, int kernel, double *ms_total, int64_t *count)
+{
+    g_err[0] = 0;
+    if (!h || !ms_total || !count) return fail(DFJK_EINVAL, "dfjk_kernel_time: NULL argument");
+    if (kernel < 0 || kernel >= DFJK_KERNEL_COUNT) return fail(DFJK_EINVAL, "dfjk_kernel_time: bad kernel id");
+    double tot = 0.0;
+    int64_t n = 0;
+    for (int i = 0; i < h->ev_used; ++i) {
+        if (h->ev_kind[i] != kernel) continue;
+        DFJK_CUDA_TRY(cudaEventSynchronize(h->ev[2 * i + 1]));
+        float ms = 0.f;
+        DFJK_CUDA_TRY(cudaEventElapsedTime(&ms, h->ev[2 * i], h->ev[2 * i + 1]));
+        tot += ms;
+        ++n;
+    }
+    *ms_total = tot;
+    *count = n;
     return DFJK_OK;
 }
