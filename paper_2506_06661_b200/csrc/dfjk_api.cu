@@ -45,7 +45,7 @@ struct dfjk_handle {
     int device, sm_count;
     int64_t l2_bytes;
     /* workspace (device) */
-    double *Ccat;        /* nao x ldc_max */
+    double *Ccat;        /* nao16 x ldc_max, k-group-major */
     int64_t ldc_max;
     double *Dt;          /* npair */
     double *d_part;      /* nchunk x naux */
@@ -166,7 +166,7 @@ extern "C" dfjk_handle *dfjk_create(int64_t naux, int64_t nao, const double *B_p
     h->nsplit_alloc = choose_splits(nb * (nb + 1) / 2, h->sm_count, 16);
 
     int rc = DFJK_OK;
-    if (rc == DFJK_OK) rc = alloc_ws(h, &h->Ccat, nao * h->ldc_max);
+    if (rc == DFJK_OK) rc = alloc_ws(h, &h->Ccat, round_up(nao, 16) * h->ldc_max);
     if (rc == DFJK_OK) rc = alloc_ws(h, &h->Dt, h->npair);
     if (rc == DFJK_OK) rc = alloc_ws(h, &h->d_part, h->nchunk * naux);
     if (rc == DFJK_OK) rc = alloc_ws(h, &h->d, naux);
@@ -259,18 +259,16 @@ int get_jk_impl(dfjk_handle *h, int nset, const double *const *C, const int64_t 
         int64_t pc = h->x_doubles / (nao * ldc);
         if (h->opt_k_chunk > 0 && h->opt_k_chunk < pc) pc = h->opt_k_chunk;
         if (pc > naux) pc = naux;
-        if (pc > 1) pc -= pc & 1;                      /* even: k groups pair up across P */
         if (pc < 1) return fail(DFJK_ENOMEM, "%s: X workspace too small", who);
-        const int64_t xpitch = pc * ldc;
         const int nsplit = h->opt_k_splits > 0 ? (int)h->opt_k_splits : h->nsplit_alloc;
         int chunk = 0;
         for (int64_t P0 = 0; P0 < naux; P0 += pc, ++chunk) {
             const int64_t np = (P0 + pc <= naux) ? pc : naux - P0;
-            { Timed t_(h, DFJK_KERNEL_K1, st); dfjk::launch_k1_half_transform(h->B, nao, npair, P0, np, h->Ccat, ldc, h->X, xpitch, st); }
+            { Timed t_(h, DFJK_KERNEL_K1, st); dfjk::launch_k1_half_transform(h->B, nao, npair, P0, np, h->Ccat, ldc, h->X, st); }
             for (int s = 0; s < nset; ++s)
                 if (K[s]) {
                     Timed t_(h, DFJK_KERNEL_K2, st);
-                    dfjk::launch_k2_syrk_lower(h->X, xpitch, nao, np, ldc, col0[s], nocc[s],
+                    dfjk::launch_k2_syrk_lower(h->X, nao, np, ldc, col0[s], nocc[s],
                                                h->Kpart + (int64_t)s * h->nsplit_alloc * nao * nao,
                                                nsplit, chunk > 0, st);
                 }

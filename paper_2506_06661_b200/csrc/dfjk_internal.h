@@ -17,7 +17,7 @@ namespace dfjk {
 /* ---------------------------------------------------------------- J path */
 
 /* J0: Dt[mu(mu+1)/2+nu] = (2 - delta_mu,nu) * sum_s w_s sum_i C_s[mu,i] C_s[nu,i].
- * Ccat is the zero-padded concatenation built by k0_pack_c: Ccat[nao][ldc], set s
+ * Ccat4 is the zero-padded, k-group-major concatenation built by k0_pack_c (see K0), set s
  * occupying columns [col0[s], col0[s]+nocc[s]). */
 void launch_j0_build_dt(const double *Ccat, int64_t ldc, int64_t nao,
                         int nset, const int *col0, const int *nocc, const double *w,
@@ -42,22 +42,23 @@ void launch_j3_unpack(const double *Jp_part, int64_t ngroup, int64_t npair, int6
 
 /* ---------------------------------------------------------------- K path */
 
-/* K0: Ccat[nao][ldc] = [C_0 | C_1 | ... | 0-pad], ldc multiple of 8. */
+/* K0: the zero-padded concatenation [C_0 | C_1 | ...] (every set padded to a multiple of 8
+ * columns, ldc columns in total) in k-group-major layout
+ *   Ccat4[(mu/4)*ldc*4 + c*4 + mu%4],  mu < nao16 = round_up(nao, 16) (rows >= nao are zero). */
 void launch_k0_pack_c(const double *const *C, const int *nocc, const int *col0, int nset,
                       int64_t nao, int64_t ldc, double *Ccat, cudaStream_t st);
 
-/* K1: for P in [P0, P0+np):  X[mu][(P-P0)*ldc + i] = sum_nu B_P(mu,nu) Ccat[nu][i]
- * X has row pitch xpitch doubles (>= np*ldc). */
+/* K1: for P in [P0, P0+np), k = (P-P0)*ldc + i:
+ *   X4[(k/4)*nao*4 + mu*4 + k%4] = sum_nu B_P(mu,nu) Ccat[nu][i]      (k-group-major X) */
 void launch_k1_half_transform(const double *B, int64_t nao, int64_t npair,
-                              int64_t P0, int64_t np, const double *Ccat, int64_t ldc,
-                              double *X, int64_t xpitch, cudaStream_t st);
+                              int64_t P0, int64_t np, const double *Ccat4, int64_t ldc,
+                              double *X4, cudaStream_t st);
 
-/* K2: Kpart[split][mu][nu] (+)= sum_{k in split's share of [kbeg,kend)} X[mu][k] X[nu][k]
- * for mu-tile >= nu-tile (lower tiles, full 128x128 tiles).  For np auxiliary rows of
- * pitch ldc, set s uses columns p*ldc + [col0, col0+ncol).  accumulate = 0 overwrites. */
-void launch_k2_syrk_lower(const double *X, int64_t xpitch, int64_t nao,
-                          int64_t np, int64_t ldc, int64_t col0, int64_t ncol,
-                          double *Kpart, int nsplit, int accumulate, cudaStream_t st);
+/* K2: Kpart[split][mu][nu] (+)= sum_{k in split's share} X[mu][k] X[nu][k]
+ * for mu-tile >= nu-tile (lower 128x128 tiles).  The set uses k = p*ldc + [col0, col0+round_up(ncol,8)),
+ * p < np.  accumulate = 0 overwrites. */
+void launch_k2_syrk_lower(const double *X4, int64_t nao, int64_t np, int64_t ldc, int64_t col0,
+                          int64_t ncol, double *Kpart, int nsplit, int accumulate, cudaStream_t st);
 
 /* K3: K[mu][nu] = K[nu][mu] = sum_split Kpart[split][mu][nu], mu >= nu. */
 void launch_k3_finish(const double *Kpart, int nsplit, int64_t nao, double *K, cudaStream_t st);

@@ -62,8 +62,9 @@ j0_build_dt_kernel(const double *__restrict__ Ccat, int64_t ldc, int64_t nao, Se
             const int row = ty + 8 * r;
             const int64_t c = c0 + tx;
             const int64_t mu = mu0 + row, nu = nu0 + row;
-            Cm[row][tx] = (mu < nao && c < ldc) ? Ccat[mu * ldc + c] : 0.0;
-            Cn[row][tx] = (nu < nao && c < ldc) ? Ccat[nu * ldc + c] : 0.0;
+            /* k-group-major Ccat4[(mu/4)][c][mu%4] */
+            Cm[row][tx] = (mu < nao && c < ldc) ? Ccat[((mu >> 2) * ldc + c) * 4 + (mu & 3)] : 0.0;
+            Cn[row][tx] = (nu < nao && c < ldc) ? Ccat[((nu >> 2) * ldc + c) * 4 + (nu & 3)] : 0.0;
         }
         __syncthreads();
 #pragma unroll 8

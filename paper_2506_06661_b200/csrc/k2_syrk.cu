@@ -4,14 +4,16 @@
  *
  *     K_s[mu][nu] += sum_{P in chunk} sum_{i in set s} X_P[mu][i] X_P[nu][i]     mu-tile >= nu-tile
  *
- * X chunk layout (written by K1): X[mu][p*ldc + i], row pitch xpitch, so the contraction
- * index k = (p, i) is contiguous per row apart from the jump between sets/P.  The k axis
- * is walked in groups of 8 columns (every set is zero-padded to a multiple of 8, so each
- * group is 64 contiguous, 16-B aligned bytes); a stage holds two groups (k = 16).
- * One CTA owns a 128 x 128 tile of K for one k-split: 8 warps as 2 (M) x 4 (N), warp tile
- * 64 x 32 = 8 x 4 DMMA.8x8x4 accumulators, 12 shared loads per 32 MMAs.  Both operands are
- * k-contiguous row tiles of X, so A (row-major) and B (col-major) fragments are read with
- * the same pattern; diagonal tiles load the panel once.
+ * X chunk layout (written by K1): k-group-major X4[k/4][mu][k%4], k = p*ldc + i, so the
+ * 128-row operand panel of one k-group (4 columns) is 4 KB of contiguous memory and lands
+ * in shared memory, by one 1-D bulk copy (TMA engine, UBLKCP), already in the dense
+ * [row][4] form whose DMMA fragment loads are bank-conflict-free.  A stage holds four
+ * k-groups (k = 16) of both operands; 6 stages, full/empty mbarriers, one producer lane.
+ * One CTA owns a 128 x 128 tile of K for one k-split: 8 consumer warps as 2 (M) x 4 (N),
+ * warp tile 64 x 32 = 8 x 4 DMMA.8x8x4 accumulators, 12 shared loads per 32 MMAs.  Both
+ * operands are row panels of X, so A (row-major) and B (col-major) fragments are read with
+ * the same pattern; diagonal tiles load the panel once; warp tiles outside the matrix or
+ * strictly above the diagonal issue no MMAs.
  * Splits: work item = (lower tile, split) with its own partial accumulator Kpart[split],
  * read-modify-written by exactly one CTA per launch => deterministic, no atomics.
  */
@@ -29,34 +31,36 @@ struct PackDesc {
     int col0[4];
 };
 
-__global__ void k0_pack_c_kernel(PackDesc pd, int64_t nao, int64_t ldc, double *__restrict__ Ccat)
+/* Ccat4[(mu/4)][c][mu%4], mu < nao16 (rows >= nao and padding columns are zero) */
+__global__ void k0_pack_c_kernel(PackDesc pd, int64_t nao, int64_t nao16, int64_t ldc,
+                                 double *__restrict__ Ccat4)
 {
     const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (idx >= nao * ldc) return;
+    if (idx >= nao16 * ldc) return;
     const int64_t mu = idx / ldc;
     const int c = (int)(idx % ldc);
     double v = 0.0;
-    for (int s = 0; s < pd.nset; ++s)
-        if (c >= pd.col0[s] && c < pd.col0[s] + pd.nocc[s])
-            v = pd.C[s][mu * pd.nocc[s] + (c - pd.col0[s])];
-    Ccat[idx] = v;
+    if (mu < nao)
+        for (int s = 0; s < pd.nset; ++s)
+            if (c >= pd.col0[s] && c < pd.col0[s] + pd.nocc[s])
+                v = pd.C[s][mu * pd.nocc[s] + (c - pd.col0[s])];
+    Ccat4[((mu >> 2) * ldc + c) * 4 + (mu & 3)] = v;
 }
 
 /* ------------------------------------------------------------------ K2 */
 constexpr int K2_T = 128;
-constexpr int K2_KC = 16;
-constexpr int K2_LD = 20;                   /* == 4 mod 16 */
-constexpr int K2_STAGES = 4;
-constexpr int K2_PANEL = K2_T * K2_LD;      /* doubles per operand per stage */
-constexpr int K2_THREADS = 256;
-constexpr int K2_SMEM_BYTES = K2_STAGES * 2 * K2_PANEL * 8;   /* 163840 */
+constexpr int K2_STAGES = 6;
+constexpr int K2_OP_BYTES = 4 * K2_T * 32;            /* one operand, one stage: [4 kg][128][4] */
+constexpr int K2_STAGE_BYTES = 2 * K2_OP_BYTES;       /* 32768 */
+constexpr int K2_CONSUMER_WARPS = 8;
+constexpr int K2_THREADS = 32 * (1 + K2_CONSUMER_WARPS);
+constexpr int K2_SMEM_BYTES = K2_STAGES * K2_STAGE_BYTES + 2 * K2_STAGES * 8 + 16;
 
 __global__ void __launch_bounds__(K2_THREADS, 1)
-k2_syrk_lower_kernel(const double *__restrict__ X, int64_t xpitch, int64_t nao, int64_t np,
-                     int64_t ldc, int64_t col0, int n8s, double *__restrict__ Kpart, int nsplit,
-                     int accumulate)
+k2_syrk_lower_kernel(const double *__restrict__ X4, int64_t nao, int64_t np, int64_t ldc4,
+                     int64_t col04, int n4s, double *__restrict__ Kpart, int nsplit, int accumulate)
 {
-    extern __shared__ __align__(16) double smem[];
+    extern __shared__ __align__(128) unsigned char smem_raw[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     /* lower-triangle tile index -> (bi, bj), bi >= bj */
     const int t = blockIdx.x;
@@ -68,69 +72,96 @@ k2_syrk_lower_kernel(const double *__restrict__ X, int64_t xpitch, int64_t nao, 
     const int split = blockIdx.y;
     const int64_t mu0 = (int64_t)bi * K2_T, nu0 = (int64_t)bj * K2_T;
 
-    /* this split's share of the k groups (8 columns each) */
-    const int64_t ng = np * n8s;
+    /* this split's share of the k groups (4 columns each) of the set */
+    const int64_t ng = np * n4s;
     const int64_t gbeg = ng * split / nsplit, gend = ng * (split + 1) / nsplit;
-    const int nk = (int)((gend - gbeg + 1) / 2);
+    const int nk = (int)((gend - gbeg + 3) / 4);
 
-    auto issue = [&](int kc, int slot) {
-        double *Xa = smem + slot * 2 * K2_PANEL;
-        double *Xb = Xa + K2_PANEL;
-        /* per operand: 128 rows x 2 groups x 4 pieces of 16 B = 1024 pieces */
-        const int npieces = diag ? 1024 : 2048;
-        for (int e = tid; e < npieces; e += K2_THREADS) {
-            const int op = e >> 10;
-            const int r = (e >> 3) & 127, q = e & 7;      /* q: piece within the 16-double row */
-            const int64_t g = gbeg + 2 * (int64_t)kc + (q >> 2);
-            const int64_t row = (op ? nu0 : mu0) + r;
-            const bool ok = g < gend && row < nao;
-            const int64_t pp = g / n8s, j = g % n8s;
-            const double *src = X + row * xpitch + pp * ldc + col0 + 8 * j + 2 * (q & 3);
-            cp_async16(smem_u32((op ? Xb : Xa) + r * K2_LD + 2 * q), ok ? src : X, ok);
+    const uint32_t smem_base = smem_u32(smem_raw);
+    const uint32_t bar_base = smem_base + K2_STAGES * K2_STAGE_BYTES;
+    auto full_bar = [&](int s) { return bar_base + 8u * s; };
+    auto empty_bar = [&](int s) { return bar_base + 8u * (K2_STAGES + s); };
+    if (tid == 0) {
+        for (int s = 0; s < K2_STAGES; ++s) {
+            mbar_init(full_bar(s), 1);
+            mbar_init(empty_bar(s), K2_CONSUMER_WARPS);
         }
-    };
+        mbar_fence_init();
+    }
+    __syncthreads();
 
+    if (warp == 0) {
+        /* ------------------------------------------------------------ producer (one lane) */
+        if (lane == 0) {
+            const int64_t rows_a = (nao - mu0 < K2_T) ? nao - mu0 : K2_T;
+            const int64_t rows_b = (nao - nu0 < K2_T) ? nao - nu0 : K2_T;
+            for (int kc = 0; kc < nk; ++kc) {
+                const int slot = kc % K2_STAGES;
+                const int round = kc / K2_STAGES;
+                if (round > 0) mbar_wait(empty_bar(slot), (round - 1) & 1);
+                const int64_t g0 = gbeg + 4 * (int64_t)kc;
+                const int n = (int)((gend - g0 < 4) ? gend - g0 : 4);
+                const uint32_t bytes = (uint32_t)(n * 32 * (rows_a + (diag ? 0 : rows_b)));
+                mbar_arrive_expect_tx(full_bar(slot), bytes);
+                const uint32_t dst = smem_base + slot * K2_STAGE_BYTES;
+                for (int q = 0; q < n; ++q) {
+                    const int64_t g = g0 + q;
+                    const int64_t kg = (g / n4s) * ldc4 + col04 + g % n4s;     /* k-group in X4 */
+                    const double *src = X4 + kg * nao * 4;
+                    bulk_g2s(dst + q * (K2_T * 32), src + mu0 * 4, (uint32_t)(rows_a * 32), full_bar(slot));
+                    if (!diag)
+                        bulk_g2s(dst + K2_OP_BYTES + q * (K2_T * 32), src + nu0 * 4,
+                                 (uint32_t)(rows_b * 32), full_bar(slot));
+                }
+            }
+        }
+        return;
+    }
+
+    /* ---------------------------------------------------------------- consumers */
+    const int cw = warp - 1;
+    const int wm = cw >> 2, wn = cw & 3;         /* warp tile: rows 64*wm.., cols 32*wn.. */
+    const int lq = lane >> 2, lr = lane & 3;
+    /* skip warp tiles that lie outside the matrix or strictly above the diagonal */
+    const bool warp_active = (mu0 + 64 * wm < nao) && (nu0 + 32 * wn < nao) &&
+                             !(diag && 32 * wn > 64 * wm + 63);
     double acc[8][4][2];
 #pragma unroll
     for (int mt = 0; mt < 8; ++mt)
 #pragma unroll
         for (int nt = 0; nt < 4; ++nt) acc[mt][nt][0] = acc[mt][nt][1] = 0.0;
 
-    const int wm = warp >> 2, wn = warp & 3;     /* warp tile: rows 64*wm.., cols 32*wn.. */
-    const int lq = lane >> 2, lr = lane & 3;
-
-#pragma unroll
-    for (int s = 0; s < K2_STAGES - 1; ++s) {
-        if (s < nk) issue(s, s);
-        cp_async_commit();
-    }
     for (int kc = 0; kc < nk; ++kc) {
-        cp_async_wait<K2_STAGES - 2>();
-        __syncthreads();
-        {
-            const int nxt = kc + K2_STAGES - 1;
-            if (nxt < nk) issue(nxt, nxt % K2_STAGES);
-            cp_async_commit();
+        const int slot = kc % K2_STAGES;
+        mbar_wait(full_bar(slot), (kc / K2_STAGES) & 1);
+        if (warp_active) {
+            const int64_t g0 = gbeg + 4 * (int64_t)kc;
+            const int n = (int)((gend - g0 < 4) ? gend - g0 : 4);
+            const double *Xa = reinterpret_cast<const double *>(smem_raw + slot * K2_STAGE_BYTES);
+            const double *Xb = diag ? Xa : Xa + K2_OP_BYTES / 8;
+            const double *a_base = Xa + (64 * wm + lq) * 4 + lr;
+            const double *b_base = Xb + (32 * wn + lq) * 4 + lr;
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                if (q < n) {
+                    double a[8], b[4];
+#pragma unroll
+                    for (int mt = 0; mt < 8; ++mt) a[mt] = a_base[q * (K2_T * 4) + mt * 32];
+#pragma unroll
+                    for (int nt = 0; nt < 4; ++nt) b[nt] = b_base[q * (K2_T * 4) + nt * 32];
+#pragma unroll
+                    for (int mt = 0; mt < 8; ++mt)
+#pragma unroll
+                        for (int nt = 0; nt < 4; ++nt)
+                            dmma884(acc[mt][nt][0], acc[mt][nt][1], a[mt], b[nt]);
+                }
+            }
         }
-        const double *Xa = smem + (kc % K2_STAGES) * 2 * K2_PANEL;
-        const double *Xb = diag ? Xa : Xa + K2_PANEL;
-        const double *a_base = Xa + (64 * wm + lq) * K2_LD + lr;
-        const double *b_base = Xb + (32 * wn + lq) * K2_LD + lr;
-#pragma unroll
-        for (int k4 = 0; k4 < K2_KC / 4; ++k4) {
-            double a[8], b[4];
-#pragma unroll
-            for (int mt = 0; mt < 8; ++mt) a[mt] = a_base[mt * 8 * K2_LD + 4 * k4];
-#pragma unroll
-            for (int nt = 0; nt < 4; ++nt) b[nt] = b_base[nt * 8 * K2_LD + 4 * k4];
-#pragma unroll
-            for (int mt = 0; mt < 8; ++mt)
-#pragma unroll
-                for (int nt = 0; nt < 4; ++nt) dmma884(acc[mt][nt][0], acc[mt][nt][1], a[mt], b[nt]);
-        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(empty_bar(slot));
     }
-    cp_async_wait<0>();
 
+    if (!warp_active) return;
     double *Kp = Kpart + (int64_t)split * nao * nao;
 #pragma unroll
     for (int mt = 0; mt < 8; ++mt) {
@@ -191,13 +222,13 @@ void launch_k0_pack_c(const double *const *C, const int *nocc, const int *col0, 
         pd.nocc[s] = s < nset ? nocc[s] : 0;
         pd.col0[s] = s < nset ? col0[s] : 0;
     }
-    const int64_t n = nao * ldc;
-    k0_pack_c_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(pd, nao, ldc, Ccat);
+    const int64_t nao16 = (nao + 15) / 16 * 16;
+    const int64_t n = nao16 * ldc;
+    k0_pack_c_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(pd, nao, nao16, ldc, Ccat);
 }
 
-void launch_k2_syrk_lower(const double *X, int64_t xpitch, int64_t nao, int64_t np, int64_t ldc,
-                          int64_t col0, int64_t ncol, double *Kpart, int nsplit, int accumulate,
-                          cudaStream_t st)
+void launch_k2_syrk_lower(const double *X4, int64_t nao, int64_t np, int64_t ldc, int64_t col0,
+                          int64_t ncol, double *Kpart, int nsplit, int accumulate, cudaStream_t st)
 {
     static bool configured = false;
     if (!configured) {
@@ -207,9 +238,9 @@ void launch_k2_syrk_lower(const double *X, int64_t xpitch, int64_t nao, int64_t 
     }
     const int nb = (int)((nao + K2_T - 1) / K2_T);
     const int ntile = nb * (nb + 1) / 2;
-    const int n8s = (int)((ncol + 7) / 8);
+    const int n4s = 2 * (int)((ncol + 7) / 8);          /* sets are padded to multiples of 8 columns */
     k2_syrk_lower_kernel<<<dim3((unsigned)ntile, (unsigned)nsplit), K2_THREADS, K2_SMEM_BYTES, st>>>(
-        X, xpitch, nao, np, ldc, col0, n8s, Kpart, nsplit, accumulate);
+        X4, nao, np, ldc / 4, col0 / 4, n4s, Kpart, nsplit, accumulate);
 }
 
 void launch_k3_finish(const double *Kpart, int nsplit, int64_t nao, double *K, cudaStream_t st)
