@@ -45,7 +45,7 @@ struct dfjk_handle {
     int device, sm_count;
     int64_t l2_bytes;
     /* workspace (device) */
-    double *Ccat;        /* nao16 x ldc_max, k-group-major */
+    double *Ccat;        /* round_up(nao,32) x ldc_max, k-group-major */
     int64_t ldc_max;
     double *Dt;          /* npair */
     double *d_part;      /* nchunk x naux */
@@ -54,7 +54,7 @@ struct dfjk_handle {
     double *X;           /* x_doubles */
     double *Kpart;       /* 2 x nsplit_alloc x nao x nao */
     int64_t nchunk, j2_groups, x_doubles;
-    int nsplit_alloc;
+    int nsplit_alloc, nsplit_default;
     int64_t ws_bytes;
     /* options */
     int64_t opt_k_chunk, opt_k_splits, opt_j_fused;
@@ -158,15 +158,16 @@ extern "C" dfjk_handle *dfjk_create(int64_t naux, int64_t nao, const double *B_p
     h->nchunk = dfjk::j1_num_chunks(h->npair);
     h->j2_groups = dfjk::j2_num_groups(naux, h->npair, h->sm_count);
     /* X chunk: ~96 MB (three quarters of L2), but at least two rows at the widest ldc */
-    int64_t xd = (96LL << 20) / 8;
+    int64_t xd = (512LL << 20) / 8;
     if (xd < 2 * nao * h->ldc_max) xd = 2 * nao * h->ldc_max;
     if (xd > naux * nao * h->ldc_max) xd = naux * nao * h->ldc_max;
     h->x_doubles = xd;
     const int nb = (int)((nao + 127) / 128);
-    h->nsplit_alloc = choose_splits(nb * (nb + 1) / 2, h->sm_count, 16);
+    h->nsplit_default = choose_splits(nb * (nb + 1) / 2, h->sm_count, 16);
+    h->nsplit_alloc = 32;
 
     int rc = DFJK_OK;
-    if (rc == DFJK_OK) rc = alloc_ws(h, &h->Ccat, round_up(nao, 16) * h->ldc_max);
+    if (rc == DFJK_OK) rc = alloc_ws(h, &h->Ccat, round_up(nao, 32) * h->ldc_max);
     if (rc == DFJK_OK) rc = alloc_ws(h, &h->Dt, h->npair);
     if (rc == DFJK_OK) rc = alloc_ws(h, &h->d_part, h->nchunk * naux);
     if (rc == DFJK_OK) rc = alloc_ws(h, &h->d, naux);
@@ -260,7 +261,7 @@ int get_jk_impl(dfjk_handle *h, int nset, const double *const *C, const int64_t 
         if (h->opt_k_chunk > 0 && h->opt_k_chunk < pc) pc = h->opt_k_chunk;
         if (pc > naux) pc = naux;
         if (pc < 1) return fail(DFJK_ENOMEM, "%s: X workspace too small", who);
-        const int nsplit = h->opt_k_splits > 0 ? (int)h->opt_k_splits : h->nsplit_alloc;
+        const int nsplit = h->opt_k_splits > 0 ? (int)h->opt_k_splits : h->nsplit_default;
         int chunk = 0;
         for (int64_t P0 = 0; P0 < naux; P0 += pc, ++chunk) {
             const int64_t np = (P0 + pc <= naux) ? pc : naux - P0;

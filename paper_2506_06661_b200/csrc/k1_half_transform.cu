@@ -5,7 +5,7 @@
  *
  * One CTA computes a 128 x NW tile of X_P for one auxiliary index P (NW = 8*NT8 <= 136
  * columns of the concatenated, zero-padded orbital block), marching over nu in stages of
- * 16.  Warp-specialised, mbarrier-pipelined (no __syncthreads in the main loop):
+ * 32.  Warp-specialised, mbarrier-pipelined (no __syncthreads in the main loop):
  *
  *   producer warpgroup (4 warps, 40 registers after setmaxnreg.dec)
  *     - A tile: the packed triangle is unpacked while staging.  Every element (mu,nu) is
@@ -34,7 +34,8 @@ namespace dfjk {
 namespace {
 
 constexpr int K1_M = 128;
-constexpr int K1_KC = 16;
+constexpr int K1_KG = 8;                          /* k-groups (of 4) per stage */
+constexpr int K1_KC = 4 * K1_KG;
 constexpr int K1_PRODUCERS = 128;                 /* one warpgroup */
 constexpr int K1_CONSUMERS = 256;                 /* two warpgroups */
 constexpr int K1_THREADS = K1_PRODUCERS + K1_CONSUMERS;
@@ -85,36 +86,40 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t nao, int64_t npai
         /* ------------------------------------------------------------ producers */
         reg_dealloc<40>();
         const double *__restrict__ Bp = B + (P0 + p) * npair;
-        const int pw = warp;                               /* k-group within the stage */
-        const int kk = 4 * pw + (lane & 3);
+        const int pw = warp;                               /* k-groups pw, pw+4, .. of the stage */
         const int mrow = lane >> 2;
         int64_t ncols = ldc - n0;                          /* valid columns of this N tile */
         if (ncols > Cfg::NW) ncols = Cfg::NW;
         const uint32_t c_bytes_g = (uint32_t)ncols * 32u;  /* per k-group */
+        int slot = 0;
+        uint32_t phase = 1;                                /* parity of the "empty" phase to wait for */
         for (int kc = 0; kc < nk; ++kc) {
-            const int slot = kc % Cfg::STAGES;
-            const int round = kc / Cfg::STAGES;
-            if (round > 0) mbar_wait(empty_bar(slot), (round - 1) & 1);
-            const uint32_t a_dst = smem_base + slot * Cfg::STAGE_BYTES + pw * 4096 + lane * 8;
-            const int64_t nu = (int64_t)kc * K1_KC + kk;
-            const bool nu_ok = nu < nao;
-            const int64_t tri_nu = nu * (nu + 1) / 2;
-#pragma unroll 4
-            for (int r = 0; r < 16; ++r) {
-                const int64_t mu = mu0 + 8 * r + mrow;
-                const bool ok = nu_ok && mu < nao;
-                const int64_t off = mu >= nu ? mu * (mu + 1) / 2 + nu : tri_nu + mu;
-                cp_async8(a_dst + r * 256, ok ? Bp + off : Bp, ok);
-            }
+            if (kc >= Cfg::STAGES) mbar_wait(empty_bar(slot), phase);
             if (tid == 0) {
                 const uint32_t c_dst = smem_base + slot * Cfg::STAGE_BYTES + K1_A_BYTES;
-                mbar_arrive_expect_tx(full_bar(slot), 4 * c_bytes_g);
+                mbar_arrive_expect_tx(full_bar(slot), K1_KG * c_bytes_g);
 #pragma unroll
-                for (int g = 0; g < 4; ++g)
-                    bulk_g2s(c_dst + g * Cfg::NW * 32, Ccat4 + (((int64_t)kc * 4 + g) * ldc + n0) * 4,
+                for (int g = 0; g < K1_KG; ++g)
+                    bulk_g2s(c_dst + g * Cfg::NW * 32, Ccat4 + (((int64_t)kc * K1_KG + g) * ldc + n0) * 4,
                              c_bytes_g, full_bar(slot));
             }
+#pragma unroll
+            for (int gg = 0; gg < K1_KG / 4; ++gg) {
+                const int g = pw + 4 * gg;
+                const uint32_t a_dst = smem_base + slot * Cfg::STAGE_BYTES + g * 4096 + lane * 8;
+                const int64_t nu = (int64_t)kc * K1_KC + 4 * g + (lane & 3);
+                const bool nu_ok = nu < nao;
+                const int64_t tri_nu = nu * (nu + 1) / 2;
+#pragma unroll 4
+                for (int r = 0; r < 16; ++r) {
+                    const int64_t mu = mu0 + 8 * r + mrow;
+                    const bool ok = nu_ok && mu < nao;
+                    const int64_t off = mu >= nu ? mu * (mu + 1) / 2 + nu : tri_nu + mu;
+                    cp_async8(a_dst + r * 256, ok ? Bp + off : Bp, ok);
+                }
+            }
             cp_async_mbar_arrive_noinc(full_bar(slot));
+            if (++slot == Cfg::STAGES) { slot = 0; phase ^= 1; }
         }
     } else {
         /* ------------------------------------------------------------ consumers */
@@ -128,16 +133,17 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t nao, int64_t npai
 #pragma unroll
             for (int nt = 0; nt < NT8; ++nt) acc[mt][nt][0] = acc[mt][nt][1] = 0.0;
 
+        int slot = 0;
+        uint32_t phase = 0;
         for (int kc = 0; kc < nk; ++kc) {
-            const int slot = kc % Cfg::STAGES;
-            mbar_wait(full_bar(slot), (kc / Cfg::STAGES) & 1);
+            mbar_wait(full_bar(slot), phase);
             if (warp_active) {
                 const double *As = reinterpret_cast<const double *>(smem_raw + slot * Cfg::STAGE_BYTES);
                 const double *Cs = As + K1_A_BYTES / 8;
                 const double *a_base = As + (16 * cw + lq) * 4 + lr;
                 const double *b_base = Cs + lq * 4 + lr;
 #pragma unroll
-                for (int g = 0; g < 4; ++g) {
+                for (int g = 0; g < K1_KG; ++g) {
                     const double a0 = a_base[g * (K1_M * 4)];
                     const double a1 = a_base[g * (K1_M * 4) + 32];
 #pragma unroll
@@ -150,6 +156,7 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t nao, int64_t npai
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(empty_bar(slot));
+            if (++slot == Cfg::STAGES) { slot = 0; phase ^= 1; }
         }
 
         if (warp_active) {

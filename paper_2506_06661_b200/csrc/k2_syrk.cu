@@ -222,7 +222,7 @@ void launch_k0_pack_c(const double *const *C, const int *nocc, const int *col0, 
         pd.nocc[s] = s < nset ? nocc[s] : 0;
         pd.col0[s] = s < nset ? col0[s] : 0;
     }
-    const int64_t nao16 = (nao + 15) / 16 * 16;
+    const int64_t nao16 = (nao + 31) / 32 * 32;   /* K1 stages cover 32 rows of C */
     const int64_t n = nao16 * ldc;
     k0_pack_c_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(pd, nao, nao16, ldc, Ccat);
 }
