@@ -185,3 +185,33 @@ class KVAccumulator:
             self.V.ctypes.data, _ptr_array(self.KV))
         if rc != 0:
             raise RuntimeError(f"oracle_kv_slab failed: {rc}")
+
+
+class KBlockAccumulator:
+    """Sampled entries of K_s, one by one from the definition (numpy, FP64).
+
+    For a list of row indices S this accumulates, slab by slab,
+        K_s[a][b] = sum_P sum_i X_P[S_a][i] X_P[S_b][i],   X_P[mu][i] = sum_nu B(P,mu,nu) C_s[nu][i]
+    (the K of the C file header restricted to the |S| x |S| block), with
+    B(P,mu,nu) = Bp[P][max(max+1)/2 + min] unpacked by explicit index arithmetic.  Used for
+    full-size parity (cfg 3-5) where the whole K is too slow on a CPU; pinned against the
+    full oracle K in tests/test_oracle_pins.py.
+    """
+
+    def __init__(self, nao: int, Cs: Sequence[np.ndarray], rows: Sequence[int]):
+        self.nao = int(nao)
+        self.Cs = [_f64c(C) for C in Cs]
+        self.rows = np.asarray(rows, dtype=np.int64)
+        mu = self.rows[:, None]
+        nu = np.arange(self.nao, dtype=np.int64)[None, :]
+        a, b = np.maximum(mu, nu), np.minimum(mu, nu)
+        self.idx = a * (a + 1) // 2 + b                  # [|S|][nao] packed index of B(P, S_a, nu)
+        self.K = [np.zeros((len(self.rows), len(self.rows))) for _ in self.Cs]
+
+    def add_slab(self, Bp_slab: np.ndarray) -> None:
+        Bp_slab = np.asarray(Bp_slab, dtype=np.float64)
+        for P in range(Bp_slab.shape[0]):
+            Bsel = Bp_slab[P][self.idx]                  # [|S|][nao]
+            for s, C in enumerate(self.Cs):
+                X = Bsel @ C                             # [|S|][nocc]
+                self.K[s] += X @ X.T

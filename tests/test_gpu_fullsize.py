@@ -1,0 +1,100 @@
+"""Full-size GPU parity (BASELINE.json configs 3-5), in the launch configuration bench.py times
+(default options, B generated on the device, first call of the config's schedule).
+
+The oracle reads back the SAME bytes the GPU used, in row slabs (B never has to fit host RAM):
+  * cfg 3 (6.7 GB): full J and full K from the oracle, element by element.
+  * cfg 4 (51 GB), cfg 5 (96 GB, unrestricted): full J from the oracle; K by
+      - sampled entries computed one by one from the definition (oracle.KBlockAccumulator):
+        a |S| x |S| block whose rows straddle 128-row tile edges and the ragged tail, and
+      - the matrix-vector identity K v = sum_P B_P C C^T B_P v for seeded random v
+        (oracle.KVAccumulator), which touches every entry of K,
+    plus exact symmetry (both triangles are written from the same lower-tile value).
+Tolerance: relative Frobenius error <= 1e-11 (north_star) on every compared object.
+"""
+import numpy as np
+import pytest
+
+import dfjk_inputs as gi
+import oracle
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-11
+SLAB_BYTES = 1 << 30
+
+
+def relerr(a, b):
+    nb = np.linalg.norm(b)
+    return np.linalg.norm(np.asarray(a) - np.asarray(b)) / (nb if nb > 0 else 1.0)
+
+
+def sample_rows(nao):
+    edge = [0, 1, 63, 64, 127, 128, 129, 255, 256, 511, 512, 1023, 1024, 1151, 1152,
+            1535, 1536, 1599, 1600, 1919, 1920, nao - 2, nao - 1]
+    rng = np.random.default_rng(nao)
+    rows = sorted({r for r in edge if 0 <= r < nao} | set(rng.integers(0, nao, 9).tolist()))
+    return rows
+
+
+def run_config(cfg_id, full_k):
+    import paper_2506_06661_b200 as pkg
+    cfg = gi.CONFIGS[cfg_id]
+    free, _ = torch.cuda.mem_get_info()
+    if free < cfg.b_bytes + (6 << 30):
+        pytest.skip(f"needs {cfg.b_bytes / 1e9:.0f} GB of free device memory")
+    B = torch.empty(cfg.naux, cfg.npair, dtype=torch.float64, device="cuda")
+    gi.fill_B_device(cfg, B)
+    h = pkg.DFJK(B, cfg.nao)
+    Cs = gi.orbitals(cfg, 0)
+    Cd = [torch.from_numpy(C).cuda() for C in Cs]
+    if len(Cs) == 1:
+        J, K0 = h.get_jk(Cd[0])
+        Ks = [K0]
+    else:
+        J, Ka, Kb = h.get_jk_u(Cd[0], Cd[1])
+        Ks = [Ka, Kb]
+    d = h.get_d()
+    torch.cuda.synchronize()
+    J = J.cpu().numpy()
+    Ks = [K.cpu().numpy() for K in Ks]
+    d = d.cpu().numpy()
+
+    rows = sample_rows(cfg.nao)
+    V = np.random.default_rng(cfg.seed).standard_normal((2, cfg.nao))
+    acc = oracle.JKAccumulator(cfg.nao, Cs, cfg.weights, with_j=True, with_k=full_k)
+    kb = oracle.KBlockAccumulator(cfg.nao, Cs, rows)
+    kv = oracle.KVAccumulator(cfg.nao, Cs, V)
+    slab = max(1, SLAB_BYTES // (cfg.npair * 8))
+    for P0 in range(0, cfg.naux, slab):
+        Bh = B[P0:P0 + slab].cpu().numpy()          # the same bytes the kernels read
+        acc.add_slab(Bh)
+        if not full_k:
+            kb.add_slab(Bh)
+            kv.add_slab(Bh)
+    h.close()
+    del B
+    torch.cuda.empty_cache()
+
+    assert relerr(d, acc.d_vector()) <= TOL
+    assert relerr(J, acc.J) <= TOL
+    assert np.array_equal(J, J.T)
+    for s, K in enumerate(Ks):
+        assert np.array_equal(K, K.T)
+        if full_k:
+            assert relerr(K, acc.K[s]) <= TOL
+        else:
+            assert relerr(K[np.ix_(rows, rows)], kb.K[s]) <= TOL
+            assert relerr(V @ K, kv.KV[s]) <= TOL     # K symmetric: rows of V K are (K v)^T
+
+
+def test_cfg3_medium_full_matrices():
+    run_config(3, full_k=True)
+
+
+def test_cfg4_large_headline():
+    run_config(4, full_k=False)
+
+
+def test_cfg5_unrestricted():
+    run_config(5, full_k=False)

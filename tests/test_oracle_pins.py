@@ -288,3 +288,20 @@ def test_argument_validation():
         oracle.get_jk(Bp[:, :-1], 4, Cs, [2.0])
     with pytest.raises(ValueError):
         oracle.get_jk(Bp, 4, [Cs[0][:3]], [2.0])
+
+
+def test_k_block_matches_full_K():
+    """KBlockAccumulator (sampled K entries from the definition) against the full oracle K
+    and against numpy on an independently unpacked B."""
+    cfg = gi.CONFIGS[1]
+    Bp = gi.fill_B_host(cfg)
+    Cs = [gi.random_orbitals(cfg.nao, 5, 3), gi.random_orbitals(cfg.nao, 3, 4, orthonormal=False)]
+    _, K, _ = oracle.get_jk(Bp, cfg.nao, Cs, [1.0, 1.0])
+    rows = [0, 1, 7, 31, 32, 47]
+    kb = oracle.KBlockAccumulator(cfg.nao, Cs, rows)
+    kb.add_slab(Bp[:70]); kb.add_slab(Bp[70:])
+    Bf = unpack_np(Bp, cfg.nao)
+    for s, C in enumerate(Cs):
+        assert relerr(kb.K[s], K[s][np.ix_(rows, rows)]) < 1e-13
+        X = Bf[:, rows, :] @ C
+        assert relerr(kb.K[s], np.einsum("pai,pbi->ab", X, X)) < 1e-13
