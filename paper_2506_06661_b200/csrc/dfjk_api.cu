@@ -265,7 +265,7 @@ int get_jk_impl(dfjk_handle *h, int nset, const double *const *C, const int64_t 
         int chunk = 0;
         for (int64_t P0 = 0; P0 < naux; P0 += pc, ++chunk) {
             const int64_t np = (P0 + pc <= naux) ? pc : naux - P0;
-            { Timed t_(h, DFJK_KERNEL_K1, st); dfjk::launch_k1_half_transform(h->B, nao, npair, P0, np, h->Ccat, ldc, h->X, st); }
+            { Timed t_(h, DFJK_KERNEL_K1, st); dfjk::launch_k1_half_transform(h->B, naux, nao, npair, P0, np, h->Ccat, ldc, h->X, st); }
             for (int s = 0; s < nset; ++s)
                 if (K[s]) {
                     Timed t_(h, DFJK_KERNEL_K2, st);

@@ -50,7 +50,7 @@ void launch_k0_pack_c(const double *const *C, const int *nocc, const int *col0, 
 
 /* K1: for P in [P0, P0+np), k = (P-P0)*ldc + i:
  *   X4[(k/4)*nao*4 + mu*4 + k%4] = sum_nu B_P(mu,nu) Ccat[nu][i]      (k-group-major X) */
-void launch_k1_half_transform(const double *B, int64_t nao, int64_t npair,
+void launch_k1_half_transform(const double *B, int64_t naux, int64_t nao, int64_t npair,
                               int64_t P0, int64_t np, const double *Ccat4, int64_t ldc,
                               double *X4, cudaStream_t st);
 

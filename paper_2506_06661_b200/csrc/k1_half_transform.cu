@@ -8,21 +8,26 @@
  * 32.  Warp-specialised, mbarrier-pipelined (no __syncthreads in the main loop):
  *
  *   producer warpgroup (4 warps, 40 registers after setmaxnreg.dec)
- *     - A tile: the packed triangle is unpacked while staging.  Every element (mu,nu) is
- *       fetched from Bp[max(max+1)/2+min] by an 8-byte cp.async (packed rows are only
- *       8-byte aligned), so tiles left of the diagonal read packed rows, tiles right of
- *       it read the transposed packed tile, and the diagonal tile mixes both; each
- *       thread's copies signal the stage's "full" mbarrier on completion
- *       (cp.async.mbarrier.arrive.noinc).  Every packed element is read twice per call
- *       (K1 is compute-bound: ~65 flop per byte of B).
- *     - C tile: Ccat is kept k-group-major ([nu/4][ldc][4]), so the 4 x NW x 4 tile of a
- *       stage is four contiguous 1-D bulk copies (TMA engine, cp.async.bulk -> UBLKCP)
- *       completing on the same mbarrier.
+ *     - A tile: the packed triangle is unpacked while staging, by the TMA engine.  A stage
+ *       left of the diagonal is 128 row copies of 32 doubles (packed rows mu, "row" form);
+ *       a stage right of it is 32 row copies of 128 doubles (packed rows nu, i.e. the
+ *       transposed tile, "col" form); each is one 1-D bulk copy (cp.async.bulk -> UBLKCP)
+ *       issued by one producer thread.  Packed rows are only 8-byte aligned: a copy whose
+ *       source index is odd starts one element early and the consumer reads that row with
+ *       a +1 column shift, which is a per-lane constant (see K1_LDD/K1_LDT).  Only the
+ *       stages that cross the diagonal (4 of 50 at nao=1600) gather element-wise with
+ *       8-byte cp.async (max/min addressing, zero fill).  An earlier version gathered every
+ *       stage with cp.async: the 4096 LDGSTS per stage cost 7 % of K1 through the LSU.
+ *       Every packed element is read twice per call (K1 is compute-bound: ~65 flop/B).
+ *     - C tile: Ccat is kept k-group-major ([nu/4][ldc][4]), so the 8 x NW x 4 tile of a
+ *       stage is eight contiguous bulk copies completing on the same mbarrier.
  *   two consumer warpgroups (8 warps, 232 registers after setmaxnreg.inc)
  *     - each warp owns 16 rows x NW columns = 2 x NT8 DMMA.8x8x4 accumulator tiles;
- *       one k4 step costs 2+NT8 shared loads for 2*NT8 MMAs.  Tiles are stored dense as
- *       [k/4][row][4] doubles: the 16 lanes of each 64-bit half-warp phase read 16
- *       consecutive doubles => conflict-free with no padding.
+ *       one k4 step costs 2+NT8 shared loads for 2*NT8 MMAs.  The C tile and X are stored
+ *       dense as [k/4][row][4] doubles: the 16 lanes of each 64-bit half-warp phase read
+ *       16 consecutive doubles => conflict-free with no padding; the A tile pitches (36,
+ *       132 doubles) are == 4 mod 16 for the same reason (one 2-way conflict per phase
+ *       remains from the alignment shift).
  *
  * Output: X in k-group-major layout X4[(p*ldc + i)/4][mu][(p*ldc + i)%4], which makes
  * every K2 operand tile a contiguous 4 KB bulk copy.
@@ -39,8 +44,33 @@ constexpr int K1_KC = 4 * K1_KG;
 constexpr int K1_PRODUCERS = 128;                 /* one warpgroup */
 constexpr int K1_CONSUMERS = 256;                 /* two warpgroups */
 constexpr int K1_THREADS = K1_PRODUCERS + K1_CONSUMERS;
-constexpr int K1_A_BYTES = K1_M * K1_KC * 8;      /* 16384 */
+/* A tile of a stage, one of two shapes (both reached by plain row copies of the packed triangle):
+ *   "row" form   [m][K1_LDD]: row m holds B_P(mu0+m, nu0 .. nu0+31) at column k + sd(m)
+ *   "col" form   [k][K1_LDT]: row k holds B_P(mu0 .. mu0+127, nu0+k) = packed(nu0+k, mu0 ..) at column m + st(k)
+ * sd/st in {0,1} is the parity of the source element's index in B: a packed row starts on an
+ * 8-byte, not a 16-byte boundary, so the bulk copy starts one element early when that index is
+ * odd and the data lands shifted by one.  mu0 is a multiple of 128 and nu0 of 32, so the shift
+ * pattern is (0,1,1,0) in (row mod 4) xor the parity of P*npair: a per-lane constant. */
+constexpr int K1_LDD = 36;                        /* 32 + shift + pad, 16-B multiple */
+constexpr int K1_LDT = 132;                       /* 128 + shift + pad, 16-B multiple */
+constexpr int K1_A_BYTES = K1_M * K1_LDD * 8;     /* 36864 >= 32 * K1_LDT * 8 = 33792 */
 constexpr int K1_SMEM_BUDGET = 220 * 1024;
+
+enum { K1_MODE_ROW = 0, K1_MODE_COL = 1, K1_MODE_GATHER = 2 };
+
+/* which form stage kc of row block mu0 takes; identical on producer and consumer side */
+__device__ __forceinline__ int k1_mode(int64_t mu0, int64_t nu0, int64_t nao, bool last_p)
+{
+    if (nu0 + K1_KC - 1 <= mu0) return K1_MODE_ROW;            /* every nu <= every mu */
+    if (nu0 >= mu0 + K1_M - 1 && !(last_p && nu0 + K1_KC >= nao))
+        return K1_MODE_COL;                                    /* every nu >= every mu */
+    return K1_MODE_GATHER;    /* crosses the diagonal (or would read past the end of B) */
+}
+
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.expect_tx.relaxed.cta.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
 
 template <int NT8>
 struct K1Cfg {
@@ -54,7 +84,7 @@ struct K1Cfg {
 
 template <int NT8>
 __global__ void __launch_bounds__(K1_THREADS, 1)
-k1_half_transform_kernel(const double *__restrict__ B, int64_t nao, int64_t npair, int64_t P0,
+k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao, int64_t npair, int64_t P0,
                          const double *__restrict__ Ccat4, int64_t ldc, int ntiles_n,
                          double *__restrict__ X4)
 {
@@ -67,6 +97,9 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t nao, int64_t npai
     const int64_t mu0 = (int64_t)ib * K1_M;
     const int64_t n0 = (int64_t)nt_idx * Cfg::NW;
     const int nk = (int)((nao + K1_KC - 1) / K1_KC);
+    const int64_t pb = (P0 + p) * npair;               /* index of B_P's first element in B */
+    const int pbpar = (int)(pb & 1);
+    const bool last_p = P0 + p == naux - 1;
 
     const uint32_t smem_base = smem_u32(smem_raw);
     const uint32_t bar_base = smem_base + Cfg::STAGES * Cfg::STAGE_BYTES;
@@ -75,7 +108,7 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t nao, int64_t npai
 
     if (tid == 0) {
         for (int s = 0; s < Cfg::STAGES; ++s) {
-            mbar_init(full_bar(s), K1_PRODUCERS + 1);
+            mbar_init(full_bar(s), K1_PRODUCERS);
             mbar_init(empty_bar(s), K1_CONSUMERS / 32);
         }
         mbar_fence_init();
@@ -85,40 +118,69 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t nao, int64_t npai
     if (warp < K1_PRODUCERS / 32) {
         /* ------------------------------------------------------------ producers */
         reg_dealloc<40>();
-        const double *__restrict__ Bp = B + (P0 + p) * npair;
-        const int pw = warp;                               /* k-groups pw, pw+4, .. of the stage */
-        const int mrow = lane >> 2;
+        const double *__restrict__ Bp = B + pb;
         int64_t ncols = ldc - n0;                          /* valid columns of this N tile */
         if (ncols > Cfg::NW) ncols = Cfg::NW;
-        const uint32_t c_bytes_g = (uint32_t)ncols * 32u;  /* per k-group */
+        const uint32_t c_bytes = K1_KG * (uint32_t)ncols * 32u;
+        int64_t rows_valid = nao - mu0;
+        if (rows_valid > K1_M) rows_valid = K1_M;
         int slot = 0;
         uint32_t phase = 1;                                /* parity of the "empty" phase to wait for */
         for (int kc = 0; kc < nk; ++kc) {
             if (kc >= Cfg::STAGES) mbar_wait(empty_bar(slot), phase);
+            const int64_t nu0 = (int64_t)kc * K1_KC;
+            const uint32_t a_dst = smem_base + slot * Cfg::STAGE_BYTES;
+            const uint32_t bar = full_bar(slot);
+            const int mode = k1_mode(mu0, nu0, nao, last_p);
+            uint32_t my_bytes = tid == 0 ? c_bytes : 0u;
+            if (mode == K1_MODE_ROW) {
+                /* thread t copies packed row mu0+t, columns nu0 .. nu0+31 (+ alignment slack) */
+                const int64_t mu = mu0 + tid;
+                const bool ok = mu < nao;
+                const int64_t e = pb + mu * (mu + 1) / 2 + nu0;
+                const int sft = (int)(e & 1);
+                const uint32_t nb = ok ? (uint32_t)(K1_KC + 2 * sft) * 8u : 0u;
+                my_bytes += nb;
+                if (my_bytes) mbar_arrive_expect_tx(bar, my_bytes); else mbar_arrive(bar);
+                if (ok) bulk_g2s(a_dst + tid * (K1_LDD * 8), B + (e - sft), nb, bar);
+            } else if (mode == K1_MODE_COL) {
+                /* thread t < 32 copies packed row nu0+t, columns mu0 .. mu0+rows_valid-1 */
+                const int64_t nu = nu0 + tid;
+                const bool ok = tid < K1_KC && nu < nao;
+                const int64_t e = pb + nu * (nu + 1) / 2 + mu0;
+                const int sft = (int)(e & 1);
+                const uint32_t nb = ok ? (uint32_t)((rows_valid + sft + 1) & ~(int64_t)1) * 8u : 0u;
+                my_bytes += nb;
+                /* rows nu >= nao of the tile multiply zero rows of C: they must not hold NaNs */
+                for (int k = (int)(nao - nu0); k < K1_KC; ++k)
+                    for (int c = tid; c < K1_LDT; c += K1_PRODUCERS)
+                        reinterpret_cast<double *>(smem_raw + slot * Cfg::STAGE_BYTES)[k * K1_LDT + c] = 0.0;
+                if (my_bytes) mbar_arrive_expect_tx(bar, my_bytes); else mbar_arrive(bar);
+                if (ok) bulk_g2s(a_dst + tid * (K1_LDT * 8), B + (e - sft), nb, bar);
+            } else {
+                /* element-wise gather into the "row" form (8-byte cp.async, zero fill outside) */
+                if (tid == 0) mbar_expect_tx(bar, c_bytes);
+                const int k = tid & 31;
+                const int64_t nu = nu0 + k;
+                const int64_t tri_nu = nu * (nu + 1) / 2;
+#pragma unroll 4
+                for (int r = 0; r < K1_M / 4; ++r) {
+                    const int m = 4 * r + (tid >> 5);
+                    const int64_t mu = mu0 + m;
+                    const bool ok = nu < nao && mu < nao;
+                    const int64_t off = mu >= nu ? mu * (mu + 1) / 2 + nu : tri_nu + mu;
+                    const int sd = (((m & 3) == 1 || (m & 3) == 2) ? 1 : 0) ^ pbpar;
+                    cp_async8(a_dst + (m * K1_LDD + k + sd) * 8, ok ? Bp + off : Bp, ok);
+                }
+                cp_async_mbar_arrive_noinc(bar);
+            }
             if (tid == 0) {
-                const uint32_t c_dst = smem_base + slot * Cfg::STAGE_BYTES + K1_A_BYTES;
-                mbar_arrive_expect_tx(full_bar(slot), K1_KG * c_bytes_g);
+                const uint32_t c_dst = a_dst + K1_A_BYTES;
 #pragma unroll
                 for (int g = 0; g < K1_KG; ++g)
                     bulk_g2s(c_dst + g * Cfg::NW * 32, Ccat4 + (((int64_t)kc * K1_KG + g) * ldc + n0) * 4,
-                             c_bytes_g, full_bar(slot));
+                             (uint32_t)ncols * 32u, bar);
             }
-#pragma unroll
-            for (int gg = 0; gg < K1_KG / 4; ++gg) {
-                const int g = pw + 4 * gg;
-                const uint32_t a_dst = smem_base + slot * Cfg::STAGE_BYTES + g * 4096 + lane * 8;
-                const int64_t nu = (int64_t)kc * K1_KC + 4 * g + (lane & 3);
-                const bool nu_ok = nu < nao;
-                const int64_t tri_nu = nu * (nu + 1) / 2;
-#pragma unroll 4
-                for (int r = 0; r < 16; ++r) {
-                    const int64_t mu = mu0 + 8 * r + mrow;
-                    const bool ok = nu_ok && mu < nao;
-                    const int64_t off = mu >= nu ? mu * (mu + 1) / 2 + nu : tri_nu + mu;
-                    cp_async8(a_dst + r * 256, ok ? Bp + off : Bp, ok);
-                }
-            }
-            cp_async_mbar_arrive_noinc(full_bar(slot));
             if (++slot == Cfg::STAGES) { slot = 0; phase ^= 1; }
         }
     } else {
@@ -127,6 +189,9 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t nao, int64_t npai
         const int cw = warp - K1_PRODUCERS / 32;           /* 0..7: rows 16*cw .. 16*cw+15 */
         const int lq = lane >> 2, lr = lane & 3;
         const bool warp_active = mu0 + 16 * cw < nao;
+        /* per-lane alignment shifts of the two tile forms (see K1_LDD / K1_LDT) */
+        const int sd_shift = (((lq & 3) == 1 || (lq & 3) == 2) ? 1 : 0) ^ pbpar;
+        const int st_shift = ((lr == 1 || lr == 2) ? 1 : 0) ^ pbpar;
         double acc[2][NT8][2];
 #pragma unroll
         for (int mt = 0; mt < 2; ++mt)
@@ -140,12 +205,16 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t nao, int64_t npai
             if (warp_active) {
                 const double *As = reinterpret_cast<const double *>(smem_raw + slot * Cfg::STAGE_BYTES);
                 const double *Cs = As + K1_A_BYTES / 8;
-                const double *a_base = As + (16 * cw + lq) * 4 + lr;
+                const bool colform = k1_mode(mu0, (int64_t)kc * K1_KC, nao, last_p) == K1_MODE_COL;
+                const double *a_base = colform ? As + lr * K1_LDT + 16 * cw + lq + st_shift
+                                               : As + (16 * cw + lq) * K1_LDD + lr + sd_shift;
+                const int a_gstep = colform ? 4 * K1_LDT : 4;        /* next k-group */
+                const int a_mstep = colform ? 8 : 8 * K1_LDD;        /* next 8 rows */
                 const double *b_base = Cs + lq * 4 + lr;
 #pragma unroll
                 for (int g = 0; g < K1_KG; ++g) {
-                    const double a0 = a_base[g * (K1_M * 4)];
-                    const double a1 = a_base[g * (K1_M * 4) + 32];
+                    const double a0 = a_base[g * a_gstep];
+                    const double a1 = a_base[g * a_gstep + a_mstep];
 #pragma unroll
                     for (int nt = 0; nt < NT8; ++nt) {
                         const double b = b_base[g * (Cfg::NW * 4) + nt * 32];
@@ -179,7 +248,7 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t nao, int64_t npai
 }
 
 template <int NT8>
-void k1_launch_t(const double *B, int64_t nao, int64_t npair, int64_t P0, int64_t np,
+void k1_launch_t(const double *B, int64_t naux, int64_t nao, int64_t npair, int64_t P0, int64_t np,
                  const double *Ccat4, int64_t ldc, int ntiles_n, double *X4, cudaStream_t st)
 {
     static bool configured = false;   /* attribute is per function, set once per process */
@@ -191,12 +260,12 @@ void k1_launch_t(const double *B, int64_t nao, int64_t npair, int64_t P0, int64_
     const unsigned nib = (unsigned)((nao + K1_M - 1) / K1_M);
     dim3 grid(nib * ntiles_n, (unsigned)np);
     k1_half_transform_kernel<NT8><<<grid, K1_THREADS, K1Cfg<NT8>::SMEM_BYTES, st>>>(
-        B, nao, npair, P0, Ccat4, ldc, ntiles_n, X4);
+        B, naux, nao, npair, P0, Ccat4, ldc, ntiles_n, X4);
 }
 
 }  // namespace
 
-void launch_k1_half_transform(const double *B, int64_t nao, int64_t npair, int64_t P0, int64_t np,
+void launch_k1_half_transform(const double *B, int64_t naux, int64_t nao, int64_t npair, int64_t P0, int64_t np,
                               const double *Ccat4, int64_t ldc, double *X4, cudaStream_t st)
 {
     const int n8 = (int)(ldc / 8);
@@ -204,7 +273,7 @@ void launch_k1_half_transform(const double *B, int64_t nao, int64_t npair, int64
     const int nt8 = (n8 + ntiles_n - 1) / ntiles_n;
     /* grid.y <= 65535: chunks are far smaller than that */
 #define DFJK_K1_CASE(N) \
-    case N: k1_launch_t<N>(B, nao, npair, P0, np, Ccat4, ldc, ntiles_n, X4, st); break;
+    case N: k1_launch_t<N>(B, naux, nao, npair, P0, np, Ccat4, ldc, ntiles_n, X4, st); break;
     switch (nt8) {
         DFJK_K1_CASE(1) DFJK_K1_CASE(2) DFJK_K1_CASE(3) DFJK_K1_CASE(4) DFJK_K1_CASE(5)
         DFJK_K1_CASE(6) DFJK_K1_CASE(7) DFJK_K1_CASE(8) DFJK_K1_CASE(9) DFJK_K1_CASE(10)
