@@ -55,8 +55,8 @@ void launch_k1_half_transform(const double *B, int64_t naux, int64_t nao, int64_
                               double *X4, cudaStream_t st);
 
 /* K2: Kpart[split][mu][nu] (+)= sum_{k in split's share} X[mu][k] X[nu][k]
- * for mu-tile >= nu-tile (lower 128x128 tiles).  The set uses k = p*ldc + [col0, col0+round_up(ncol,8)),
- * p < np.  accumulate = 0 overwrites. */
+ * for mu-tile >= nu-tile (lower 128x128 tiles).  The set uses k = p*ldc + [col0, col0+round_up(ncol,4)),
+ * p < np: K2's MMA k step is 4, so the 8-padding columns of Ccat beyond that are never read.  accumulate = 0 overwrites. */
 void launch_k2_syrk_lower(const double *X4, int64_t nao, int64_t np, int64_t ldc, int64_t col0,
                           int64_t ncol, double *Kpart, int nsplit, int accumulate, cudaStream_t st);
 

@@ -7,8 +7,8 @@
  * X chunk layout (written by K1): k-group-major X4[k/4][mu][k%4], k = p*ldc + i, so the
  * 128-row operand panel of one k-group (4 columns) is 4 KB of contiguous memory and lands
  * in shared memory, by one 1-D bulk copy (TMA engine, UBLKCP), already in the dense
- * [row][4] form whose DMMA fragment loads are bank-conflict-free.  A stage holds four
- * k-groups (k = 16) of both operands; 6 stages, full/empty mbarriers, one producer lane.
+ * [row][4] form whose DMMA fragment loads are bank-conflict-free.  A stage holds eight
+ * k-groups (k = 32) of both operands; 3 stages, full/empty mbarriers, one producer lane.
  * One CTA owns a 128 x 128 tile of K for one k-split: 8 consumer warps as 2 (M) x 4 (N),
  * warp tile 64 x 32 = 8 x 4 DMMA.8x8x4 accumulators, 12 shared loads per 32 MMAs.  Both
  * operands are row panels of X, so A (row-major) and B (col-major) fragments are read with
@@ -49,9 +49,10 @@ __global__ void k0_pack_c_kernel(PackDesc pd, int64_t nao, int64_t nao16, int64_
 
 /* ------------------------------------------------------------------ K2 */
 constexpr int K2_T = 128;
-constexpr int K2_STAGES = 6;
-constexpr int K2_OP_BYTES = 4 * K2_T * 32;            /* one operand, one stage: [4 kg][128][4] */
-constexpr int K2_STAGE_BYTES = 2 * K2_OP_BYTES;       /* 32768 */
+constexpr int K2_KG = 8;                              /* k-groups (of 4) per stage: k = 32 */
+constexpr int K2_STAGES = 3;
+constexpr int K2_OP_BYTES = K2_KG * K2_T * 32;        /* one operand, one stage: [kg][128][4] */
+constexpr int K2_STAGE_BYTES = 2 * K2_OP_BYTES;       /* 65536 */
 constexpr int K2_CONSUMER_WARPS = 8;
 constexpr int K2_THREADS = 32 * (1 + K2_CONSUMER_WARPS);
 constexpr int K2_SMEM_BYTES = K2_STAGES * K2_STAGE_BYTES + 2 * K2_STAGES * 8 + 16;
@@ -75,7 +76,7 @@ k2_syrk_lower_kernel(const double *__restrict__ X4, int64_t nao, int64_t np, int
     /* this split's share of the k groups (4 columns each) of the set */
     const int64_t ng = np * n4s;
     const int64_t gbeg = ng * split / nsplit, gend = ng * (split + 1) / nsplit;
-    const int nk = (int)((gend - gbeg + 3) / 4);
+    const int nk = (int)((gend - gbeg + K2_KG - 1) / K2_KG);
 
     const uint32_t smem_base = smem_u32(smem_raw);
     const uint32_t bar_base = smem_base + K2_STAGES * K2_STAGE_BYTES;
@@ -99,8 +100,8 @@ k2_syrk_lower_kernel(const double *__restrict__ X4, int64_t nao, int64_t np, int
                 const int slot = kc % K2_STAGES;
                 const int round = kc / K2_STAGES;
                 if (round > 0) mbar_wait(empty_bar(slot), (round - 1) & 1);
-                const int64_t g0 = gbeg + 4 * (int64_t)kc;
-                const int n = (int)((gend - g0 < 4) ? gend - g0 : 4);
+                const int64_t g0 = gbeg + K2_KG * (int64_t)kc;
+                const int n = (int)((gend - g0 < K2_KG) ? gend - g0 : K2_KG);
                 const uint32_t bytes = (uint32_t)(n * 32 * (rows_a + (diag ? 0 : rows_b)));
                 mbar_arrive_expect_tx(full_bar(slot), bytes);
                 const uint32_t dst = smem_base + slot * K2_STAGE_BYTES;
@@ -135,14 +136,14 @@ k2_syrk_lower_kernel(const double *__restrict__ X4, int64_t nao, int64_t np, int
         const int slot = kc % K2_STAGES;
         mbar_wait(full_bar(slot), (kc / K2_STAGES) & 1);
         if (warp_active) {
-            const int64_t g0 = gbeg + 4 * (int64_t)kc;
-            const int n = (int)((gend - g0 < 4) ? gend - g0 : 4);
+            const int64_t g0 = gbeg + K2_KG * (int64_t)kc;
+            const int n = (int)((gend - g0 < K2_KG) ? gend - g0 : K2_KG);
             const double *Xa = reinterpret_cast<const double *>(smem_raw + slot * K2_STAGE_BYTES);
             const double *Xb = diag ? Xa : Xa + K2_OP_BYTES / 8;
             const double *a_base = Xa + (64 * wm + lq) * 4 + lr;
             const double *b_base = Xb + (32 * wn + lq) * 4 + lr;
 #pragma unroll
-            for (int q = 0; q < 4; ++q) {
+            for (int q = 0; q < K2_KG; ++q) {
                 if (q < n) {
                     double a[8], b[4];
 #pragma unroll
@@ -238,7 +239,7 @@ void launch_k2_syrk_lower(const double *X4, int64_t nao, int64_t np, int64_t ldc
     }
     const int nb = (int)((nao + K2_T - 1) / K2_T);
     const int ntile = nb * (nb + 1) / 2;
-    const int n4s = 2 * (int)((ncol + 7) / 8);          /* sets are padded to multiples of 8 columns */
+    const int n4s = (int)((ncol + 3) / 4);              /* k step 4: Ccat's padding to 8 is not read */
     k2_syrk_lower_kernel<<<dim3((unsigned)ntile, (unsigned)nsplit), K2_THREADS, K2_SMEM_BYTES, st>>>(
         X4, nao, np, ldc / 4, col0 / 4, n4s, Kpart, nsplit, accumulate);
 }
