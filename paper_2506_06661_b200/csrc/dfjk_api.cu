@@ -98,16 +98,18 @@ struct Timed {
     ~Timed() { if (slot >= 0) cudaEventRecord(h->ev[2 * slot + 1], st); }
 };
 
-/* split count that fills the SMs best: work items = ntile * s, one CTA per SM */
+/* split count that fills the SMs best: work items = ntile * s on sm_count SMs (one CTA each).
+ * Whole waves matter because a CTA's duration is fixed by its k range; a small penalty per
+ * split accounts for the read-modify-write of the partial tile. */
 int choose_splits(int ntile, int sm_count, int max_splits)
 {
     int best = 1;
-    double best_eff = 0.0;
+    double best_score = -1.0;
     for (int s = 1; s <= max_splits; ++s) {
         const int items = ntile * s;
         const int waves = (items + sm_count - 1) / sm_count;
-        const double eff = (double)items / ((double)waves * sm_count);
-        if (eff > best_eff + 0.02) { best_eff = eff; best = s; }
+        const double score = (double)items / ((double)waves * sm_count) - 0.002 * s;
+        if (score > best_score) { best_score = score; best = s; }
     }
     return best;
 }
@@ -163,7 +165,7 @@ extern "C" dfjk_handle *dfjk_create(int64_t naux, int64_t nao, const double *B_p
     if (xd > naux * nao * h->ldc_max) xd = naux * nao * h->ldc_max;
     h->x_doubles = xd;
     const int nb = (int)((nao + 127) / 128);
-    h->nsplit_default = choose_splits(nb * (nb + 1) / 2, h->sm_count, 16);
+    h->nsplit_default = choose_splits(nb * (nb + 1) / 2, h->sm_count, 32);
     h->nsplit_alloc = 32;
 
     int rc = DFJK_OK;

@@ -64,13 +64,16 @@ k2_syrk_lower_kernel(const double *__restrict__ X4, int64_t nao, int64_t np, int
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     /* lower-triangle tile index -> (bi, bj), bi >= bj */
-    const int t = blockIdx.x;
+    /* blockIdx.x = split (fastest), blockIdx.y = tile: the hardware dispatches CTAs in linear
+     * order, so the last block row -- the ragged, cheaper tiles -- runs last and the launch's
+     * tail is made of short CTAs */
+    const int t = blockIdx.y;
     int bi = (int)((sqrtf(8.0f * (float)t + 1.0f) - 1.0f) * 0.5f);
     while (bi * (bi + 1) / 2 > t) --bi;
     while ((bi + 1) * (bi + 2) / 2 <= t) ++bi;
     const int bj = t - bi * (bi + 1) / 2;
     const bool diag = bi == bj;
-    const int split = blockIdx.y;
+    const int split = blockIdx.x;
     const int64_t mu0 = (int64_t)bi * K2_T, nu0 = (int64_t)bj * K2_T;
 
     /* this split's share of the k groups (4 columns each) of the set */
@@ -240,7 +243,7 @@ void launch_k2_syrk_lower(const double *X4, int64_t nao, int64_t np, int64_t ldc
     const int nb = (int)((nao + K2_T - 1) / K2_T);
     const int ntile = nb * (nb + 1) / 2;
     const int n4s = (int)((ncol + 3) / 4);              /* k step 4: Ccat's padding to 8 is not read */
-    k2_syrk_lower_kernel<<<dim3((unsigned)ntile, (unsigned)nsplit), K2_THREADS, K2_SMEM_BYTES, st>>>(
+    k2_syrk_lower_kernel<<<dim3((unsigned)nsplit, (unsigned)ntile), K2_THREADS, K2_SMEM_BYTES, st>>>(
         X4, nao, np, ldc / 4, col0 / 4, n4s, Kpart, nsplit, accumulate);
 }
 
