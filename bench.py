@@ -275,10 +275,16 @@ def run_ours(args, cfg):
     k2_ms, k2_n = kt["K2"]
     j_ms = sum(kt[n][0] for n in ("J0", "J1", "J1R", "J2", "J3")) / args.steps
     k_ms = sum(kt[n][0] for n in ("K1", "K2", "K3")) / args.steps
+    # DRAM bytes of the dominant kernel from the committed ncu --set full capture
+    # (profiles/traffic.csv), scaled from the captured launch's rows to the average launch
     traffic = None
     try:
-        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
-            traffic = json.load(f).get(f"cfg{cfg.index}", {}).get("k1_dram_bytes_per_launch")
+        import csv
+        with open(os.path.join(ROOT, "profiles", "traffic.csv")) as f:
+            for row in csv.DictReader(f):
+                if int(row["cfg"]) == cfg.index and row["kernel"] == "K1" and k1_n > 0:
+                    per_row = (float(row["dram_read_bytes"]) + float(row["dram_write_bytes"])) / float(row["rows_in_launch"])
+                    traffic = per_row * cfg.naux * args.steps / k1_n
     except Exception:
         pass
     k1_tflops = flops_k1(cfg) * args.steps / (k1_ms * 1e-3) / 1e12 if k1_ms > 0 else 0.0
