@@ -55,6 +55,19 @@ def _load():
         lib.oracle_kv_slab.argtypes = [
             ctypes.c_int64, ctypes.c_int64, ctypes.c_void_p, ctypes.c_int,
             pp, ctypes.c_void_p, ctypes.c_int64, ctypes.c_void_p, pp]
+        lib.oracle_jk_dm_slab.restype = ctypes.c_int
+        lib.oracle_jk_dm_slab.argtypes = [
+            ctypes.c_int64, ctypes.c_int64, ctypes.c_void_p, ctypes.c_void_p,
+            ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
+        lib.oracle_jk_pair_slab.restype = ctypes.c_int
+        lib.oracle_jk_pair_slab.argtypes = [
+            ctypes.c_int64, ctypes.c_int64, ctypes.c_void_p, ctypes.c_int64,
+            ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p,
+            ctypes.c_void_p]
+        lib.oracle_bruteforce_jk_dm.restype = ctypes.c_int
+        lib.oracle_bruteforce_jk_dm.argtypes = [
+            ctypes.c_int64, ctypes.c_int64, ctypes.c_void_p, ctypes.c_void_p,
+            ctypes.c_void_p, ctypes.c_void_p]
         _lib = lib
     return _lib
 
@@ -215,3 +228,58 @@ class KBlockAccumulator:
             for s, C in enumerate(self.Cs):
                 X = Bsel @ C                             # [|S|][nocc]
                 self.K[s] += X @ X.T
+
+
+# ---------------------------------------------------------------- general densities
+def get_jk_dm(Bp: np.ndarray, nao: int, dm: np.ndarray, with_j: bool = True,
+              with_k: bool = True):
+    """J[dm], K[dm] (both linear in dm, any real nao x nao dm; oracle_jk_dm_slab).
+
+    Returns (J, K, d).  PAPER.md:96 ("arbitrary number of density matrices").
+    """
+    Bp, dm = _f64c(Bp), _f64c(dm)
+    _check_inputs(Bp, nao, [])
+    if dm.shape != (nao, nao):
+        raise ValueError("dm must be nao x nao")
+    J = np.zeros((nao, nao)) if with_j else None
+    K = np.zeros((nao, nao)) if with_k else None
+    d = np.zeros(Bp.shape[0])
+    rc = _load().oracle_jk_dm_slab(
+        Bp.shape[0], nao, Bp.ctypes.data, dm.ctypes.data,
+        None if J is None else J.ctypes.data, None if K is None else K.ctypes.data,
+        d.ctypes.data)
+    if rc != 0:
+        raise RuntimeError(f"oracle_jk_dm_slab failed: {rc}")
+    return J, K, d
+
+
+def get_jk_pair(Bp: np.ndarray, nao: int, C1: np.ndarray, C2: np.ndarray,
+                with_j: bool = True, with_k: bool = True):
+    """dm = C1 C2^T given by its factors: K = sum_P (B_P C1)(B_P C2)^T, J = J[dm]
+    (oracle_jk_pair_slab).  Returns (J, K, d)."""
+    Bp, C1, C2 = _f64c(Bp), _f64c(C1), _f64c(C2)
+    _check_inputs(Bp, nao, [C1, C2])
+    if C1.shape != C2.shape:
+        raise ValueError("C1 and C2 must have the same shape")
+    J = np.zeros((nao, nao)) if with_j else None
+    K = np.zeros((nao, nao)) if with_k else None
+    d = np.zeros(Bp.shape[0])
+    rc = _load().oracle_jk_pair_slab(
+        Bp.shape[0], nao, Bp.ctypes.data, C1.shape[1], C1.ctypes.data, C2.ctypes.data,
+        None if J is None else J.ctypes.data, None if K is None else K.ctypes.data,
+        d.ctypes.data)
+    if rc != 0:
+        raise RuntimeError(f"oracle_jk_pair_slab failed: {rc}")
+    return J, K, d
+
+
+def bruteforce_jk_dm(Bp: np.ndarray, nao: int, dm: np.ndarray):
+    """Eq. 1 materialised + textbook J/K with an arbitrary dm (tiny inputs).  Returns (J, K)."""
+    Bp, dm = _f64c(Bp), _f64c(dm)
+    _check_inputs(Bp, nao, [])
+    J, K = np.zeros((nao, nao)), np.zeros((nao, nao))
+    rc = _load().oracle_bruteforce_jk_dm(Bp.shape[0], nao, Bp.ctypes.data, dm.ctypes.data,
+                                         J.ctypes.data, K.ctypes.data)
+    if rc != 0:
+        raise RuntimeError(f"oracle_bruteforce_jk_dm failed: {rc}")
+    return J, K

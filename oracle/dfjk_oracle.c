@@ -40,8 +40,10 @@
  * Parity pins (tests/test_oracle_pins.py): brute force over the explicit 4-index
  * tensor built by oracle_bruteforce_jk() below (itself a different formula:
  * Eq. 1 materialised, then the textbook J/K contractions), closed forms,
- * invariants, single-element probes, numpy library reductions.  No function in
- * this file is "parity unpinned".
+ * invariants, single-element probes, numpy library reductions; the general-density
+ * functions at the end of the file (oracle_jk_dm_slab, oracle_jk_pair_slab) are pinned
+ * the same way in tests/test_oracle_general_pins.py.  No function in this file is
+ * "parity unpinned".
  *
  * Build: gcc -O2 -fopenmp -shared -fPIC (no -ffast-math; no reassociation).
  */
@@ -355,4 +357,207 @@ int oracle_kv_slab(int64_t nrows, int64_t nao, const double *Bp_slab,
         free(t); free(u); free(y); free(acc);
     }
     return rc;
+}
+
+/* ======================================================================================
+ * General densities.  PAPER.md:96: get_jk "supports an
+ * arbitrary number of density matrices"; the DF-approximated orbital
+ * Hessian of SOSCF contracts the same integrals with NON-idempotent, in general
+ * non-symmetric, response densities.  With Eq. 1 in the textbook
+ * contractions, for ANY real nao x nao matrix dm:
+ *
+ *     J[dm][m][n] = sum_{l,s} (mn|ls) dm[l][s] = sum_P B(P,m,n) * ( sum_{l,s} B(P,l,s) dm[l][s] )
+ *     K[dm][m][n] = sum_{l,s} (ml|ns) dm[l][s] = sum_P sum_{l,s} B(P,m,l) dm[l][s] B(P,n,s)
+ *
+ * Both are LINEAR in dm (this is PySCF's vj, vk).  The occupied-orbital build above is the
+ * special case  K_s = K[C_s C_s^T]  (no weight: reading R1) and  J = J[sum_s w_s C_s C_s^T].
+ * ====================================================================================== */
+
+/*
+ * oracle_jk_dm_slab: accumulate J[dm] and K[dm] of `nrows` packed rows, straight from the
+ * two formulas above: plain triple loops, full squares, nothing factorised.
+ *   dm  nao x nao row-major, ANY real matrix;  J, K accumulated (either may be NULL);
+ *   d_out[r] = sum_{l,s} B(P,l,s) dm[l][s]  (may be NULL).
+ */
+int oracle_jk_dm_slab(int64_t nrows, int64_t nao, const double *Bp_slab, const double *dm,
+                      double *J, double *K, double *d_out)
+{
+    if (nrows < 0 || nao < 1 || !Bp_slab || !dm) return ORACLE_EINVAL;
+    const int64_t npair = nao * (nao + 1) / 2;
+    double *Bf = (double *)malloc(sizeof(double) * nao * nao);
+    double *T = (double *)malloc(sizeof(double) * nao * nao);
+    double *rowsum = (double *)malloc(sizeof(double) * nao);
+    if (!Bf || !T || !rowsum) { free(Bf); free(T); free(rowsum); return ORACLE_ENOMEM; }
+
+    for (int64_t r = 0; r < nrows; ++r) {
+        const double *Bp_row = Bp_slab + r * npair;
+#pragma omp parallel for schedule(static)
+        for (int64_t m = 0; m < nao; ++m)
+            for (int64_t n = 0; n < nao; ++n)
+                Bf[m * nao + n] = b_elem(Bp_row, m, n);
+
+        /* d_P = sum_l ( sum_s B(P,l,s) dm[l][s] )  -- two-level, reading R9 */
+#pragma omp parallel for schedule(static)
+        for (int64_t l = 0; l < nao; ++l) {
+            double t = 0.0;
+            for (int64_t s = 0; s < nao; ++s)
+                t += Bf[l * nao + s] * dm[l * nao + s];
+            rowsum[l] = t;
+        }
+        double dP = 0.0;
+        for (int64_t l = 0; l < nao; ++l) dP += rowsum[l];
+        if (d_out) d_out[r] = dP;
+
+        if (J) {
+#pragma omp parallel for schedule(static)
+            for (int64_t m = 0; m < nao; ++m)
+                for (int64_t n = 0; n < nao; ++n)
+                    J[m * nao + n] += dP * Bf[m * nao + n];
+        }
+        if (K) {
+            /* T[m][s] = sum_l B(P,m,l) dm[l][s]   (s innermost: axpy form) */
+#pragma omp parallel for schedule(static)
+            for (int64_t m = 0; m < nao; ++m) {
+                double *Trow = T + m * nao;
+                for (int64_t s = 0; s < nao; ++s) Trow[s] = 0.0;
+                for (int64_t l = 0; l < nao; ++l) {
+                    const double b = Bf[m * nao + l];
+                    const double *drow = dm + l * nao;
+                    for (int64_t s = 0; s < nao; ++s) Trow[s] += b * drow[s];
+                }
+            }
+            /* K[m][n] += sum_s T[m][s] B(P,n,s)  =  sum_s T[m][s] Bf[s][n]  (B_P symmetric
+             * BY CONSTRUCTION of Bf: Bf[s][n] and Bf[n][s] are the same packed element) */
+#pragma omp parallel for schedule(static)
+            for (int64_t m = 0; m < nao; ++m) {
+                double *Krow = K + m * nao;
+                for (int64_t s = 0; s < nao; ++s) {
+                    const double t = T[m * nao + s];
+                    const double *brow = Bf + s * nao;
+                    for (int64_t n = 0; n < nao; ++n) Krow[n] += t * brow[n];
+                }
+            }
+        }
+    }
+    free(Bf); free(T); free(rowsum);
+    return ORACLE_OK;
+}
+
+/*
+ * oracle_jk_pair_slab: the factorised form used when dm = C1 C2^T is given by its factors
+ * (response densities of SOSCF / TDDFT):
+ *
+ *     X1_P = B_P C1,  X2_P = B_P C2   (nao x ncol each)
+ *     K[m][n] += sum_i X1_P[m][i] X2_P[n][i]                 (= K[C1 C2^T], not symmetric)
+ *     d_P = sum_{l,s} B(P,l,s) (C1 C2^T)[l][s],   J += d_P B_P
+ *
+ * Pinned against oracle_jk_dm_slab (a different formula) and the brute force below.
+ */
+int oracle_jk_pair_slab(int64_t nrows, int64_t nao, const double *Bp_slab, int64_t ncol,
+                        const double *C1, const double *C2, double *J, double *K, double *d_out)
+{
+    if (nrows < 0 || nao < 1 || ncol < 1 || !Bp_slab || !C1 || !C2) return ORACLE_EINVAL;
+    const int64_t npair = nao * (nao + 1) / 2;
+    double *D = (double *)malloc(sizeof(double) * nao * nao);
+    double *Bf = (double *)malloc(sizeof(double) * nao * nao);
+    double *X1 = (double *)malloc(sizeof(double) * nao * ncol);
+    double *X2t = (double *)malloc(sizeof(double) * nao * ncol);
+    double *rowsum = (double *)malloc(sizeof(double) * nao);
+    if (!D || !Bf || !X1 || !X2t || !rowsum) {
+        free(D); free(Bf); free(X1); free(X2t); free(rowsum);
+        return ORACLE_ENOMEM;
+    }
+#pragma omp parallel for schedule(static)
+    for (int64_t l = 0; l < nao; ++l)
+        for (int64_t s = 0; s < nao; ++s) {
+            double t = 0.0;
+            for (int64_t i = 0; i < ncol; ++i) t += C1[l * ncol + i] * C2[s * ncol + i];
+            D[l * nao + s] = t;
+        }
+    for (int64_t r = 0; r < nrows; ++r) {
+        const double *Bp_row = Bp_slab + r * npair;
+#pragma omp parallel for schedule(static)
+        for (int64_t m = 0; m < nao; ++m)
+            for (int64_t n = 0; n < nao; ++n)
+                Bf[m * nao + n] = b_elem(Bp_row, m, n);
+#pragma omp parallel for schedule(static)
+        for (int64_t l = 0; l < nao; ++l) {
+            double t = 0.0;
+            for (int64_t s = 0; s < nao; ++s) t += Bf[l * nao + s] * D[l * nao + s];
+            rowsum[l] = t;
+        }
+        double dP = 0.0;
+        for (int64_t l = 0; l < nao; ++l) dP += rowsum[l];
+        if (d_out) d_out[r] = dP;
+        if (J) {
+#pragma omp parallel for schedule(static)
+            for (int64_t m = 0; m < nao; ++m)
+                for (int64_t n = 0; n < nao; ++n)
+                    J[m * nao + n] += dP * Bf[m * nao + n];
+        }
+        if (K) {
+            /* X1[m][i] = sum_l B(P,m,l) C1[l][i];  X2t[i][n] = sum_l B(P,n,l) C2[l][i] */
+#pragma omp parallel for schedule(static)
+            for (int64_t m = 0; m < nao; ++m) {
+                for (int64_t i = 0; i < ncol; ++i) {
+                    double a = 0.0, b = 0.0;
+                    for (int64_t l = 0; l < nao; ++l) {
+                        a += Bf[m * nao + l] * C1[l * ncol + i];
+                        b += Bf[m * nao + l] * C2[l * ncol + i];
+                    }
+                    X1[m * ncol + i] = a;
+                    X2t[i * nao + m] = b;
+                }
+            }
+#pragma omp parallel for schedule(static)
+            for (int64_t m = 0; m < nao; ++m) {
+                double *Krow = K + m * nao;
+                for (int64_t i = 0; i < ncol; ++i) {
+                    const double x = X1[m * ncol + i];
+                    const double *x2 = X2t + i * nao;
+                    for (int64_t n = 0; n < nao; ++n) Krow[n] += x * x2[n];
+                }
+            }
+        }
+    }
+    free(D); free(Bf); free(X1); free(X2t); free(rowsum);
+    return ORACLE_OK;
+}
+
+/*
+ * oracle_bruteforce_jk_dm: Eq. 1 materialised, then the textbook contractions with an
+ * arbitrary dm (tiny inputs only).  J, K OVERWRITTEN.
+ *     eri[m][n][l][s] = sum_P B(P,m,n) B(P,l,s)
+ *     J[m][n] = sum_{l,s} eri[m][n][l][s] dm[l][s];   K[m][n] = sum_{l,s} eri[m][l][n][s] dm[l][s]
+ */
+int oracle_bruteforce_jk_dm(int64_t naux, int64_t nao, const double *Bp, const double *dm,
+                            double *J, double *K)
+{
+    if (naux < 1 || nao < 1 || nao > 40 || !Bp || !dm) return ORACLE_EINVAL;
+    const int64_t npair = nao * (nao + 1) / 2;
+    const int64_t n2 = nao * nao, n3 = n2 * nao, n4 = n3 * nao;
+    double *eri = (double *)calloc((size_t)n4, sizeof(double));
+    if (!eri) return ORACLE_ENOMEM;
+    for (int64_t m = 0; m < nao; ++m)
+        for (int64_t n = 0; n < nao; ++n)
+            for (int64_t l = 0; l < nao; ++l)
+                for (int64_t s = 0; s < nao; ++s) {
+                    double acc = 0.0;
+                    for (int64_t P = 0; P < naux; ++P)
+                        acc += b_elem(Bp + P * npair, m, n) * b_elem(Bp + P * npair, l, s);
+                    eri[m * n3 + n * n2 + l * nao + s] = acc;
+                }
+    for (int64_t m = 0; m < nao; ++m)
+        for (int64_t n = 0; n < nao; ++n) {
+            double aj = 0.0, ak = 0.0;
+            for (int64_t l = 0; l < nao; ++l)
+                for (int64_t s = 0; s < nao; ++s) {
+                    aj += eri[m * n3 + n * n2 + l * nao + s] * dm[l * nao + s];
+                    ak += eri[m * n3 + l * n2 + n * nao + s] * dm[l * nao + s];
+                }
+            if (J) J[m * nao + n] = aj;
+            if (K) K[m * nao + n] = ak;
+        }
+    free(eri);
+    return ORACLE_OK;
 }
