@@ -94,6 +94,45 @@ int dfjk_get_jk_u(dfjk_handle *h, const double *C_a, int64_t nocc_a,
                   double *J, double *K_a, double *K_b, void *stream);
 
 /*
+ * General densities.  PAPER.md:96: get_jk "supports an
+ * arbitrary number of density matrices"; the DF-approximated
+ * orbital Hessian of SOSCF contracts Eq. 1's integrals with response densities that are
+ * neither idempotent nor symmetric.  For ANY real nao x nao matrix dm, with Eq. 1:
+ *
+ *     J[dm] = sum_P B_P <B_P, dm>          (only dm + dm^T matters; J is symmetric)
+ *     K[dm] = sum_P B_P dm B_P             (K[dm^T] = K[dm]^T; not symmetric in general)
+ *
+ * Both are LINEAR in dm (PySCF's vj, vk).  Relation to dfjk_get_jk: its J is J[2 C C^T]
+ * and its K is K[C C^T] (no factor 2, R1).
+ *
+ * dfjk_get_jk_pair -- dm = C1 C2^T given by its factors (the usual form of a response
+ * density, e.g. C_occ and the rotated orbitals C_vir kappa):
+ *     K = sum_P (B_P C1)(B_P C2)^T        one half transform over [C1|C2], then a
+ *                                          full (non-symmetric) DMMA product
+ *   C1, C2  DEVICE, nao x ncol row-major, 1 <= ncol <= nao (any dm has such a factorisation).
+ *   J, K    DEVICE, nao x nao, OVERWRITTEN; either may be NULL, not both.
+ */
+int dfjk_get_jk_pair(dfjk_handle *h, const double *C1, const double *C2, int64_t ncol,
+                     double *J, double *K, void *stream);
+
+/*
+ * dfjk_get_jk_dm -- the same for a raw density matrix (no factorisation needed):
+ *   dm      DEVICE, nao x nao row-major, any real matrix.
+ * K is built as the pair (dm, I): X_P = B_P dm by the half transform, then
+ * K = sum_P X_P B_P^T.  Cost ~ 6 naux nao^3 flop: prefer dfjk_get_jk / dfjk_get_jk_pair
+ * whenever factors with few columns are known.
+ */
+int dfjk_get_jk_dm(dfjk_handle *h, const double *dm, double *J, double *K, void *stream);
+
+/*
+ * dfjk_get_jk_dms -- "an arbitrary number of density matrices":
+ *   dms     DEVICE, ndm x nao x nao;  Js, Ks  DEVICE, ndm x nao x nao (either may be NULL).
+ * Equivalent to ndm stream-ordered dfjk_get_jk_dm calls.
+ */
+int dfjk_get_jk_dms(dfjk_handle *h, int64_t ndm, const double *dms, double *Js, double *Ks,
+                    void *stream);
+
+/*
  * dfjk_get_jk_host -- the same restricted build for a caller whose orbitals and
  * results live in HOST memory (the end-to-end call bench.py times):
  * copies C_occ host->device, runs dfjk_get_jk on an internal stream, copies J and

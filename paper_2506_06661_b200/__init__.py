@@ -29,6 +29,7 @@ SYMBOLS = (
     "dfjk_create", "dfjk_get_jk", "dfjk_get_jk_u", "dfjk_get_jk_host", "dfjk_get_d",
     "dfjk_set_option", "dfjk_workspace_bytes", "dfjk_destroy", "dfjk_last_error",
     "dfjk_version", "dfjk_launch_count", "dfjk_kernel_time",
+    "dfjk_get_jk_pair", "dfjk_get_jk_dm", "dfjk_get_jk_dms",
 )
 
 # DFJK_KERNEL_* ids of include/dfjk.h
@@ -65,6 +66,12 @@ def lib() -> ctypes.CDLL:
     L.dfjk_get_jk.argtypes = [vp, vp, i64, vp, vp, vp]
     L.dfjk_get_jk_u.restype = ci
     L.dfjk_get_jk_u.argtypes = [vp, vp, i64, vp, i64, vp, vp, vp, vp]
+    L.dfjk_get_jk_pair.restype = ci
+    L.dfjk_get_jk_pair.argtypes = [vp, vp, vp, i64, vp, vp, vp]
+    L.dfjk_get_jk_dm.restype = ci
+    L.dfjk_get_jk_dm.argtypes = [vp, vp, vp, vp, vp]
+    L.dfjk_get_jk_dms.restype = ci
+    L.dfjk_get_jk_dms.argtypes = [vp, i64, vp, vp, vp, vp]
     L.dfjk_get_jk_host.restype = ci
     L.dfjk_get_jk_host.argtypes = [vp, vp, i64, vp, vp]
     L.dfjk_get_d.restype = ci
@@ -162,6 +169,43 @@ class DFJK:
                                        Ka.data_ptr() if with_k else None,
                                        Kb.data_ptr() if with_k else None, st), "dfjk_get_jk_u")
         return J, Ka, Kb
+
+    # -- general densities: dm = C1 C2^T (pair) or a raw nao x nao matrix; J, K linear in dm
+    def _out(self, with_it: bool, lead=()):
+        import torch
+        return torch.empty(*lead, self.nao, self.nao, dtype=torch.float64,
+                           device=self.device) if with_it else None
+
+    def get_jk_pair(self, C1, C2, with_j: bool = True, with_k: bool = True, stream=None):
+        import torch
+        if C1.dim() != 2 or C1.shape[0] != self.nao or C1.shape != C2.shape:
+            raise ValueError("C1, C2 must both be nao x ncol")
+        p1, p2 = _dev_f64(C1, "C1"), _dev_f64(C2, "C2")
+        J, K = self._out(with_j), self._out(with_k)
+        with torch.cuda.device(self.device):
+            st = (stream or torch.cuda.current_stream(self.device)).cuda_stream
+            _check(lib().dfjk_get_jk_pair(self._h, p1, p2, int(C1.shape[1]),
+                                          J.data_ptr() if with_j else None,
+                                          K.data_ptr() if with_k else None, st), "dfjk_get_jk_pair")
+        return J, K
+
+    def get_jk_dm(self, dm, with_j: bool = True, with_k: bool = True, stream=None):
+        """dm: nao x nao (one density) or ndm x nao x nao (a batch)."""
+        import torch
+        batched = dm.dim() == 3
+        if dm.shape[-2:] != (self.nao, self.nao) or dm.dim() not in (2, 3):
+            raise ValueError("dm must be nao x nao or ndm x nao x nao")
+        dp = _dev_f64(dm, "dm")
+        lead = (dm.shape[0],) if batched else ()
+        J, K = self._out(with_j, lead), self._out(with_k, lead)
+        jp, kp = (J.data_ptr() if with_j else None), (K.data_ptr() if with_k else None)
+        with torch.cuda.device(self.device):
+            st = (stream or torch.cuda.current_stream(self.device)).cuda_stream
+            if batched:
+                _check(lib().dfjk_get_jk_dms(self._h, int(dm.shape[0]), dp, jp, kp, st), "dfjk_get_jk_dms")
+            else:
+                _check(lib().dfjk_get_jk_dm(self._h, dp, jp, kp, st), "dfjk_get_jk_dm")
+        return J, K
 
     # -- host buffers in, host buffers out (B stays resident); synchronous
     def get_jk_host(self, C_occ_host, J_host=None, K_host=None):

@@ -287,7 +287,88 @@ int get_jk_impl(dfjk_handle *h, int nset, const double *const *C, const int64_t 
     return DFJK_OK;
 }
 
+
+/* general density: dm = C1 C2^T (pair form) or dm = C1 with C2 == NULL (raw nao x nao matrix,
+ * built as the pair (dm, I)).  J = J[dm], K = K[dm] = sum_P (B_P C1)(B_P C2)^T, both linear. */
+int get_jk_general_impl(dfjk_handle *h, const double *C1, const double *C2, int64_t ncol,
+                        double *J, double *K, cudaStream_t st, const char *who)
+{
+    g_err[0] = 0;
+    if (!h) return fail(DFJK_EINVAL, "%s: NULL handle", who);
+    if (!C1) return fail(DFJK_EINVAL, "%s: density / factor pointer is NULL", who);
+    if (ncol < 1 || ncol > h->nao)
+        return fail(DFJK_EINVAL, "%s: ncol=%lld outside [1, nao=%lld]", who, (long long)ncol, (long long)h->nao);
+    if (!J && !K) return fail(DFJK_EINVAL, "%s: no output requested", who);
+    int dev = -1;
+    DFJK_CUDA_TRY(cudaGetDevice(&dev));
+    if (dev != h->device) return fail(DFJK_EINVAL, "%s: handle belongs to device %d, current is %d", who, h->device, dev);
+
+    const int64_t nao = h->nao, naux = h->naux, npair = h->npair;
+    if (J) {
+        { Timed t_(h, DFJK_KERNEL_J0, st); dfjk::launch_j0_general_dt(C1, C2, ncol, nao, h->Dt, st); }
+        { Timed t_(h, DFJK_KERNEL_J1, st); dfjk::launch_j1_dot(h->B, naux, npair, h->Dt, h->d_part, h->sm_count, st); }
+        { Timed t_(h, DFJK_KERNEL_J1R, st); dfjk::launch_j1_reduce(h->d_part, h->nchunk, naux, h->d, st); }
+        { Timed t_(h, DFJK_KERNEL_J2, st); dfjk::launch_j2_axpy(h->B, naux, npair, h->d, h->Jp_part, h->j2_groups, st); }
+        { Timed t_(h, DFJK_KERNEL_J3, st); dfjk::launch_j3_unpack(h->Jp_part, h->j2_groups, npair, nao, J, st); }
+        h->have_d = true;
+    }
+    if (K) {
+        /* Ccat = [C1 | C2] (a NULL second factor packs the identity), each padded to 8 columns */
+        const double *Cp[2] = {C1, C2};
+        const int nocc[2] = {(int)ncol, (int)ncol};
+        const int64_t w8 = round_up(ncol, 8);
+        const int col0[2] = {0, (int)w8};
+        const int64_t ldc = 2 * w8;
+        { Timed t_(h, DFJK_KERNEL_K0, st); dfjk::launch_k0_pack_c(Cp, nocc, col0, 2, nao, ldc, h->Ccat, st); }
+        int64_t pc = h->x_doubles / (nao * ldc);
+        if (h->opt_k_chunk > 0 && h->opt_k_chunk < pc) pc = h->opt_k_chunk;
+        if (pc > naux) pc = naux;
+        if (pc < 1) return fail(DFJK_ENOMEM, "%s: X workspace too small", who);
+        const int nb = (int)((nao + 127) / 128);
+        const int nsplit = h->opt_k_splits > 0 ? (int)h->opt_k_splits
+                                               : choose_splits(nb * nb, h->sm_count, h->nsplit_alloc);
+        int chunk = 0;
+        for (int64_t P0 = 0; P0 < naux; P0 += pc, ++chunk) {
+            const int64_t np = (P0 + pc <= naux) ? pc : naux - P0;
+            { Timed t_(h, DFJK_KERNEL_K1, st); dfjk::launch_k1_half_transform(h->B, naux, nao, npair, P0, np, h->Ccat, ldc, h->X, st); }
+            { Timed t_(h, DFJK_KERNEL_K2, st);
+              dfjk::launch_k2_gemm_full(h->X, nao, np, ldc, col0[0], col0[1], ncol, h->Kpart, nsplit, chunk > 0, st); }
+        }
+        { Timed t_(h, DFJK_KERNEL_K3, st); dfjk::launch_k3_sum(h->Kpart, nsplit, nao, K, st); }
+    }
+    DFJK_CUDA_TRY(cudaGetLastError());
+    return DFJK_OK;
+}
+
 }  // namespace
+
+extern "C" int dfjk_get_jk_pair(dfjk_handle *h, const double *C1, const double *C2, int64_t ncol,
+                                double *J, double *K, void *stream)
+{
+    if (!C2) { g_err[0] = 0; return fail(DFJK_EINVAL, "dfjk_get_jk_pair: C2 is NULL"); }
+    return get_jk_general_impl(h, C1, C2, ncol, J, K, (cudaStream_t)stream, "dfjk_get_jk_pair");
+}
+
+extern "C" int dfjk_get_jk_dm(dfjk_handle *h, const double *dm, double *J, double *K, void *stream)
+{
+    return get_jk_general_impl(h, dm, nullptr, h ? h->nao : 1, J, K, (cudaStream_t)stream, "dfjk_get_jk_dm");
+}
+
+extern "C" int dfjk_get_jk_dms(dfjk_handle *h, int64_t ndm, const double *dms, double *Js, double *Ks,
+                               void *stream)
+{
+    g_err[0] = 0;
+    if (!h) return fail(DFJK_EINVAL, "dfjk_get_jk_dms: NULL handle");
+    if (ndm < 1) return fail(DFJK_EINVAL, "dfjk_get_jk_dms: ndm must be >= 1");
+    const int64_t n2 = h->nao * h->nao;
+    for (int64_t i = 0; i < ndm; ++i) {
+        const int rc = get_jk_general_impl(h, dms ? dms + i * n2 : nullptr, nullptr, h->nao,
+                                           Js ? Js + i * n2 : nullptr, Ks ? Ks + i * n2 : nullptr,
+                                           (cudaStream_t)stream, "dfjk_get_jk_dms");
+        if (rc != DFJK_OK) return rc;
+    }
+    return DFJK_OK;
+}
 
 extern "C" int dfjk_get_jk(dfjk_handle *h, const double *C_occ, int64_t nocc, double *J, double *K,
                            void *stream)

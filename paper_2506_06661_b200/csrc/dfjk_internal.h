@@ -23,6 +23,11 @@ void launch_j0_build_dt(const double *Ccat, int64_t ldc, int64_t nao,
                         int nset, const int *col0, const int *nocc, const double *w,
                         double *Dt, cudaStream_t st);
 
+/* J0 for a general density: Dt[mu(mu+1)/2+nu] = dm[mu][nu] + (mu != nu) dm[nu][mu] where dm is either
+ * given (C2 == NULL, C1 = dm, nao x nao row-major) or the product C1 C2^T of two nao x ncol factors. */
+void launch_j0_general_dt(const double *C1, const double *C2, int64_t ncol, int64_t nao, double *Dt,
+                          cudaStream_t st);
+
 /* J1: d_part[c][P] = sum_{pair in chunk c} B[P][pair] Dt[pair];  nchunk = j1_num_chunks(npair). */
 int64_t j1_num_chunks(int64_t npair);
 void launch_j1_dot(const double *B, int64_t naux, int64_t npair, const double *Dt,
@@ -45,6 +50,7 @@ void launch_j3_unpack(const double *Jp_part, int64_t ngroup, int64_t npair, int6
 /* K0: the zero-padded concatenation [C_0 | C_1 | ...] (every set padded to a multiple of 8
  * columns, ldc columns in total) in k-group-major layout
  *   Ccat4[(mu/4)*ldc*4 + c*4 + mu%4],  mu < round_up(nao, 32) (rows >= nao are zero). */
+/* A NULL C[s] stands for the nao x nao identity (nocc[s] = nao): used by the raw-dm build. */
 void launch_k0_pack_c(const double *const *C, const int *nocc, const int *col0, int nset,
                       int64_t nao, int64_t ldc, double *Ccat, cudaStream_t st);
 
@@ -59,6 +65,16 @@ void launch_k1_half_transform(const double *B, int64_t naux, int64_t nao, int64_
  * p < np: K2's MMA k step is 4, so the 8-padding columns of Ccat beyond that are never read.  accumulate = 0 overwrites. */
 void launch_k2_syrk_lower(const double *X4, int64_t nao, int64_t np, int64_t ldc, int64_t col0,
                           int64_t ncol, double *Kpart, int nsplit, int accumulate, cudaStream_t st);
+
+/* K2 general: Kpart[split][mu][nu] (+)= sum_k X[mu][k_a] X[nu][k_b] over ALL tiles, with
+ * k_a = p*ldc + col0a + j, k_b = p*ldc + col0b + j, j < round_up(ncol,4): the product
+ * sum_P (B_P C1)(B_P C2)^T of two column ranges of the same X chunk (not symmetric). */
+void launch_k2_gemm_full(const double *X4, int64_t nao, int64_t np, int64_t ldc, int64_t col0a,
+                         int64_t col0b, int64_t ncol, double *Kpart, int nsplit, int accumulate,
+                         cudaStream_t st);
+
+/* K3 general: K[mu][nu] = sum_split Kpart[split][mu][nu] for every (mu, nu). */
+void launch_k3_sum(const double *Kpart, int nsplit, int64_t nao, double *K, cudaStream_t st);
 
 /* K3: K[mu][nu] = K[nu][mu] = sum_split Kpart[split][mu][nu], mu >= nu. */
 void launch_k3_finish(const double *Kpart, int nsplit, int64_t nao, double *K, cudaStream_t st);

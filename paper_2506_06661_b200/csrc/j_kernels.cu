@@ -83,6 +83,74 @@ j0_build_dt_kernel(const double *__restrict__ Ccat, int64_t ldc, int64_t nao, Se
     }
 }
 
+/* J0 for a general (non-symmetric, non-idempotent) density, 32 x 32 lower tiles:
+ *   C2 == NULL:  dm = C1 (nao x nao);   else dm = C1 C2^T (nao x ncol factors)
+ *   Dt[mu(mu+1)/2 + nu] = dm[mu][nu] + (mu != nu) * dm[nu][mu]       (J sees only dm + dm^T) */
+__global__ void __launch_bounds__(256)
+j0_general_dt_kernel(const double *__restrict__ C1, const double *__restrict__ C2, int64_t ncol,
+                     int64_t nao, double *__restrict__ Dt)
+{
+    const int bi = blockIdx.y, bj = blockIdx.x;
+    if (bj > bi) return;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    const int64_t mu0 = (int64_t)bi * J0_T, nu0 = (int64_t)bj * J0_T;
+    __shared__ double A1[J0_T][J0_T + 1];      /* C1 rows mu0.. (or dm tile [mu][nu]) */
+    __shared__ double A2[J0_T][J0_T + 1];      /* C2 rows mu0.. (or dm tile [nu][mu]) */
+    __shared__ double B1[J0_T][J0_T + 1];      /* C1 rows nu0.. */
+    __shared__ double B2[J0_T][J0_T + 1];      /* C2 rows nu0.. */
+    if (C2 == nullptr) {
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            const int row = ty + 8 * r;
+            const int64_t mu = mu0 + row, nu = nu0 + tx;
+            A1[row][tx] = (mu < nao && nu < nao) ? C1[mu * nao + nu] : 0.0;
+            const int64_t a = nu0 + row, b = mu0 + tx;
+            A2[row][tx] = (a < nao && b < nao) ? C1[a * nao + b] : 0.0;
+        }
+        __syncthreads();
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            const int row = ty + 8 * r;
+            const int64_t mu = mu0 + row, nu = nu0 + tx;
+            if (mu < nao && nu <= mu)
+                Dt[mu * (mu + 1) / 2 + nu] = A1[row][tx] + (mu == nu ? 0.0 : A2[tx][row]);
+        }
+        return;
+    }
+    double acc[4] = {0.0, 0.0, 0.0, 0.0};      /* dm[mu][nu] */
+    double acct[4] = {0.0, 0.0, 0.0, 0.0};     /* dm[nu][mu] */
+    for (int64_t c0 = 0; c0 < ncol; c0 += J0_T) {
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            const int row = ty + 8 * r;
+            const int64_t c = c0 + tx;
+            const int64_t mu = mu0 + row, nu = nu0 + row;
+            const bool okm = mu < nao && c < ncol, okn = nu < nao && c < ncol;
+            A1[row][tx] = okm ? C1[mu * ncol + c] : 0.0;
+            A2[row][tx] = okm ? C2[mu * ncol + c] : 0.0;
+            B1[row][tx] = okn ? C1[nu * ncol + c] : 0.0;
+            B2[row][tx] = okn ? C2[nu * ncol + c] : 0.0;
+        }
+        __syncthreads();
+#pragma unroll 8
+        for (int c = 0; c < J0_T; ++c) {
+            const double b1 = B1[tx][c], b2 = B2[tx][c];
+#pragma unroll
+            for (int r = 0; r < 4; ++r) {
+                acc[r] += A1[ty + 8 * r][c] * b2;
+                acct[r] += A2[ty + 8 * r][c] * b1;
+            }
+        }
+        __syncthreads();
+    }
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+        const int64_t mu = mu0 + ty + 8 * r, nu = nu0 + tx;
+        if (mu < nao && nu <= mu)
+            Dt[mu * (mu + 1) / 2 + nu] = acc[r] + (mu == nu ? 0.0 : acct[r]);
+    }
+}
+
 /* ------------------------------------------------------------------ J1 */
 constexpr int J1_CH = 4096;          /* columns (pairs) per chunk; Dt chunk = 32 KB of smem */
 constexpr int J1_WARPS = 8;
@@ -262,6 +330,13 @@ void launch_j0_build_dt(const double *Ccat, int64_t ldc, int64_t nao, int nset, 
     }
     const unsigned nb = (unsigned)((nao + J0_T - 1) / J0_T);
     j0_build_dt_kernel<<<dim3(nb, nb), 256, 0, st>>>(Ccat, ldc, nao, sd, Dt);
+}
+
+void launch_j0_general_dt(const double *C1, const double *C2, int64_t ncol, int64_t nao, double *Dt,
+                          cudaStream_t st)
+{
+    const unsigned nb = (unsigned)((nao + J0_T - 1) / J0_T);
+    j0_general_dt_kernel<<<dim3(nb, nb), 256, 0, st>>>(C1, C2, ncol, nao, Dt);
 }
 
 int64_t j1_num_chunks(int64_t npair) { return (npair + J1_CH - 1) / J1_CH; }

@@ -29,6 +29,7 @@ struct PackDesc {
     const double *C[4];
     int nocc[4];
     int col0[4];
+    int identity[4];      /* 1: the set is the nao x nao identity (C[s] unused) */
 };
 
 /* Ccat4[(mu/4)][c][mu%4], mu < nao16 (rows >= nao and padding columns are zero) */
@@ -43,7 +44,8 @@ __global__ void k0_pack_c_kernel(PackDesc pd, int64_t nao, int64_t nao16, int64_
     if (mu < nao)
         for (int s = 0; s < pd.nset; ++s)
             if (c >= pd.col0[s] && c < pd.col0[s] + pd.nocc[s])
-                v = pd.C[s][mu * pd.nocc[s] + (c - pd.col0[s])];
+                v = pd.identity[s] ? (mu == c - pd.col0[s] ? 1.0 : 0.0)
+                                   : pd.C[s][mu * pd.nocc[s] + (c - pd.col0[s])];
     Ccat4[((mu >> 2) * ldc + c) * 4 + (mu & 3)] = v;
 }
 
@@ -57,9 +59,15 @@ constexpr int K2_CONSUMER_WARPS = 8;
 constexpr int K2_THREADS = 32 * (1 + K2_CONSUMER_WARPS);
 constexpr int K2_SMEM_BYTES = K2_STAGES * K2_STAGE_BYTES + 2 * K2_STAGES * 8 + 16;
 
+/* FULL == false: the SYRK above (one column range, lower tiles only).
+ * FULL == true : the general product  Kpart += X[:, range a] X[:, range b]^T  over ALL nb x nb
+ *                tiles (K[C1 C2^T] = sum_P (B_P C1)(B_P C2)^T is not symmetric); blockIdx.y is the
+ *                row-major tile index and the operands come from two column ranges of X. */
+template <bool FULL>
 __global__ void __launch_bounds__(K2_THREADS, 1)
 k2_syrk_lower_kernel(const double *__restrict__ X4, int64_t nao, int64_t np, int64_t ldc4,
-                     int64_t col04, int n4s, double *__restrict__ Kpart, int nsplit, int accumulate)
+                     int64_t col04, int64_t col04b, int n4s, double *__restrict__ Kpart, int nsplit,
+                     int accumulate)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -68,11 +76,18 @@ k2_syrk_lower_kernel(const double *__restrict__ X4, int64_t nao, int64_t np, int
      * order, so the last block row -- the ragged, cheaper tiles -- runs last and the launch's
      * tail is made of short CTAs */
     const int t = blockIdx.y;
-    int bi = (int)((sqrtf(8.0f * (float)t + 1.0f) - 1.0f) * 0.5f);
-    while (bi * (bi + 1) / 2 > t) --bi;
-    while ((bi + 1) * (bi + 2) / 2 <= t) ++bi;
-    const int bj = t - bi * (bi + 1) / 2;
-    const bool diag = bi == bj;
+    int bi, bj;
+    if (FULL) {
+        const int nb = (int)((nao + K2_T - 1) / K2_T);
+        bi = t / nb;
+        bj = t - bi * nb;
+    } else {
+        bi = (int)((sqrtf(8.0f * (float)t + 1.0f) - 1.0f) * 0.5f);
+        while (bi * (bi + 1) / 2 > t) --bi;
+        while ((bi + 1) * (bi + 2) / 2 <= t) ++bi;
+        bj = t - bi * (bi + 1) / 2;
+    }
+    const bool diag = !FULL && bi == bj;         /* both operands are the same panel */
     const int split = blockIdx.x;
     const int64_t mu0 = (int64_t)bi * K2_T, nu0 = (int64_t)bj * K2_T;
 
@@ -113,9 +128,11 @@ k2_syrk_lower_kernel(const double *__restrict__ X4, int64_t nao, int64_t np, int
                     const int64_t kg = (g / n4s) * ldc4 + col04 + g % n4s;     /* k-group in X4 */
                     const double *src = X4 + kg * nao * 4;
                     bulk_g2s(dst + q * (K2_T * 32), src + mu0 * 4, (uint32_t)(rows_a * 32), full_bar(slot));
-                    if (!diag)
-                        bulk_g2s(dst + K2_OP_BYTES + q * (K2_T * 32), src + nu0 * 4,
+                    if (!diag) {
+                        const double *srcb = FULL ? src + (col04b - col04) * nao * 4 : src;
+                        bulk_g2s(dst + K2_OP_BYTES + q * (K2_T * 32), srcb + nu0 * 4,
                                  (uint32_t)(rows_b * 32), full_bar(slot));
+                    }
                 }
             }
         }
@@ -128,7 +145,7 @@ k2_syrk_lower_kernel(const double *__restrict__ X4, int64_t nao, int64_t np, int
     const int lq = lane >> 2, lr = lane & 3;
     /* skip warp tiles that lie outside the matrix or strictly above the diagonal */
     const bool warp_active = (mu0 + 64 * wm < nao) && (nu0 + 32 * wn < nao) &&
-                             !(diag && 32 * wn > 64 * wm + 63);
+                             !(diag && 32 * wn > 64 * wm + 63);    /* diag is false when FULL */
     double acc[8][4][2];
 #pragma unroll
     for (int mt = 0; mt < 8; ++mt)
@@ -214,6 +231,17 @@ k3_finish_kernel(const double *__restrict__ Kpart, int nsplit, int64_t nao, doub
     }
 }
 
+/* general (non-symmetric) finish: K[mu][nu] = sum_split Kpart[split][mu][nu], every entry */
+__global__ void __launch_bounds__(256)
+k3_sum_kernel(const double *__restrict__ Kpart, int nsplit, int64_t n2, double *__restrict__ K)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n2) return;
+    double v = 0.0;
+    for (int s = 0; s < nsplit; ++s) v += Kpart[(int64_t)s * n2 + i];
+    K[i] = v;
+}
+
 }  // namespace
 
 void launch_k0_pack_c(const double *const *C, const int *nocc, const int *col0, int nset, int64_t nao,
@@ -225,6 +253,7 @@ void launch_k0_pack_c(const double *const *C, const int *nocc, const int *col0, 
         pd.C[s] = s < nset ? C[s] : nullptr;
         pd.nocc[s] = s < nset ? nocc[s] : 0;
         pd.col0[s] = s < nset ? col0[s] : 0;
+        pd.identity[s] = (s < nset && C[s] == nullptr) ? 1 : 0;   /* NULL set = identity */
     }
     const int64_t nao16 = (nao + 31) / 32 * 32;   /* K1 stages cover 32 rows of C */
     const int64_t n = nao16 * ldc;
@@ -236,21 +265,43 @@ void launch_k2_syrk_lower(const double *X4, int64_t nao, int64_t np, int64_t ldc
 {
     static bool configured = false;
     if (!configured) {
-        cudaFuncSetAttribute(k2_syrk_lower_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        cudaFuncSetAttribute(k2_syrk_lower_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                              K2_SMEM_BYTES);
         configured = true;
     }
     const int nb = (int)((nao + K2_T - 1) / K2_T);
     const int ntile = nb * (nb + 1) / 2;
     const int n4s = (int)((ncol + 3) / 4);              /* k step 4: Ccat's padding to 8 is not read */
-    k2_syrk_lower_kernel<<<dim3((unsigned)nsplit, (unsigned)ntile), K2_THREADS, K2_SMEM_BYTES, st>>>(
-        X4, nao, np, ldc / 4, col0 / 4, n4s, Kpart, nsplit, accumulate);
+    k2_syrk_lower_kernel<false><<<dim3((unsigned)nsplit, (unsigned)ntile), K2_THREADS, K2_SMEM_BYTES, st>>>(
+        X4, nao, np, ldc / 4, col0 / 4, col0 / 4, n4s, Kpart, nsplit, accumulate);
+}
+
+void launch_k2_gemm_full(const double *X4, int64_t nao, int64_t np, int64_t ldc, int64_t col0a,
+                         int64_t col0b, int64_t ncol, double *Kpart, int nsplit, int accumulate,
+                         cudaStream_t st)
+{
+    static bool configured = false;
+    if (!configured) {
+        cudaFuncSetAttribute(k2_syrk_lower_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             K2_SMEM_BYTES);
+        configured = true;
+    }
+    const int nb = (int)((nao + K2_T - 1) / K2_T);
+    const int n4s = (int)((ncol + 3) / 4);
+    k2_syrk_lower_kernel<true><<<dim3((unsigned)nsplit, (unsigned)(nb * nb)), K2_THREADS, K2_SMEM_BYTES, st>>>(
+        X4, nao, np, ldc / 4, col0a / 4, col0b / 4, n4s, Kpart, nsplit, accumulate);
 }
 
 void launch_k3_finish(const double *Kpart, int nsplit, int64_t nao, double *K, cudaStream_t st)
 {
     const unsigned nb = (unsigned)((nao + K3_T - 1) / K3_T);
     k3_finish_kernel<<<dim3(nb, nb), 256, 0, st>>>(Kpart, nsplit, nao, K);
+}
+
+void launch_k3_sum(const double *Kpart, int nsplit, int64_t nao, double *K, cudaStream_t st)
+{
+    const int64_t n2 = nao * nao;
+    k3_sum_kernel<<<(unsigned)((n2 + 255) / 256), 256, 0, st>>>(Kpart, nsplit, n2, K);
 }
 
 }  // namespace dfjk

@@ -35,6 +35,11 @@ def test_version_and_null_handling(L):
     assert b"NULL handle" in L.dfjk_last_error()
     assert L.dfjk_get_jk_host(None, None, 1, None, None) == -1
     assert L.dfjk_set_option(None, b"k_chunk", 1) == -1
+    # general-density entry points (section 8f rank 1)
+    assert L.dfjk_get_jk_pair(None, None, None, 1, None, None, None) == -1
+    assert b"NULL" in L.dfjk_last_error()
+    assert L.dfjk_get_jk_dm(None, None, None, None, None) == -1
+    assert L.dfjk_get_jk_dms(None, 1, None, None, None, None) == -1
 
 
 def test_create_rejects_bad_arguments_without_touching_memory(L):

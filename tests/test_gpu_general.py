@@ -1,0 +1,155 @@
+"""GPU parity of the general-density entry points (dfjk_get_jk_pair / _dm / _dms) against the
+CPU oracle, element by element.
+
+Bar: relative Frobenius error <= 1e-11 for J and K, FP64, full matrices (north_star tolerance).
+Shapes span several 128 x 128 K tiles (full, non-symmetric tile grid), ragged tails, odd npair,
+ncol = 1 ... nao, several X chunks and k splits.
+"""
+import numpy as np
+import pytest
+
+import dfjk_inputs as gi
+import oracle
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-11
+
+
+def relerr(a, b):
+    nb = np.linalg.norm(b)
+    return np.linalg.norm(np.asarray(a) - np.asarray(b)) / (nb if nb > 0 else 1.0)
+
+
+@pytest.fixture(scope="module")
+def dfjk():
+    import paper_2506_06661_b200 as pkg
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    pkg.lib()
+    return pkg
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def make_B(nao, naux, seed):
+    return gi.fill_B_host(gi.custom_config(nao, naux, (1,), seed=seed))
+
+
+@pytest.mark.parametrize("nao,naux,ncol", [
+    (1, 1, 1),
+    (2, 3, 2),
+    (5, 7, 3),
+    (17, 9, 17),         # ncol = nao
+    (33, 5, 8),
+    (64, 16, 9),
+    (129, 12, 31),       # 2 x 2 tiles, ragged
+    (200, 40, 13),
+    (290, 60, 25),       # 3 x 3 tiles, npair odd
+    (300, 7, 130),
+])
+def test_pair_parity(dfjk, nao, naux, ncol):
+    Bp = make_B(nao, naux, 100 + nao)
+    rng = np.random.default_rng(nao + ncol)
+    C1, C2 = rng.standard_normal((nao, ncol)), rng.standard_normal((nao, ncol))
+    h = dfjk.DFJK(dev(Bp), nao)
+    J, K = h.get_jk_pair(dev(C1), dev(C2))
+    d = h.get_d()
+    torch.cuda.synchronize()
+    Jo, Ko, do = oracle.get_jk_pair(Bp, nao, C1, C2)
+    assert relerr(d.cpu().numpy(), do) <= TOL
+    assert relerr(J.cpu().numpy(), Jo) <= TOL
+    assert relerr(K.cpu().numpy(), Ko) <= TOL
+    h.close()
+
+
+@pytest.mark.parametrize("nao,naux", [(1, 2), (3, 4), (31, 6), (130, 9), (257, 5)])
+def test_dm_parity(dfjk, nao, naux):
+    Bp = make_B(nao, naux, 300 + nao)
+    dm = np.random.default_rng(nao).standard_normal((nao, nao))       # neither symmetric nor PSD
+    h = dfjk.DFJK(dev(Bp), nao)
+    J, K = h.get_jk_dm(dev(dm))
+    torch.cuda.synchronize()
+    Jo, Ko, _ = oracle.get_jk_dm(Bp, nao, dm)
+    assert relerr(J.cpu().numpy(), Jo) <= TOL
+    assert relerr(K.cpu().numpy(), Ko) <= TOL
+    h.close()
+
+
+def test_dm_batch_and_options(dfjk):
+    nao, naux = 150, 11
+    Bp = make_B(nao, naux, 7)
+    rng = np.random.default_rng(3)
+    dms = rng.standard_normal((3, nao, nao))
+    dms[1] = dms[1] + dms[1].T                                       # one symmetric member
+    h = dfjk.DFJK(dev(Bp), nao)
+    h.set_option("k_chunk", 3)                                       # several X chunks
+    h.set_option("k_splits", 2)
+    J, K = h.get_jk_dm(dev(dms))
+    torch.cuda.synchronize()
+    for i in range(3):
+        Jo, Ko, _ = oracle.get_jk_dm(Bp, nao, dms[i])
+        assert relerr(J[i].cpu().numpy(), Jo) <= TOL
+        assert relerr(K[i].cpu().numpy(), Ko) <= TOL
+    # J only / K only
+    Jonly, none = h.get_jk_dm(dev(dms[0]), with_k=False)
+    assert none is None and torch.equal(Jonly, J[0])
+    none, Konly = h.get_jk_dm(dev(dms[0]), with_j=False)
+    assert none is None and torch.equal(Konly, K[0])                 # deterministic: bitwise repeatable
+    h.close()
+
+
+def test_general_reduces_to_restricted(dfjk):
+    """pair(C, C) K == get_jk K; dm = 2 C C^T: same J, K[dm] = 2 K (reading R1)."""
+    cfg = gi.CONFIGS[1]
+    Bp = gi.fill_B_host(cfg)
+    C = gi.orbitals(cfg, 0)[0]
+    h = dfjk.DFJK(dev(Bp), cfg.nao)
+    J0, K0 = h.get_jk(dev(C))
+    Jp, Kp = h.get_jk_pair(dev(C), dev(C))
+    Jd, Kd = h.get_jk_dm(dev(2.0 * C @ C.T))
+    torch.cuda.synchronize()
+    assert relerr(Kp.cpu().numpy(), K0.cpu().numpy()) <= 1e-13
+    assert relerr(2.0 * Jp.cpu().numpy(), J0.cpu().numpy()) <= 1e-13
+    assert relerr(Jd.cpu().numpy(), J0.cpu().numpy()) <= 1e-13
+    assert relerr(Kd.cpu().numpy(), 2.0 * K0.cpu().numpy()) <= 1e-13
+    h.close()
+
+
+def test_general_after_restricted_call_shares_workspace(dfjk):
+    """Interleaved calls on one handle (different Ccat widths, split counts) stay correct."""
+    nao, naux = 140, 10
+    Bp = make_B(nao, naux, 21)
+    rng = np.random.default_rng(5)
+    C = gi.random_orbitals(nao, 12, 4)
+    C1, C2 = rng.standard_normal((nao, 5)), rng.standard_normal((nao, 5))
+    h = dfjk.DFJK(dev(Bp), nao)
+    for _ in range(2):
+        J, K = h.get_jk(dev(C))
+        Jp, Kp = h.get_jk_pair(dev(C1), dev(C2))
+    torch.cuda.synchronize()
+    Jo, Ko, _ = oracle.get_jk(Bp, nao, [C], [2.0])
+    Jpo, Kpo, _ = oracle.get_jk_pair(Bp, nao, C1, C2)
+    assert relerr(J.cpu().numpy(), Jo) <= TOL and relerr(K.cpu().numpy(), Ko[0]) <= TOL
+    assert relerr(Jp.cpu().numpy(), Jpo) <= TOL and relerr(Kp.cpu().numpy(), Kpo) <= TOL
+    h.close()
+
+
+def test_general_error_paths(dfjk):
+    nao, naux = 6, 3
+    h = dfjk.DFJK(dev(make_B(nao, naux, 1)), nao)
+    C = dev(np.ones((nao, 2)))
+    with pytest.raises(ValueError):
+        h.get_jk_pair(C, dev(np.ones((nao, 3))))
+    with pytest.raises(dfjk.DFJKError):
+        h.get_jk_pair(C, C, with_j=False, with_k=False)
+    with pytest.raises(ValueError):
+        h.get_jk_dm(dev(np.ones((nao, nao + 1))))
+    L = dfjk.lib()
+    assert L.dfjk_get_jk_pair(h._h, C.data_ptr(), None, 2, None, C.data_ptr(), None) == -1
+    assert L.dfjk_get_jk_pair(h._h, C.data_ptr(), C.data_ptr(), nao + 1, None, C.data_ptr(), None) == -1
+    assert L.dfjk_get_jk_dm(None, None, None, None, None) == -1
+    assert L.dfjk_get_jk_dms(h._h, 0, C.data_ptr(), C.data_ptr(), None, None) == -1
+    h.close()
