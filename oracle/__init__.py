@@ -68,6 +68,9 @@ def _load():
         lib.oracle_bruteforce_jk_dm.argtypes = [
             ctypes.c_int64, ctypes.c_int64, ctypes.c_void_p, ctypes.c_void_p,
             ctypes.c_void_p, ctypes.c_void_p]
+        lib.oracle_df_diag_slab.restype = ctypes.c_int
+        lib.oracle_df_diag_slab.argtypes = [ctypes.c_int64, ctypes.c_int64, ctypes.c_void_p,
+                                            ctypes.c_void_p]
         _lib = lib
     return _lib
 
@@ -283,3 +286,15 @@ def bruteforce_jk_dm(Bp: np.ndarray, nao: int, dm: np.ndarray):
     if rc != 0:
         raise RuntimeError(f"oracle_bruteforce_jk_dm failed: {rc}")
     return J, K
+
+
+def df_diag(Bp: np.ndarray, nao: int, out: Optional[np.ndarray] = None) -> np.ndarray:
+    """diag[m][n] (+)= sum_P B(P,m,n)^2 -- the DF term of Eq. 7.
+    Pass ``out`` to accumulate slab by slab."""
+    Bp = _f64c(Bp)
+    _check_inputs(Bp, nao, [])
+    diag = np.zeros((nao, nao)) if out is None else out
+    rc = _load().oracle_df_diag_slab(Bp.shape[0], nao, Bp.ctypes.data, diag.ctypes.data)
+    if rc != 0:
+        raise RuntimeError(f"oracle_df_diag_slab failed: {rc}")
+    return diag

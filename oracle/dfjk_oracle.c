@@ -561,3 +561,26 @@ int oracle_bruteforce_jk_dm(int64_t naux, int64_t nao, const double *Bp, const d
     free(eri);
     return ORACLE_OK;
 }
+
+/*
+ * oracle_df_diag_slab: the DF term of Eq. 7,
+ *     diag[m][n] += sum_{P in slab} B(P,m,n)^2        = (mn|mn) of Eq. 1 with kappa lambda = mu nu
+ * full square, accumulated over slabs.  Pinned (tests/test_oracle_general_pins.py) against the
+ * materialised eri[m][n][m][n] of oracle_bruteforce_jk, numpy, and the identity
+ * sum_n diag[m][n] = K[m][m] for C = I (K = sum_P B_P^2).
+ */
+int oracle_df_diag_slab(int64_t nrows, int64_t nao, const double *Bp_slab, double *diag)
+{
+    if (nrows < 0 || nao < 1 || !Bp_slab || !diag) return ORACLE_EINVAL;
+    const int64_t npair = nao * (nao + 1) / 2;
+    for (int64_t r = 0; r < nrows; ++r) {
+        const double *Bp_row = Bp_slab + r * npair;
+#pragma omp parallel for schedule(static)
+        for (int64_t m = 0; m < nao; ++m)
+            for (int64_t n = 0; n < nao; ++n) {
+                const double b = b_elem(Bp_row, m, n);
+                diag[m * nao + n] += b * b;
+            }
+    }
+    return ORACLE_OK;
+}

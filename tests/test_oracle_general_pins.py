@@ -168,3 +168,29 @@ def test_library_reduction_general(cfg_id):
     X1, X2 = Bf @ C1, Bf @ C2
     assert relerr(Kp, np.einsum("pmi,pni->mn", X1, X2)) < 1e-12
     assert relerr(Jp, np.einsum("p,pmn->mn", np.einsum("pls,ls->p", Bf, C1 @ C2.T), Bf)) < 1e-12
+
+
+# ---------------------------------------------------------------- Eq. 7 DF diagonal
+def test_df_diag_pins():
+    """oracle.df_diag against the materialised (mn|mn) of the brute force, numpy, the trace
+    identity and K[C = I]'s diagonal (K = sum_P B_P^2  =>  K[m][m] = sum_n diag[m][n])."""
+    nao, naux = 9, 6
+    Bp = rand_B(nao, naux, 23)
+    diag = oracle.df_diag(Bp, nao)
+    _, _, diag_bf = oracle.bruteforce_jk(Bp, nao, [np.eye(nao)], [2.0])
+    assert relerr(diag, diag_bf) < RTOL
+    Bf = unpack_np(Bp, nao)
+    assert relerr(diag, (Bf ** 2).sum(0)) < RTOL
+    assert np.array_equal(diag, diag.T)
+    assert abs(diag.sum() - sum(np.linalg.norm(Bf[p]) ** 2 for p in range(naux))) <= 1e-12 * diag.sum()
+    _, K, _ = oracle.get_jk(Bp, nao, [np.eye(nao)], [2.0])
+    assert relerr(diag.sum(1), np.diag(K[0])) < RTOL
+    # slab accumulation
+    acc = oracle.df_diag(Bp[:2], nao)
+    oracle.df_diag(Bp[2:], nao, out=acc)
+    assert relerr(acc, diag) < RTOL
+    # single-element probe
+    Bp1 = np.zeros((2, nao * (nao + 1) // 2)); Bp1[1, 4 * 5 // 2 + 2] = 3.0     # (mu, nu) = (4, 2)
+    d1 = oracle.df_diag(Bp1, nao)
+    ref = np.zeros((nao, nao)); ref[4, 2] = ref[2, 4] = 9.0
+    assert np.array_equal(d1, ref)
