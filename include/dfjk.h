@@ -143,6 +143,16 @@ int dfjk_get_jk_host(dfjk_handle *h, const double *C_occ_host, int64_t nocc,
                      double *J_host, double *K_host);
 
 /*
+ * dfjk_get_df_diag -- the DF term of the diagonal-error diagnostic, Eq. 7:
+ *     diag[mu][nu] = (mu nu|mu nu)_DF = sum_P T_{P,mu nu}^2
+ * (Delta of Eq. 7 is sum_{mu nu} [(mu nu|mu nu)_exact - diag[mu][nu]]; the exact integrals
+ * need an integral engine and are outside this library).  One streaming pass over B
+ * (HBM-bound, |B| bytes), same kernel as J2 with each element weighted by itself.
+ *   diag    DEVICE, nao x nao, OVERWRITTEN, both triangles written.
+ */
+int dfjk_get_df_diag(dfjk_handle *h, double *diag, void *stream);
+
+/*
  * dfjk_get_d -- debug/inspection getter: copies the naux fitting coefficients
  * d_P of the most recent J build on this handle into d_out (DEVICE, naux doubles),
  * enqueued on `stream`.  DFJK_EINVAL if no J has been built yet.

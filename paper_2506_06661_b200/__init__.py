@@ -29,7 +29,7 @@ SYMBOLS = (
     "dfjk_create", "dfjk_get_jk", "dfjk_get_jk_u", "dfjk_get_jk_host", "dfjk_get_d",
     "dfjk_set_option", "dfjk_workspace_bytes", "dfjk_destroy", "dfjk_last_error",
     "dfjk_version", "dfjk_launch_count", "dfjk_kernel_time",
-    "dfjk_get_jk_pair", "dfjk_get_jk_dm", "dfjk_get_jk_dms",
+    "dfjk_get_jk_pair", "dfjk_get_jk_dm", "dfjk_get_jk_dms", "dfjk_get_df_diag",
 )
 
 # DFJK_KERNEL_* ids of include/dfjk.h
@@ -72,6 +72,8 @@ def lib() -> ctypes.CDLL:
     L.dfjk_get_jk_dm.argtypes = [vp, vp, vp, vp, vp]
     L.dfjk_get_jk_dms.restype = ci
     L.dfjk_get_jk_dms.argtypes = [vp, i64, vp, vp, vp, vp]
+    L.dfjk_get_df_diag.restype = ci
+    L.dfjk_get_df_diag.argtypes = [vp, vp, vp]
     L.dfjk_get_jk_host.restype = ci
     L.dfjk_get_jk_host.argtypes = [vp, vp, i64, vp, vp]
     L.dfjk_get_d.restype = ci
@@ -225,6 +227,15 @@ class DFJK:
                                           K_host.data_ptr() if K_host is not None else None),
                    "dfjk_get_jk_host")
         return J_host, K_host
+
+    def get_df_diag(self, stream=None):
+        """diag[mu][nu] = sum_P B_P[mu,nu]^2, the DF term of Eq. 7."""
+        import torch
+        out = self._out(True)
+        with torch.cuda.device(self.device):
+            st = (stream or torch.cuda.current_stream(self.device)).cuda_stream
+            _check(lib().dfjk_get_df_diag(self._h, out.data_ptr(), st), "dfjk_get_df_diag")
+        return out
 
     def get_d(self, stream=None):
         """Fitting coefficients d_P of the most recent J build (debug getter)."""

@@ -390,6 +390,20 @@ extern "C" int dfjk_get_jk_u(dfjk_handle *h, const double *C_a, int64_t nocc_a, 
     return get_jk_impl(h, 2, C, no, w, J, Ks, (cudaStream_t)stream, "dfjk_get_jk_u");
 }
 
+extern "C" int dfjk_get_df_diag(dfjk_handle *h, double *diag, void *stream)
+{
+    g_err[0] = 0;
+    if (!h || !diag) return fail(DFJK_EINVAL, "dfjk_get_df_diag: NULL argument");
+    int dev = -1;
+    DFJK_CUDA_TRY(cudaGetDevice(&dev));
+    if (dev != h->device) return fail(DFJK_EINVAL, "dfjk_get_df_diag: handle belongs to device %d, current is %d", h->device, dev);
+    cudaStream_t st = (cudaStream_t)stream;
+    { Timed t_(h, DFJK_KERNEL_J2, st); dfjk::launch_j2_axpy(h->B, h->naux, h->npair, nullptr, h->Jp_part, h->j2_groups, st); }
+    { Timed t_(h, DFJK_KERNEL_J3, st); dfjk::launch_j3_unpack(h->Jp_part, h->j2_groups, h->npair, h->nao, diag, st); }
+    DFJK_CUDA_TRY(cudaGetLastError());
+    return DFJK_OK;
+}
+
 extern "C" int dfjk_get_d(dfjk_handle *h, double *d_out, void *stream)
 {
     g_err[0] = 0;

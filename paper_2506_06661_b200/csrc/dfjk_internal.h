@@ -36,7 +36,8 @@ void launch_j1_dot(const double *B, int64_t naux, int64_t npair, const double *D
 void launch_j1_reduce(const double *d_part, int64_t nchunk, int64_t naux, double *d,
                       cudaStream_t st);
 
-/* J2: Jp_part[g][pair] = sum_{P in row group g} d[P] B[P][pair];  ngroup = j2_num_groups(...). */
+/* J2: Jp_part[g][pair] = sum_{P in row group g} d[P] B[P][pair];  ngroup = j2_num_groups(...).
+ * d == NULL: the same stream with every element weighted by itself, sum_P B[P][pair]^2 (Eq. 7). */
 int64_t j2_num_groups(int64_t naux, int64_t npair, int sm_count);
 void launch_j2_axpy(const double *B, int64_t naux, int64_t npair, const double *d,
                     double *Jp_part, int64_t ngroup, cudaStream_t st);

@@ -160,13 +160,17 @@ __global__ void __launch_bounds__(J1_WARPS * 32)
 j1_dot_kernel(const double *__restrict__ B, int64_t naux, int64_t npair,
               const double *__restrict__ Dt, double *__restrict__ d_part)
 {
-    /* sDt[k] = Dt[c0 - 1 + k], k = 0 .. CH+1 (zero outside [c0, c1)) */
-    __shared__ double sDt[J1_CH + 2];
+    /* sDt[k] = Dt[c0 - 2 + k], k = 0 .. CH+3 (zero outside [c0, c1)): column c0 sits at the 16-B
+     * aligned index 2, so a row segment that starts on the 16-B grid of B (always, when npair is
+     * even) reads its Dt pairs with one conflict-free 128-bit shared load per 128-bit global load;
+     * two 64-bit loads at a 16-B lane stride would cost twice the shared-memory wavefronts
+     * (profiles/r01b: mio_throttle was J1's top stall). */
+    __shared__ __align__(16) double sDt[J1_CH + 4];
     const int64_t chunk = blockIdx.x;
     const int64_t c0 = chunk * J1_CH;
     const int64_t c1 = (c0 + J1_CH < npair) ? c0 + J1_CH : npair;
-    for (int k = threadIdx.x; k < J1_CH + 2; k += blockDim.x) {
-        const int64_t col = c0 - 1 + k;
+    for (int k = threadIdx.x; k < J1_CH + 4; k += blockDim.x) {
+        const int64_t col = c0 - 2 + k;
         sDt[k] = (col >= c0 && col < c1) ? Dt[col] : 0.0;
     }
     __syncthreads();
@@ -181,31 +185,53 @@ j1_dot_kernel(const double *__restrict__ B, int64_t naux, int64_t npair,
         double acc0 = 0.0, acc1 = 0.0;
         if (fa <= fb) {
             /* head / tail scalars */
-            if (lane == 0 && f0 < fa) acc0 += ldg_stream1(B + f0) * sDt[1];
-            if (lane == 1 && fb < f1) acc1 += ldg_stream1(B + fb) * sDt[fb - f0 + 1];
+            if (lane == 0 && f0 < fa) acc0 += ldg_stream1(B + f0) * sDt[2];
+            if (lane == 1 && fb < f1) acc1 += ldg_stream1(B + fb) * sDt[fb - f0 + 2];
             const int64_t nvec = (fb - fa) >> 1;
             const double *bp = B + fa;
-            const double *sp = sDt + (fa - f0 + 1);
+            const double *sp = sDt + (fa - f0 + 2);
             int64_t v = lane;
-            for (; v + 32 * (J1_UNROLL - 1) < nvec; v += 32 * J1_UNROLL) {
-                double2 b[J1_UNROLL];
+            if (fa == f0) {
+                /* aligned segment: 128-bit shared loads */
+                const double2 *sp2 = reinterpret_cast<const double2 *>(sp);
+                for (; v + 32 * (J1_UNROLL - 1) < nvec; v += 32 * J1_UNROLL) {
+                    double2 b[J1_UNROLL];
 #pragma unroll
-                for (int u = 0; u < J1_UNROLL; ++u) b[u] = ldg_stream2(bp + 2 * (v + 32 * u));
+                    for (int u = 0; u < J1_UNROLL; ++u) b[u] = ldg_stream2(bp + 2 * (v + 32 * u));
 #pragma unroll
-                for (int u = 0; u < J1_UNROLL; ++u) {
-                    const int64_t k = 2 * (v + 32 * u);
-                    acc0 += b[u].x * sp[k];
-                    acc1 += b[u].y * sp[k + 1];
+                    for (int u = 0; u < J1_UNROLL; ++u) {
+                        const double2 t = sp2[v + 32 * u];
+                        acc0 += b[u].x * t.x;
+                        acc1 += b[u].y * t.y;
+                    }
                 }
-            }
-            for (; v < nvec; v += 32) {
-                const double2 b = ldg_stream2(bp + 2 * v);
-                acc0 += b.x * sp[2 * v];
-                acc1 += b.y * sp[2 * v + 1];
+                for (; v < nvec; v += 32) {
+                    const double2 b = ldg_stream2(bp + 2 * v);
+                    const double2 t = sp2[v];
+                    acc0 += b.x * t.x;
+                    acc1 += b.y * t.y;
+                }
+            } else {
+                for (; v + 32 * (J1_UNROLL - 1) < nvec; v += 32 * J1_UNROLL) {
+                    double2 b[J1_UNROLL];
+#pragma unroll
+                    for (int u = 0; u < J1_UNROLL; ++u) b[u] = ldg_stream2(bp + 2 * (v + 32 * u));
+#pragma unroll
+                    for (int u = 0; u < J1_UNROLL; ++u) {
+                        const int64_t k = 2 * (v + 32 * u);
+                        acc0 += b[u].x * sp[k];
+                        acc1 += b[u].y * sp[k + 1];
+                    }
+                }
+                for (; v < nvec; v += 32) {
+                    const double2 b = ldg_stream2(bp + 2 * v);
+                    acc0 += b.x * sp[2 * v];
+                    acc1 += b.y * sp[2 * v + 1];
+                }
             }
         } else {
             /* segment of a single element straddling the 16-B grid */
-            if (lane == 0) acc0 += ldg_stream1(B + f0) * sDt[1];
+            if (lane == 0) acc0 += ldg_stream1(B + f0) * sDt[2];
         }
         double acc = acc0 + acc1;
 #pragma unroll
@@ -228,6 +254,10 @@ __global__ void j1_reduce_kernel(const double *__restrict__ d_part, int64_t nchu
 constexpr int J2_THREADS = 256;
 constexpr int J2_UNROLL = 8;
 
+/* SQ == false: J2 proper, Jp_part[g][pair] = sum_{P in group g} d[P] B[P][pair].
+ * SQ == true : the DF diagonal of Eq. 7, sum_P B[P][pair]^2 -- the same stream
+ *              with each element weighted by itself (d is not read). */
+template <bool SQ>
 __global__ void __launch_bounds__(J2_THREADS)
 j2_axpy_kernel(const double *__restrict__ B, int64_t naux, int64_t npair,
                const double *__restrict__ d, double *__restrict__ Jp_part, int64_t ngroup)
@@ -250,24 +280,27 @@ j2_axpy_kernel(const double *__restrict__ B, int64_t naux, int64_t npair,
 #pragma unroll
             for (int u = 0; u < J2_UNROLL; ++u) {
                 b[u] = ldg_stream2(bp + (P + u * ngroup) * npair);
-                dv[u] = __ldg(d + P + u * ngroup);
+                dv[u] = SQ ? 0.0 : __ldg(d + P + u * ngroup);
             }
 #pragma unroll
             for (int u = 0; u < J2_UNROLL; ++u) {
-                ax += dv[u] * b[u].x;
-                ay += dv[u] * b[u].y;
+                ax += (SQ ? b[u].x : dv[u]) * b[u].x;
+                ay += (SQ ? b[u].y : dv[u]) * b[u].y;
             }
         }
         for (; P < naux; P += ngroup) {
             const double2 b = ldg_stream2(bp + P * npair);
-            const double dv = __ldg(d + P);
-            ax += dv * b.x;
-            ay += dv * b.y;
+            const double dv = SQ ? 0.0 : __ldg(d + P);
+            ax += (SQ ? b.x : dv) * b.x;
+            ay += (SQ ? b.y : dv) * b.y;
         }
     } else {
         const int64_t col = okx ? colx : coly;
         double a = 0.0;
-        for (int64_t P = g; P < naux; P += ngroup) a += __ldg(d + P) * ldg_stream1(B + P * npair + col);
+        for (int64_t P = g; P < naux; P += ngroup) {
+            const double b = ldg_stream1(B + P * npair + col);
+            a += (SQ ? b : __ldg(d + P)) * b;
+        }
         if (okx) ax = a; else ay = a;
     }
     double *out = Jp_part + g * npair;
@@ -377,8 +410,12 @@ void launch_j2_axpy(const double *B, int64_t naux, int64_t npair, const double *
 {
     const int64_t nvec = (npair + 1) / 2 + 1;               /* one spare vector for shifted rows */
     const unsigned nbx = (unsigned)((nvec + J2_THREADS - 1) / J2_THREADS);
-    j2_axpy_kernel<<<dim3(nbx, (unsigned)ngroup), J2_THREADS, 0, st>>>(B, naux, npair, d, Jp_part,
-                                                                       ngroup);
+    if (d)
+        j2_axpy_kernel<false><<<dim3(nbx, (unsigned)ngroup), J2_THREADS, 0, st>>>(B, naux, npair, d,
+                                                                                  Jp_part, ngroup);
+    else    /* d == NULL: Eq. 7's DF diagonal, sum_P B[P][pair]^2 */
+        j2_axpy_kernel<true><<<dim3(nbx, (unsigned)ngroup), J2_THREADS, 0, st>>>(B, naux, npair, nullptr,
+                                                                                 Jp_part, ngroup);
 }
 
 void launch_j3_unpack(const double *Jp_part, int64_t ngroup, int64_t npair, int64_t nao, double *J,

@@ -153,3 +153,14 @@ def test_general_error_paths(dfjk):
     assert L.dfjk_get_jk_dm(None, None, None, None, None) == -1
     assert L.dfjk_get_jk_dms(h._h, 0, C.data_ptr(), C.data_ptr(), None, None) == -1
     h.close()
+
+
+@pytest.mark.parametrize("nao,naux", [(1, 1), (5, 7), (64, 16), (129, 12), (290, 60)])
+def test_df_diag_parity(dfjk, nao, naux):
+    """Eq. 7's DF diagonal sum_P B_Pmn^2 against the oracle."""
+    Bp = make_B(nao, naux, 500 + nao)
+    h = dfjk.DFJK(dev(Bp), nao)
+    diag = h.get_df_diag()
+    torch.cuda.synchronize()
+    assert relerr(diag.cpu().numpy(), oracle.df_diag(Bp, nao)) <= TOL
+    h.close()
