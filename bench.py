@@ -168,7 +168,9 @@ def run_reference(args, cfg):
 
 
 def workload_config(cfg, args):
-    return {"workload": f"BASELINE.json configs[{cfg.index - 1}] '{cfg.name}': nao={cfg.nao} "
+    origin = (f"BASELINE.json configs[{cfg.index - 1}]" if cfg.index <= 5 else
+              "LRDF-shaped workload (PAPER.md:433-450, naux = nao/10; not a BASELINE config)")
+    return {"workload": f"{origin} '{cfg.name}': nao={cfg.nao} "
                         f"naux={cfg.naux} nocc={'+'.join(map(str, cfg.nocc))} seed={cfg.seed}",
             "nao": cfg.nao, "naux": cfg.naux, "nocc": list(cfg.nocc),
             "b_bytes": cfg.b_bytes, "calls_per_step": 1,

@@ -62,6 +62,9 @@ CONFIGS = {
     3: Config(3, "medium", 2, 800, 2600, (66,), 10, "rotate"),
     4: Config(4, "large", 3, 1600, 5000, (130,), 5, "rotate"),
     5: Config(5, "unrestricted", 4, 2000, 6000, (170, 160), 3, "rotate"),
+    # not a BASELINE.json config: the LRDF shape of PAPER.md:433-450 ("the auxiliary dimension
+    # needed is approximately only 1/10 of the size of the orbital basis"): few, long rows
+    6: Config(6, "lrdf-shape", 5, 4000, 400, (330,), 3, "rotate"),
 }
 
 

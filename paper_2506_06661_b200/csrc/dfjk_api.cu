@@ -166,7 +166,12 @@ extern "C" dfjk_handle *dfjk_create(int64_t naux, int64_t nao, const double *B_p
     h->x_doubles = xd;
     const int nb = (int)((nao + 127) / 128);
     h->nsplit_default = choose_splits(nb * (nb + 1) / 2, h->sm_count, 32);
-    h->nsplit_alloc = 32;
+    /* partial-K slots: what the two automatic choices (lower tiles; all tiles for the general
+     * product) need, at least 8 for the "k_splits" option -- 2*32 slots would be 8 GB at nao=4000 */
+    h->nsplit_alloc = h->nsplit_default;
+    if (choose_splits(nb * nb, h->sm_count, 32) > h->nsplit_alloc)
+        h->nsplit_alloc = choose_splits(nb * nb, h->sm_count, 32);
+    if (h->nsplit_alloc < 8) h->nsplit_alloc = 8;
 
     int rc = DFJK_OK;
     if (rc == DFJK_OK) rc = alloc_ws(h, &h->Ccat, round_up(nao, 32) * h->ldc_max);

@@ -31,7 +31,7 @@ def relerr(a, b):
 
 def sample_rows(nao):
     edge = [0, 1, 63, 64, 127, 128, 129, 255, 256, 511, 512, 1023, 1024, 1151, 1152,
-            1535, 1536, 1599, 1600, 1919, 1920, nao - 2, nao - 1]
+            1535, 1536, 1599, 1600, 1919, 1920, 3967, 3968, nao - 2, nao - 1]
     rng = np.random.default_rng(nao)
     rows = sorted({r for r in edge if 0 <= r < nao} | set(rng.integers(0, nao, 9).tolist()))
     return rows
@@ -98,3 +98,22 @@ def test_cfg4_large_headline():
 
 def test_cfg5_unrestricted():
     run_config(5, full_k=False)
+
+
+def test_cfg6_lrdf_shape():
+    """naux = nao/10: few, long rows -- 32 x 32 K tiles, 9 X chunks of 49 rows,
+    1955 J1 column chunks over only 400 rows; plus Eq. 7's DF diagonal at this size."""
+    import paper_2506_06661_b200 as pkg
+    run_config(6, full_k=False)
+    cfg = gi.CONFIGS[6]
+    B = torch.empty(cfg.naux, cfg.npair, dtype=torch.float64, device="cuda")
+    gi.fill_B_device(cfg, B)
+    h = pkg.DFJK(B, cfg.nao)
+    diag = h.get_df_diag()
+    torch.cuda.synchronize()
+    ref = np.zeros((cfg.nao, cfg.nao))
+    slab = max(1, SLAB_BYTES // (cfg.npair * 8))
+    for P0 in range(0, cfg.naux, slab):
+        oracle.df_diag(B[P0:P0 + slab].cpu().numpy(), cfg.nao, out=ref)
+    h.close()
+    assert relerr(diag.cpu().numpy(), ref) <= TOL
