@@ -29,7 +29,7 @@ _DEV_LIB = os.path.join(_HERE, "libdfjk_gen_device.so")
 _host = None
 _dev = None
 
-STREAM_X, STREAM_A, STREAM_Z, STREAM_C, STREAM_ROT = 0, 1, 2, 10, 1000
+STREAM_X, STREAM_A, STREAM_Z, STREAM_Y, STREAM_C, STREAM_ROT = 0, 1, 2, 3, 10, 1000
 
 
 @dataclass(frozen=True)
@@ -233,3 +233,15 @@ def random_orbitals(nao: int, nocc: int, seed: int, orthonormal: bool = True) ->
     """A free-standing nao x nocc block for tests (optionally NOT orthonormal, reading R8)."""
     M = normals(seed, STREAM_C, nao * nocc).reshape(nao, nocc)
     return _orth(M) if orthonormal else np.ascontiguousarray(M)
+
+
+def metric(cfg: Config) -> np.ndarray:
+    """Synthetic auxiliary metric M_PQ of Eq. 2, naux x naux, symmetric
+    positive definite and moderately conditioned (the real Coulomb metric needs an integral engine):
+        y_P = U(0,10) (stream 3),   M_PQ = exp(-|y_P - y_Q| / 2) + 0.1 delta_PQ
+    (an exponential kernel is positive definite; the 0.1 ridge bounds cond(M) by ~(1+naux)/0.1).
+    The raw 3-centre tensor (Q|mu nu) of Eq. 3 is ``fill_B_host`` / ``fill_B_device`` unchanged."""
+    y = 10.0 * uniform(cfg.seed, STREAM_Y, cfg.naux)
+    M = np.exp(-np.abs(y[:, None] - y[None, :]) / 2.0)
+    M[np.diag_indices(cfg.naux)] += 0.1
+    return np.ascontiguousarray(M)

@@ -71,6 +71,11 @@ def _load():
         lib.oracle_df_diag_slab.restype = ctypes.c_int
         lib.oracle_df_diag_slab.argtypes = [ctypes.c_int64, ctypes.c_int64, ctypes.c_void_p,
                                             ctypes.c_void_p]
+        lib.oracle_cholesky_lower.restype = ctypes.c_int
+        lib.oracle_cholesky_lower.argtypes = [ctypes.c_int64, ctypes.c_void_p, ctypes.c_void_p]
+        lib.oracle_whiten.restype = ctypes.c_int
+        lib.oracle_whiten.argtypes = [ctypes.c_int64, ctypes.c_int64, ctypes.c_void_p,
+                                      ctypes.c_void_p, ctypes.c_void_p]
         _lib = lib
     return _lib
 
@@ -298,3 +303,35 @@ def df_diag(Bp: np.ndarray, nao: int, out: Optional[np.ndarray] = None) -> np.nd
     if rc != 0:
         raise RuntimeError(f"oracle_df_diag_slab failed: {rc}")
     return diag
+
+
+# ---------------------------------------------------------------- building B (Eq. 2-3)
+def cholesky_lower(M: np.ndarray) -> np.ndarray:
+    """L with M = L L^T (Eq. 2), textbook recurrence; raises if M is not SPD."""
+    M = _f64c(M)
+    if M.ndim != 2 or M.shape[0] != M.shape[1]:
+        raise ValueError("M must be square")
+    L = np.zeros_like(M)
+    rc = _load().oracle_cholesky_lower(M.shape[0], M.ctypes.data, L.ctypes.data)
+    if rc != 0:
+        raise RuntimeError(f"oracle_cholesky_lower failed: {rc} (not positive definite?)")
+    return L
+
+
+def whiten(L: np.ndarray, R: np.ndarray) -> np.ndarray:
+    """B = L^-1 R by forward substitution per column (Eq. 3).
+    R is [naux][ncols] (the packed raw 3-centre tensor (Q|mu nu))."""
+    L, R = _f64c(L), _f64c(R)
+    if R.ndim != 2 or L.shape != (R.shape[0], R.shape[0]):
+        raise ValueError("L must be naux x naux and R naux x ncols")
+    B = np.empty_like(R)
+    rc = _load().oracle_whiten(R.shape[0], R.shape[1], L.ctypes.data, R.ctypes.data, B.ctypes.data)
+    if rc != 0:
+        raise RuntimeError(f"oracle_whiten failed: {rc}")
+    return B
+
+
+def build_b(M: np.ndarray, R: np.ndarray):
+    """Eq. 2-3 together: returns (L, B)."""
+    L = cholesky_lower(M)
+    return L, whiten(L, R)

@@ -584,3 +584,60 @@ int oracle_df_diag_slab(int64_t nrows, int64_t nao, const double *Bp_slab, doubl
     }
     return ORACLE_OK;
 }
+
+/* ======================================================================================
+ * Building the whitened tensor -- PAPER.md:353-356, Eq. 2-3:
+ *
+ *     M_PQ = (chi_P|chi_Q) = L L^T                                            (Eq. 2)
+ *     T_{P,mu nu} = sum_Q (L^-1)_{PQ} (chi_Q|mu nu)                            (Eq. 3)
+ *
+ * T is this library's B.  The oracle follows the two equations literally: the textbook
+ * Cholesky-Banachiewicz recurrence for L (row by row), then, for every packed column, the
+ * forward substitution that applies L^-1 (no explicit inverse, no blocking).
+ * ====================================================================================== */
+#include <math.h>
+
+/*
+ * oracle_cholesky_lower: L (n x n row-major, lower triangle; the strict upper triangle is set
+ * to 0) with M = L L^T, M symmetric positive definite (only its lower triangle is read):
+ *     L[i][j] = ( M[i][j] - sum_{k<j} L[i][k] L[j][k] ) / L[j][j]      j < i
+ *     L[i][i] = sqrt( M[i][i] - sum_{k<i} L[i][k]^2 )
+ * Returns ORACLE_EINVAL and stops at the first non-positive pivot.
+ */
+int oracle_cholesky_lower(int64_t n, const double *M, double *L)
+{
+    if (n < 1 || !M || !L) return ORACLE_EINVAL;
+    for (int64_t i = 0; i < n * n; ++i) L[i] = 0.0;
+    for (int64_t i = 0; i < n; ++i) {
+        for (int64_t j = 0; j <= i; ++j) {
+            double s = M[i * n + j];
+            for (int64_t k = 0; k < j; ++k) s -= L[i * n + k] * L[j * n + k];
+            if (i == j) {
+                if (!(s > 0.0)) return ORACLE_EINVAL;
+                L[i * n + i] = sqrt(s);
+            } else {
+                L[i * n + j] = s / L[j * n + j];
+            }
+        }
+    }
+    return ORACLE_OK;
+}
+
+/*
+ * oracle_whiten: B[P][c] = sum_Q (L^-1)[P][Q] R[Q][c] for every column c < ncols (Eq. 3), by
+ * forward substitution  B[P][c] = ( R[P][c] - sum_{Q<P} L[P][Q] B[Q][c] ) / L[P][P].
+ * R and B are naux x ncols row-major (ncols = npair for the packed tensor); B may alias R.
+ */
+int oracle_whiten(int64_t naux, int64_t ncols, const double *L, const double *R, double *B)
+{
+    if (naux < 1 || ncols < 1 || !L || !R || !B) return ORACLE_EINVAL;
+#pragma omp parallel for schedule(static)
+    for (int64_t c = 0; c < ncols; ++c) {
+        for (int64_t P = 0; P < naux; ++P) {
+            double s = R[P * ncols + c];
+            for (int64_t Q = 0; Q < P; ++Q) s -= L[P * naux + Q] * B[Q * ncols + c];
+            B[P * ncols + c] = s / L[P * naux + P];
+        }
+    }
+    return ORACLE_OK;
+}
