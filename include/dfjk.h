@@ -143,6 +143,32 @@ int dfjk_get_jk_host(dfjk_handle *h, const double *C_occ_host, int64_t nocc,
                      double *J_host, double *K_host);
 
 /*
+ * dfjk_build_b -- build the whitened tensor on the device,
+ * PAPER.md:353-356, Eq. 2-3:
+ *     M_PQ = (chi_P|chi_Q) = L L^T                              Eq. 2
+ *     T_{P,mu nu} = sum_Q (L^-1)_{PQ} (chi_Q|mu nu)             Eq. 3      (T is this library's B)
+ *
+ *   naux, nao  as in dfjk_create;  npair = nao*(nao+1)/2
+ *   M          DEVICE, naux x naux row-major, symmetric positive definite.  Only the lower
+ *              triangle is read.  OVERWRITTEN: on exit the lower triangle holds L; the strict
+ *              upper triangle is left as it was, except inside the 128 x 128 diagonal blocks,
+ *              where it is zeroed.  16-byte aligned.
+ *   R_packed   DEVICE, naux x npair, the raw 3-centre tensor (Q|mu nu), packed like B_packed.
+ *              OVERWRITTEN IN PLACE by B = L^-1 R (the tensor is up to 96 GB: no second copy).
+ *              16-byte aligned.  Pass the result to dfjk_create.
+ *   info       DEVICE int64 flag or NULL: 0 on success, j+1 if pivot j of the Cholesky
+ *              factorisation was not positive (LAPACK's convention; B is then garbage).
+ *   stream     cudaStream_t; the call only enqueues (workspace of ~naux^2 doubles comes from
+ *              the stream-ordered allocator, cudaMallocAsync / cudaFreeAsync).
+ *
+ * Cost: naux^2 npair flop for the solve (3.2e13 at naux=5000, nao=1600; FP64 DMMA, in place,
+ * block row by block row) + naux^3/3 for the factorisation.  The integrals (chi_P|chi_Q) and
+ * (chi_Q|mu nu) themselves need an integral engine and are inputs here.
+ */
+int dfjk_build_b(int64_t naux, int64_t nao, double *M, double *R_packed, int64_t *info,
+                 void *stream);
+
+/*
  * dfjk_get_df_diag -- the DF term of the diagonal-error diagnostic, Eq. 7:
  *     diag[mu][nu] = (mu nu|mu nu)_DF = sum_P T_{P,mu nu}^2
  * (Delta of Eq. 7 is sum_{mu nu} [(mu nu|mu nu)_exact - diag[mu][nu]]; the exact integrals

@@ -17,7 +17,7 @@ import os
 import subprocess
 from typing import Optional, Tuple
 
-__all__ = ["build", "lib", "DFJK", "DFJKError", "SYMBOLS", "KERNELS", "LIB_PATH", "HEADER_PATH"]
+__all__ = ["build", "lib", "build_b", "DFJK", "DFJKError", "SYMBOLS", "KERNELS", "LIB_PATH", "HEADER_PATH"]
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libdfjk.so")
@@ -30,6 +30,7 @@ SYMBOLS = (
     "dfjk_set_option", "dfjk_workspace_bytes", "dfjk_destroy", "dfjk_last_error",
     "dfjk_version", "dfjk_launch_count", "dfjk_kernel_time",
     "dfjk_get_jk_pair", "dfjk_get_jk_dm", "dfjk_get_jk_dms", "dfjk_get_df_diag",
+    "dfjk_build_b",
 )
 
 # DFJK_KERNEL_* ids of include/dfjk.h
@@ -72,6 +73,8 @@ def lib() -> ctypes.CDLL:
     L.dfjk_get_jk_dm.argtypes = [vp, vp, vp, vp, vp]
     L.dfjk_get_jk_dms.restype = ci
     L.dfjk_get_jk_dms.argtypes = [vp, i64, vp, vp, vp, vp]
+    L.dfjk_build_b.restype = ci
+    L.dfjk_build_b.argtypes = [i64, i64, vp, vp, vp, vp]
     L.dfjk_get_df_diag.restype = ci
     L.dfjk_get_df_diag.argtypes = [vp, vp, vp]
     L.dfjk_get_jk_host.restype = ci
@@ -109,6 +112,25 @@ def _dev_f64(t, name: str, numel: Optional[int] = None):
     if numel is not None and t.numel() != numel:
         raise ValueError(f"{name} has {t.numel()} elements, expected {numel}")
     return t.data_ptr()
+
+
+def build_b(M, R_packed, nao: int, stream=None):
+    """Eq. 2-3 on the device, IN PLACE: ``M`` (naux x naux, SPD) becomes its
+    Cholesky factor L (lower triangle), ``R_packed`` ([naux][npair] raw 3-centre tensor) becomes
+    B = L^-1 R.  Returns the device int64 ``info`` flag (0 = ok, j+1 = pivot j not positive)."""
+    import torch
+    nao = int(nao)
+    naux = int(R_packed.shape[0])
+    if R_packed.dim() != 2 or R_packed.shape[1] != nao * (nao + 1) // 2:
+        raise ValueError("R_packed must be [naux][nao(nao+1)/2]")
+    if M.dim() != 2 or tuple(M.shape) != (naux, naux):
+        raise ValueError("M must be naux x naux")
+    mp, rp = _dev_f64(M, "M"), _dev_f64(R_packed, "R_packed")
+    with torch.cuda.device(R_packed.device):
+        info = torch.zeros(1, dtype=torch.int64, device=R_packed.device)
+        st = (stream or torch.cuda.current_stream(R_packed.device)).cuda_stream
+        _check(lib().dfjk_build_b(naux, nao, mp, rp, info.data_ptr(), st), "dfjk_build_b")
+    return info
 
 
 class DFJK:

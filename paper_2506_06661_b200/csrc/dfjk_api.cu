@@ -13,6 +13,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <initializer_list>
 #include <new>
 
 namespace {
@@ -393,6 +394,38 @@ extern "C" int dfjk_get_jk_u(dfjk_handle *h, const double *C_a, int64_t nocc_a, 
     const double w[2] = {1.0, 1.0};
     double *Ks[2] = {K_a, K_b};
     return get_jk_impl(h, 2, C, no, w, J, Ks, (cudaStream_t)stream, "dfjk_get_jk_u");
+}
+
+extern "C" int dfjk_build_b(int64_t naux, int64_t nao, double *M, double *R_packed, int64_t *info,
+                            void *stream)
+{
+    g_err[0] = 0;
+    if (naux < 1 || nao < 1 || nao > 46340) return fail(DFJK_EINVAL, "dfjk_build_b: naux and nao must be >= 1");
+    if (!M || !R_packed) return fail(DFJK_EINVAL, "dfjk_build_b: NULL pointer");
+    if (((uintptr_t)R_packed & 15) != 0 || ((uintptr_t)M & 15) != 0)
+        return fail(DFJK_EINVAL, "dfjk_build_b: M and R_packed must be 16-byte aligned");
+    for (const void *p : {(const void *)M, (const void *)R_packed}) {
+        cudaPointerAttributes pa;
+        const cudaError_t e = cudaPointerGetAttributes(&pa, p);
+        if (e != cudaSuccess || (pa.type != cudaMemoryTypeDevice && pa.type != cudaMemoryTypeManaged)) {
+            cudaGetLastError();
+            return fail(DFJK_EINVAL, "dfjk_build_b: M / R_packed is not a device pointer (no CPU fallback)");
+        }
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    const int64_t npair = nao * (nao + 1) / 2;
+    double *ws = nullptr;
+    const size_t bytes = (size_t)dfjk::build_b_workspace_doubles(naux) * sizeof(double);
+    cudaError_t e = cudaMallocAsync((void **)&ws, bytes, st);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return fail(DFJK_ENOMEM, "dfjk_build_b: cudaMallocAsync of %zu bytes: %s", bytes, cudaGetErrorString(e));
+    }
+    static_assert(sizeof(long long) == sizeof(int64_t), "info is a 64-bit flag");
+    e = dfjk::launch_build_b(naux, npair, M, R_packed, ws, (long long *)info, st);
+    cudaFreeAsync(ws, st);
+    if (e != cudaSuccess) return fail(DFJK_ECUDA, "dfjk_build_b: %s", cudaGetErrorString(e));
+    return DFJK_OK;
 }
 
 extern "C" int dfjk_get_df_diag(dfjk_handle *h, double *diag, void *stream)

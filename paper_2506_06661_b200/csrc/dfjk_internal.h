@@ -80,5 +80,14 @@ void launch_k3_sum(const double *Kpart, int nsplit, int64_t nao, double *K, cuda
 /* K3: K[mu][nu] = K[nu][mu] = sum_split Kpart[split][mu][nu], mu >= nu. */
 void launch_k3_finish(const double *Kpart, int nsplit, int64_t nao, double *K, cudaStream_t st);
 
+/* ---------------------------------------------------------------- building B (Eq. 2-3) */
+
+/* Workspace (doubles) and launch sequence of dfjk_build_b: M = L L^T in place (lower triangle),
+ * T (packed R, naux x npair) overwritten by B = L^-1 R.  info: device flag (0 ok, j+1 = first
+ * non-positive pivot) or NULL. */
+int64_t build_b_workspace_doubles(int64_t naux);
+cudaError_t launch_build_b(int64_t naux, int64_t npair, double *M, double *T, double *ws,
+                           long long *info, cudaStream_t st);
+
 }  // namespace dfjk
 #endif

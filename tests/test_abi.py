@@ -41,6 +41,9 @@ def test_version_and_null_handling(L):
     assert L.dfjk_get_jk_dm(None, None, None, None, None) == -1
     assert L.dfjk_get_jk_dms(None, 1, None, None, None, None) == -1
     assert L.dfjk_get_df_diag(None, None, None) == -1
+    assert L.dfjk_build_b(0, 4, None, None, None, None) == -1
+    assert L.dfjk_build_b(4, 4, None, None, None, None) == -1
+    assert b"NULL" in L.dfjk_last_error()
 
 
 def test_create_rejects_bad_arguments_without_touching_memory(L):
