@@ -327,6 +327,76 @@ def run_ours(args, cfg):
         dist.destroy_process_group()
 
 
+def run_extra(args, cfg):
+    """--op build_b | pair | dm | diag: the section-8f rows, timed alone with CUDA events (one JSON
+    line, same keys as the main line where they apply; no cpu_baseline / e2e legs)."""
+    import torch
+    import paper_2506_06661_b200 as pkg
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    pkg.lib()
+    B = torch.empty(cfg.naux, cfg.npair, dtype=torch.float64, device=dev)
+    gi.fill_B_device(cfg, B)
+    nao, naux, nocc = cfg.nao, cfg.naux, cfg.nocc[0]
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+          for _ in range(args.steps)]
+    sampler = ClockSampler(0)
+    if args.op == "build_b":
+        Mh = torch.from_numpy(gi.metric(cfg)).pin_memory()
+        Md = torch.empty(naux, naux, dtype=torch.float64, device=dev)
+        flops = float(naux) ** 2 * cfg.npair + float(naux) ** 3 / 3.0
+        what = "dfjk_build_b: Cholesky of the metric + in-place whitening (Eq. 2-3)"
+
+        def prep():
+            Md.copy_(Mh, non_blocking=True)
+            gi.fill_B_device(cfg, B)                 # R is overwritten in place: regenerate it
+
+        def run():
+            pkg.build_b(Md, B, nao)
+    else:
+        h = pkg.DFJK(B, nao)
+        rng = np.random.default_rng(cfg.seed)
+        if args.op == "pair":
+            C1 = torch.from_numpy(rng.standard_normal((nao, nocc))).to(dev)
+            C2 = torch.from_numpy(rng.standard_normal((nao, nocc))).to(dev)
+            flops = flops_j(cfg) + 2.0 * naux * nao ** 2 * (2 * nocc) + 2.0 * naux * nao ** 2 * nocc
+            what = f"dfjk_get_jk_pair, ncol={nocc}: J[C1 C2^T] + K = sum_P (B_P C1)(B_P C2)^T"
+            run = lambda: h.get_jk_pair(C1, C2)
+        elif args.op == "dm":
+            dm = torch.from_numpy(rng.standard_normal((nao, nao))).to(dev)
+            flops = flops_j(cfg) + 2.0 * naux * nao ** 3 + 2.0 * naux * nao ** 3
+            what = "dfjk_get_jk_dm: J[dm], K[dm] = sum_P B_P dm B_P for a raw nao x nao dm"
+            run = lambda: h.get_jk_dm(dm)
+        else:
+            flops = 2.0 * naux * cfg.npair
+            what = "dfjk_get_df_diag: sum_P B_Pmn^2 (Eq. 7), one pass over B"
+            run = lambda: h.get_df_diag()
+        prep = lambda: None
+    for _ in range(max(args.warmup, 1)):
+        prep(); run()
+    torch.cuda.synchronize()
+    sampler.start()
+    for k in range(args.steps):
+        prep()
+        ev[k][0].record()
+        run()
+        ev[k][1].record()
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    ms = [a.elapsed_time(b) for a, b in ev]
+    t = float(np.mean(ms))
+    out = {"metric": f"df_{args.op}_gflops_fp64", "value": flops / (t * 1e-3) / 1e9, "unit": "GFLOP/s",
+           "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "ms_per_step": t,
+           "higher_is_better": True, "dtype": "f64", "data": "synthetic", "op": what,
+           "config": workload_config(cfg, args), "clocks": clocks, "step_ms": ms,
+           "algorithmic_flops": flops}
+    if args.op == "diag":
+        out["gbs"] = cfg.b_bytes / (t * 1e-3) / 1e9
+    else:
+        out["frac_fp64_peak"] = flops / (t * 1e-3) / 1e12 / FP64_PEAK_TFLOPS
+    print(json.dumps(out))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -334,12 +404,16 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=4, choices=sorted(gi.CONFIGS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--op", default="get_jk", choices=["get_jk", "build_b", "pair", "dm", "diag"],
+                    help="get_jk (default, the contract line) or one of the section-8f rows")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         print("bench.py: warning: fewer than 3 warm-up steps", file=sys.stderr)
     cfg = gi.CONFIGS[args.config]
     if args.impl == "reference":
         run_reference(args, cfg)
+    elif args.op != "get_jk":
+        run_extra(args, cfg)
     else:
         run_ours(args, cfg)
 

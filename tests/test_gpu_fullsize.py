@@ -117,3 +117,35 @@ def test_cfg6_lrdf_shape():
         oracle.df_diag(B[P0:P0 + slab].cpu().numpy(), cfg.nao, out=ref)
     h.close()
     assert relerr(diag.cpu().numpy(), ref) <= TOL
+
+
+def test_cfg4_build_b_sampled_columns():
+    """dfjk_build_b at the headline size (naux=5000, nao=1600, R = 51 GB in place): L against the
+    oracle's Cholesky in full; B on sampled packed columns, each computed by the oracle's forward
+    substitution one by one (columns of Eq. 3 are independent), spanning the first / last column
+    tiles, tile edges and the element-wise edge tile; every row block is covered by each column."""
+    import paper_2506_06661_b200 as pkg
+    cfg = gi.CONFIGS[4]
+    free, _ = torch.cuda.mem_get_info()
+    if free < cfg.b_bytes + (6 << 30):
+        pytest.skip(f"needs {cfg.b_bytes / 1e9:.0f} GB of free device memory")
+    M = gi.metric(cfg)
+    R = torch.empty(cfg.naux, cfg.npair, dtype=torch.float64, device="cuda")
+    gi.fill_B_device(cfg, R)
+    rng = np.random.default_rng(4)
+    edge = [0, 1, 126, 127, 128, 129, 255, 256, cfg.npair - 130, cfg.npair - 129, cfg.npair - 128,
+            cfg.npair - 127, cfg.npair - 2, cfg.npair - 1]
+    cols = np.array(sorted(set(edge) | set(rng.integers(0, cfg.npair, 500).tolist())), dtype=np.int64)
+    ct = torch.from_numpy(cols).cuda()
+    Rs = R[:, ct].cpu().numpy()                      # the sampled columns of the raw tensor
+    Md = torch.from_numpy(M).cuda()
+    info = pkg.build_b(Md, R, cfg.nao)
+    torch.cuda.synchronize()
+    assert int(info.item()) == 0
+    Bs = R[:, ct].cpu().numpy()
+    Lg = np.tril(Md.cpu().numpy())
+    del R
+    torch.cuda.empty_cache()
+    Lo = oracle.cholesky_lower(M)
+    assert relerr(Lg, Lo) <= TOL
+    assert relerr(Bs, oracle.whiten(Lo, Rs)) <= TOL
