@@ -118,9 +118,9 @@ int dfjk_get_jk_pair(dfjk_handle *h, const double *C1, const double *C2, int64_t
 /*
  * dfjk_get_jk_dm -- the same for a raw density matrix (no factorisation needed):
  *   dm      DEVICE, nao x nao row-major, any real matrix.
- * K is built as the pair (dm, I): X_P = B_P dm by the half transform, then
- * K = sum_P X_P B_P^T.  Cost ~ 6 naux nao^3 flop: prefer dfjk_get_jk / dfjk_get_jk_pair
- * whenever factors with few columns are known.
+ * K is built as the pair (dm, I): X_P = B_P dm by the half transform, B_P itself unpacked
+ * beside it, then K = sum_P X_P B_P^T as a full DMMA product.  Cost 4 naux nao^3 flop: prefer
+ * dfjk_get_jk / dfjk_get_jk_pair whenever factors with few columns are known.
  */
 int dfjk_get_jk_dm(dfjk_handle *h, const double *dm, double *J, double *K, void *stream);
 

@@ -273,7 +273,7 @@ int get_jk_impl(dfjk_handle *h, int nset, const double *const *C, const int64_t 
         int chunk = 0;
         for (int64_t P0 = 0; P0 < naux; P0 += pc, ++chunk) {
             const int64_t np = (P0 + pc <= naux) ? pc : naux - P0;
-            { Timed t_(h, DFJK_KERNEL_K1, st); dfjk::launch_k1_half_transform(h->B, naux, nao, npair, P0, np, h->Ccat, ldc, h->X, st); }
+            { Timed t_(h, DFJK_KERNEL_K1, st); dfjk::launch_k1_half_transform(h->B, naux, nao, npair, P0, np, h->Ccat, ldc, ldc, h->X, st); }
             for (int s = 0; s < nset; ++s)
                 if (K[s]) {
                     Timed t_(h, DFJK_KERNEL_K2, st);
@@ -319,14 +319,17 @@ int get_jk_general_impl(dfjk_handle *h, const double *C1, const double *C2, int6
         h->have_d = true;
     }
     if (K) {
-        /* Ccat = [C1 | C2] (a NULL second factor packs the identity), each padded to 8 columns */
+        /* X chunk columns [0, w8) = B_P C1 and [w8, 2 w8) = B_P C2.  Pair form: one half transform
+         * over Ccat = [C1 | C2].  Raw dm (C2 == NULL, the pair (dm, I)): the half transform runs over
+         * Ccat = [dm] only and the identity half, B_P itself, is unpacked straight into X (K1U). */
+        const bool raw = C2 == nullptr;
         const double *Cp[2] = {C1, C2};
         const int nocc[2] = {(int)ncol, (int)ncol};
         const int64_t w8 = round_up(ncol, 8);
         const int col0[2] = {0, (int)w8};
-        const int64_t ldc = 2 * w8;
-        { Timed t_(h, DFJK_KERNEL_K0, st); dfjk::launch_k0_pack_c(Cp, nocc, col0, 2, nao, ldc, h->Ccat, st); }
-        int64_t pc = h->x_doubles / (nao * ldc);
+        const int64_t ldx = 2 * w8, ldc = raw ? w8 : ldx;
+        { Timed t_(h, DFJK_KERNEL_K0, st); dfjk::launch_k0_pack_c(Cp, nocc, col0, raw ? 1 : 2, nao, ldc, h->Ccat, st); }
+        int64_t pc = h->x_doubles / (nao * ldx);
         if (h->opt_k_chunk > 0 && h->opt_k_chunk < pc) pc = h->opt_k_chunk;
         if (pc > naux) pc = naux;
         if (pc < 1) return fail(DFJK_ENOMEM, "%s: X workspace too small", who);
@@ -336,9 +339,10 @@ int get_jk_general_impl(dfjk_handle *h, const double *C1, const double *C2, int6
         int chunk = 0;
         for (int64_t P0 = 0; P0 < naux; P0 += pc, ++chunk) {
             const int64_t np = (P0 + pc <= naux) ? pc : naux - P0;
-            { Timed t_(h, DFJK_KERNEL_K1, st); dfjk::launch_k1_half_transform(h->B, naux, nao, npair, P0, np, h->Ccat, ldc, h->X, st); }
+            { Timed t_(h, DFJK_KERNEL_K1, st); dfjk::launch_k1_half_transform(h->B, naux, nao, npair, P0, np, h->Ccat, ldc, ldx, h->X, st); }
+            if (raw) { Timed t_(h, DFJK_KERNEL_K1, st); dfjk::launch_k1u_unpack(h->B, nao, npair, P0, np, ldx, w8, h->X, st); }
             { Timed t_(h, DFJK_KERNEL_K2, st);
-              dfjk::launch_k2_gemm_full(h->X, nao, np, ldc, col0[0], col0[1], ncol, h->Kpart, nsplit, chunk > 0, st); }
+              dfjk::launch_k2_gemm_full(h->X, nao, np, ldx, col0[0], col0[1], ncol, h->Kpart, nsplit, chunk > 0, st); }
         }
         { Timed t_(h, DFJK_KERNEL_K3, st); dfjk::launch_k3_sum(h->Kpart, nsplit, nao, K, st); }
     }

@@ -56,10 +56,15 @@ void launch_k0_pack_c(const double *const *C, const int *nocc, const int *col0, 
                       int64_t nao, int64_t ldc, double *Ccat, cudaStream_t st);
 
 /* K1: for P in [P0, P0+np), k = (P-P0)*ldc + i:
- *   X4[(k/4)*nao*4 + mu*4 + k%4] = sum_nu B_P(mu,nu) Ccat[nu][i]      (k-group-major X) */
+ *   X4[(k/4)*nao*4 + mu*4 + k%4] = sum_nu B_P(mu,nu) Ccat[nu][i]      (k-group-major X)
+ * with k = (P-P0)*ldx + i: ldx >= ldc is X's row pitch (ldx > ldc leaves room for K1U's columns). */
 void launch_k1_half_transform(const double *B, int64_t naux, int64_t nao, int64_t npair,
-                              int64_t P0, int64_t np, const double *Ccat4, int64_t ldc,
+                              int64_t P0, int64_t np, const double *Ccat4, int64_t ldc, int64_t ldx,
                               double *X4, cudaStream_t st);
+
+/* K1U: X4 columns [col0, col0 + round_up(nao,4)) of the chunk = B_P unpacked (X_P = B_P . I). */
+void launch_k1u_unpack(const double *B, int64_t nao, int64_t npair, int64_t P0, int64_t np, int64_t ldx,
+                       int64_t col0, double *X4, cudaStream_t st);
 
 /* K2: Kpart[split][mu][nu] (+)= sum_{k in split's share} X[mu][k] X[nu][k]
  * for mu-tile >= nu-tile (lower 128x128 tiles).  The set uses k = p*ldc + [col0, col0+round_up(ncol,4)),

@@ -85,7 +85,7 @@ struct K1Cfg {
 template <int NT8>
 __global__ void __launch_bounds__(K1_THREADS, 1)
 k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao, int64_t npair, int64_t P0,
-                         const double *__restrict__ Ccat4, int64_t ldc, int ntiles_n,
+                         const double *__restrict__ Ccat4, int64_t ldc, int64_t ldx, int ntiles_n,
                          double *__restrict__ X4)
 {
     using Cfg = K1Cfg<NT8>;
@@ -237,7 +237,7 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
                 for (int nt = 0; nt < NT8; ++nt) {
                     const int64_t col = n0 + 8 * nt + 2 * lr;          /* even */
                     if (col < ldc) {
-                        const int64_t k = p * ldc + col;
+                        const int64_t k = p * ldx + col;       /* ldx >= ldc: X row pitch */
                         double *dst = X4 + ((k >> 2) * nao + mu) * 4 + (k & 3);
                         *reinterpret_cast<double2 *>(dst) = make_double2(acc[mt][nt][0], acc[mt][nt][1]);
                     }
@@ -247,9 +247,35 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
     }
 }
 
+/* K1U: the identity half of the raw-dm build, X_P = B_P . I = B_P unpacked, written straight
+ * into X's k-group-major layout without touching the FP64 pipe:
+ *     X4[(k/4)][mu][k%4] = B_P(mu, i),   k = p*ldx + col0 + i,   i < round_up(nao, 4) (0 for i >= nao)
+ * One thread per (mu, group of four i): four packed loads (max/min addressing), one 32-byte store;
+ * consecutive threads own consecutive mu, so the stores are contiguous. */
+__global__ void __launch_bounds__(128)
+k1u_unpack_kernel(const double *__restrict__ B, int64_t nao, int64_t npair, int64_t P0, int64_t ldx,
+                  int64_t col0, double *__restrict__ X4)
+{
+    const int64_t mu = (int64_t)blockIdx.x * 128 + threadIdx.x;
+    if (mu >= nao) return;
+    const int64_t i0 = 4 * (int64_t)blockIdx.y, p = blockIdx.z;
+    const double *Bp = B + (P0 + p) * npair;
+    double v[4];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        const int64_t i = i0 + q;
+        const int64_t a = mu > i ? mu : i, b = mu > i ? i : mu;
+        v[q] = i < nao ? Bp[a * (a + 1) / 2 + b] : 0.0;
+    }
+    const int64_t k = p * ldx + col0 + i0;                 /* multiple of 4 */
+    double2 *dst = reinterpret_cast<double2 *>(X4 + ((k >> 2) * nao + mu) * 4);
+    dst[0] = make_double2(v[0], v[1]);
+    dst[1] = make_double2(v[2], v[3]);
+}
+
 template <int NT8>
 void k1_launch_t(const double *B, int64_t naux, int64_t nao, int64_t npair, int64_t P0, int64_t np,
-                 const double *Ccat4, int64_t ldc, int ntiles_n, double *X4, cudaStream_t st)
+                 const double *Ccat4, int64_t ldc, int64_t ldx, int ntiles_n, double *X4, cudaStream_t st)
 {
     static bool configured = false;   /* attribute is per function, set once per process */
     if (!configured) {
@@ -260,20 +286,20 @@ void k1_launch_t(const double *B, int64_t naux, int64_t nao, int64_t npair, int6
     const unsigned nib = (unsigned)((nao + K1_M - 1) / K1_M);
     dim3 grid(nib * ntiles_n, (unsigned)np);
     k1_half_transform_kernel<NT8><<<grid, K1_THREADS, K1Cfg<NT8>::SMEM_BYTES, st>>>(
-        B, naux, nao, npair, P0, Ccat4, ldc, ntiles_n, X4);
+        B, naux, nao, npair, P0, Ccat4, ldc, ldx, ntiles_n, X4);
 }
 
 }  // namespace
 
 void launch_k1_half_transform(const double *B, int64_t naux, int64_t nao, int64_t npair, int64_t P0, int64_t np,
-                              const double *Ccat4, int64_t ldc, double *X4, cudaStream_t st)
+                              const double *Ccat4, int64_t ldc, int64_t ldx, double *X4, cudaStream_t st)
 {
     const int n8 = (int)(ldc / 8);
     const int ntiles_n = (n8 + 16) / 17;
     const int nt8 = (n8 + ntiles_n - 1) / ntiles_n;
     /* grid.y <= 65535: chunks are far smaller than that */
 #define DFJK_K1_CASE(N) \
-    case N: k1_launch_t<N>(B, naux, nao, npair, P0, np, Ccat4, ldc, ntiles_n, X4, st); break;
+    case N: k1_launch_t<N>(B, naux, nao, npair, P0, np, Ccat4, ldc, ldx, ntiles_n, X4, st); break;
     switch (nt8) {
         DFJK_K1_CASE(1) DFJK_K1_CASE(2) DFJK_K1_CASE(3) DFJK_K1_CASE(4) DFJK_K1_CASE(5)
         DFJK_K1_CASE(6) DFJK_K1_CASE(7) DFJK_K1_CASE(8) DFJK_K1_CASE(9) DFJK_K1_CASE(10)
@@ -282,6 +308,13 @@ void launch_k1_half_transform(const double *B, int64_t naux, int64_t nao, int64_
     default: break;
     }
 #undef DFJK_K1_CASE
+}
+
+void launch_k1u_unpack(const double *B, int64_t nao, int64_t npair, int64_t P0, int64_t np, int64_t ldx,
+                       int64_t col0, double *X4, cudaStream_t st)
+{
+    dim3 grid((unsigned)((nao + 127) / 128), (unsigned)((nao + 3) / 4), (unsigned)np);
+    k1u_unpack_kernel<<<grid, 128, 0, st>>>(B, nao, npair, P0, ldx, col0, X4);
 }
 
 }  // namespace dfjk
