@@ -64,6 +64,23 @@ def measured_peaks():
         return {"hbm_gbs": HBM_FALLBACK_GBS}, "fallback"
 
 
+def max_over_ranks(x, dist=None, device="cpu"):
+    """MAX over ranks of a host scalar (the timing rule: a multi-GPU step takes as long as its
+    slowest replica).  dist=None (single process) returns x."""
+    if dist is None:
+        return float(x)
+    import torch
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(flops_per_step, steps, total_ms, world):
+    """Aggregate GFLOP/s of `world` independent replicas ("replicas only", weak scaling): every
+    rank does `steps` steps of flops_per_step in the max-over-ranks time total_ms."""
+    return world * flops_per_step * steps / (total_ms * 1e-3) / 1e9
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons sampled during the timed region."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
@@ -239,10 +256,7 @@ def run_ours(args, cfg):
     total_ms = float(sum(step_ms))
     kt = {name: h.kernel_time(name) for name in pkg.KERNELS}
     h.set_option("time_kernels", 0)
-    if dist is not None:
-        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = max_over_ranks(total_ms, dist, dev)
 
     # ---- end to end through the host entry point (restricted configs)
     e2e = None
@@ -257,11 +271,8 @@ def run_ours(args, cfg):
         for k in range(args.steps):
             h.get_jk_host(Ch[args.warmup + k], Jh, Kh)
         e2e_s = time.perf_counter() - t0
-        if dist is not None:
-            t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            e2e_s = float(t.item())
-        e2e = {"value": world * flops_step(cfg) * args.steps / e2e_s / 1e9, "unit": "GFLOP/s",
+        e2e_s = max_over_ranks(e2e_s, dist, dev)
+        e2e = {"value": whole_job_value(flops_step(cfg), args.steps, e2e_s * 1e3, world), "unit": "GFLOP/s",
                "ms_per_step": e2e_s * 1e3 / args.steps,
                "h2d_bytes_per_step": cfg.nao * nocc * 8, "d2h_bytes_per_step": 2 * cfg.nao * cfg.nao * 8,
                "api": "dfjk_get_jk_host (pinned host C_occ in, pinned host J and K out; B resident)"}
@@ -272,7 +283,7 @@ def run_ours(args, cfg):
 
     peaks, peak_src = measured_peaks()
     ms_per_step = total_ms / args.steps
-    value = world * flops_step(cfg) * args.steps / (total_ms * 1e-3) / 1e9
+    value = whole_job_value(flops_step(cfg), args.steps, total_ms, world)
     k1_ms, k1_n = kt["K1"]
     k2_ms, k2_n = kt["K2"]
     j_ms = sum(kt[n][0] for n in ("J0", "J1", "J1R", "J2", "J3")) / args.steps
