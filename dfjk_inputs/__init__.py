@@ -245,3 +245,28 @@ def metric(cfg: Config) -> np.ndarray:
     M = np.exp(-np.abs(y[:, None] - y[None, :]) / 2.0)
     M[np.diag_indices(cfg.naux)] += 0.1
     return np.ascontiguousarray(M)
+
+
+def overlap(cfg: Config) -> np.ndarray:
+    """Synthetic overlap matrix S of a non-orthogonal basis (SCF driver tests, section 8f rank 4):
+    S_mn = 0.7 delta_mn + 0.3 exp(-|x_m - x_n| / 0.5) on the basis-function centres x -- symmetric,
+    unit diagonal, positive definite (exponential kernel) and well conditioned."""
+    x = centers(cfg)
+    S = 0.3 * np.exp(-np.abs(x[:, None] - x[None, :]) / 0.5)
+    S[np.diag_indices(cfg.nao)] += 0.7
+    return np.ascontiguousarray(S)
+
+
+def core_hamiltonian(cfg: Config) -> np.ndarray:
+    """Synthetic one-electron Hamiltonian with a clear occupied/virtual gap (so that plain DIIS
+    converges, PAPER.md:260): every (nao // nocc)-th site is "deep", -(4 + u_m), the others are
+    shallow, -(0.5 + 0.5 u_m), u = U(0,1) (stream 4); plus a short-range hopping
+    -0.2 exp(-|x_m - x_n|) between different sites.  Symmetric."""
+    x = centers(cfg)
+    u = uniform(cfg.seed, 4, cfg.nao)
+    nocc = cfg.nocc[0]
+    deep = np.zeros(cfg.nao, dtype=bool)
+    deep[(np.arange(nocc) * cfg.nao) // nocc] = True
+    h = -0.2 * np.exp(-np.abs(x[:, None] - x[None, :]))
+    h[np.diag_indices(cfg.nao)] = np.where(deep, -(4.0 + u), -(0.5 + 0.5 * u))
+    return np.ascontiguousarray(h)
