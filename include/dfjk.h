@@ -143,6 +143,32 @@ int dfjk_get_jk_host(dfjk_handle *h, const double *C_occ_host, int64_t nocc,
                      double *J_host, double *K_host);
 
 /*
+ * dfjk_scf_rhf -- a closed-shell DF-SCF driver around dfjk_get_jk.
+ * The paper gives the loop in words (Fock build -> diagonalisation -> new density, DIIS by
+ * default: PAPER.md:258-262; mf.kernel(dm0): PAPER.md:154-159); written out (Roothaan-Hall + Pulay
+ * DIIS):
+ *     core guess  hcore C = S C eps;   then per iteration k = 0, 1, ...
+ *     C_occ = nocc lowest orbitals;  J, K = get_jk(C_occ);  F = hcore + J - K
+ *     E_k = 1/2 sum D o (hcore + F), D = 2 C_occ C_occ^T;   e = F D S - S D F
+ *     stop when k > 0, |E_k - E_{k-1}| <= conv_tol max(1, |E_k|) and max|e| <= sqrt(conv_tol)
+ *     DIIS over the last diis_space (F, e) pairs;  F_ext C = S C eps
+ *   hcore, S   DEVICE nao x nao, symmetric (S positive definite); read only
+ *   nocc       doubly occupied orbitals, 1 <= nocc <= nao;  max_iter >= 1;  1 <= diis_space <= 16
+ *   C          DEVICE nao x nao OUT, C[mu*nao + i], orbitals of the last diagonalisation (C^T S C = 1)
+ *   mo_energy  DEVICE nao OUT or NULL;  D, F  DEVICE nao x nao OUT or NULL (density and Fock matrix of
+ *              the last energy evaluation)
+ *   e_hist     HOST max_iter doubles OUT (E_k);  n_iter, converged  HOST OUT
+ * SYNCHRONOUS: the host reads E and max|e| back every iteration.  Allocates its workspace
+ * (about (9 + 2 diis_space) nao^2 doubles) for the duration of the call.  Every step runs in this
+ * library's kernels except the generalised symmetric eigenproblem, which is cuSOLVER's Dsygvd
+ * (loaded with dlopen at the first call; DFJK_ECUDA if libcusolver is not available).
+ */
+int dfjk_scf_rhf(dfjk_handle *h, const double *hcore, const double *S, int64_t nocc,
+                 int64_t max_iter, double conv_tol, int64_t diis_space, double *C,
+                 double *mo_energy, double *D, double *F, double *e_hist, int64_t *n_iter,
+                 int *converged, void *stream);
+
+/*
  * dfjk_build_b -- build the whitened tensor on the device,
  * PAPER.md:353-356, Eq. 2-3:
  *     M_PQ = (chi_P|chi_Q) = L L^T                              Eq. 2

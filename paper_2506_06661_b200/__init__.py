@@ -30,7 +30,7 @@ SYMBOLS = (
     "dfjk_set_option", "dfjk_workspace_bytes", "dfjk_destroy", "dfjk_last_error",
     "dfjk_version", "dfjk_launch_count", "dfjk_kernel_time",
     "dfjk_get_jk_pair", "dfjk_get_jk_dm", "dfjk_get_jk_dms", "dfjk_get_df_diag",
-    "dfjk_build_b",
+    "dfjk_build_b", "dfjk_scf_rhf",
 )
 
 # DFJK_KERNEL_* ids of include/dfjk.h
@@ -73,6 +73,10 @@ def lib() -> ctypes.CDLL:
     L.dfjk_get_jk_dm.argtypes = [vp, vp, vp, vp, vp]
     L.dfjk_get_jk_dms.restype = ci
     L.dfjk_get_jk_dms.argtypes = [vp, i64, vp, vp, vp, vp]
+    L.dfjk_scf_rhf.restype = ci
+    L.dfjk_scf_rhf.argtypes = [vp, vp, vp, i64, i64, ctypes.c_double, i64, vp, vp, vp, vp,
+                               ctypes.POINTER(ctypes.c_double), ctypes.POINTER(i64),
+                               ctypes.POINTER(ci), vp]
     L.dfjk_build_b.restype = ci
     L.dfjk_build_b.argtypes = [i64, i64, vp, vp, vp, vp]
     L.dfjk_get_df_diag.restype = ci
@@ -249,6 +253,26 @@ class DFJK:
                                           K_host.data_ptr() if K_host is not None else None),
                    "dfjk_get_jk_host")
         return J_host, K_host
+
+    def scf_rhf(self, hcore, S, nocc: int, max_iter: int = 50, conv_tol: float = 1e-10,
+                diis_space: int = 8, stream=None):
+        """Closed-shell DF-SCF around get_jk (dfjk_scf_rhf; synchronous).  Returns a dict with
+        converged, e_hist (list), C, mo_energy, D, F (device tensors)."""
+        import torch
+        n2 = self.nao * self.nao
+        hp, sp = _dev_f64(hcore, "hcore", n2), _dev_f64(S, "S", n2)
+        C, D, F = self._out(True), self._out(True), self._out(True)
+        eps = torch.empty(self.nao, dtype=torch.float64, device=self.device)
+        e_hist = (ctypes.c_double * int(max_iter))()
+        n_iter, conv = ctypes.c_int64(0), ctypes.c_int(0)
+        with torch.cuda.device(self.device):
+            st = (stream or torch.cuda.current_stream(self.device)).cuda_stream
+            _check(lib().dfjk_scf_rhf(self._h, hp, sp, int(nocc), int(max_iter), float(conv_tol),
+                                      int(diis_space), C.data_ptr(), eps.data_ptr(), D.data_ptr(),
+                                      F.data_ptr(), e_hist, ctypes.byref(n_iter), ctypes.byref(conv), st),
+                   "dfjk_scf_rhf")
+        return dict(converged=bool(conv.value), e_hist=list(e_hist[:n_iter.value]), C=C,
+                    mo_energy=eps, D=D, F=F)
 
     def get_df_diag(self, stream=None):
         """diag[mu][nu] = sum_P B_P[mu,nu]^2, the DF term of Eq. 7."""

@@ -329,6 +329,13 @@ whiten_gemm_kernel(double *__restrict__ T, int64_t naux, int64_t npair,
 
 }  // namespace
 
+void launch_fp64_tile_gemm(const double *A, int64_t lda, const double *Bop, int64_t sbk, int64_t sbn,
+                           double *C, int64_t ldc, int64_t Mr, int64_t Nc, int64_t Kd, double alpha,
+                           double beta, int lower_only, cudaStream_t st)
+{
+    small_gemm(A, lda, Bop, sbk, sbn, C, ldc, Mr, Nc, Kd, alpha, beta, lower_only, st);
+}
+
 int64_t build_b_workspace_doubles(int64_t naux)
 {
     const int64_t ldw = (naux + NB - 1) / NB * NB;

@@ -400,6 +400,27 @@ extern "C" int dfjk_get_jk_u(dfjk_handle *h, const double *C_a, int64_t nocc_a, 
     return get_jk_impl(h, 2, C, no, w, J, Ks, (cudaStream_t)stream, "dfjk_get_jk_u");
 }
 
+extern "C" int dfjk_scf_rhf(dfjk_handle *h, const double *hcore, const double *S, int64_t nocc,
+                            int64_t max_iter, double conv_tol, int64_t diis_space, double *C,
+                            double *mo_energy, double *D, double *F, double *e_hist, int64_t *n_iter,
+                            int *converged, void *stream)
+{
+    g_err[0] = 0;
+    if (!h) return fail(DFJK_EINVAL, "dfjk_scf_rhf: NULL handle");
+    if (!hcore || !S || !C || !e_hist || !n_iter || !converged)
+        return fail(DFJK_EINVAL, "dfjk_scf_rhf: NULL pointer");
+    if (nocc < 1 || nocc > h->nao) return fail(DFJK_EINVAL, "dfjk_scf_rhf: nocc outside [1, nao]");
+    if (max_iter < 1) return fail(DFJK_EINVAL, "dfjk_scf_rhf: max_iter must be >= 1");
+    if (diis_space < 1 || diis_space > 16) return fail(DFJK_EINVAL, "dfjk_scf_rhf: diis_space outside [1, 16]");
+    if (!(conv_tol > 0.0)) return fail(DFJK_EINVAL, "dfjk_scf_rhf: conv_tol must be positive");
+    if (h->nao > 32768) return fail(DFJK_EINVAL, "dfjk_scf_rhf: nao too large for the dense eigensolver");
+    int dev = -1;
+    DFJK_CUDA_TRY(cudaGetDevice(&dev));
+    if (dev != h->device) return fail(DFJK_EINVAL, "dfjk_scf_rhf: handle belongs to device %d, current is %d", h->device, dev);
+    return dfjk::scf_rhf_run(h, h->nao, hcore, S, nocc, max_iter, conv_tol, diis_space, C, mo_energy, D, F,
+                             e_hist, n_iter, converged, (cudaStream_t)stream, g_err, sizeof g_err);
+}
+
 extern "C" int dfjk_build_b(int64_t naux, int64_t nao, double *M, double *R_packed, int64_t *info,
                             void *stream)
 {

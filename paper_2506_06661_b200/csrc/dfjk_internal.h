@@ -10,6 +10,7 @@
 #define DFJK_INTERNAL_H
 
 #include <cuda_runtime.h>
+#include <stddef.h>
 #include <stdint.h>
 
 namespace dfjk {
@@ -94,5 +95,21 @@ int64_t build_b_workspace_doubles(int64_t naux);
 cudaError_t launch_build_b(int64_t naux, int64_t npair, double *M, double *T, double *ws,
                            long long *info, cudaStream_t st);
 
+/* Plain FP64 FMA tile product for the small dense steps around the hot kernels (Cholesky panels,
+ * SCF driver):  C[m][n] = beta C[m][n] + alpha sum_k A[m*lda + k] * Bop[k*sbk + n*sbn],
+ * m < Mr, n < Nc, k < Kd; (sbk, sbn) = (ldb, 1) is A.B, (1, ldb) is A.B^T. */
+void launch_fp64_tile_gemm(const double *A, int64_t lda, const double *Bop, int64_t sbk, int64_t sbn,
+                           double *C, int64_t ldc, int64_t Mr, int64_t Nc, int64_t Kd, double alpha,
+                           double beta, int lower_only, cudaStream_t st);
+
+}  // namespace dfjk
+
+/* ---------------------------------------------------------------- SCF driver (scf_rhf.cu) */
+struct dfjk_handle;
+namespace dfjk {
+int scf_rhf_run(dfjk_handle *h, int64_t nao, const double *hcore, const double *S, int64_t nocc,
+                int64_t max_iter, double conv_tol, int64_t diis_space, double *C_out,
+                double *mo_energy_out, double *D_out, double *F_out, double *e_hist, int64_t *n_iter,
+                int *converged, cudaStream_t st, char *err, size_t errlen);
 }  // namespace dfjk
 #endif

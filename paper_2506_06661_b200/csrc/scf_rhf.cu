@@ -1,0 +1,359 @@
+/*
+ * scf_rhf.cu -- a closed-shell DF-SCF driver around the get_jk kernels (include/dfjk.h,
+ * dfjk_scf_rhf).  The paper describes the loop in words only: the
+ * mean-field object iterates Fock build -> diagonalisation -> new density, DIIS being the default
+ * accelerator (mf.kernel(dm0)), with get_jk(dm) -> (vj, vk)
+ * as the expensive step.  Per iteration, all on the device:
+ *
+ *     J, K = get_jk(C_occ)                       this library's hot path (J0-J3, K0-K3)
+ *     F    = hcore + J - K                        S1 (elementwise)
+ *     D    = 2 C_occ C_occ^T                      FP64 tile product
+ *     E    = 1/2 sum D o (hcore + F)              S2 (two-stage deterministic reduction)
+ *     e    = F D S - (F D S)^T                    two FP64 tile products + S3
+ *     DIIS: B_ij = <e_i, e_j> (S2), the (m+1) x (m+1) system on the host, F_ext = sum c_i F_i (S4)
+ *     F_ext C = S C eps                           cuSOLVER Dsygvd -- the one library step, loaded
+ *                                                 with dlopen so libdfjk.so itself has no
+ *                                                 dependency on it
+ *     C (row-major), C_occ                        S5 (transpose of the column-major eigenvectors)
+ *
+ * The host reads back two scalars per iteration (E and max|e|) to decide convergence.
+ */
+#include "../../include/dfjk.h"
+#include "dfjk_internal.h"
+
+#include <cusolverDn.h>
+#include <dlfcn.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <vector>
+
+namespace dfjk {
+namespace {
+
+/* ------------------------------------------------------------------ cuSOLVER through dlopen */
+struct Cusolver {
+    void *lib = nullptr;
+    cusolverStatus_t (*create)(cusolverDnHandle_t *) = nullptr;
+    cusolverStatus_t (*destroy)(cusolverDnHandle_t) = nullptr;
+    cusolverStatus_t (*set_stream)(cusolverDnHandle_t, cudaStream_t) = nullptr;
+    cusolverStatus_t (*sygvd_bufsize)(cusolverDnHandle_t, cusolverEigType_t, cusolverEigMode_t,
+                                      cublasFillMode_t, int, const double *, int, const double *, int,
+                                      const double *, int *) = nullptr;
+    cusolverStatus_t (*sygvd)(cusolverDnHandle_t, cusolverEigType_t, cusolverEigMode_t, cublasFillMode_t,
+                              int, double *, int, double *, int, double *, double *, int, int *) = nullptr;
+    bool ok() const { return lib && create && destroy && set_stream && sygvd_bufsize && sygvd; }
+};
+
+Cusolver &cusolver()
+{
+    static Cusolver cs;
+    static bool tried = false;
+    if (!tried) {
+        tried = true;
+        const char *names[] = {"libcusolver.so.11", "libcusolver.so",
+                               "/usr/local/cuda/lib64/libcusolver.so.11", "libcusolver.so.12"};
+        for (const char *n : names) {
+            cs.lib = dlopen(n, RTLD_NOW | RTLD_LOCAL);
+            if (cs.lib) break;
+        }
+        if (cs.lib) {
+            cs.create = (decltype(cs.create))dlsym(cs.lib, "cusolverDnCreate");
+            cs.destroy = (decltype(cs.destroy))dlsym(cs.lib, "cusolverDnDestroy");
+            cs.set_stream = (decltype(cs.set_stream))dlsym(cs.lib, "cusolverDnSetStream");
+            cs.sygvd_bufsize = (decltype(cs.sygvd_bufsize))dlsym(cs.lib, "cusolverDnDsygvd_bufferSize");
+            cs.sygvd = (decltype(cs.sygvd))dlsym(cs.lib, "cusolverDnDsygvd");
+        }
+    }
+    return cs;
+}
+
+/* ------------------------------------------------------------------ S1-S5: small kernels */
+__global__ void fock_kernel(const double *__restrict__ h, const double *__restrict__ J,
+                            const double *__restrict__ K, int64_t n2, double *__restrict__ F)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n2) F[i] = h[i] + J[i] - K[i];
+}
+
+/* partial[b] = reduction over this block's grid-stride share; mode 0: sum a*b, 1: sum a*(b+c),
+ * 2: max |a|.  Fixed grid + fixed-order second stage => deterministic. */
+constexpr int RED_BLOCKS = 256, RED_THREADS = 256;
+
+__global__ void __launch_bounds__(RED_THREADS)
+reduce_partial_kernel(int mode, const double *__restrict__ a, const double *__restrict__ b,
+                      const double *__restrict__ c, int64_t n, double *__restrict__ partial)
+{
+    __shared__ double sh[RED_THREADS];
+    double acc = 0.0;
+    for (int64_t i = (int64_t)blockIdx.x * RED_THREADS + threadIdx.x; i < n; i += (int64_t)RED_BLOCKS * RED_THREADS) {
+        if (mode == 0) acc += a[i] * b[i];
+        else if (mode == 1) acc += a[i] * (b[i] + c[i]);
+        else acc = fmax(acc, fabs(a[i]));
+    }
+    sh[threadIdx.x] = acc;
+    __syncthreads();
+    for (int s = RED_THREADS / 2; s > 0; s >>= 1) {
+        if (threadIdx.x < s)
+            sh[threadIdx.x] = mode == 2 ? fmax(sh[threadIdx.x], sh[threadIdx.x + s])
+                                        : sh[threadIdx.x] + sh[threadIdx.x + s];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) partial[blockIdx.x] = sh[0];
+}
+
+__global__ void reduce_final_kernel(int mode, const double *__restrict__ partial, double scale,
+                                    double *__restrict__ out)
+{
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    double acc = 0.0;
+    for (int i = 0; i < RED_BLOCKS; ++i) acc = mode == 2 ? fmax(acc, partial[i]) : acc + partial[i];
+    *out = scale * acc;
+}
+
+/* e = T - T^T (T = F D S, so e = F D S - S D F) */
+__global__ void antisym_kernel(const double *__restrict__ T, int64_t n, double *__restrict__ e)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n * n) return;
+    const int64_t r = i / n, c = i - r * n;
+    e[i] = T[i] - T[c * n + r];
+}
+
+struct Coefs { double c[16]; const double *F[16]; int m; };
+
+__global__ void lincomb_kernel(Coefs cf, int64_t n2, double *__restrict__ out)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n2) return;
+    double acc = 0.0;
+    for (int k = 0; k < cf.m; ++k) acc += cf.c[k] * cf.F[k][i];
+    out[i] = acc;
+}
+
+/* V holds the eigenvectors as columns of a column-major matrix: V[mu + i*n] = C[mu][i].
+ * Writes C row-major (C[mu*n + i]) and the occupied block C_occ[mu*nocc + i], i < nocc. */
+__global__ void __launch_bounds__(256)
+unpack_vectors_kernel(const double *__restrict__ V, int64_t n, int64_t nocc, double *__restrict__ C,
+                      double *__restrict__ C_occ)
+{
+    __shared__ double t[32][33];
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    const int64_t i0 = (int64_t)blockIdx.y * 32, m0 = (int64_t)blockIdx.x * 32;
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+        const int64_t i = i0 + ty + 8 * r, mu = m0 + tx;
+        t[ty + 8 * r][tx] = (i < n && mu < n) ? V[i * n + mu] : 0.0;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+        const int64_t mu = m0 + ty + 8 * r, i = i0 + tx;
+        if (mu < n && i < n) {
+            const double v = t[tx][ty + 8 * r];
+            C[mu * n + i] = v;
+            if (i < nocc) C_occ[mu * nocc + i] = v;
+        }
+    }
+}
+
+/* (m+1) x (m+1) DIIS system on the host: Gaussian elimination with partial pivoting */
+bool solve_dense(std::vector<double> &A, std::vector<double> &b, int n)
+{
+    for (int k = 0; k < n; ++k) {
+        int p = k;
+        for (int i = k + 1; i < n; ++i)
+            if (std::fabs(A[i * n + k]) > std::fabs(A[p * n + k])) p = i;
+        if (A[p * n + k] == 0.0) return false;
+        if (p != k) {
+            for (int j = 0; j < n; ++j) std::swap(A[k * n + j], A[p * n + j]);
+            std::swap(b[k], b[p]);
+        }
+        for (int i = k + 1; i < n; ++i) {
+            const double f = A[i * n + k] / A[k * n + k];
+            for (int j = k; j < n; ++j) A[i * n + j] -= f * A[k * n + j];
+            b[i] -= f * b[k];
+        }
+    }
+    for (int k = n - 1; k >= 0; --k) {
+        double s = b[k];
+        for (int j = k + 1; j < n; ++j) s -= A[k * n + j] * b[j];
+        b[k] = s / A[k * n + k];
+    }
+    return true;
+}
+
+}  // namespace
+
+#define SCF_TRY(expr)                                                                      \
+    do {                                                                                   \
+        cudaError_t e_ = (expr);                                                           \
+        if (e_ != cudaSuccess) {                                                           \
+            snprintf(err, errlen, "dfjk_scf_rhf: %s: %s", #expr, cudaGetErrorString(e_));  \
+            rc = DFJK_ECUDA;                                                               \
+            goto done;                                                                     \
+        }                                                                                  \
+    } while (0)
+
+/* The loop of the file header.  All pointers except e_hist / n_iter / converged are DEVICE.
+ * Returns a DFJK_* code; on failure `err` holds the message. */
+int scf_rhf_run(dfjk_handle *h, int64_t nao, const double *hcore, const double *S, int64_t nocc,
+                int64_t max_iter, double conv_tol, int64_t diis_space, double *C_out,
+                double *mo_energy_out, double *D_out, double *F_out, double *e_hist, int64_t *n_iter,
+                int *converged, cudaStream_t st, char *err, size_t errlen)
+{
+    Cusolver &cs = cusolver();
+    if (!cs.ok()) {
+        snprintf(err, errlen, "dfjk_scf_rhf: libcusolver could not be loaded (%s)", dlerror() ? dlerror() : "symbols missing");
+        return DFJK_ECUDA;
+    }
+    const int64_t n2 = nao * nao;
+    const int m_max = (int)diis_space;
+    int rc = DFJK_OK;
+    cusolverDnHandle_t sol = nullptr;
+    double *ws = nullptr, *work = nullptr;
+    int *dev_info = nullptr;
+    int lwork = 0;
+    std::vector<double> Bmat((size_t)m_max * m_max, 0.0);
+    std::vector<int> slot_of;                        /* history, oldest first: ring slot ids */
+    double e_prev = 0.0;
+    *n_iter = 0;
+    *converged = 0;
+
+    /* workspace layout (doubles): F, D, T1, T2, Va (eigenvector / A copy), Sb (B copy), C, J, K,
+     * C_occ, W, partials, scalars, then the DIIS rings */
+    const int64_t fixed = 9 * n2 + nao * nocc + nao + RED_BLOCKS + 8;
+    const int64_t total = fixed + 2 * (int64_t)m_max * n2;
+    double *F, *D, *T1, *T2, *Va, *Sb, *C, *J, *K, *Cocc, *W, *part, *scal, *Fring, *Ering;
+    const unsigned eb = (unsigned)((n2 + 255) / 256);
+    const dim3 tgrid((unsigned)((nao + 31) / 32), (unsigned)((nao + 31) / 32));
+
+    if (cs.create(&sol) != CUSOLVER_STATUS_SUCCESS || cs.set_stream(sol, st) != CUSOLVER_STATUS_SUCCESS) {
+        snprintf(err, errlen, "dfjk_scf_rhf: cusolverDnCreate / SetStream failed");
+        rc = DFJK_ECUDA;
+        goto done;
+    }
+    SCF_TRY(cudaMalloc((void **)&ws, (size_t)total * sizeof(double)));
+    F = ws; D = F + n2; T1 = D + n2; T2 = T1 + n2; Va = T2 + n2; Sb = Va + n2; C = Sb + n2;
+    J = C + n2; K = J + n2; Cocc = K + n2; W = Cocc + nao * nocc; part = W + nao;
+    scal = part + RED_BLOCKS; Fring = scal + 8; Ering = Fring + (int64_t)m_max * n2;
+    if (cs.sygvd_bufsize(sol, CUSOLVER_EIG_TYPE_1, CUSOLVER_EIG_MODE_VECTOR, CUBLAS_FILL_MODE_LOWER,
+                         (int)nao, Va, (int)nao, Sb, (int)nao, W, &lwork) != CUSOLVER_STATUS_SUCCESS) {
+        snprintf(err, errlen, "dfjk_scf_rhf: cusolverDnDsygvd_bufferSize failed");
+        rc = DFJK_ECUDA;
+        goto done;
+    }
+    SCF_TRY(cudaMalloc((void **)&work, (size_t)lwork * sizeof(double)));
+    SCF_TRY(cudaMalloc((void **)&dev_info, sizeof(int)));
+
+    /* generalised symmetric eigenproblem A C = S C eps; a symmetric row-major matrix is its own
+     * column-major image, the eigenvectors come back as columns of the column-major Va */
+    {
+        auto diagonalise = [&](const double *A) -> int {
+            if (cudaMemcpyAsync(Va, A, (size_t)n2 * 8, cudaMemcpyDeviceToDevice, st) != cudaSuccess) return 1;
+            if (cudaMemcpyAsync(Sb, S, (size_t)n2 * 8, cudaMemcpyDeviceToDevice, st) != cudaSuccess) return 1;
+            if (cs.sygvd(sol, CUSOLVER_EIG_TYPE_1, CUSOLVER_EIG_MODE_VECTOR, CUBLAS_FILL_MODE_LOWER, (int)nao,
+                         Va, (int)nao, Sb, (int)nao, W, work, lwork, dev_info) != CUSOLVER_STATUS_SUCCESS)
+                return 2;
+            unpack_vectors_kernel<<<tgrid, 256, 0, st>>>(Va, nao, nocc, C, Cocc);
+            int info = 0;
+            if (cudaMemcpyAsync(&info, dev_info, sizeof(int), cudaMemcpyDeviceToHost, st) != cudaSuccess) return 1;
+            if (cudaStreamSynchronize(st) != cudaSuccess) return 1;
+            return info == 0 ? 0 : 3;
+        };
+        auto reduce = [&](int mode, const double *a, const double *b, const double *c, double scale, double *out) {
+            reduce_partial_kernel<<<RED_BLOCKS, RED_THREADS, 0, st>>>(mode, a, b, c, n2, part);
+            reduce_final_kernel<<<1, 32, 0, st>>>(mode, part, scale, out);
+        };
+
+        int dr = diagonalise(hcore);                                    /* 0. core guess */
+        if (dr != 0) {
+            snprintf(err, errlen, "dfjk_scf_rhf: Dsygvd failed on the core guess (%d; S not positive definite?)", dr);
+            rc = DFJK_ECUDA;
+            goto done;
+        }
+        for (int64_t k = 0; k < max_iter; ++k) {
+            rc = dfjk_get_jk(h, Cocc, nocc, J, K, (void *)st);
+            if (rc != DFJK_OK) { snprintf(err, errlen, "%s", dfjk_last_error()); goto done; }
+            fock_kernel<<<eb, 256, 0, st>>>(hcore, J, K, n2, F);
+            launch_fp64_tile_gemm(Cocc, nocc, Cocc, 1, nocc, D, nao, nao, nao, nocc, 2.0, 0.0, 0, st);
+            reduce(1, D, hcore, F, 0.5, scal + 0);                      /* E */
+            launch_fp64_tile_gemm(F, nao, D, nao, 1, T1, nao, nao, nao, nao, 1.0, 0.0, 0, st);   /* F D */
+            launch_fp64_tile_gemm(T1, nao, S, nao, 1, T2, nao, nao, nao, nao, 1.0, 0.0, 0, st);  /* F D S */
+            /* the new pair goes into the ring slot of the entry it evicts (or a fresh one) */
+            int slot;
+            if ((int)slot_of.size() < m_max) slot = (int)slot_of.size();
+            else slot = slot_of.front();
+            double *e_new = Ering + (int64_t)slot * n2, *f_new = Fring + (int64_t)slot * n2;
+            antisym_kernel<<<eb, 256, 0, st>>>(T2, nao, T1);            /* T1 = e (F D no longer needed) */
+            reduce(2, T1, nullptr, nullptr, 1.0, scal + 1);             /* max |e| */
+            double host2[2];
+            SCF_TRY(cudaMemcpyAsync(host2, scal, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+            SCF_TRY(cudaStreamSynchronize(st));
+            const double E = host2[0], emax = host2[1];
+            e_hist[k] = E;
+            *n_iter = k + 1;
+            if (k > 0 && std::fabs(E - e_prev) <= conv_tol * std::fmax(1.0, std::fabs(E)) &&
+                emax <= std::sqrt(conv_tol)) {
+                *converged = 1;
+                break;
+            }
+            e_prev = E;
+            if (k + 1 == max_iter) break;
+            /* DIIS history (oldest first) */
+            if ((int)slot_of.size() == m_max) {
+                slot_of.erase(slot_of.begin());
+                for (int i = 0; i + 1 < m_max; ++i)
+                    for (int j = 0; j + 1 < m_max; ++j) Bmat[i * m_max + j] = Bmat[(i + 1) * m_max + j + 1];
+            }
+            slot_of.push_back(slot);
+            SCF_TRY(cudaMemcpyAsync(e_new, T1, (size_t)n2 * 8, cudaMemcpyDeviceToDevice, st));
+            SCF_TRY(cudaMemcpyAsync(f_new, F, (size_t)n2 * 8, cudaMemcpyDeviceToDevice, st));
+            const int m = (int)slot_of.size();
+            /* one dot per launch pair, read back one by one (m <= 16 scalars per iteration) */
+            for (int i = 0; i < m; ++i) {
+                reduce(0, Ering + (int64_t)slot_of[i] * n2, e_new, nullptr, 1.0, scal + 2);
+                double v;
+                SCF_TRY(cudaMemcpyAsync(&v, scal + 2, sizeof(double), cudaMemcpyDeviceToHost, st));
+                SCF_TRY(cudaStreamSynchronize(st));
+                Bmat[i * m_max + (m - 1)] = Bmat[(m - 1) * m_max + i] = v;
+            }
+            std::vector<double> A((size_t)(m + 1) * (m + 1), 0.0), rhs(m + 1, 0.0);
+            for (int i = 0; i < m; ++i) {
+                for (int j = 0; j < m; ++j) A[i * (m + 1) + j] = Bmat[i * m_max + j];
+                A[i * (m + 1) + m] = A[m * (m + 1) + i] = -1.0;
+            }
+            rhs[m] = -1.0;
+            if (!solve_dense(A, rhs, m + 1)) {
+                snprintf(err, errlen, "dfjk_scf_rhf: singular DIIS system at iteration %lld", (long long)k);
+                rc = DFJK_ECUDA;
+                goto done;
+            }
+            Coefs cf;
+            cf.m = m;
+            for (int i = 0; i < m; ++i) { cf.c[i] = rhs[i]; cf.F[i] = Fring + (int64_t)slot_of[i] * n2; }
+            lincomb_kernel<<<eb, 256, 0, st>>>(cf, n2, T2);             /* T2 = F_ext */
+            dr = diagonalise(T2);
+            if (dr != 0) {
+                snprintf(err, errlen, "dfjk_scf_rhf: Dsygvd failed at iteration %lld (%d)", (long long)k, dr);
+                rc = DFJK_ECUDA;
+                goto done;
+            }
+        }
+        SCF_TRY(cudaMemcpyAsync(C_out, C, (size_t)n2 * 8, cudaMemcpyDeviceToDevice, st));
+        if (mo_energy_out) SCF_TRY(cudaMemcpyAsync(mo_energy_out, W, (size_t)nao * 8, cudaMemcpyDeviceToDevice, st));
+        if (D_out) SCF_TRY(cudaMemcpyAsync(D_out, D, (size_t)n2 * 8, cudaMemcpyDeviceToDevice, st));
+        if (F_out) SCF_TRY(cudaMemcpyAsync(F_out, F, (size_t)n2 * 8, cudaMemcpyDeviceToDevice, st));
+        SCF_TRY(cudaStreamSynchronize(st));
+        SCF_TRY(cudaGetLastError());
+    }
+done:
+    if (sol) cs.destroy(sol);
+    cudaFree(ws);
+    cudaFree(work);
+    cudaFree(dev_info);
+    return rc;
+}
+
+}  // namespace dfjk

@@ -41,6 +41,8 @@ def test_version_and_null_handling(L):
     assert L.dfjk_get_jk_dm(None, None, None, None, None) == -1
     assert L.dfjk_get_jk_dms(None, 1, None, None, None, None) == -1
     assert L.dfjk_get_df_diag(None, None, None) == -1
+    assert L.dfjk_scf_rhf(None, None, None, 1, 1, 1e-8, 4, None, None, None, None, None, None, None, None) == -1
+    assert b"NULL handle" in L.dfjk_last_error()
     assert L.dfjk_build_b(0, 4, None, None, None, None) == -1
     assert L.dfjk_build_b(4, 4, None, None, None, None) == -1
     assert b"NULL" in L.dfjk_last_error()
