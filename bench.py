@@ -352,7 +352,22 @@ def run_extra(args, cfg):
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
           for _ in range(args.steps)]
     sampler = ClockSampler(0)
-    if args.op == "build_b":
+    if args.op == "scf":
+        # SCF driver: max_iter fixed iterations of (get_jk + Fock + DIIS + Dsygvd); B scaled so that
+        # the two-electron term is a perturbation of the gapped synthetic core Hamiltonian
+        B.mul_(0.02)
+        h = pkg.DFJK(B, nao)
+        hc = torch.from_numpy(gi.core_hamiltonian(cfg)).to(dev)
+        S = torch.from_numpy(gi.overlap(cfg)).to(dev)
+        iters = 6
+        flops = iters * flops_step(cfg)
+        what = f"dfjk_scf_rhf: {iters} SCF iterations (get_jk + Fock + DIIS + Dsygvd), flops = get_jk only"
+        res = {}
+        prep = lambda: None
+
+        def run():
+            res.update(h.scf_rhf(hc, S, nocc, max_iter=iters, conv_tol=1e-300))
+    elif args.op == "build_b":
         Mh = torch.from_numpy(gi.metric(cfg)).pin_memory()
         Md = torch.empty(naux, naux, dtype=torch.float64, device=dev)
         flops = float(naux) ** 2 * cfg.npair + float(naux) ** 3 / 3.0
@@ -401,6 +416,9 @@ def run_extra(args, cfg):
            "higher_is_better": True, "dtype": "f64", "data": "synthetic", "op": what,
            "config": workload_config(cfg, args), "clocks": clocks, "step_ms": ms,
            "algorithmic_flops": flops}
+    if args.op == "scf":
+        out["e_hist"] = res.get("e_hist")
+        out["ms_per_iteration"] = t / 6
     if args.op == "diag":
         out["gbs"] = cfg.b_bytes / (t * 1e-3) / 1e9
     else:
@@ -415,7 +433,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=4, choices=sorted(gi.CONFIGS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--op", default="get_jk", choices=["get_jk", "build_b", "pair", "dm", "diag"],
+    ap.add_argument("--op", default="get_jk", choices=["get_jk", "build_b", "pair", "dm", "diag", "scf"],
                     help="get_jk (default, the contract line) or one of the section-8f rows")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
