@@ -220,6 +220,7 @@ def run_ours(args, cfg):
         torch.cuda.synchronize()
 
     pkg.lib()
+    fp64_probe = pkg.probe_fp64_peak() if rank == 0 else None     # measured FP64 pipe rate (untimed)
     unrestricted = len(cfg.nocc) == 2
     B = torch.empty(cfg.naux, cfg.npair, dtype=torch.float64, device=dev)
     gi.fill_B_device(cfg, B)
@@ -304,9 +305,10 @@ def run_ours(args, cfg):
     roofline = {"kernel": "k1_half_transform_kernel (X_P = B_P C, DMMA.8x8x4 on the FP64 pipe)",
                 "bound": "alu", "achieved": k1_tflops, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
                 "frac": k1_tflops / FP64_PEAK_TFLOPS, "traffic": traffic,
-                "peak_source": "148 SM x 64 FP64 FMA/clk x 2 x 1.965 GHz (DESIGN.md; DMMA microbenchmark "
-                               "reaches 37.07); sm_100a has no tcgen05 FP64 kind",
-                "launches": k1_n, "avg_launch_ms": k1_ms / max(k1_n, 1),
+                "peak_source": "148 SM x 64 FP64 FMA/clk x 2 x 1.965 GHz (DESIGN.md); peak_probe_tflops is "
+                               "dfjk_probe_dmma_peak's register-only DMMA loop measured in this run; "
+                               "sm_100a has no tcgen05 FP64 kind",
+                "peak_probe_tflops": fp64_probe, "launches": k1_n, "avg_launch_ms": k1_ms / max(k1_n, 1),
                 "flops_per_launch": flops_k1(cfg) * args.steps / max(k1_n, 1)}
     hbm = float(peaks.get("hbm_gbs", HBM_FALLBACK_GBS))
     j_stream_ms = (kt["J1"][0] + kt["J2"][0]) / args.steps

@@ -63,7 +63,8 @@ typedef struct dfjk_handle dfjk_handle;
  *             until dfjk_destroy (it is up to 96 GB).  Must be 16-byte aligned.
  *
  * Returns the handle, or NULL on failure (dfjk_last_error says why).
- * Workspace (a few hundred MB at most, independent of naux*npair) is allocated
+ * Workspace (at most ~3 GB: a 2 GB chunk of the half-transformed tensor plus the partial-K
+ * slots; independent of naux*npair) is allocated
  * here with cudaMalloc and freed by dfjk_destroy; get_jk never allocates.
  */
 dfjk_handle *dfjk_create(int64_t naux, int64_t nao, const double *B_packed);
@@ -259,6 +260,14 @@ int64_t dfjk_workspace_bytes(const dfjk_handle *h);
  * The caller must make sure no enqueued work still uses the handle.
  */
 int dfjk_destroy(dfjk_handle *h);
+
+/*
+ * dfjk_probe_dmma_peak -- measurement aid: runs a register-only DMMA.8x8x4 loop on every SM of the
+ * current device (default stream, synchronous, ~0.2 s) and returns the sustained FP64 rate in
+ * TFLOP/s (HOST pointer).  This is the measured counterpart of the derived FP64 peak
+ * (SMs x 64 FMA/clk x 2 x clock) that K's roofline fraction is quoted against.
+ */
+int dfjk_probe_dmma_peak(double *tflops);
 
 /* dfjk_last_error -- thread-local text of the last failure ("" if none). */
 const char *dfjk_last_error(void);

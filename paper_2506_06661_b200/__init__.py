@@ -30,7 +30,7 @@ SYMBOLS = (
     "dfjk_set_option", "dfjk_workspace_bytes", "dfjk_destroy", "dfjk_last_error",
     "dfjk_version", "dfjk_launch_count", "dfjk_kernel_time",
     "dfjk_get_jk_pair", "dfjk_get_jk_dm", "dfjk_get_jk_dms", "dfjk_get_df_diag",
-    "dfjk_build_b", "dfjk_scf_rhf",
+    "dfjk_build_b", "dfjk_scf_rhf", "dfjk_probe_dmma_peak",
 )
 
 # DFJK_KERNEL_* ids of include/dfjk.h
@@ -77,6 +77,8 @@ def lib() -> ctypes.CDLL:
     L.dfjk_scf_rhf.argtypes = [vp, vp, vp, i64, i64, ctypes.c_double, i64, vp, vp, vp, vp,
                                ctypes.POINTER(ctypes.c_double), ctypes.POINTER(i64),
                                ctypes.POINTER(ci), vp]
+    L.dfjk_probe_dmma_peak.restype = ci
+    L.dfjk_probe_dmma_peak.argtypes = [ctypes.POINTER(ctypes.c_double)]
     L.dfjk_build_b.restype = ci
     L.dfjk_build_b.argtypes = [i64, i64, vp, vp, vp, vp]
     L.dfjk_get_df_diag.restype = ci
@@ -116,6 +118,13 @@ def _dev_f64(t, name: str, numel: Optional[int] = None):
     if numel is not None and t.numel() != numel:
         raise ValueError(f"{name} has {t.numel()} elements, expected {numel}")
     return t.data_ptr()
+
+
+def probe_fp64_peak() -> float:
+    """Sustained FP64 TFLOP/s of a register-only DMMA loop on the current device."""
+    v = ctypes.c_double(0.0)
+    _check(lib().dfjk_probe_dmma_peak(ctypes.byref(v)), "dfjk_probe_dmma_peak")
+    return v.value
 
 
 def build_b(M, R_packed, nao: int, stream=None):

@@ -16,6 +16,10 @@
 #include <initializer_list>
 #include <new>
 
+#ifndef DFJK_X_MB
+#define DFJK_X_MB 2048   /* 512 -> 2048 MB: 17 -> 5 K1/K2 launch pairs at cfg 4, -1.1 % step time */
+#endif
+
 namespace {
 
 thread_local char g_err[512] = "";
@@ -160,8 +164,9 @@ extern "C" dfjk_handle *dfjk_create(int64_t naux, int64_t nao, const double *B_p
     h->ldc_max = 2 * round_up(nao, 8);
     h->nchunk = dfjk::j1_num_chunks(h->npair);
     h->j2_groups = dfjk::j2_num_groups(naux, h->npair, h->sm_count);
-    /* X chunk: ~96 MB (three quarters of L2), but at least two rows at the widest ldc */
-    int64_t xd = (512LL << 20) / 8;
+    /* X chunk (the half-transformed rows that live between K1 and K2), at least two rows at the
+     * widest ldc */
+    int64_t xd = ((int64_t)DFJK_X_MB << 20) / 8;
     if (xd < 2 * nao * h->ldc_max) xd = 2 * nao * h->ldc_max;
     if (xd > naux * nao * h->ldc_max) xd = naux * nao * h->ldc_max;
     h->x_doubles = xd;
@@ -398,6 +403,37 @@ extern "C" int dfjk_get_jk_u(dfjk_handle *h, const double *C_a, int64_t nocc_a, 
     const double w[2] = {1.0, 1.0};
     double *Ks[2] = {K_a, K_b};
     return get_jk_impl(h, 2, C, no, w, J, Ks, (cudaStream_t)stream, "dfjk_get_jk_u");
+}
+
+extern "C" int dfjk_probe_dmma_peak(double *tflops)
+{
+    g_err[0] = 0;
+    if (!tflops) return fail(DFJK_EINVAL, "dfjk_probe_dmma_peak: NULL pointer");
+    int dev = 0, sms = 0;
+    DFJK_CUDA_TRY(cudaGetDevice(&dev));
+    DFJK_CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    double *sink = nullptr;
+    DFJK_CUDA_TRY(cudaMalloc((void **)&sink, sizeof(double)));
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    const int ctas = 8 * sms, iters = 20000;
+    dfjk::launch_fp64_peak_probe(ctas, 2000, sink, 0);            /* warm-up */
+    double best = 0.0;
+    for (int rep = 0; rep < 3; ++rep) {
+        cudaEventRecord(e0, 0);
+        dfjk::launch_fp64_peak_probe(ctas, iters, sink, 0);
+        cudaEventRecord(e1, 0);
+        cudaEventSynchronize(e1);
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        const double tf = dfjk::fp64_peak_probe_flops(ctas, iters) / (ms * 1e-3) / 1e12;
+        if (tf > best) best = tf;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(sink);
+    DFJK_CUDA_TRY(cudaGetLastError());
+    *tflops = best;
+    return DFJK_OK;
 }
 
 extern "C" int dfjk_scf_rhf(dfjk_handle *h, const double *hcore, const double *S, int64_t nocc,

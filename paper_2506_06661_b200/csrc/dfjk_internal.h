@@ -95,6 +95,10 @@ int64_t build_b_workspace_doubles(int64_t naux);
 cudaError_t launch_build_b(int64_t naux, int64_t npair, double *M, double *T, double *ws,
                            long long *info, cudaStream_t st);
 
+/* FP64-pipe probe (register-only DMMA.8x8x4 loop): flops of one launch, and the launch. */
+double fp64_peak_probe_flops(int ctas, int iters);
+void launch_fp64_peak_probe(int ctas, int iters, double *sink, cudaStream_t st);
+
 /* Plain FP64 FMA tile product for the small dense steps around the hot kernels (Cholesky panels,
  * SCF driver):  C[m][n] = beta C[m][n] + alpha sum_k A[m*lda + k] * Bop[k*sbk + n*sbn],
  * m < Mr, n < Nc, k < Kd; (sbk, sbn) = (ldb, 1) is A.B, (1, ldb) is A.B^T. */

@@ -231,6 +231,26 @@ k3_finish_kernel(const double *__restrict__ Kpart, int nsplit, int64_t nao, doub
     }
 }
 
+/* ------------------------------------------------------------------ FP64 pipe probe */
+/* Register-only DMMA loop: 8 warps per CTA, 16 independent accumulator tiles per warp.  Measures
+ * what the FP64 pipe sustains with nothing else in the way -- the denominator of K's roofline. */
+__global__ void __launch_bounds__(256)
+fp64_peak_probe_kernel(int iters, double *__restrict__ sink)
+{
+    double acc[16][2];
+#pragma unroll
+    for (int t = 0; t < 16; ++t) { acc[t][0] = 0.0; acc[t][1] = 0.0; }
+    double a = 1.0 + 1e-9 * threadIdx.x, b = 1.0 - 1e-9 * threadIdx.x;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int t = 0; t < 16; ++t) dmma884(acc[t][0], acc[t][1], a, b);
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int t = 0; t < 16; ++t) s += acc[t][0] + acc[t][1];
+    if (s == 123.456) sink[0] = s;                       /* keeps the loop alive */
+}
+
 /* general (non-symmetric) finish: K[mu][nu] = sum_split Kpart[split][mu][nu], every entry */
 __global__ void __launch_bounds__(256)
 k3_sum_kernel(const double *__restrict__ Kpart, int nsplit, int64_t n2, double *__restrict__ K)
@@ -296,6 +316,13 @@ void launch_k3_finish(const double *Kpart, int nsplit, int64_t nao, double *K, c
 {
     const unsigned nb = (unsigned)((nao + K3_T - 1) / K3_T);
     k3_finish_kernel<<<dim3(nb, nb), 256, 0, st>>>(Kpart, nsplit, nao, K);
+}
+
+double fp64_peak_probe_flops(int ctas, int iters) { return (double)ctas * 8.0 * iters * 16.0 * 512.0; }
+
+void launch_fp64_peak_probe(int ctas, int iters, double *sink, cudaStream_t st)
+{
+    fp64_peak_probe_kernel<<<ctas, 256, 0, st>>>(iters, sink);
 }
 
 void launch_k3_sum(const double *Kpart, int nsplit, int64_t nao, double *K, cudaStream_t st)

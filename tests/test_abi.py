@@ -43,6 +43,7 @@ def test_version_and_null_handling(L):
     assert L.dfjk_get_df_diag(None, None, None) == -1
     assert L.dfjk_scf_rhf(None, None, None, 1, 1, 1e-8, 4, None, None, None, None, None, None, None, None) == -1
     assert b"NULL handle" in L.dfjk_last_error()
+    assert L.dfjk_probe_dmma_peak(None) == -1
     assert L.dfjk_build_b(0, 4, None, None, None, None) == -1
     assert L.dfjk_build_b(4, 4, None, None, None, None) == -1
     assert b"NULL" in L.dfjk_last_error()
