@@ -82,24 +82,22 @@ struct K1Cfg {
     static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 2 * STAGES * 8 + 16;
 };
 
+/* PERSISTENT: the grid is one CTA per SM; CTA b processes the work items b, b + gridDim.x, ...
+ * (item = (p, row block, column tile), p slowest) with the mbarrier ring running THROUGH item
+ * boundaries: while the consumers write one item's X tile, the producers are already filling the
+ * stages of the next one.  Producers and consumers walk the same item sequence independently.
+ * (One CTA per item cost a pipeline fill + drain per 25-50 stages: 16 % of K1 at nao = 290.) */
 template <int NT8>
 __global__ void __launch_bounds__(K1_THREADS, 1)
 k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao, int64_t npair, int64_t P0,
                          const double *__restrict__ Ccat4, int64_t ldc, int64_t ldx, int ntiles_n,
-                         double *__restrict__ X4)
+                         int64_t nitems, double *__restrict__ X4)
 {
     using Cfg = K1Cfg<NT8>;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int nt_idx = blockIdx.x % ntiles_n;
-    const int ib = blockIdx.x / ntiles_n;
-    const int64_t p = blockIdx.y;
-    const int64_t mu0 = (int64_t)ib * K1_M;
-    const int64_t n0 = (int64_t)nt_idx * Cfg::NW;
     const int nk = (int)((nao + K1_KC - 1) / K1_KC);
-    const int64_t pb = (P0 + p) * npair;               /* index of B_P's first element in B */
-    const int pbpar = (int)(pb & 1);
-    const bool last_p = P0 + p == naux - 1;
+    const int items_per_p = (int)((nao + K1_M - 1) / K1_M) * ntiles_n;
 
     const uint32_t smem_base = smem_u32(smem_raw);
     const uint32_t bar_base = smem_base + Cfg::STAGES * Cfg::STAGE_BYTES;
@@ -118,16 +116,25 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
     if (warp < K1_PRODUCERS / 32) {
         /* ------------------------------------------------------------ producers */
         reg_dealloc<40>();
+        int slot = 0;
+        uint32_t phase = 1;                                /* parity of the "empty" phase to wait for */
+        bool ring_full = false;                            /* all STAGES slots have been used once */
+        for (int64_t item = blockIdx.x; item < nitems; item += gridDim.x) {
+        const int64_t p = item / items_per_p;
+        const int rem = (int)(item - p * items_per_p);
+        const int64_t mu0 = (int64_t)(rem / ntiles_n) * K1_M;
+        const int64_t n0 = (int64_t)(rem % ntiles_n) * Cfg::NW;
+        const int64_t pb = (P0 + p) * npair;               /* index of B_P's first element in B */
+        const int pbpar = (int)(pb & 1);
+        const bool last_p = P0 + p == naux - 1;
         const double *__restrict__ Bp = B + pb;
         int64_t ncols = ldc - n0;                          /* valid columns of this N tile */
         if (ncols > Cfg::NW) ncols = Cfg::NW;
         const uint32_t c_bytes = K1_KG * (uint32_t)ncols * 32u;
         int64_t rows_valid = nao - mu0;
         if (rows_valid > K1_M) rows_valid = K1_M;
-        int slot = 0;
-        uint32_t phase = 1;                                /* parity of the "empty" phase to wait for */
         for (int kc = 0; kc < nk; ++kc) {
-            if (kc >= Cfg::STAGES) mbar_wait(empty_bar(slot), phase);
+            if (ring_full) mbar_wait(empty_bar(slot), phase);
             const int64_t nu0 = (int64_t)kc * K1_KC;
             const uint32_t a_dst = smem_base + slot * Cfg::STAGE_BYTES;
             const uint32_t bar = full_bar(slot);
@@ -181,13 +188,23 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
                     bulk_g2s(c_dst + g * Cfg::NW * 32, Ccat4 + (((int64_t)kc * K1_KG + g) * ldc + n0) * 4,
                              (uint32_t)ncols * 32u, bar);
             }
-            if (++slot == Cfg::STAGES) { slot = 0; phase ^= 1; }
+            if (++slot == Cfg::STAGES) { slot = 0; phase ^= 1; ring_full = true; }
         }
+        }   /* items */
     } else {
         /* ------------------------------------------------------------ consumers */
         reg_alloc<232>();
         const int cw = warp - K1_PRODUCERS / 32;           /* 0..7: rows 16*cw .. 16*cw+15 */
         const int lq = lane >> 2, lr = lane & 3;
+        int slot = 0;
+        uint32_t phase = 0;
+        for (int64_t item = blockIdx.x; item < nitems; item += gridDim.x) {
+        const int64_t p = item / items_per_p;
+        const int rem = (int)(item - p * items_per_p);
+        const int64_t mu0 = (int64_t)(rem / ntiles_n) * K1_M;
+        const int64_t n0 = (int64_t)(rem % ntiles_n) * Cfg::NW;
+        const int pbpar = (int)(((P0 + p) * npair) & 1);
+        const bool last_p = P0 + p == naux - 1;
         const bool warp_active = mu0 + 16 * cw < nao;
         /* per-lane alignment shifts of the two tile forms (see K1_LDD / K1_LDT) */
         const int sd_shift = (((lq & 3) == 1 || (lq & 3) == 2) ? 1 : 0) ^ pbpar;
@@ -198,8 +215,6 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
 #pragma unroll
             for (int nt = 0; nt < NT8; ++nt) acc[mt][nt][0] = acc[mt][nt][1] = 0.0;
 
-        int slot = 0;
-        uint32_t phase = 0;
         for (int kc = 0; kc < nk; ++kc) {
             mbar_wait(full_bar(slot), phase);
             if (warp_active) {
@@ -244,6 +259,7 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
                 }
             }
         }
+        }   /* items */
     }
 }
 
@@ -283,10 +299,18 @@ void k1_launch_t(const double *B, int64_t naux, int64_t nao, int64_t npair, int6
                              K1Cfg<NT8>::SMEM_BYTES);
         configured = true;
     }
-    const unsigned nib = (unsigned)((nao + K1_M - 1) / K1_M);
-    dim3 grid(nib * ntiles_n, (unsigned)np);
+    static int sm_count = 0;
+    if (!sm_count) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev);
+        if (sm_count <= 0) sm_count = 148;
+    }
+    const int64_t nib = (nao + K1_M - 1) / K1_M;
+    const int64_t nitems = nib * ntiles_n * np;
+    const unsigned grid = (unsigned)(nitems < sm_count ? nitems : sm_count);   /* persistent: 1 CTA / SM */
     k1_half_transform_kernel<NT8><<<grid, K1_THREADS, K1Cfg<NT8>::SMEM_BYTES, st>>>(
-        B, naux, nao, npair, P0, Ccat4, ldc, ldx, ntiles_n, X4);
+        B, naux, nao, npair, P0, Ccat4, ldc, ldx, ntiles_n, nitems, X4);
 }
 
 }  // namespace
