@@ -141,11 +141,16 @@ k2_syrk_lower_kernel(const double *__restrict__ X4, int64_t nao, int64_t np, int
 
     /* ---------------------------------------------------------------- consumers */
     const int cw = warp - 1;
-    const int wm = cw >> 2, wn = cw & 3;         /* warp tile: rows 64*wm.., cols 32*wn.. */
+    /* warp tiles: 2 (M) x 4 (N) of 64 x 32.  A tile of the ragged last block row with <= 64 valid
+     * rows would leave the lower four warps idle: it is covered 1 (M) x 8 (N) with 64 x 16 warp
+     * tiles instead, so all eight warps share the work ("narrow"; CTA-uniform). */
+    const bool narrow = nao - mu0 <= 64;
+    const int wm = narrow ? 0 : cw >> 2, wn = narrow ? cw : cw & 3;
+    const int wcols = narrow ? 16 : 32;          /* columns per warp tile */
     const int lq = lane >> 2, lr = lane & 3;
     /* skip warp tiles that lie outside the matrix or strictly above the diagonal */
-    const bool warp_active = (mu0 + 64 * wm < nao) && (nu0 + 32 * wn < nao) &&
-                             !(diag && 32 * wn > 64 * wm + 63);    /* diag is false when FULL */
+    const bool warp_active = (mu0 + 64 * wm < nao) && (nu0 + wcols * wn < nao) &&
+                             !(diag && wcols * wn > 64 * wm + 63);    /* diag is false when FULL */
     double acc[8][4][2];
 #pragma unroll
     for (int mt = 0; mt < 8; ++mt)
@@ -161,20 +166,38 @@ k2_syrk_lower_kernel(const double *__restrict__ X4, int64_t nao, int64_t np, int
             const double *Xa = reinterpret_cast<const double *>(smem_raw + slot * K2_STAGE_BYTES);
             const double *Xb = diag ? Xa : Xa + K2_OP_BYTES / 8;
             const double *a_base = Xa + (64 * wm + lq) * 4 + lr;
-            const double *b_base = Xb + (32 * wn + lq) * 4 + lr;
+            const double *b_base = Xb + (wcols * wn + lq) * 4 + lr;
+            if (!narrow) {
 #pragma unroll
-            for (int q = 0; q < K2_KG; ++q) {
-                if (q < n) {
-                    double a[8], b[4];
+                for (int q = 0; q < K2_KG; ++q) {
+                    if (q < n) {
+                        double a[8], b[4];
 #pragma unroll
-                    for (int mt = 0; mt < 8; ++mt) a[mt] = a_base[q * (K2_T * 4) + mt * 32];
+                        for (int mt = 0; mt < 8; ++mt) a[mt] = a_base[q * (K2_T * 4) + mt * 32];
 #pragma unroll
-                    for (int nt = 0; nt < 4; ++nt) b[nt] = b_base[q * (K2_T * 4) + nt * 32];
+                        for (int nt = 0; nt < 4; ++nt) b[nt] = b_base[q * (K2_T * 4) + nt * 32];
 #pragma unroll
-                    for (int mt = 0; mt < 8; ++mt)
+                        for (int mt = 0; mt < 8; ++mt)
 #pragma unroll
-                        for (int nt = 0; nt < 4; ++nt)
-                            dmma884(acc[mt][nt][0], acc[mt][nt][1], a[mt], b[nt]);
+                            for (int nt = 0; nt < 4; ++nt)
+                                dmma884(acc[mt][nt][0], acc[mt][nt][1], a[mt], b[nt]);
+                    }
+                }
+            } else {
+#pragma unroll
+                for (int q = 0; q < K2_KG; ++q) {
+                    if (q < n) {
+                        double a[8], b[2];
+#pragma unroll
+                        for (int mt = 0; mt < 8; ++mt) a[mt] = a_base[q * (K2_T * 4) + mt * 32];
+#pragma unroll
+                        for (int nt = 0; nt < 2; ++nt) b[nt] = b_base[q * (K2_T * 4) + nt * 32];
+#pragma unroll
+                        for (int mt = 0; mt < 8; ++mt)
+#pragma unroll
+                            for (int nt = 0; nt < 2; ++nt)
+                                dmma884(acc[mt][nt][0], acc[mt][nt][1], a[mt], b[nt]);
+                    }
                 }
             }
         }
@@ -190,7 +213,8 @@ k2_syrk_lower_kernel(const double *__restrict__ X4, int64_t nao, int64_t np, int
         if (mu >= nao) continue;
 #pragma unroll
         for (int nt = 0; nt < 4; ++nt) {
-            const int64_t nu = nu0 + 32 * wn + 8 * nt + 2 * lr;
+            if (narrow && nt >= 2) continue;
+            const int64_t nu = nu0 + wcols * wn + 8 * nt + 2 * lr;
             double *dst = Kp + mu * nao + nu;
             if (nu < nao) dst[0] = accumulate ? dst[0] + acc[mt][nt][0] : acc[mt][nt][0];
             if (nu + 1 < nao) dst[1] = accumulate ? dst[1] + acc[mt][nt][1] : acc[mt][nt][1];
