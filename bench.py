@@ -412,7 +412,7 @@ def run_extra(args, cfg):
     torch.cuda.synchronize()
     clocks = sampler.stop()
     ms = [a.elapsed_time(b) for a, b in ev]
-    t = float(np.mean(ms))
+    t = float(np.median(ms))                      # median: one-second steps see the odd outlier
     out = {"metric": f"df_{args.op}_gflops_fp64", "value": flops / (t * 1e-3) / 1e9, "unit": "GFLOP/s",
            "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "ms_per_step": t,
            "higher_is_better": True, "dtype": "f64", "data": "synthetic", "op": what,

@@ -153,8 +153,14 @@ j0_general_dt_kernel(const double *__restrict__ C1, const double *__restrict__ C
 
 /* ------------------------------------------------------------------ J1 */
 constexpr int J1_CH = 4096;          /* columns (pairs) per chunk; Dt chunk = 32 KB of smem */
-constexpr int J1_WARPS = 8;
-constexpr int J1_UNROLL = 8;         /* 128-bit loads in flight per lane */
+#ifndef DFJK_J1_WARPS
+#define DFJK_J1_WARPS 16   /* swept on B200 at cfg 4 (warps x unroll): 8x8 7.51 ms, 16x8 7.12, 16x6 7.07, 32x8 7.10, 16x16 7.62 */
+#endif
+#ifndef DFJK_J1_UNROLL
+#define DFJK_J1_UNROLL 8
+#endif
+constexpr int J1_WARPS = DFJK_J1_WARPS;
+constexpr int J1_UNROLL = DFJK_J1_UNROLL;         /* 128-bit loads in flight per lane */
 
 __global__ void __launch_bounds__(J1_WARPS * 32)
 j1_dot_kernel(const double *__restrict__ B, int64_t naux, int64_t npair,
@@ -251,8 +257,14 @@ __global__ void j1_reduce_kernel(const double *__restrict__ d_part, int64_t nchu
 }
 
 /* ------------------------------------------------------------------ J2 */
-constexpr int J2_THREADS = 256;
-constexpr int J2_UNROLL = 8;
+#ifndef DFJK_J2_THREADS
+#define DFJK_J2_THREADS 256
+#endif
+#ifndef DFJK_J2_UNROLL
+#define DFJK_J2_UNROLL 12  /* swept on B200 at cfg 4: 8 -> 8.13 ms, 12 -> 7.18, 16 -> 7.22, 32 -> 7.43 */
+#endif
+constexpr int J2_THREADS = DFJK_J2_THREADS;
+constexpr int J2_UNROLL = DFJK_J2_UNROLL;
 
 /* SQ == false: J2 proper, Jp_part[g][pair] = sum_{P in group g} d[P] B[P][pair].
  * SQ == true : the DF diagonal of Eq. 7, sum_P B[P][pair]^2 -- the same stream
