@@ -145,17 +145,24 @@ k2_syrk_lower_kernel(const double *__restrict__ X4, int64_t nao, int64_t np, int
      * rows would leave the lower four warps idle: it is covered 1 (M) x 8 (N) with 64 x 16 warp
      * tiles instead, so all eight warps share the work ("narrow"; CTA-uniform). */
     const bool narrow = nao - mu0 <= 64;
+    /* A full-height diagonal tile needs only its lower triangle: 20 units of 32 x 16 touch it.  They
+     * are dealt 3,3,3,3,2,2,2,2 to the eight warps as 32 x 48 / 32 x 32 warp tiles ("tri"), so the tile
+     * costs 24 instead of 32 DMMAs per warp and k-group (the 2 x 4 layout would leave two warps idle
+     * and the CTA would take as long as an off-diagonal one). */
+    const bool tri = diag && !narrow;
+    const int tr = (cw < 2 || cw == 4) ? 3 : (cw < 4 ? 2 : (cw < 7 ? 1 : 0));   /* 32-row strip */
+    const int tc0 = (cw == 1 || cw == 3) ? 3 : (cw == 4 ? 6 : (cw == 6 ? 2 : 0)); /* first 16-col unit */
     const int wm = narrow ? 0 : cw >> 2, wn = narrow ? cw : cw & 3;
-    const int wcols = narrow ? 16 : 32;          /* columns per warp tile */
+    const int wcols = narrow ? 16 : 32;          /* columns per warp tile (2 x 4 and 1 x 8 layouts) */
     const int lq = lane >> 2, lr = lane & 3;
+    const int row_w = tri ? 32 * tr : 64 * wm;   /* first row / column of this warp's tile */
+    const int col_w = tri ? 16 * tc0 : wcols * wn;
     /* skip warp tiles that lie outside the matrix or strictly above the diagonal */
-    const bool warp_active = (mu0 + 64 * wm < nao) && (nu0 + wcols * wn < nao) &&
-                             !(diag && wcols * wn > 64 * wm + 63);    /* diag is false when FULL */
-    double acc[8][4][2];
+    const bool warp_active = (mu0 + row_w < nao) && (nu0 + col_w < nao) &&
+                             !(diag && !tri && col_w > row_w + 63);    /* diag is false when FULL */
+    double acc[32][2];                           /* [mt*4+nt] (8 x 4, or 8 x 2 narrow); tri: [mt*6+nt] (4 x 6) */
 #pragma unroll
-    for (int mt = 0; mt < 8; ++mt)
-#pragma unroll
-        for (int nt = 0; nt < 4; ++nt) acc[mt][nt][0] = acc[mt][nt][1] = 0.0;
+    for (int t = 0; t < 32; ++t) acc[t][0] = acc[t][1] = 0.0;
 
     for (int kc = 0; kc < nk; ++kc) {
         const int slot = kc % K2_STAGES;
@@ -165,9 +172,43 @@ k2_syrk_lower_kernel(const double *__restrict__ X4, int64_t nao, int64_t np, int
             const int n = (int)((gend - g0 < K2_KG) ? gend - g0 : K2_KG);
             const double *Xa = reinterpret_cast<const double *>(smem_raw + slot * K2_STAGE_BYTES);
             const double *Xb = diag ? Xa : Xa + K2_OP_BYTES / 8;
-            const double *a_base = Xa + (64 * wm + lq) * 4 + lr;
-            const double *b_base = Xb + (wcols * wn + lq) * 4 + lr;
-            if (!narrow) {
+            const double *a_base = Xa + (row_w + lq) * 4 + lr;
+            const double *b_base = Xb + (col_w + lq) * 4 + lr;
+            if (tri) {
+                if (cw < 4) {
+#pragma unroll
+                    for (int q = 0; q < K2_KG; ++q) {
+                        if (q < n) {
+                            double a[4], b[6];
+#pragma unroll
+                            for (int mt = 0; mt < 4; ++mt) a[mt] = a_base[q * (K2_T * 4) + mt * 32];
+#pragma unroll
+                            for (int nt = 0; nt < 6; ++nt) b[nt] = b_base[q * (K2_T * 4) + nt * 32];
+#pragma unroll
+                            for (int mt = 0; mt < 4; ++mt)
+#pragma unroll
+                                for (int nt = 0; nt < 6; ++nt)
+                                    dmma884(acc[mt * 6 + nt][0], acc[mt * 6 + nt][1], a[mt], b[nt]);
+                        }
+                    }
+                } else {
+#pragma unroll
+                    for (int q = 0; q < K2_KG; ++q) {
+                        if (q < n) {
+                            double a[4], b[4];
+#pragma unroll
+                            for (int mt = 0; mt < 4; ++mt) a[mt] = a_base[q * (K2_T * 4) + mt * 32];
+#pragma unroll
+                            for (int nt = 0; nt < 4; ++nt) b[nt] = b_base[q * (K2_T * 4) + nt * 32];
+#pragma unroll
+                            for (int mt = 0; mt < 4; ++mt)
+#pragma unroll
+                                for (int nt = 0; nt < 4; ++nt)
+                                    dmma884(acc[mt * 6 + nt][0], acc[mt * 6 + nt][1], a[mt], b[nt]);
+                        }
+                    }
+                }
+            } else if (!narrow) {
 #pragma unroll
                 for (int q = 0; q < K2_KG; ++q) {
                     if (q < n) {
@@ -180,7 +221,7 @@ k2_syrk_lower_kernel(const double *__restrict__ X4, int64_t nao, int64_t np, int
                         for (int mt = 0; mt < 8; ++mt)
 #pragma unroll
                             for (int nt = 0; nt < 4; ++nt)
-                                dmma884(acc[mt][nt][0], acc[mt][nt][1], a[mt], b[nt]);
+                                dmma884(acc[mt * 4 + nt][0], acc[mt * 4 + nt][1], a[mt], b[nt]);
                     }
                 }
             } else {
@@ -196,7 +237,7 @@ k2_syrk_lower_kernel(const double *__restrict__ X4, int64_t nao, int64_t np, int
                         for (int mt = 0; mt < 8; ++mt)
 #pragma unroll
                             for (int nt = 0; nt < 2; ++nt)
-                                dmma884(acc[mt][nt][0], acc[mt][nt][1], a[mt], b[nt]);
+                                dmma884(acc[mt * 4 + nt][0], acc[mt * 4 + nt][1], a[mt], b[nt]);
                     }
                 }
             }
@@ -207,17 +248,34 @@ k2_syrk_lower_kernel(const double *__restrict__ X4, int64_t nao, int64_t np, int
 
     if (!warp_active) return;
     double *Kp = Kpart + (int64_t)split * nao * nao;
+    if (tri) {
+        const int ntw = cw < 4 ? 6 : 4;
+#pragma unroll
+        for (int mt = 0; mt < 4; ++mt) {
+            const int64_t mu = mu0 + row_w + 8 * mt + lq;
+            if (mu >= nao) continue;
+#pragma unroll
+            for (int nt = 0; nt < 6; ++nt) {
+                if (nt >= ntw) continue;
+                const int64_t nu = nu0 + col_w + 8 * nt + 2 * lr;
+                double *dst = Kp + mu * nao + nu;
+                if (nu < nao) dst[0] = accumulate ? dst[0] + acc[mt * 6 + nt][0] : acc[mt * 6 + nt][0];
+                if (nu + 1 < nao) dst[1] = accumulate ? dst[1] + acc[mt * 6 + nt][1] : acc[mt * 6 + nt][1];
+            }
+        }
+        return;
+    }
 #pragma unroll
     for (int mt = 0; mt < 8; ++mt) {
-        const int64_t mu = mu0 + 64 * wm + 8 * mt + lq;
+        const int64_t mu = mu0 + row_w + 8 * mt + lq;
         if (mu >= nao) continue;
 #pragma unroll
         for (int nt = 0; nt < 4; ++nt) {
             if (narrow && nt >= 2) continue;
-            const int64_t nu = nu0 + wcols * wn + 8 * nt + 2 * lr;
+            const int64_t nu = nu0 + col_w + 8 * nt + 2 * lr;
             double *dst = Kp + mu * nao + nu;
-            if (nu < nao) dst[0] = accumulate ? dst[0] + acc[mt][nt][0] : acc[mt][nt][0];
-            if (nu + 1 < nao) dst[1] = accumulate ? dst[1] + acc[mt][nt][1] : acc[mt][nt][1];
+            if (nu < nao) dst[0] = accumulate ? dst[0] + acc[mt * 4 + nt][0] : acc[mt * 4 + nt][0];
+            if (nu + 1 < nao) dst[1] = accumulate ? dst[1] + acc[mt * 4 + nt][1] : acc[mt * 4 + nt][1];
         }
     }
 }
