@@ -205,7 +205,11 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
         const int64_t n0 = (int64_t)(rem % ntiles_n) * Cfg::NW;
         const int pbpar = (int)(((P0 + p) * npair) & 1);
         const bool last_p = P0 + p == naux - 1;
-        const bool warp_active = mu0 + 16 * cw < nao;
+        /* a ragged last row block with <= 64 valid rows: each warp takes 8 rows instead of 16, so
+         * all eight warps share it (otherwise the upper four would idle) */
+        const bool half = nao - mu0 <= 64;
+        const int row_w = half ? 8 * cw : 16 * cw;
+        const bool warp_active = mu0 + row_w < nao;
         /* per-lane alignment shifts of the two tile forms (see K1_LDD / K1_LDT) */
         const int sd_shift = (((lq & 3) == 1 || (lq & 3) == 2) ? 1 : 0) ^ pbpar;
         const int st_shift = ((lr == 1 || lr == 2) ? 1 : 0) ^ pbpar;
@@ -221,20 +225,31 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
                 const double *As = reinterpret_cast<const double *>(smem_raw + slot * Cfg::STAGE_BYTES);
                 const double *Cs = As + K1_A_BYTES / 8;
                 const bool colform = k1_mode(mu0, (int64_t)kc * K1_KC, nao, last_p) == K1_MODE_COL;
-                const double *a_base = colform ? As + lr * K1_LDT + 16 * cw + lq + st_shift
-                                               : As + (16 * cw + lq) * K1_LDD + lr + sd_shift;
+                const double *a_base = colform ? As + lr * K1_LDT + row_w + lq + st_shift
+                                               : As + (row_w + lq) * K1_LDD + lr + sd_shift;
                 const int a_gstep = colform ? 4 * K1_LDT : 4;        /* next k-group */
                 const int a_mstep = colform ? 8 : 8 * K1_LDD;        /* next 8 rows */
                 const double *b_base = Cs + lq * 4 + lr;
 #pragma unroll
-                for (int g = 0; g < K1_KG; ++g) {
-                    const double a0 = a_base[g * a_gstep];
-                    const double a1 = a_base[g * a_gstep + a_mstep];
+                if (!half) {
 #pragma unroll
-                    for (int nt = 0; nt < NT8; ++nt) {
-                        const double b = b_base[g * (Cfg::NW * 4) + nt * 32];
-                        dmma884(acc[0][nt][0], acc[0][nt][1], a0, b);
-                        dmma884(acc[1][nt][0], acc[1][nt][1], a1, b);
+                    for (int g = 0; g < K1_KG; ++g) {
+                        const double a0 = a_base[g * a_gstep];
+                        const double a1 = a_base[g * a_gstep + a_mstep];
+#pragma unroll
+                        for (int nt = 0; nt < NT8; ++nt) {
+                            const double b = b_base[g * (Cfg::NW * 4) + nt * 32];
+                            dmma884(acc[0][nt][0], acc[0][nt][1], a0, b);
+                            dmma884(acc[1][nt][0], acc[1][nt][1], a1, b);
+                        }
+                    }
+                } else {
+#pragma unroll
+                    for (int g = 0; g < K1_KG; ++g) {
+                        const double a0 = a_base[g * a_gstep];
+#pragma unroll
+                        for (int nt = 0; nt < NT8; ++nt)
+                            dmma884(acc[0][nt][0], acc[0][nt][1], a0, b_base[g * (Cfg::NW * 4) + nt * 32]);
                     }
                 }
             }
@@ -246,8 +261,8 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
         if (warp_active) {
 #pragma unroll
             for (int mt = 0; mt < 2; ++mt) {
-                const int64_t mu = mu0 + 16 * cw + 8 * mt + lq;
-                if (mu >= nao) continue;
+                const int64_t mu = mu0 + row_w + 8 * mt + lq;
+                if (mu >= nao || (half && mt == 1)) continue;
 #pragma unroll
                 for (int nt = 0; nt < NT8; ++nt) {
                     const int64_t col = n0 + 8 * nt + 2 * lr;          /* even */
