@@ -220,15 +220,18 @@ int dfjk_get_d(dfjk_handle *h, double *d_out, void *stream);
  *   "k_splits"  number of partial-K accumulators the SYRK is split over (0 = automatic)
  *   "time_kernels"  1 = bracket every kernel launch with CUDA events on the call's stream
  *               (read back with dfjk_kernel_time); setting it (to 0 or 1) clears the record
- *   "j_fused"   1 = J in one HBM pass (row groups kept in L2 between the dot and
- *               the axpy), 0 = two plain streaming passes (default)
+ *   "j_fused"   1 (default) = in a call that builds J and K together, the fitting coefficients
+ *               d_P = <B_P, D> are read off the half-transformed tensor the K build produces
+ *               anyway (<B_P, C C^T> = <B_P C, C>), so B is streamed ONCE for J (the axpy pass)
+ *               instead of twice; 0 = always the two plain streaming passes over B (dot, then
+ *               axpy).  J-only calls and the general-density entry points always use two passes.
  */
 int dfjk_set_option(dfjk_handle *h, const char *name, int64_t value);
 
 /* kernel ids for dfjk_kernel_time (one per step of the path) */
 #define DFJK_KERNEL_K0   0   /* pack / zero-pad C_occ */
 #define DFJK_KERNEL_J0   1   /* build D-tilde */
-#define DFJK_KERNEL_J1   2   /* d_P = <B_P, D-tilde>       (streams B) */
+#define DFJK_KERNEL_J1   2   /* d_P = <B_P, D-tilde> (streams B), or <X_P, C> (streams X) when fused */
 #define DFJK_KERNEL_J1R  3   /* reduce d partials */
 #define DFJK_KERNEL_J2   4   /* Jp = sum_P d_P B_P         (streams B) */
 #define DFJK_KERNEL_J3   5   /* unpack Jp -> J */

@@ -157,6 +157,7 @@ extern "C" dfjk_handle *dfjk_create(int64_t naux, int64_t nao, const double *B_p
     if (!h) { fail(DFJK_ENOMEM, "dfjk_create: host allocation failed"); return nullptr; }
     memset(h, 0, sizeof *h);
     h->naux = naux; h->nao = nao; h->npair = nao * (nao + 1) / 2; h->B = B_packed; h->device = dev;
+    h->opt_j_fused = 1;
     int v = 0;
     cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev); h->sm_count = v > 0 ? v : 148;
     cudaDeviceGetAttribute(&v, cudaDevAttrL2CacheSize, dev); h->l2_bytes = v;
@@ -182,7 +183,10 @@ extern "C" dfjk_handle *dfjk_create(int64_t naux, int64_t nao, const double *B_p
     int rc = DFJK_OK;
     if (rc == DFJK_OK) rc = alloc_ws(h, &h->Ccat, round_up(nao, 32) * h->ldc_max);
     if (rc == DFJK_OK) rc = alloc_ws(h, &h->Dt, h->npair);
-    if (rc == DFJK_OK) rc = alloc_ws(h, &h->d_part, h->nchunk * naux);
+    /* d partials: J1's column chunks, or J1X's blocks at the widest ldc */
+    int64_t dparts = dfjk::j1x_num_blocks(nao, h->ldc_max);
+    if (dparts < h->nchunk) dparts = h->nchunk;
+    if (rc == DFJK_OK) rc = alloc_ws(h, &h->d_part, dparts * naux);
     if (rc == DFJK_OK) rc = alloc_ws(h, &h->d, naux);
     if (rc == DFJK_OK) rc = alloc_ws(h, &h->Jp_part, h->j2_groups * h->npair);
     if (rc == DFJK_OK) rc = alloc_ws(h, &h->X, h->x_doubles);
@@ -221,10 +225,7 @@ extern "C" int dfjk_set_option(dfjk_handle *h, const char *name, int64_t value)
         }
         h->opt_time_kernels = value; h->ev_used = 0; return DFJK_OK;
     }
-    if (!strcmp(name, "j_fused")) {
-        if (value != 0) return fail(DFJK_EINVAL, "j_fused=1 is not available in this build");
-        h->opt_j_fused = value; return DFJK_OK;
-    }
+    if (!strcmp(name, "j_fused")) { h->opt_j_fused = value != 0; return DFJK_OK; }
     return fail(DFJK_EINVAL, "dfjk_set_option: unknown option '%s'", name);
 }
 
@@ -260,7 +261,10 @@ int get_jk_impl(dfjk_handle *h, int nset, const double *const *C, const int64_t 
     /* K0: zero-padded concatenation [C_0 | C_1], each set padded to a multiple of 8 columns */
     { Timed t_(h, DFJK_KERNEL_K0, st); dfjk::launch_k0_pack_c(C, nocc, col0, nset, nao, ldc, h->Ccat, st); }
 
-    if (J) {
+    /* J and K in one call: d_P = <B_P, D> = sum_s w_s <X_P^s, C_s> is read off the half-transformed
+     * X that K1 writes anyway (J1X), so B is streamed once for J (J2) instead of twice */
+    const bool fused = J && any_k && h->opt_j_fused != 0;
+    if (J && !fused) {
         { Timed t_(h, DFJK_KERNEL_J0, st); dfjk::launch_j0_build_dt(h->Ccat, ldc, nao, nset, col0, nocc, w, h->Dt, st); }
         { Timed t_(h, DFJK_KERNEL_J1, st); dfjk::launch_j1_dot(h->B, naux, npair, h->Dt, h->d_part, h->sm_count, st); }
         { Timed t_(h, DFJK_KERNEL_J1R, st); dfjk::launch_j1_reduce(h->d_part, h->nchunk, naux, h->d, st); }
@@ -279,6 +283,10 @@ int get_jk_impl(dfjk_handle *h, int nset, const double *const *C, const int64_t 
         for (int64_t P0 = 0; P0 < naux; P0 += pc, ++chunk) {
             const int64_t np = (P0 + pc <= naux) ? pc : naux - P0;
             { Timed t_(h, DFJK_KERNEL_K1, st); dfjk::launch_k1_half_transform(h->B, naux, nao, npair, P0, np, h->Ccat, ldc, ldc, h->X, st); }
+            if (fused) {
+                Timed t_(h, DFJK_KERNEL_J1, st);
+                dfjk::launch_j1x_dot(h->X, h->Ccat, nao, np, ldc, ldc, nset, col0, nocc, w, P0, naux, h->d_part, st);
+            }
             for (int s = 0; s < nset; ++s)
                 if (K[s]) {
                     Timed t_(h, DFJK_KERNEL_K2, st);
@@ -293,6 +301,12 @@ int get_jk_impl(dfjk_handle *h, int nset, const double *const *C, const int64_t 
                 dfjk::launch_k3_finish(h->Kpart + (int64_t)s * h->nsplit_alloc * nao * nao, nsplit,
                                        nao, K[s], st);
             }
+    }
+    if (fused) {
+        { Timed t_(h, DFJK_KERNEL_J1R, st); dfjk::launch_j1_reduce(h->d_part, dfjk::j1x_num_blocks(nao, ldc), naux, h->d, st); }
+        { Timed t_(h, DFJK_KERNEL_J2, st); dfjk::launch_j2_axpy(h->B, naux, npair, h->d, h->Jp_part, h->j2_groups, st); }
+        { Timed t_(h, DFJK_KERNEL_J3, st); dfjk::launch_j3_unpack(h->Jp_part, h->j2_groups, npair, nao, J, st); }
+        h->have_d = true;
     }
     DFJK_CUDA_TRY(cudaGetLastError());
     return DFJK_OK;

@@ -246,6 +246,78 @@ j1_dot_kernel(const double *__restrict__ B, int64_t naux, int64_t npair,
     }
 }
 
+/* ------------------------------------------------------------------ J1X */
+/* d_P without a pass over B, for calls that also build K:  <B_P, C C^T> = <B_P C, C> = <X_P, C>, and
+ * X_P = B_P C is what K1 has just written.  So
+ *     d_P = sum_s w_s sum_{mu,i} X_P^s[mu][i] C_s[mu][i]
+ * is one pass over the X chunk (8.7 GB per call at cfg 4 instead of the 51 GB of B that J1 streams).
+ * X4[(p*ldx4 + cg)][mu][4] and Ccat4[(mu/4)][col][4] hold the same 4 x 4 block (4 rows mu, 4 columns)
+ * transposed to each other, each as 128 contiguous bytes.  A thread keeps ONE block of C in
+ * registers and walks 16 consecutive P with it; consecutive threads own consecutive row groups, so
+ * every X load of a warp is 4 KB contiguous.  The 256 shares of each P go through shared memory and
+ * are added in a fixed order: d_part[blockIdx.x][P] (deterministic; J1R adds the blocks). */
+constexpr int J1X_PB = 16;            /* P per CTA (16 x 264 doubles of static shared memory) */
+constexpr int J1X_PARTS = 256 / J1X_PB;
+
+__global__ void __launch_bounds__(256)
+j1x_dot_kernel(const double *__restrict__ X4, const double *__restrict__ Ccat4, int64_t nao, int64_t np,
+               int64_t ldx4, int64_t ldc, SetDesc sd, int64_t P0, int64_t naux, double *__restrict__ d_part)
+{
+    __shared__ double ts[J1X_PB][264];                     /* this thread's share of d_P, P in the CTA's range */
+    const int64_t nmg = (nao + 3) / 4, ncg = ldc / 4;
+    const int64_t blk = (int64_t)blockIdx.x * 256 + threadIdx.x;
+    const int64_t cg = blk / nmg, mg = blk - cg * nmg;
+    double w = 0.0;
+    if (cg < ncg)
+        for (int s = 0; s < sd.nset; ++s)
+            if (4 * cg >= sd.col0[s] && 4 * cg < sd.col0[s] + sd.nocc[s]) w = sd.w[s];
+    const int nrow = w != 0.0 ? (int)((nao - 4 * mg < 4) ? nao - 4 * mg : 4) : 0;
+    double c[4][4];                                        /* c[col][mu], pre-multiplied by w */
+#pragma unroll
+    for (int j = 0; j < 4; ++j)
+#pragma unroll
+        for (int m = 0; m < 4; ++m) c[j][m] = 0.0;
+    if (nrow > 0) {
+        const double2 *cp = reinterpret_cast<const double2 *>(Ccat4 + (mg * ldc + 4 * cg) * 4);
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const double2 a = cp[2 * j], b = cp[2 * j + 1];
+            c[j][0] = w * a.x; c[j][1] = w * a.y; c[j][2] = w * b.x; c[j][3] = w * b.y;
+        }
+    }
+    const int64_t p0 = (int64_t)blockIdx.y * J1X_PB;
+    const double *xbase = X4 + (cg * nao + 4 * mg) * 4;   /* + p * ldx4 * nao * 4 */
+    const int64_t pstride = ldx4 * nao * 4;
+#pragma unroll 4
+    for (int pp = 0; pp < J1X_PB; ++pp) {
+        const int64_t p = p0 + pp;
+        double t = 0.0;
+        if (p < np) {
+            const double2 *x = reinterpret_cast<const double2 *>(xbase + p * pstride);
+#pragma unroll
+            for (int m = 0; m < 4; ++m) {
+                if (m < nrow) {
+                    const double2 x01 = __ldcs(x + 2 * m), x23 = __ldcs(x + 2 * m + 1);
+                    t += x01.x * c[0][m] + x01.y * c[1][m] + x23.x * c[2][m] + x23.y * c[3][m];
+                }
+            }
+        }
+        ts[pp][threadIdx.x] = t;
+    }
+    __syncthreads();
+    /* thread (pp, part) adds 256 / PARTS of the 256 shares of P = p0 + pp, then the parts are added
+     * across lanes: a fixed order */
+    {
+        const int pp = threadIdx.x / J1X_PARTS, part = threadIdx.x % J1X_PARTS;
+        double acc = 0.0;
+#pragma unroll 8
+        for (int j = 0; j < 256 / J1X_PARTS; ++j) acc += ts[pp][part + J1X_PARTS * j];
+#pragma unroll
+        for (int o = 1; o < J1X_PARTS; o <<= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+        if (part == 0 && p0 + pp < np) d_part[(int64_t)blockIdx.x * naux + P0 + p0 + pp] = acc;
+    }
+}
+
 __global__ void j1_reduce_kernel(const double *__restrict__ d_part, int64_t nchunk, int64_t naux,
                                  double *__restrict__ d)
 {
@@ -397,6 +469,23 @@ void launch_j1_dot(const double *B, int64_t naux, int64_t npair, const double *D
     if (rg > 65535) rg = 65535;
     j1_dot_kernel<<<dim3((unsigned)nchunk, (unsigned)rg), J1_WARPS * 32, 0, st>>>(B, naux, npair, Dt,
                                                                                   d_part);
+}
+
+int64_t j1x_num_blocks(int64_t nao, int64_t ldc) { return (((nao + 3) / 4) * (ldc / 4) + 255) / 256; }
+
+void launch_j1x_dot(const double *X4, const double *Ccat4, int64_t nao, int64_t np, int64_t ldx, int64_t ldc,
+                    int nset, const int *col0, const int *nocc, const double *w, int64_t P0, int64_t naux,
+                    double *d_part, cudaStream_t st)
+{
+    SetDesc sd;
+    sd.nset = nset;
+    for (int s = 0; s < 4; ++s) {
+        sd.col0[s] = s < nset ? col0[s] : 0;
+        sd.nocc[s] = s < nset ? nocc[s] : 0;
+        sd.w[s] = s < nset ? w[s] : 0.0;
+    }
+    dim3 grid((unsigned)j1x_num_blocks(nao, ldc), (unsigned)((np + J1X_PB - 1) / J1X_PB));
+    j1x_dot_kernel<<<grid, 256, 0, st>>>(X4, Ccat4, nao, np, ldx / 4, ldc, sd, P0, naux, d_part);
 }
 
 void launch_j1_reduce(const double *d_part, int64_t nchunk, int64_t naux, double *d, cudaStream_t st)

@@ -55,7 +55,13 @@ def run_config(cfg_id, full_k):
         J, Ka, Kb = h.get_jk_u(Cd[0], Cd[1])
         Ks = [Ka, Kb]
     d = h.get_d()
+    # the same J by the two plain streaming passes over B (J-only calls never fuse)
+    J2 = h.get_jk(Cd[0], with_k=False)[0] if len(Cs) == 1 else h.get_jk_u(Cd[0], Cd[1], with_k=False)[0]
+    d2 = h.get_d()
     torch.cuda.synchronize()
+    assert relerr(J2.cpu().numpy(), J.cpu().numpy()) <= 1e-12
+    assert relerr(d2.cpu().numpy(), d.cpu().numpy()) <= 1e-12
+    del J2, d2
     J = J.cpu().numpy()
     Ks = [K.cpu().numpy() for K in Ks]
     d = d.cpu().numpy()

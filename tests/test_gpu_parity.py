@@ -102,7 +102,7 @@ def test_non_orthonormal_orbitals(dfjk):
 
 
 @pytest.mark.parametrize("opts", [dict(k_chunk=1), dict(k_chunk=3), dict(k_chunk=4, k_splits=1),
-                                  dict(k_chunk=7, k_splits=2)])
+                                  dict(k_chunk=7, k_splits=2), dict(j_fused=0), dict(j_fused=0, k_chunk=5)])
 def test_chunk_and_split_options(dfjk, opts):
     Bp, (C,) = rand_case(260, 23, (13,), seed=3)
     J, K, _ = run_restricted(dfjk, Bp, 260, C, **opts)
@@ -110,13 +110,18 @@ def test_chunk_and_split_options(dfjk, opts):
     assert relerr(J, Jo) <= TOL and relerr(K, Ko[0]) <= TOL
 
 
-def test_unrestricted(dfjk):
+@pytest.mark.parametrize("fused", [1, 0])
+def test_unrestricted(dfjk, fused):
     nao, naux = 210, 33
     Bp, (Ca, Cb) = rand_case(nao, naux, (19, 14), seed=8)
     h = dfjk.DFJK(dev(Bp), nao)
+    h.set_option("j_fused", fused)      # d_P from the half-transformed X (default) or by a pass over B
     J, Ka, Kb = h.get_jk_u(dev(Ca), dev(Cb))
+    d = h.get_d()
     torch.cuda.synchronize()
     Jo, Kao, Kbo = oracle.get_jk_unrestricted(Bp, nao, Ca, Cb)
+    _, _, do = oracle.get_jk(Bp, nao, [Ca, Cb], [1.0, 1.0], with_k=False)
+    assert relerr(d.cpu().numpy(), do) <= TOL
     assert relerr(J.cpu().numpy(), Jo) <= TOL
     assert relerr(Ka.cpu().numpy(), Kao) <= TOL
     assert relerr(Kb.cpu().numpy(), Kbo) <= TOL
@@ -133,8 +138,15 @@ def test_j_only_k_only_and_repeatability(dfjk):
     none_j, K2 = h.get_jk(Cd, with_j=False)
     torch.cuda.synchronize()
     assert none_k is None and none_j is None
+    # K is the same kernel sequence either way; J of a J-only call comes from two passes over B, J of a
+    # J+K call from the fused route (d_P read off X): same numbers up to summation order
+    assert torch.equal(K1, K2)
+    assert relerr(J2.cpu().numpy(), J1.cpu().numpy()) <= 1e-13
     # deterministic reductions: repeat calls are bitwise identical
-    assert torch.equal(J1, J2) and torch.equal(K1, K2)
+    J3, K3 = h.get_jk(Cd)
+    J4, _ = h.get_jk(Cd, with_k=False)
+    torch.cuda.synchronize()
+    assert torch.equal(J1, J3) and torch.equal(K1, K3) and torch.equal(J2, J4)
     # outputs are overwritten, not accumulated
     Jpre = torch.full((nao, nao), 7.0, dtype=torch.float64, device="cuda")
     Kpre = torch.full((nao, nao), -3.0, dtype=torch.float64, device="cuda")
