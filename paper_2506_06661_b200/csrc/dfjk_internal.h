@@ -59,7 +59,6 @@ void launch_j3_unpack(const double *Jp_part, int64_t ngroup, int64_t npair, int6
 /* K0: the zero-padded concatenation [C_0 | C_1 | ...] (every set padded to a multiple of 8
  * columns, ldc columns in total) in k-group-major layout
  *   Ccat4[(mu/4)*ldc*4 + c*4 + mu%4],  mu < round_up(nao, 32) (rows >= nao are zero). */
-/* A NULL C[s] stands for the nao x nao identity (nocc[s] = nao): used by the raw-dm build. */
 void launch_k0_pack_c(const double *const *C, const int *nocc, const int *col0, int nset,
                       int64_t nao, int64_t ldc, double *Ccat, cudaStream_t st);
 

@@ -12,8 +12,11 @@
  * One CTA owns a 128 x 128 tile of K for one k-split: 8 consumer warps as 2 (M) x 4 (N),
  * warp tile 64 x 32 = 8 x 4 DMMA.8x8x4 accumulators, 12 shared loads per 32 MMAs.  Both
  * operands are row panels of X, so A (row-major) and B (col-major) fragments are read with
- * the same pattern; diagonal tiles load the panel once; warp tiles outside the matrix or
- * strictly above the diagonal issue no MMAs.
+ * the same pattern; diagonal tiles load the panel once and use a triangular warp layout (the
+ * 20 units of 32 x 16 that touch the lower triangle, dealt 3,3,3,3,2,2,2,2); block rows with
+ * <= 64 valid rows use a 1 x 8 layout of 64 x 16 warp tiles, so no warp idles on ragged tiles.
+ * The same kernel with FULL = true covers all nb x nb tiles with operands from two column
+ * ranges of X (the non-symmetric product of the general-density entry points).
  * Splits: work item = (lower tile, split) with its own partial accumulator Kpart[split],
  * read-modify-written by exactly one CTA per launch => deterministic, no atomics.
  */
@@ -29,7 +32,6 @@ struct PackDesc {
     const double *C[4];
     int nocc[4];
     int col0[4];
-    int identity[4];      /* 1: the set is the nao x nao identity (C[s] unused) */
 };
 
 /* Ccat4[(mu/4)][c][mu%4], mu < nao16 (rows >= nao and padding columns are zero) */
@@ -44,8 +46,7 @@ __global__ void k0_pack_c_kernel(PackDesc pd, int64_t nao, int64_t nao16, int64_
     if (mu < nao)
         for (int s = 0; s < pd.nset; ++s)
             if (c >= pd.col0[s] && c < pd.col0[s] + pd.nocc[s])
-                v = pd.identity[s] ? (mu == c - pd.col0[s] ? 1.0 : 0.0)
-                                   : pd.C[s][mu * pd.nocc[s] + (c - pd.col0[s])];
+                v = pd.C[s][mu * pd.nocc[s] + (c - pd.col0[s])];
     Ccat4[((mu >> 2) * ldc + c) * 4 + (mu & 3)] = v;
 }
 
@@ -355,7 +356,6 @@ void launch_k0_pack_c(const double *const *C, const int *nocc, const int *col0, 
         pd.C[s] = s < nset ? C[s] : nullptr;
         pd.nocc[s] = s < nset ? nocc[s] : 0;
         pd.col0[s] = s < nset ? col0[s] : 0;
-        pd.identity[s] = (s < nset && C[s] == nullptr) ? 1 : 0;   /* NULL set = identity */
     }
     const int64_t nao16 = (nao + 31) / 32 * 32;   /* K1 stages cover 32 rows of C */
     const int64_t n = nao16 * ldc;
