@@ -224,7 +224,8 @@ int dfjk_get_d(dfjk_handle *h, double *d_out, void *stream);
  *               d_P = <B_P, D> are read off the half-transformed tensor the K build produces
  *               anyway (<B_P, C C^T> = <B_P C, C>), so B is streamed ONCE for J (the axpy pass)
  *               instead of twice; 0 = always the two plain streaming passes over B (dot, then
- *               axpy).  J-only calls and the general-density entry points always use two passes.
+ *               axpy).  Applies to dfjk_get_jk, dfjk_get_jk_u and dfjk_get_jk_pair (there
+ *               <B_P, C1 C2^T> = <B_P C1, C2>); J-only calls and raw-dm calls always use two passes.
  */
 int dfjk_set_option(dfjk_handle *h, const char *name, int64_t value);
 

@@ -285,7 +285,7 @@ int get_jk_impl(dfjk_handle *h, int nset, const double *const *C, const int64_t 
             { Timed t_(h, DFJK_KERNEL_K1, st); dfjk::launch_k1_half_transform(h->B, naux, nao, npair, P0, np, h->Ccat, ldc, ldc, h->X, st); }
             if (fused) {
                 Timed t_(h, DFJK_KERNEL_J1, st);
-                dfjk::launch_j1x_dot(h->X, h->Ccat, nao, np, ldc, ldc, nset, col0, nocc, w, P0, naux, h->d_part, st);
+                dfjk::launch_j1x_dot(h->X, h->Ccat, nao, np, ldc, ldc, 0, nset, col0, nocc, w, P0, naux, h->d_part, st);
             }
             for (int s = 0; s < nset; ++s)
                 if (K[s]) {
@@ -329,7 +329,9 @@ int get_jk_general_impl(dfjk_handle *h, const double *C1, const double *C2, int6
     if (dev != h->device) return fail(DFJK_EINVAL, "%s: handle belongs to device %d, current is %d", who, h->device, dev);
 
     const int64_t nao = h->nao, naux = h->naux, npair = h->npair;
-    if (J) {
+    /* pair form with J and K in one call: d_P = <B_P, C1 C2^T> = <B_P C1, C2> is read off X (J1X) */
+    const bool fused = J && K && C2 != nullptr && h->opt_j_fused != 0;
+    if (J && !fused) {
         { Timed t_(h, DFJK_KERNEL_J0, st); dfjk::launch_j0_general_dt(C1, C2, ncol, nao, h->Dt, st); }
         { Timed t_(h, DFJK_KERNEL_J1, st); dfjk::launch_j1_dot(h->B, naux, npair, h->Dt, h->d_part, h->sm_count, st); }
         { Timed t_(h, DFJK_KERNEL_J1R, st); dfjk::launch_j1_reduce(h->d_part, h->nchunk, naux, h->d, st); }
@@ -360,10 +362,21 @@ int get_jk_general_impl(dfjk_handle *h, const double *C1, const double *C2, int6
             const int64_t np = (P0 + pc <= naux) ? pc : naux - P0;
             { Timed t_(h, DFJK_KERNEL_K1, st); dfjk::launch_k1_half_transform(h->B, naux, nao, npair, P0, np, h->Ccat, ldc, ldx, h->X, st); }
             if (raw) { Timed t_(h, DFJK_KERNEL_K1, st); dfjk::launch_k1u_unpack(h->B, nao, npair, P0, np, ldx, w8, h->X, st); }
+            if (fused) {
+                const double one = 1.0;
+                Timed t_(h, DFJK_KERNEL_J1, st);
+                dfjk::launch_j1x_dot(h->X, h->Ccat, nao, np, ldx, ldc, w8, 1, col0, nocc, &one, P0, naux, h->d_part, st);
+            }
             { Timed t_(h, DFJK_KERNEL_K2, st);
               dfjk::launch_k2_gemm_full(h->X, nao, np, ldx, col0[0], col0[1], ncol, h->Kpart, nsplit, chunk > 0, st); }
         }
         { Timed t_(h, DFJK_KERNEL_K3, st); dfjk::launch_k3_sum(h->Kpart, nsplit, nao, K, st); }
+        if (fused) {
+            { Timed t_(h, DFJK_KERNEL_J1R, st); dfjk::launch_j1_reduce(h->d_part, dfjk::j1x_num_blocks(nao, ldc), naux, h->d, st); }
+            { Timed t_(h, DFJK_KERNEL_J2, st); dfjk::launch_j2_axpy(h->B, naux, npair, h->d, h->Jp_part, h->j2_groups, st); }
+            { Timed t_(h, DFJK_KERNEL_J3, st); dfjk::launch_j3_unpack(h->Jp_part, h->j2_groups, npair, nao, J, st); }
+            h->have_d = true;
+        }
     }
     DFJK_CUDA_TRY(cudaGetLastError());
     return DFJK_OK;

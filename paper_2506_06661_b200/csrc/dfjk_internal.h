@@ -35,11 +35,13 @@ void launch_j1_dot(const double *B, int64_t naux, int64_t npair, const double *D
                    double *d_part, int sm_count, cudaStream_t st);
 /* J1X: d_part[b][P0 + p] = block b's share of sum_s w_s <X_P^s, C_s> for the np rows of the X chunk
  * K1 has just written (= <B_P, sum_s w_s C_s C_s^T>: d_P without streaming B; used when K is built in
- * the same call).  b < j1x_num_blocks(nao, ldc); J1R adds the blocks. */
+ * the same call).  b < j1x_num_blocks(nao, ldc); J1R adds the blocks.  c_shift (columns, multiple of
+ * 4): the C block of X column c is Ccat column c + c_shift -- 0 for C C^T densities, the width of C1
+ * for the pair form, where d_P = <B_P C1, C2>. */
 int64_t j1x_num_blocks(int64_t nao, int64_t ldc);
 void launch_j1x_dot(const double *X4, const double *Ccat4, int64_t nao, int64_t np, int64_t ldx, int64_t ldc,
-                    int nset, const int *col0, const int *nocc, const double *w, int64_t P0, int64_t naux,
-                    double *d_part, cudaStream_t st);
+                    int64_t c_shift, int nset, const int *col0, const int *nocc, const double *w, int64_t P0,
+                    int64_t naux, double *d_part, cudaStream_t st);
 /* J1b: d[P] = sum_c d_part[c][P] (fixed order: deterministic). */
 void launch_j1_reduce(const double *d_part, int64_t nchunk, int64_t naux, double *d,
                       cudaStream_t st);

@@ -261,7 +261,8 @@ constexpr int J1X_PARTS = 256 / J1X_PB;
 
 __global__ void __launch_bounds__(256)
 j1x_dot_kernel(const double *__restrict__ X4, const double *__restrict__ Ccat4, int64_t nao, int64_t np,
-               int64_t ldx4, int64_t ldc, SetDesc sd, int64_t P0, int64_t naux, double *__restrict__ d_part)
+               int64_t ldx4, int64_t ldc, int64_t c_shift, SetDesc sd, int64_t P0, int64_t naux,
+               double *__restrict__ d_part)
 {
     __shared__ double ts[J1X_PB][264];                     /* this thread's share of d_P, P in the CTA's range */
     const int64_t nmg = (nao + 3) / 4, ncg = ldc / 4;
@@ -278,7 +279,9 @@ j1x_dot_kernel(const double *__restrict__ X4, const double *__restrict__ Ccat4, 
 #pragma unroll
         for (int m = 0; m < 4; ++m) c[j][m] = 0.0;
     if (nrow > 0) {
-        const double2 *cp = reinterpret_cast<const double2 *>(Ccat4 + (mg * ldc + 4 * cg) * 4);
+        /* c_shift: the C block is taken c_shift columns to the right of the X block (pair form:
+         * d_P = <B_P C1, C2> with Ccat = [C1 | C2]) */
+        const double2 *cp = reinterpret_cast<const double2 *>(Ccat4 + (mg * ldc + 4 * cg + c_shift) * 4);
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
             const double2 a = cp[2 * j], b = cp[2 * j + 1];
@@ -474,8 +477,8 @@ void launch_j1_dot(const double *B, int64_t naux, int64_t npair, const double *D
 int64_t j1x_num_blocks(int64_t nao, int64_t ldc) { return (((nao + 3) / 4) * (ldc / 4) + 255) / 256; }
 
 void launch_j1x_dot(const double *X4, const double *Ccat4, int64_t nao, int64_t np, int64_t ldx, int64_t ldc,
-                    int nset, const int *col0, const int *nocc, const double *w, int64_t P0, int64_t naux,
-                    double *d_part, cudaStream_t st)
+                    int64_t c_shift, int nset, const int *col0, const int *nocc, const double *w, int64_t P0,
+                    int64_t naux, double *d_part, cudaStream_t st)
 {
     SetDesc sd;
     sd.nset = nset;
@@ -485,7 +488,7 @@ void launch_j1x_dot(const double *X4, const double *Ccat4, int64_t nao, int64_t 
         sd.w[s] = s < nset ? w[s] : 0.0;
     }
     dim3 grid((unsigned)j1x_num_blocks(nao, ldc), (unsigned)((np + J1X_PB - 1) / J1X_PB));
-    j1x_dot_kernel<<<grid, 256, 0, st>>>(X4, Ccat4, nao, np, ldx / 4, ldc, sd, P0, naux, d_part);
+    j1x_dot_kernel<<<grid, 256, 0, st>>>(X4, Ccat4, nao, np, ldx / 4, ldc, c_shift, sd, P0, naux, d_part);
 }
 
 void launch_j1_reduce(const double *d_part, int64_t nchunk, int64_t naux, double *d, cudaStream_t st)

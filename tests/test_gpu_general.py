@@ -55,13 +55,15 @@ def test_pair_parity(dfjk, nao, naux, ncol):
     rng = np.random.default_rng(nao + ncol)
     C1, C2 = rng.standard_normal((nao, ncol)), rng.standard_normal((nao, ncol))
     h = dfjk.DFJK(dev(Bp), nao)
-    J, K = h.get_jk_pair(dev(C1), dev(C2))
-    d = h.get_d()
-    torch.cuda.synchronize()
     Jo, Ko, do = oracle.get_jk_pair(Bp, nao, C1, C2)
-    assert relerr(d.cpu().numpy(), do) <= TOL
-    assert relerr(J.cpu().numpy(), Jo) <= TOL
-    assert relerr(K.cpu().numpy(), Ko) <= TOL
+    for fused in (1, 0):             # d_P read off X = B_P C1 (default), or by a pass over B
+        h.set_option("j_fused", fused)
+        J, K = h.get_jk_pair(dev(C1), dev(C2))
+        d = h.get_d()
+        torch.cuda.synchronize()
+        assert relerr(d.cpu().numpy(), do) <= TOL
+        assert relerr(J.cpu().numpy(), Jo) <= TOL
+        assert relerr(K.cpu().numpy(), Ko) <= TOL
     h.close()
 
 
