@@ -4,8 +4,12 @@
  * kernels of j_kernels.cu / k1_half_transform.cu / k2_syrk.cu; there is no CPU
  * fallback (a missing device is DFJK_ECUDA).
  *
- *   get_jk = K0 pack C -> [J0 Dt -> J1 dot -> J1b reduce -> J2 axpy -> J3 unpack]
- *                      -> [for P-chunks: K1 half transform -> K2 SYRK (per set)] -> K3 finish
+ *   J and K together (default, "j_fused"):
+ *     K0 pack C -> for P-chunks: [K1 half transform -> J1X d_P from X -> K2 SYRK (per set)]
+ *               -> K3 finish -> J1R reduce -> J2 axpy (the one pass over B for J) -> J3 unpack
+ *   J only, or j_fused = 0:
+ *     K0 -> J0 Dt -> J1 dot -> J1R -> J2 axpy -> J3  (two streaming passes over B), then the K chain
+ *   general densities (get_jk_pair / _dm), building B (build_b) and the SCF driver live below.
  */
 #include "../../include/dfjk.h"
 #include "dfjk_internal.h"
