@@ -347,13 +347,10 @@ int64_t build_b_workspace_doubles(int64_t naux)
 cudaError_t launch_build_b(int64_t naux, int64_t npair, double *M, double *T, double *ws,
                            long long *info, cudaStream_t st)
 {
-    static bool configured = false;
-    if (!configured) {
-        cudaFuncSetAttribute(chol_diag_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, NB * (NB + 1) * 8);
-        cudaFuncSetAttribute(tri_inv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, NB * NB * 8);
-        cudaFuncSetAttribute(whiten_gemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, W_SMEM_BYTES);
-        configured = true;
-    }
+    static unsigned long long ok1 = 0, ok2 = 0, ok3 = 0;
+    ensure_dynamic_smem(chol_diag_kernel, NB * (NB + 1) * 8, ok1);
+    ensure_dynamic_smem(tri_inv_kernel, NB * NB * 8, ok2);
+    ensure_dynamic_smem(whiten_gemm_kernel, W_SMEM_BYTES, ok3);
     const int64_t ldw = (naux + NB - 1) / NB * NB;
     double *Aw = ws, *panel = ws + ldw * ldw;
     cudaError_t e = cudaMemsetAsync(Aw, 0, (size_t)(ldw * ldw) * sizeof(double), st);

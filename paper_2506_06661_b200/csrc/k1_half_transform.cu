@@ -308,19 +308,12 @@ template <int NT8>
 void k1_launch_t(const double *B, int64_t naux, int64_t nao, int64_t npair, int64_t P0, int64_t np,
                  const double *Ccat4, int64_t ldc, int64_t ldx, int ntiles_n, double *X4, cudaStream_t st)
 {
-    static bool configured = false;   /* attribute is per function, set once per process */
-    if (!configured) {
-        cudaFuncSetAttribute(k1_half_transform_kernel<NT8>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             K1Cfg<NT8>::SMEM_BYTES);
-        configured = true;
-    }
-    static int sm_count = 0;
-    if (!sm_count) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev);
-        if (sm_count <= 0) sm_count = 148;
-    }
+    static unsigned long long smem_ok = 0;
+    ensure_dynamic_smem(k1_half_transform_kernel<NT8>, K1Cfg<NT8>::SMEM_BYTES, smem_ok);
+    int dev = 0, sm_count = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev);
+    if (sm_count <= 0) sm_count = 148;
     const int64_t nib = (nao + K1_M - 1) / K1_M;
     const int64_t nitems = nib * ntiles_n * np;
     const unsigned grid = (unsigned)(nitems < sm_count ? nitems : sm_count);   /* persistent: 1 CTA / SM */

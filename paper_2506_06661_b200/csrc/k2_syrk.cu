@@ -365,12 +365,8 @@ void launch_k0_pack_c(const double *const *C, const int *nocc, const int *col0, 
 void launch_k2_syrk_lower(const double *X4, int64_t nao, int64_t np, int64_t ldc, int64_t col0,
                           int64_t ncol, double *Kpart, int nsplit, int accumulate, cudaStream_t st)
 {
-    static bool configured = false;
-    if (!configured) {
-        cudaFuncSetAttribute(k2_syrk_lower_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             K2_SMEM_BYTES);
-        configured = true;
-    }
+    static unsigned long long smem_ok = 0;
+    ensure_dynamic_smem(k2_syrk_lower_kernel<false>, K2_SMEM_BYTES, smem_ok);
     const int nb = (int)((nao + K2_T - 1) / K2_T);
     const int ntile = nb * (nb + 1) / 2;
     const int n4s = (int)((ncol + 3) / 4);              /* k step 4: Ccat's padding to 8 is not read */
@@ -382,12 +378,8 @@ void launch_k2_gemm_full(const double *X4, int64_t nao, int64_t np, int64_t ldc,
                          int64_t col0b, int64_t ncol, double *Kpart, int nsplit, int accumulate,
                          cudaStream_t st)
 {
-    static bool configured = false;
-    if (!configured) {
-        cudaFuncSetAttribute(k2_syrk_lower_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             K2_SMEM_BYTES);
-        configured = true;
-    }
+    static unsigned long long smem_ok = 0;
+    ensure_dynamic_smem(k2_syrk_lower_kernel<true>, K2_SMEM_BYTES, smem_ok);
     const int nb = (int)((nao + K2_T - 1) / K2_T);
     const int n4s = (int)((ncol + 3) / 4);
     k2_syrk_lower_kernel<true><<<dim3((unsigned)nsplit, (unsigned)(nb * nb)), K2_THREADS, K2_SMEM_BYTES, st>>>(

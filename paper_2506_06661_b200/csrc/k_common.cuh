@@ -104,5 +104,19 @@ __device__ __forceinline__ void reg_dealloc() { asm volatile("setmaxnreg.dec.syn
 template <int N>
 __device__ __forceinline__ void reg_alloc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
 
+/* Host side: the opt-in to more than 48 KB of dynamic shared memory is per function AND per device;
+ * `done` (one static word per call site) remembers the devices that already have it. */
+template <class F>
+inline void ensure_dynamic_smem(F func, int bytes, unsigned long long &done)
+{
+    int dev = 0;
+    cudaGetDevice(&dev);
+    const unsigned long long bit = 1ull << (dev & 63);
+    if (!(done & bit)) {
+        cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+        done |= bit;
+    }
+}
+
 }  // namespace dfjk
 #endif
