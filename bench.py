@@ -304,9 +304,22 @@ def run_ours(args, cfg):
     h.set_option("time_kernels", 0)
     total_ms = max_over_ranks(total_ms, dist, dev)
 
-    # ---- end to end through the host entry point (restricted configs)
+    # ---- end to end through the host entry points
     e2e = None
-    if not unrestricted:
+    if unrestricted:
+        Ch = [[torch.from_numpy(c).pin_memory() for c in s] for s in Cs_host]
+        Jh, Kah, Kbh = (torch.empty(cfg.nao, cfg.nao, dtype=torch.float64).pin_memory() for _ in range(3))
+        h.get_jk_u_host(Ch[0][0], Ch[0][1], Jh, Kah, Kbh)
+        barrier()
+        t0 = time.perf_counter()
+        for k in range(args.steps):
+            h.get_jk_u_host(Ch[args.warmup + k][0], Ch[args.warmup + k][1], Jh, Kah, Kbh)
+        e2e_s = max_over_ranks(time.perf_counter() - t0, dist, dev)
+        e2e = {"value": whole_job_value(flops_step(cfg), args.steps, e2e_s * 1e3, world), "unit": "GFLOP/s",
+               "ms_per_step": e2e_s * 1e3 / args.steps,
+               "h2d_bytes_per_step": cfg.nao * sum(cfg.nocc) * 8, "d2h_bytes_per_step": 3 * cfg.nao * cfg.nao * 8,
+               "api": "dfjk_get_jk_u_host (pinned host C_a, C_b in, pinned host J, K_a, K_b out; B resident)"}
+    else:
         nocc = cfg.nocc[0]
         Ch = [torch.from_numpy(s[0]).pin_memory() for s in Cs_host]
         Jh = torch.empty(cfg.nao, cfg.nao, dtype=torch.float64).pin_memory()

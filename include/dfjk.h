@@ -206,6 +206,16 @@ int dfjk_build_b(int64_t naux, int64_t nao, double *M, double *R_packed, int64_t
 int dfjk_get_df_diag(dfjk_handle *h, double *diag, void *stream);
 
 /*
+ * dfjk_get_jk_u_host -- the unrestricted build (dfjk_get_jk_u) for HOST orbitals and results, with the
+ * same copy-in / run / copy-out / synchronise sequence as dfjk_get_jk_host.
+ *   C_a_host (nao x nocc_a), C_b_host (nao x nocc_b): HOST;  J_host, K_a_host, K_b_host: HOST nao x nao,
+ *   any may be NULL, not all three.
+ */
+int dfjk_get_jk_u_host(dfjk_handle *h, const double *C_a_host, int64_t nocc_a,
+                       const double *C_b_host, int64_t nocc_b,
+                       double *J_host, double *K_a_host, double *K_b_host);
+
+/*
  * dfjk_get_d -- debug/inspection getter: copies the naux fitting coefficients
  * d_P of the most recent J build on this handle into d_out (DEVICE, naux doubles),
  * enqueued on `stream`.  DFJK_EINVAL if no J has been built yet.

@@ -31,6 +31,7 @@ SYMBOLS = (
     "dfjk_version", "dfjk_launch_count", "dfjk_kernel_time",
     "dfjk_get_jk_pair", "dfjk_get_jk_dm", "dfjk_get_jk_dms", "dfjk_get_df_diag",
     "dfjk_build_b", "dfjk_scf_rhf", "dfjk_probe_dmma_peak",
+    "dfjk_get_jk_u_host",
 )
 
 # DFJK_KERNEL_* ids of include/dfjk.h
@@ -85,6 +86,8 @@ def lib() -> ctypes.CDLL:
     L.dfjk_get_df_diag.argtypes = [vp, vp, vp]
     L.dfjk_get_jk_host.restype = ci
     L.dfjk_get_jk_host.argtypes = [vp, vp, i64, vp, vp]
+    L.dfjk_get_jk_u_host.restype = ci
+    L.dfjk_get_jk_u_host.argtypes = [vp, vp, i64, vp, i64, vp, vp, vp]
     L.dfjk_get_d.restype = ci
     L.dfjk_get_d.argtypes = [vp, vp, vp]
     L.dfjk_set_option.restype = ci
@@ -291,6 +294,27 @@ class DFJK:
             st = (stream or torch.cuda.current_stream(self.device)).cuda_stream
             _check(lib().dfjk_get_df_diag(self._h, out.data_ptr(), st), "dfjk_get_df_diag")
         return out
+
+    def get_jk_u_host(self, C_a_host, C_b_host, J_host=None, K_a_host=None, K_b_host=None):
+        """Unrestricted build with host orbitals / results (synchronous; B stays resident)."""
+        import torch
+        for t, name in ((C_a_host, "C_a_host"), (C_b_host, "C_b_host"), (J_host, "J_host"),
+                        (K_a_host, "K_a_host"), (K_b_host, "K_b_host")):
+            if t is not None and not (isinstance(t, torch.Tensor) and not t.is_cuda
+                                      and t.dtype == torch.float64 and t.is_contiguous()):
+                raise ValueError(f"{name} must be a contiguous CPU float64 tensor")
+        for C in (C_a_host, C_b_host):
+            if C.dim() != 2 or C.shape[0] != self.nao:
+                raise ValueError("C_a_host, C_b_host must be nao x nocc")
+        for t in (J_host, K_a_host, K_b_host):
+            if t is not None and t.numel() != self.nao * self.nao:
+                raise ValueError("J_host / K_host must be nao x nao")
+        ptr = lambda t: t.data_ptr() if t is not None else None
+        with torch.cuda.device(self.device):
+            _check(lib().dfjk_get_jk_u_host(self._h, C_a_host.data_ptr(), int(C_a_host.shape[1]),
+                                            C_b_host.data_ptr(), int(C_b_host.shape[1]),
+                                            ptr(J_host), ptr(K_a_host), ptr(K_b_host)), "dfjk_get_jk_u_host")
+        return J_host, K_a_host, K_b_host
 
     def get_d(self, stream=None):
         """Fitting coefficients d_P of the most recent J build (debug getter)."""

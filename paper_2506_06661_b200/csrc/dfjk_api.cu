@@ -76,7 +76,7 @@ struct dfjk_handle {
     int ev_cap, ev_used;
     /* host-call resources (lazy) */
     cudaStream_t host_stream;
-    double *hostC, *hostJ, *hostK;
+    double *hostC, *hostJ, *hostK, *hostC2, *hostK2;
 };
 
 namespace {
@@ -85,7 +85,7 @@ void free_all(dfjk_handle *h)
 {
     cudaFree(h->Ccat); cudaFree(h->Dt); cudaFree(h->d_part); cudaFree(h->d);
     cudaFree(h->Jp_part); cudaFree(h->X); cudaFree(h->Kpart);
-    cudaFree(h->hostC); cudaFree(h->hostJ); cudaFree(h->hostK);
+    cudaFree(h->hostC); cudaFree(h->hostJ); cudaFree(h->hostK); cudaFree(h->hostC2); cudaFree(h->hostK2);
     if (h->host_stream) cudaStreamDestroy(h->host_stream);
     for (int i = 0; i < 2 * h->ev_cap; ++i) cudaEventDestroy(h->ev[i]);
     delete[] h->ev;
@@ -566,6 +566,36 @@ extern "C" int dfjk_get_jk_host(dfjk_handle *h, const double *C_occ_host, int64_
     if (rc != DFJK_OK) return rc;
     if (J_host) DFJK_CUDA_TRY(cudaMemcpyAsync(J_host, h->hostJ, (size_t)n2 * 8, cudaMemcpyDeviceToHost, st));
     if (K_host) DFJK_CUDA_TRY(cudaMemcpyAsync(K_host, h->hostK, (size_t)n2 * 8, cudaMemcpyDeviceToHost, st));
+    DFJK_CUDA_TRY(cudaStreamSynchronize(st));
+    return DFJK_OK;
+}
+
+extern "C" int dfjk_get_jk_u_host(dfjk_handle *h, const double *C_a_host, int64_t nocc_a,
+                                  const double *C_b_host, int64_t nocc_b, double *J_host,
+                                  double *K_a_host, double *K_b_host)
+{
+    g_err[0] = 0;
+    if (!h) return fail(DFJK_EINVAL, "dfjk_get_jk_u_host: NULL handle");
+    if (!C_a_host || !C_b_host) return fail(DFJK_EINVAL, "dfjk_get_jk_u_host: orbital pointer is NULL");
+    if (nocc_a < 1 || nocc_a > h->nao || nocc_b < 1 || nocc_b > h->nao)
+        return fail(DFJK_EINVAL, "dfjk_get_jk_u_host: nocc outside [1, nao]");
+    if (!J_host && !K_a_host && !K_b_host) return fail(DFJK_EINVAL, "dfjk_get_jk_u_host: no output requested");
+    const int64_t n2 = h->nao * h->nao;
+    if (!h->host_stream) {
+        DFJK_CUDA_TRY(cudaStreamCreateWithFlags(&h->host_stream, cudaStreamNonBlocking));
+        if (alloc_ws(h, &h->hostC, n2) || alloc_ws(h, &h->hostJ, n2) || alloc_ws(h, &h->hostK, n2))
+            return DFJK_ENOMEM;
+    }
+    if (!h->hostC2 && (alloc_ws(h, &h->hostC2, n2) || alloc_ws(h, &h->hostK2, n2))) return DFJK_ENOMEM;
+    cudaStream_t st = h->host_stream;
+    DFJK_CUDA_TRY(cudaMemcpyAsync(h->hostC, C_a_host, (size_t)h->nao * nocc_a * 8, cudaMemcpyHostToDevice, st));
+    DFJK_CUDA_TRY(cudaMemcpyAsync(h->hostC2, C_b_host, (size_t)h->nao * nocc_b * 8, cudaMemcpyHostToDevice, st));
+    const int rc = dfjk_get_jk_u(h, h->hostC, nocc_a, h->hostC2, nocc_b, J_host ? h->hostJ : nullptr,
+                                 K_a_host ? h->hostK : nullptr, K_b_host ? h->hostK2 : nullptr, st);
+    if (rc != DFJK_OK) return rc;
+    if (J_host) DFJK_CUDA_TRY(cudaMemcpyAsync(J_host, h->hostJ, (size_t)n2 * 8, cudaMemcpyDeviceToHost, st));
+    if (K_a_host) DFJK_CUDA_TRY(cudaMemcpyAsync(K_a_host, h->hostK, (size_t)n2 * 8, cudaMemcpyDeviceToHost, st));
+    if (K_b_host) DFJK_CUDA_TRY(cudaMemcpyAsync(K_b_host, h->hostK2, (size_t)n2 * 8, cudaMemcpyDeviceToHost, st));
     DFJK_CUDA_TRY(cudaStreamSynchronize(st));
     return DFJK_OK;
 }

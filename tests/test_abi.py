@@ -34,6 +34,7 @@ def test_version_and_null_handling(L):
     assert L.dfjk_get_jk(None, None, 1, None, None, None) == -1
     assert b"NULL handle" in L.dfjk_last_error()
     assert L.dfjk_get_jk_host(None, None, 1, None, None) == -1
+    assert L.dfjk_get_jk_u_host(None, None, 1, None, 1, None, None, None) == -1
     assert L.dfjk_set_option(None, b"k_chunk", 1) == -1
     # general-density entry points (section 8f rank 1)
     assert L.dfjk_get_jk_pair(None, None, None, 1, None, None, None) == -1

@@ -181,6 +181,13 @@ def test_host_entry_point(dfjk):
     h.get_jk_host(Ch, Jh, Kh)
     Jo, Ko, _ = oracle.get_jk(Bp, nao, [C], [2.0])
     assert relerr(Jh.numpy(), Jo) <= TOL and relerr(Kh.numpy(), Ko[0]) <= TOL
+    # unrestricted host entry
+    Ca, Cb = gi.random_orbitals(nao, 7, 21), gi.random_orbitals(nao, 5, 22)
+    Kah = torch.empty(nao, nao, dtype=torch.float64).pin_memory()
+    Kbh = torch.empty(nao, nao, dtype=torch.float64).pin_memory()
+    h.get_jk_u_host(torch.from_numpy(Ca).pin_memory(), torch.from_numpy(Cb).pin_memory(), Jh, Kah, Kbh)
+    Juo, Kao, Kbo = oracle.get_jk_unrestricted(Bp, nao, Ca, Cb)
+    assert relerr(Jh.numpy(), Juo) <= TOL and relerr(Kah.numpy(), Kao) <= TOL and relerr(Kbh.numpy(), Kbo) <= TOL
     # pageable memory is accepted too
     Jp = torch.empty(nao, nao, dtype=torch.float64)
     h.get_jk_host(torch.from_numpy(C), Jp, None)
