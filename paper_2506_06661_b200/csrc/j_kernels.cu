@@ -251,13 +251,15 @@ j1_dot_kernel(const double *__restrict__ B, int64_t naux, int64_t npair,
  * X_P = B_P C is what K1 has just written.  So
  *     d_P = sum_s w_s sum_{mu,i} X_P^s[mu][i] C_s[mu][i]
  * is one pass over the X chunk (8.7 GB per call at cfg 4 instead of the 51 GB of B that J1 streams).
- * X4[(p*ldx4 + cg)][mu][4] and Ccat4[(mu/4)][col][4] hold the same 4 x 4 block (4 rows mu, 4 columns)
- * transposed to each other, each as 128 contiguous bytes.  A thread keeps ONE block of C in
- * registers and walks 16 consecutive P with it; consecutive threads own consecutive row groups, so
- * every X load of a warp is 4 KB contiguous.  The 256 shares of each P go through shared memory and
- * are added in a fixed order: d_part[blockIdx.x][P] (deterministic; J1R adds the blocks). */
-constexpr int J1X_PB = 16;            /* P per CTA (16 x 264 doubles of static shared memory) */
+ * For one P, X4[(p*ldx4 + cg)][mu][4] is a contiguous array of nao*ldx doubles; "unit" u is its
+ * u-th 16-byte piece = X_P[mu][col], X_P[mu][col+1] with col = 4 cg + 2 h, u = (cg*nao + mu)*2 + h.
+ * A thread takes one unit per tile of 256, keeps the two matching C values (times w) in registers
+ * and walks J1X_PB consecutive P with them: every warp load is 512 contiguous bytes.  A CTA covers
+ * J1X_TILES tiles; its 256 x PB shares are reduced through shared memory in a fixed order into
+ * d_part[blockIdx.x][P] (deterministic; J1R adds the blocks). */
+constexpr int J1X_PB = 16;            /* P per CTA */
 constexpr int J1X_PARTS = 256 / J1X_PB;
+constexpr int J1X_TILES = 8;          /* tiles of 256 units per CTA */
 
 __global__ void __launch_bounds__(256)
 j1x_dot_kernel(const double *__restrict__ X4, const double *__restrict__ Ccat4, int64_t nao, int64_t np,
@@ -265,48 +267,37 @@ j1x_dot_kernel(const double *__restrict__ X4, const double *__restrict__ Ccat4, 
                double *__restrict__ d_part)
 {
     __shared__ double ts[J1X_PB][264];                     /* this thread's share of d_P, P in the CTA's range */
-    const int64_t nmg = (nao + 3) / 4, ncg = ldc / 4;
-    const int64_t blk = (int64_t)blockIdx.x * 256 + threadIdx.x;
-    const int64_t cg = blk / nmg, mg = blk - cg * nmg;
-    double w = 0.0;
-    if (cg < ncg)
-        for (int s = 0; s < sd.nset; ++s)
-            if (4 * cg >= sd.col0[s] && 4 * cg < sd.col0[s] + sd.nocc[s]) w = sd.w[s];
-    const int nrow = w != 0.0 ? (int)((nao - 4 * mg < 4) ? nao - 4 * mg : 4) : 0;
-    double c[4][4];                                        /* c[col][mu], pre-multiplied by w */
-#pragma unroll
-    for (int j = 0; j < 4; ++j)
-#pragma unroll
-        for (int m = 0; m < 4; ++m) c[j][m] = 0.0;
-    if (nrow > 0) {
-        /* c_shift: the C block is taken c_shift columns to the right of the X block (pair form:
-         * d_P = <B_P C1, C2> with Ccat = [C1 | C2]) */
-        const double2 *cp = reinterpret_cast<const double2 *>(Ccat4 + (mg * ldc + 4 * cg + c_shift) * 4);
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            const double2 a = cp[2 * j], b = cp[2 * j + 1];
-            c[j][0] = w * a.x; c[j][1] = w * a.y; c[j][2] = w * b.x; c[j][3] = w * b.y;
-        }
-    }
+    const int64_t nunit = (ldc / 4) * nao * 2;             /* units that face columns of Ccat */
     const int64_t p0 = (int64_t)blockIdx.y * J1X_PB;
-    const double *xbase = X4 + (cg * nao + 4 * mg) * 4;   /* + p * ldx4 * nao * 4 */
-    const int64_t pstride = ldx4 * nao * 4;
-#pragma unroll 4
-    for (int pp = 0; pp < J1X_PB; ++pp) {
-        const int64_t p = p0 + pp;
-        double t = 0.0;
-        if (p < np) {
-            const double2 *x = reinterpret_cast<const double2 *>(xbase + p * pstride);
+    const int64_t pstride = ldx4 * nao * 4;                /* doubles between consecutive P */
+    double t[J1X_PB];
 #pragma unroll
-            for (int m = 0; m < 4; ++m) {
-                if (m < nrow) {
-                    const double2 x01 = __ldcs(x + 2 * m), x23 = __ldcs(x + 2 * m + 1);
-                    t += x01.x * c[0][m] + x01.y * c[1][m] + x23.x * c[2][m] + x23.y * c[3][m];
-                }
+    for (int pp = 0; pp < J1X_PB; ++pp) t[pp] = 0.0;
+    for (int tile = 0; tile < J1X_TILES; ++tile) {
+        const int64_t u = ((int64_t)blockIdx.x * J1X_TILES + tile) * 256 + threadIdx.x;
+        if (u >= nunit) break;
+        const int64_t row = u >> 1;                        /* cg*nao + mu */
+        const int64_t cg = row / nao, mu = row - cg * nao;
+        const int64_t col = 4 * cg + 2 * (u & 1);
+        double w = 0.0;
+        for (int s = 0; s < sd.nset; ++s)
+            if (col >= sd.col0[s] && col < sd.col0[s] + sd.nocc[s]) w = sd.w[s];
+        if (w == 0.0) continue;                            /* padding columns: C is zero there */
+        /* c_shift: the C columns are taken c_shift to the right of the X columns (pair form:
+         * d_P = <B_P C1, C2> with Ccat = [C1 | C2]) */
+        const double *cp = Ccat4 + ((mu >> 2) * ldc + col + c_shift) * 4 + (mu & 3);
+        const double c0 = w * cp[0], c1 = w * cp[4];
+        const double2 *x = reinterpret_cast<const double2 *>(X4) + u + p0 * (pstride / 2);
+#pragma unroll
+        for (int pp = 0; pp < J1X_PB; ++pp) {
+            if (p0 + pp < np) {
+                const double2 v = __ldcs(x + pp * (pstride / 2));
+                t[pp] += v.x * c0 + v.y * c1;
             }
         }
-        ts[pp][threadIdx.x] = t;
     }
+#pragma unroll
+    for (int pp = 0; pp < J1X_PB; ++pp) ts[pp][threadIdx.x] = t[pp];
     __syncthreads();
     /* thread (pp, part) adds 256 / PARTS of the 256 shares of P = p0 + pp, then the parts are added
      * across lanes: a fixed order */
@@ -474,7 +465,11 @@ void launch_j1_dot(const double *B, int64_t naux, int64_t npair, const double *D
                                                                                   d_part);
 }
 
-int64_t j1x_num_blocks(int64_t nao, int64_t ldc) { return (((nao + 3) / 4) * (ldc / 4) + 255) / 256; }
+int64_t j1x_num_blocks(int64_t nao, int64_t ldc)
+{
+    const int64_t per_cta = 256LL * J1X_TILES;
+    return ((ldc / 4) * nao * 2 + per_cta - 1) / per_cta;
+}
 
 void launch_j1x_dot(const double *X4, const double *Ccat4, int64_t nao, int64_t np, int64_t ldx, int64_t ldc,
                     int64_t c_shift, int nset, const int *col0, const int *nocc, const double *w, int64_t P0,
