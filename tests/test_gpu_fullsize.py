@@ -155,3 +155,44 @@ def test_cfg4_build_b_sampled_columns():
     Lo = oracle.cholesky_lower(M)
     assert relerr(Lg, Lo) <= TOL
     assert relerr(Bs, oracle.whiten(Lo, Rs)) <= TOL
+
+
+def test_cfg3_pair_full_matrices():
+    """dfjk_get_jk_pair at cfg 3's size (nao=800, naux=2600, ncol=66; B generated on the device):
+    full J and the full, non-symmetric K against the oracle, which reads the same bytes in slabs."""
+    import paper_2506_06661_b200 as pkg
+    cfg = gi.CONFIGS[3]
+    B = torch.empty(cfg.naux, cfg.npair, dtype=torch.float64, device="cuda")
+    gi.fill_B_device(cfg, B)
+    rng = np.random.default_rng(33)
+    C1 = gi.orbitals(cfg, 0)[0]
+    C2 = np.ascontiguousarray(C1 + 0.3 * rng.standard_normal(C1.shape))      # a response-like partner
+    h = pkg.DFJK(B, cfg.nao)
+    J, K = h.get_jk_pair(torch.from_numpy(C1).cuda(), torch.from_numpy(C2).cuda())
+    torch.cuda.synchronize()
+    Jo, Ko = np.zeros((cfg.nao, cfg.nao)), np.zeros((cfg.nao, cfg.nao))
+    slab = max(1, SLAB_BYTES // (cfg.npair * 8))
+    for P0 in range(0, cfg.naux, slab):
+        Js, Ks, _ = oracle.get_jk_pair(B[P0:P0 + slab].cpu().numpy(), cfg.nao, C1, C2)
+        Jo += Js
+        Ko += Ks
+    h.close()
+    assert relerr(J.cpu().numpy(), Jo) <= TOL
+    assert relerr(K.cpu().numpy(), Ko) <= TOL
+    assert relerr(K.cpu().numpy(), Ko.T) > 1e-3                  # K really is non-symmetric here
+
+
+def test_raw_dm_mid_size():
+    """dfjk_get_jk_dm at nao=400, naux=600 (4 x 4 K tiles, several X chunks of the 2 nao wide
+    half-transformed tensor): full J and K for a random non-symmetric dm."""
+    import paper_2506_06661_b200 as pkg
+    cfg = gi.custom_config(400, 600, (1,), seed=12)
+    Bp = gi.fill_B_host(cfg)
+    dm = np.random.default_rng(8).standard_normal((400, 400))
+    h = pkg.DFJK(torch.from_numpy(Bp).cuda(), 400)
+    J, K = h.get_jk_dm(torch.from_numpy(dm).cuda())
+    torch.cuda.synchronize()
+    Jo, Ko, _ = oracle.get_jk_dm(Bp, 400, dm)
+    h.close()
+    assert relerr(J.cpu().numpy(), Jo) <= TOL
+    assert relerr(K.cpu().numpy(), Ko) <= TOL
