@@ -96,3 +96,50 @@ def test_generators_for_the_scf_inputs():
     assert ev.min() > 0.5 and ev.max() / ev.min() < 100
     eps = scipy.linalg.eigh(h, S, eigvals_only=True)
     assert eps[9] - eps[8] > 1.0                                  # occupied/virtual gap
+
+
+# ---------------------------------------------------------------- unrestricted
+def uhf_energy_4index(Bp, nao, h, Ca, Cb):
+    il = np.tril_indices(nao)
+    Bf = np.zeros((Bp.shape[0], nao, nao)); Bf[:, il[0], il[1]] = Bp; Bf[:, il[1], il[0]] = Bp
+    eri = np.einsum("pmn,pls->mnls", Bf, Bf)
+    Da, Db = Ca @ Ca.T, Cb @ Cb.T
+    Dt = Da + Db
+    return float(np.sum(Dt * h) + 0.5 * np.einsum("mn,ls,mnls->", Dt, Dt, eri)
+                 - 0.5 * np.einsum("mn,ls,mlns->", Da, Da, eri) - 0.5 * np.einsum("mn,ls,mlns->", Db, Db, eri))
+
+
+def test_uhf_reduces_to_rhf_for_a_closed_shell():
+    """nocc_a = nocc_b from the same core guess: the spin blocks stay equal, every energy equals RHF's."""
+    cfg, Bp, h, S = case(20, 60, 4, 0.3)
+    r = scf.scf_rhf(Bp, 20, h, S, 4)
+    u = scf.scf_uhf(Bp, 20, h, S, 4, 4)
+    assert u["converged"] and len(u["e_hist"]) == len(r["e_hist"])
+    assert np.allclose(u["e_hist"], r["e_hist"], rtol=1e-11, atol=0)
+    assert np.allclose(u["D"][0] + u["D"][1], r["D"], rtol=0, atol=1e-9)
+
+
+def test_uhf_energy_formula_and_stationarity():
+    cfg, Bp, h, S = case(9, 20, 3, 0.3)
+    u = scf.scf_uhf(Bp, 9, h, S, 3, 1, max_iter=1)
+    C0 = scipy.linalg.eigh(h, S)[1]
+    E0 = uhf_energy_4index(Bp, 9, h, C0[:, :3], C0[:, :1])
+    assert abs(u["e_hist"][0] - E0) <= 1e-12 * abs(E0)            # textbook UHF energy, incl. the K factors
+    u = scf.scf_uhf(Bp, 9, h, S, 3, 1, conv_tol=1e-12)
+    assert u["converged"]
+    for s, n in ((0, 3), (1, 1)):
+        C, D, F = u["C"][s], u["D"][s], u["F"][s]
+        assert np.abs(F @ D @ S - S @ D @ F).max() <= 1e-6
+        assert np.abs(C.T @ S @ C - np.eye(9)).max() <= 1e-12
+        assert abs(np.trace(D @ S) - n) <= 1e-12
+        assert np.abs(D @ S @ D - D).max() <= 1e-12                # idempotent with weight 1
+    Efin = uhf_energy_4index(Bp, 9, h, u["C"][0][:, :3], u["C"][1][:, :1])
+    assert abs(u["e_hist"][-1] - Efin) <= 1e-9 * abs(Efin)
+
+
+def test_uhf_no_two_electron_term():
+    cfg, Bp, h, S = case(12, 4, 3, 0.0)
+    u = scf.scf_uhf(Bp, 12, h, S, 4, 2)
+    eps = scipy.linalg.eigh(h, S, eigvals_only=True)
+    assert u["converged"] and len(u["e_hist"]) == 2
+    assert abs(u["e_hist"][-1] - (eps[:4].sum() + eps[:2].sum())) <= 1e-12 * abs(eps[:4].sum())
