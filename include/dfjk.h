@@ -170,6 +170,23 @@ int dfjk_scf_rhf(dfjk_handle *h, const double *hcore, const double *S, int64_t n
                  int *converged, void *stream);
 
 /*
+ * dfjk_scf_uhf -- the unrestricted (two-spin) counterpart of dfjk_scf_rhf around dfjk_get_jk_u (the
+ * paper's UKS/UHF objects): Pople-Nesbet equations,
+ *     D_s = C_s,occ C_s,occ^T;  J = J[D_a + D_b];  K_s = K[D_s];  F_s = hcore + J - K_s
+ *     E = 1/2 sum_s sum D_s o (hcore + F_s);  e_s = F_s D_s S - S D_s F_s
+ * one DIIS over both spin blocks (B_ij = <e_a^i, e_a^j> + <e_b^i, e_b^j>), both spins started from the
+ * core guess, the same stopping rule (max over both spins of max|e_s|).
+ *   C_a, C_b             DEVICE nao x nao OUT;  mo_energy_a/b  DEVICE nao OUT or NULL
+ *   D_a, D_b             DEVICE nao x nao OUT or NULL (weight-1 spin densities)
+ *   other arguments as in dfjk_scf_rhf.  SYNCHRONOUS.
+ */
+int dfjk_scf_uhf(dfjk_handle *h, const double *hcore, const double *S, int64_t nocc_a,
+                 int64_t nocc_b, int64_t max_iter, double conv_tol, int64_t diis_space,
+                 double *C_a, double *C_b, double *mo_energy_a, double *mo_energy_b,
+                 double *D_a, double *D_b, double *e_hist, int64_t *n_iter, int *converged,
+                 void *stream);
+
+/*
  * dfjk_build_b -- build the whitened tensor on the device,
  * PAPER.md:353-356, Eq. 2-3:
  *     M_PQ = (chi_P|chi_Q) = L L^T                              Eq. 2

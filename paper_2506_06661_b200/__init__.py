@@ -31,7 +31,7 @@ SYMBOLS = (
     "dfjk_version", "dfjk_launch_count", "dfjk_kernel_time",
     "dfjk_get_jk_pair", "dfjk_get_jk_dm", "dfjk_get_jk_dms", "dfjk_get_df_diag",
     "dfjk_build_b", "dfjk_scf_rhf", "dfjk_probe_dmma_peak",
-    "dfjk_get_jk_u_host",
+    "dfjk_get_jk_u_host", "dfjk_scf_uhf",
 )
 
 # DFJK_KERNEL_* ids of include/dfjk.h
@@ -80,6 +80,10 @@ def lib() -> ctypes.CDLL:
                                ctypes.POINTER(ci), vp]
     L.dfjk_probe_dmma_peak.restype = ci
     L.dfjk_probe_dmma_peak.argtypes = [ctypes.POINTER(ctypes.c_double)]
+    L.dfjk_scf_uhf.restype = ci
+    L.dfjk_scf_uhf.argtypes = [vp, vp, vp, i64, i64, i64, ctypes.c_double, i64, vp, vp, vp, vp, vp, vp,
+                               ctypes.POINTER(ctypes.c_double), ctypes.POINTER(i64),
+                               ctypes.POINTER(ci), vp]
     L.dfjk_build_b.restype = ci
     L.dfjk_build_b.argtypes = [i64, i64, vp, vp, vp, vp]
     L.dfjk_get_df_diag.restype = ci
@@ -285,6 +289,26 @@ class DFJK:
                    "dfjk_scf_rhf")
         return dict(converged=bool(conv.value), e_hist=list(e_hist[:n_iter.value]), C=C,
                     mo_energy=eps, D=D, F=F)
+
+    def scf_uhf(self, hcore, S, nocc_a: int, nocc_b: int, max_iter: int = 50, conv_tol: float = 1e-10,
+                diis_space: int = 8, stream=None):
+        """Unrestricted DF-SCF around get_jk_u (dfjk_scf_uhf; synchronous).  Returns a dict with
+        converged, e_hist and two-element lists C, mo_energy, D."""
+        import torch
+        n2 = self.nao * self.nao
+        hp, sp = _dev_f64(hcore, "hcore", n2), _dev_f64(S, "S", n2)
+        C = [self._out(True), self._out(True)]
+        D = [self._out(True), self._out(True)]
+        eps = [torch.empty(self.nao, dtype=torch.float64, device=self.device) for _ in range(2)]
+        e_hist = (ctypes.c_double * int(max_iter))()
+        n_iter, conv = ctypes.c_int64(0), ctypes.c_int(0)
+        with torch.cuda.device(self.device):
+            st = (stream or torch.cuda.current_stream(self.device)).cuda_stream
+            _check(lib().dfjk_scf_uhf(self._h, hp, sp, int(nocc_a), int(nocc_b), int(max_iter),
+                                      float(conv_tol), int(diis_space), C[0].data_ptr(), C[1].data_ptr(),
+                                      eps[0].data_ptr(), eps[1].data_ptr(), D[0].data_ptr(), D[1].data_ptr(),
+                                      e_hist, ctypes.byref(n_iter), ctypes.byref(conv), st), "dfjk_scf_uhf")
+        return dict(converged=bool(conv.value), e_hist=list(e_hist[:n_iter.value]), C=C, mo_energy=eps, D=D)
 
     def get_df_diag(self, stream=None):
         """diag[mu][nu] = sum_P B_P[mu,nu]^2, the DF term of Eq. 7."""

@@ -484,8 +484,35 @@ extern "C" int dfjk_scf_rhf(dfjk_handle *h, const double *hcore, const double *S
     int dev = -1;
     DFJK_CUDA_TRY(cudaGetDevice(&dev));
     if (dev != h->device) return fail(DFJK_EINVAL, "dfjk_scf_rhf: handle belongs to device %d, current is %d", h->device, dev);
-    return dfjk::scf_rhf_run(h, h->nao, hcore, S, nocc, max_iter, conv_tol, diis_space, C, mo_energy, D, F,
-                             e_hist, n_iter, converged, (cudaStream_t)stream, g_err, sizeof g_err);
+    const int64_t no[1] = {nocc};
+    double *Cs[1] = {C}, *Ws[1] = {mo_energy}, *Ds[1] = {D}, *Fs[1] = {F};
+    return dfjk::scf_run(h, h->nao, 1, hcore, S, no, max_iter, conv_tol, diis_space, Cs, Ws, Ds, Fs,
+                         e_hist, n_iter, converged, (cudaStream_t)stream, g_err, sizeof g_err);
+}
+
+extern "C" int dfjk_scf_uhf(dfjk_handle *h, const double *hcore, const double *S, int64_t nocc_a,
+                            int64_t nocc_b, int64_t max_iter, double conv_tol, int64_t diis_space,
+                            double *C_a, double *C_b, double *mo_energy_a, double *mo_energy_b,
+                            double *D_a, double *D_b, double *e_hist, int64_t *n_iter, int *converged,
+                            void *stream)
+{
+    g_err[0] = 0;
+    if (!h) return fail(DFJK_EINVAL, "dfjk_scf_uhf: NULL handle");
+    if (!hcore || !S || !C_a || !C_b || !e_hist || !n_iter || !converged)
+        return fail(DFJK_EINVAL, "dfjk_scf_uhf: NULL pointer");
+    if (nocc_a < 1 || nocc_a > h->nao || nocc_b < 1 || nocc_b > h->nao)
+        return fail(DFJK_EINVAL, "dfjk_scf_uhf: nocc outside [1, nao]");
+    if (max_iter < 1) return fail(DFJK_EINVAL, "dfjk_scf_uhf: max_iter must be >= 1");
+    if (diis_space < 1 || diis_space > 16) return fail(DFJK_EINVAL, "dfjk_scf_uhf: diis_space outside [1, 16]");
+    if (!(conv_tol > 0.0)) return fail(DFJK_EINVAL, "dfjk_scf_uhf: conv_tol must be positive");
+    if (h->nao > 32768) return fail(DFJK_EINVAL, "dfjk_scf_uhf: nao too large for the dense eigensolver");
+    int dev = -1;
+    DFJK_CUDA_TRY(cudaGetDevice(&dev));
+    if (dev != h->device) return fail(DFJK_EINVAL, "dfjk_scf_uhf: handle belongs to device %d, current is %d", h->device, dev);
+    const int64_t no[2] = {nocc_a, nocc_b};
+    double *Cs[2] = {C_a, C_b}, *Ws[2] = {mo_energy_a, mo_energy_b}, *Ds[2] = {D_a, D_b}, *Fs[2] = {nullptr, nullptr};
+    return dfjk::scf_run(h, h->nao, 2, hcore, S, no, max_iter, conv_tol, diis_space, Cs, Ws, Ds, Fs,
+                         e_hist, n_iter, converged, (cudaStream_t)stream, g_err, sizeof g_err);
 }
 
 extern "C" int dfjk_build_b(int64_t naux, int64_t nao, double *M, double *R_packed, int64_t *info,

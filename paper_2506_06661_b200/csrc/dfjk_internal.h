@@ -119,9 +119,11 @@ void launch_fp64_tile_gemm(const double *A, int64_t lda, const double *Bop, int6
 /* ---------------------------------------------------------------- SCF driver (scf_rhf.cu) */
 struct dfjk_handle;
 namespace dfjk {
-int scf_rhf_run(dfjk_handle *h, int64_t nao, const double *hcore, const double *S, int64_t nocc,
-                int64_t max_iter, double conv_tol, int64_t diis_space, double *C_out,
-                double *mo_energy_out, double *D_out, double *F_out, double *e_hist, int64_t *n_iter,
-                int *converged, cudaStream_t st, char *err, size_t errlen);
+/* nspin = 1: restricted (get_jk), nspin = 2: unrestricted (get_jk_u); per-spin arguments are arrays */
+int scf_run(dfjk_handle *h, int64_t nao, int nspin, const double *hcore, const double *S,
+            const int64_t *nocc, int64_t max_iter, double conv_tol, int64_t diis_space,
+            double *const *C_out, double *const *mo_energy_out, double *const *D_out,
+            double *const *F_out, double *e_hist, int64_t *n_iter, int *converged, cudaStream_t st,
+            char *err, size_t errlen);
 }  // namespace dfjk
 #endif

@@ -190,26 +190,30 @@ bool solve_dense(std::vector<double> &A, std::vector<double> &b, int n)
     do {                                                                                   \
         cudaError_t e_ = (expr);                                                           \
         if (e_ != cudaSuccess) {                                                           \
-            snprintf(err, errlen, "dfjk_scf_rhf: %s: %s", #expr, cudaGetErrorString(e_));  \
+            snprintf(err, errlen, "dfjk_scf: %s: %s", #expr, cudaGetErrorString(e_));      \
             rc = DFJK_ECUDA;                                                               \
             goto done;                                                                     \
         }                                                                                  \
     } while (0)
 
-/* The loop of the file header.  All pointers except e_hist / n_iter / converged are DEVICE.
- * Returns a DFJK_* code; on failure `err` holds the message. */
-int scf_rhf_run(dfjk_handle *h, int64_t nao, const double *hcore, const double *S, int64_t nocc,
-                int64_t max_iter, double conv_tol, int64_t diis_space, double *C_out,
-                double *mo_energy_out, double *D_out, double *F_out, double *e_hist, int64_t *n_iter,
-                int *converged, cudaStream_t st, char *err, size_t errlen)
+/* The loop of the file header for nspin = 1 (restricted: D = 2 C_occ C_occ^T, get_jk) or nspin = 2
+ * (unrestricted: D_s = C_s,occ C_s,occ^T, get_jk_u; Pople-Nesbet with one DIIS over both spin
+ * blocks).  Per-spin arrays are indexed [s].  All pointers except e_hist / n_iter / converged are
+ * DEVICE.  Returns a DFJK_* code; on failure `err` holds the message. */
+int scf_run(dfjk_handle *h, int64_t nao, int nspin, const double *hcore, const double *S,
+            const int64_t *nocc, int64_t max_iter, double conv_tol, int64_t diis_space,
+            double *const *C_out, double *const *mo_energy_out, double *const *D_out,
+            double *const *F_out, double *e_hist, int64_t *n_iter, int *converged, cudaStream_t st,
+            char *err, size_t errlen)
 {
     Cusolver &cs = cusolver();
     if (!cs.ok()) {
-        snprintf(err, errlen, "dfjk_scf_rhf: libcusolver could not be loaded (%s)", dlerror() ? dlerror() : "symbols missing");
+        snprintf(err, errlen, "dfjk_scf: libcusolver could not be loaded (%s)", dlerror() ? dlerror() : "symbols missing");
         return DFJK_ECUDA;
     }
     const int64_t n2 = nao * nao;
     const int m_max = (int)diis_space;
+    const double dw = nspin == 1 ? 2.0 : 1.0;           /* density weight of one spin block */
     int rc = DFJK_OK;
     cusolverDnHandle_t sol = nullptr;
     double *ws = nullptr, *work = nullptr;
@@ -221,26 +225,34 @@ int scf_rhf_run(dfjk_handle *h, int64_t nao, const double *hcore, const double *
     *n_iter = 0;
     *converged = 0;
 
-    /* workspace layout (doubles): F, D, T1, T2, Va (eigenvector / A copy), Sb (B copy), C, J, K,
-     * C_occ, W, partials, scalars, then the DIIS rings */
-    const int64_t fixed = 9 * n2 + nao * nocc + nao + RED_BLOCKS + 8;
-    const int64_t total = fixed + 2 * (int64_t)m_max * n2;
-    double *F, *D, *T1, *T2, *Va, *Sb, *C, *J, *K, *Cocc, *W, *part, *scal, *Fring, *Ering;
+    /* workspace (doubles): per spin F, D, E(rr), C, K, C_occ, W and the DIIS rings; shared T1, T2, Va
+     * (eigenvector / A copy), Sb (B copy), J, partials, scalars */
+    const int64_t per_spin = 5 * n2 + nao * nao + nao + 2 * (int64_t)m_max * n2;
+    const int64_t total = nspin * per_spin + 5 * n2 + RED_BLOCKS + 8;
+    double *F[2], *D[2], *Er[2], *C[2], *K[2], *Cocc[2], *W[2], *Fring[2], *Ering[2];
+    double *T1, *T2, *Va, *Sb, *J, *part, *scal;
     const unsigned eb = (unsigned)((n2 + 255) / 256);
     const dim3 tgrid((unsigned)((nao + 31) / 32), (unsigned)((nao + 31) / 32));
 
     if (cs.create(&sol) != CUSOLVER_STATUS_SUCCESS || cs.set_stream(sol, st) != CUSOLVER_STATUS_SUCCESS) {
-        snprintf(err, errlen, "dfjk_scf_rhf: cusolverDnCreate / SetStream failed");
+        snprintf(err, errlen, "dfjk_scf: cusolverDnCreate / SetStream failed");
         rc = DFJK_ECUDA;
         goto done;
     }
     SCF_TRY(cudaMalloc((void **)&ws, (size_t)total * sizeof(double)));
-    F = ws; D = F + n2; T1 = D + n2; T2 = T1 + n2; Va = T2 + n2; Sb = Va + n2; C = Sb + n2;
-    J = C + n2; K = J + n2; Cocc = K + n2; W = Cocc + nao * nocc; part = W + nao;
-    scal = part + RED_BLOCKS; Fring = scal + 8; Ering = Fring + (int64_t)m_max * n2;
+    {
+        double *q = ws;
+        for (int s = 0; s < nspin; ++s) {
+            F[s] = q; q += n2; D[s] = q; q += n2; Er[s] = q; q += n2; C[s] = q; q += n2; K[s] = q; q += n2;
+            Cocc[s] = q; q += nao * nao; W[s] = q; q += nao;
+            Fring[s] = q; q += (int64_t)m_max * n2; Ering[s] = q; q += (int64_t)m_max * n2;
+        }
+        T1 = q; q += n2; T2 = q; q += n2; Va = q; q += n2; Sb = q; q += n2; J = q; q += n2;
+        part = q; q += RED_BLOCKS; scal = q;
+    }
     if (cs.sygvd_bufsize(sol, CUSOLVER_EIG_TYPE_1, CUSOLVER_EIG_MODE_VECTOR, CUBLAS_FILL_MODE_LOWER,
-                         (int)nao, Va, (int)nao, Sb, (int)nao, W, &lwork) != CUSOLVER_STATUS_SUCCESS) {
-        snprintf(err, errlen, "dfjk_scf_rhf: cusolverDnDsygvd_bufferSize failed");
+                         (int)nao, Va, (int)nao, Sb, (int)nao, W[0], &lwork) != CUSOLVER_STATUS_SUCCESS) {
+        snprintf(err, errlen, "dfjk_scf: cusolverDnDsygvd_bufferSize failed");
         rc = DFJK_ECUDA;
         goto done;
     }
@@ -250,13 +262,13 @@ int scf_rhf_run(dfjk_handle *h, int64_t nao, const double *hcore, const double *
     /* generalised symmetric eigenproblem A C = S C eps; a symmetric row-major matrix is its own
      * column-major image, the eigenvectors come back as columns of the column-major Va */
     {
-        auto diagonalise = [&](const double *A) -> int {
+        auto diagonalise = [&](const double *A, int s) -> int {
             if (cudaMemcpyAsync(Va, A, (size_t)n2 * 8, cudaMemcpyDeviceToDevice, st) != cudaSuccess) return 1;
             if (cudaMemcpyAsync(Sb, S, (size_t)n2 * 8, cudaMemcpyDeviceToDevice, st) != cudaSuccess) return 1;
             if (cs.sygvd(sol, CUSOLVER_EIG_TYPE_1, CUSOLVER_EIG_MODE_VECTOR, CUBLAS_FILL_MODE_LOWER, (int)nao,
-                         Va, (int)nao, Sb, (int)nao, W, work, lwork, dev_info) != CUSOLVER_STATUS_SUCCESS)
+                         Va, (int)nao, Sb, (int)nao, W[s], work, lwork, dev_info) != CUSOLVER_STATUS_SUCCESS)
                 return 2;
-            unpack_vectors_kernel<<<tgrid, 256, 0, st>>>(Va, nao, nocc, C, Cocc);
+            unpack_vectors_kernel<<<tgrid, 256, 0, st>>>(Va, nao, nocc[s], C[s], Cocc[s]);
             int info = 0;
             if (cudaMemcpyAsync(&info, dev_info, sizeof(int), cudaMemcpyDeviceToHost, st) != cudaSuccess) return 1;
             if (cudaStreamSynchronize(st) != cudaSuccess) return 1;
@@ -266,32 +278,40 @@ int scf_rhf_run(dfjk_handle *h, int64_t nao, const double *hcore, const double *
             reduce_partial_kernel<<<RED_BLOCKS, RED_THREADS, 0, st>>>(mode, a, b, c, n2, part);
             reduce_final_kernel<<<1, 32, 0, st>>>(mode, part, scale, out);
         };
+        auto read_scalars = [&](double *dst, int n) -> cudaError_t {
+            cudaError_t e = cudaMemcpyAsync(dst, scal, n * sizeof(double), cudaMemcpyDeviceToHost, st);
+            return e != cudaSuccess ? e : cudaStreamSynchronize(st);
+        };
 
-        int dr = diagonalise(hcore);                                    /* 0. core guess */
-        if (dr != 0) {
-            snprintf(err, errlen, "dfjk_scf_rhf: Dsygvd failed on the core guess (%d; S not positive definite?)", dr);
-            rc = DFJK_ECUDA;
-            goto done;
+        for (int s = 0; s < nspin; ++s) {                               /* 0. core guess, both spins */
+            const int dr = diagonalise(hcore, s);
+            if (dr != 0) {
+                snprintf(err, errlen, "dfjk_scf: Dsygvd failed on the core guess (%d; S not positive definite?)", dr);
+                rc = DFJK_ECUDA;
+                goto done;
+            }
         }
         for (int64_t k = 0; k < max_iter; ++k) {
-            rc = dfjk_get_jk(h, Cocc, nocc, J, K, (void *)st);
+            rc = nspin == 1 ? dfjk_get_jk(h, Cocc[0], nocc[0], J, K[0], (void *)st)
+                            : dfjk_get_jk_u(h, Cocc[0], nocc[0], Cocc[1], nocc[1], J, K[0], K[1], (void *)st);
             if (rc != DFJK_OK) { snprintf(err, errlen, "%s", dfjk_last_error()); goto done; }
-            fock_kernel<<<eb, 256, 0, st>>>(hcore, J, K, n2, F);
-            launch_fp64_tile_gemm(Cocc, nocc, Cocc, 1, nocc, D, nao, nao, nao, nocc, 2.0, 0.0, 0, st);
-            reduce(1, D, hcore, F, 0.5, scal + 0);                      /* E */
-            launch_fp64_tile_gemm(F, nao, D, nao, 1, T1, nao, nao, nao, nao, 1.0, 0.0, 0, st);   /* F D */
-            launch_fp64_tile_gemm(T1, nao, S, nao, 1, T2, nao, nao, nao, nao, 1.0, 0.0, 0, st);  /* F D S */
-            /* the new pair goes into the ring slot of the entry it evicts (or a fresh one) */
+            /* the new (F, e) pair goes into the ring slot of the entry it evicts (or a fresh one) */
             int slot;
             if ((int)slot_of.size() < m_max) slot = (int)slot_of.size();
             else slot = slot_of.front();
-            double *e_new = Ering + (int64_t)slot * n2, *f_new = Fring + (int64_t)slot * n2;
-            antisym_kernel<<<eb, 256, 0, st>>>(T2, nao, T1);            /* T1 = e (F D no longer needed) */
-            reduce(2, T1, nullptr, nullptr, 1.0, scal + 1);             /* max |e| */
-            double host2[2];
-            SCF_TRY(cudaMemcpyAsync(host2, scal, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
-            SCF_TRY(cudaStreamSynchronize(st));
-            const double E = host2[0], emax = host2[1];
+            for (int s = 0; s < nspin; ++s) {
+                fock_kernel<<<eb, 256, 0, st>>>(hcore, J, K[s], n2, F[s]);
+                launch_fp64_tile_gemm(Cocc[s], nocc[s], Cocc[s], 1, nocc[s], D[s], nao, nao, nao, nocc[s], dw, 0.0, 0, st);
+                reduce(1, D[s], hcore, F[s], 0.5, scal + s);            /* E_s = 1/2 sum D_s o (h + F_s) */
+                launch_fp64_tile_gemm(F[s], nao, D[s], nao, 1, T1, nao, nao, nao, nao, 1.0, 0.0, 0, st);   /* F D */
+                launch_fp64_tile_gemm(T1, nao, S, nao, 1, T2, nao, nao, nao, nao, 1.0, 0.0, 0, st);        /* F D S */
+                antisym_kernel<<<eb, 256, 0, st>>>(T2, nao, Er[s]);     /* e_s = F D S - S D F */
+                reduce(2, Er[s], nullptr, nullptr, 1.0, scal + 2 + s);  /* max |e_s| */
+            }
+            double hs[4] = {0.0, 0.0, 0.0, 0.0};
+            SCF_TRY(read_scalars(hs, 4));
+            const double E = nspin == 1 ? hs[0] : hs[0] + hs[1];
+            const double emax = nspin == 1 ? hs[2] : std::fmax(hs[2], hs[3]);
             e_hist[k] = E;
             *n_iter = k + 1;
             if (k > 0 && std::fabs(E - e_prev) <= conv_tol * std::fmax(1.0, std::fabs(E)) &&
@@ -308,16 +328,19 @@ int scf_rhf_run(dfjk_handle *h, int64_t nao, const double *hcore, const double *
                     for (int j = 0; j + 1 < m_max; ++j) Bmat[i * m_max + j] = Bmat[(i + 1) * m_max + j + 1];
             }
             slot_of.push_back(slot);
-            SCF_TRY(cudaMemcpyAsync(e_new, T1, (size_t)n2 * 8, cudaMemcpyDeviceToDevice, st));
-            SCF_TRY(cudaMemcpyAsync(f_new, F, (size_t)n2 * 8, cudaMemcpyDeviceToDevice, st));
+            for (int s = 0; s < nspin; ++s) {
+                SCF_TRY(cudaMemcpyAsync(Ering[s] + (int64_t)slot * n2, Er[s], (size_t)n2 * 8, cudaMemcpyDeviceToDevice, st));
+                SCF_TRY(cudaMemcpyAsync(Fring[s] + (int64_t)slot * n2, F[s], (size_t)n2 * 8, cudaMemcpyDeviceToDevice, st));
+            }
             const int m = (int)slot_of.size();
-            /* one dot per launch pair, read back one by one (m <= 16 scalars per iteration) */
+            /* B_im = sum_s <e_s^i, e_s^m>: one dot per launch pair, read back (m <= 16 per iteration) */
             for (int i = 0; i < m; ++i) {
-                reduce(0, Ering + (int64_t)slot_of[i] * n2, e_new, nullptr, 1.0, scal + 2);
-                double v;
-                SCF_TRY(cudaMemcpyAsync(&v, scal + 2, sizeof(double), cudaMemcpyDeviceToHost, st));
+                for (int s = 0; s < nspin; ++s)
+                    reduce(0, Ering[s] + (int64_t)slot_of[i] * n2, Er[s], nullptr, 1.0, scal + 4 + s);
+                double v[2] = {0.0, 0.0};
+                SCF_TRY(cudaMemcpyAsync(v, scal + 4, nspin * sizeof(double), cudaMemcpyDeviceToHost, st));
                 SCF_TRY(cudaStreamSynchronize(st));
-                Bmat[i * m_max + (m - 1)] = Bmat[(m - 1) * m_max + i] = v;
+                Bmat[i * m_max + (m - 1)] = Bmat[(m - 1) * m_max + i] = nspin == 1 ? v[0] : v[0] + v[1];
             }
             std::vector<double> A((size_t)(m + 1) * (m + 1), 0.0), rhs(m + 1, 0.0);
             for (int i = 0; i < m; ++i) {
@@ -326,25 +349,30 @@ int scf_rhf_run(dfjk_handle *h, int64_t nao, const double *hcore, const double *
             }
             rhs[m] = -1.0;
             if (!solve_dense(A, rhs, m + 1)) {
-                snprintf(err, errlen, "dfjk_scf_rhf: singular DIIS system at iteration %lld", (long long)k);
+                snprintf(err, errlen, "dfjk_scf: singular DIIS system at iteration %lld", (long long)k);
                 rc = DFJK_ECUDA;
                 goto done;
             }
-            Coefs cf;
-            cf.m = m;
-            for (int i = 0; i < m; ++i) { cf.c[i] = rhs[i]; cf.F[i] = Fring + (int64_t)slot_of[i] * n2; }
-            lincomb_kernel<<<eb, 256, 0, st>>>(cf, n2, T2);             /* T2 = F_ext */
-            dr = diagonalise(T2);
-            if (dr != 0) {
-                snprintf(err, errlen, "dfjk_scf_rhf: Dsygvd failed at iteration %lld (%d)", (long long)k, dr);
-                rc = DFJK_ECUDA;
-                goto done;
+            for (int s = 0; s < nspin; ++s) {
+                Coefs cf;
+                cf.m = m;
+                for (int i = 0; i < m; ++i) { cf.c[i] = rhs[i]; cf.F[i] = Fring[s] + (int64_t)slot_of[i] * n2; }
+                lincomb_kernel<<<eb, 256, 0, st>>>(cf, n2, T2);         /* T2 = F_s,ext */
+                const int dr = diagonalise(T2, s);
+                if (dr != 0) {
+                    snprintf(err, errlen, "dfjk_scf: Dsygvd failed at iteration %lld (%d)", (long long)k, dr);
+                    rc = DFJK_ECUDA;
+                    goto done;
+                }
             }
         }
-        SCF_TRY(cudaMemcpyAsync(C_out, C, (size_t)n2 * 8, cudaMemcpyDeviceToDevice, st));
-        if (mo_energy_out) SCF_TRY(cudaMemcpyAsync(mo_energy_out, W, (size_t)nao * 8, cudaMemcpyDeviceToDevice, st));
-        if (D_out) SCF_TRY(cudaMemcpyAsync(D_out, D, (size_t)n2 * 8, cudaMemcpyDeviceToDevice, st));
-        if (F_out) SCF_TRY(cudaMemcpyAsync(F_out, F, (size_t)n2 * 8, cudaMemcpyDeviceToDevice, st));
+        for (int s = 0; s < nspin; ++s) {
+            SCF_TRY(cudaMemcpyAsync(C_out[s], C[s], (size_t)n2 * 8, cudaMemcpyDeviceToDevice, st));
+            if (mo_energy_out && mo_energy_out[s])
+                SCF_TRY(cudaMemcpyAsync(mo_energy_out[s], W[s], (size_t)nao * 8, cudaMemcpyDeviceToDevice, st));
+            if (D_out && D_out[s]) SCF_TRY(cudaMemcpyAsync(D_out[s], D[s], (size_t)n2 * 8, cudaMemcpyDeviceToDevice, st));
+            if (F_out && F_out[s]) SCF_TRY(cudaMemcpyAsync(F_out[s], F[s], (size_t)n2 * 8, cudaMemcpyDeviceToDevice, st));
+        }
         SCF_TRY(cudaStreamSynchronize(st));
         SCF_TRY(cudaGetLastError());
     }

@@ -84,3 +84,46 @@ def test_scf_not_converged_and_errors(dfjk):
     with pytest.raises(dfjk.DFJKError):                                  # S not positive definite
         hd.scf_rhf(dev(h), dev(-S), 4)
     hd.close()
+
+
+@pytest.mark.parametrize("nao,naux,na,nb,scale,diis", [
+    (20, 60, 5, 3, 0.3, 8),
+    (48, 160, 6, 5, 0.2, 3),      # small DIIS space: the ring wraps
+    (150, 400, 14, 12, 0.2, 8),
+    (290, 300, 26, 24, 0.1, 6),
+])
+def test_uhf_matches_oracle(dfjk, nao, naux, na, nb, scale, diis):
+    """dfjk_scf_uhf against oracle.scf.scf_uhf: every iteration's energy, the spin densities and
+    orbital energies (same tolerances as the restricted test)."""
+    cfg = gi.custom_config(nao, naux, (na,), seed=3)
+    Bp = gi.fill_B_host(cfg) * scale
+    h, S = gi.core_hamiltonian(cfg), gi.overlap(cfg)
+    ref = scf.scf_uhf(Bp, nao, h, S, na, nb, conv_tol=1e-10, diis_space=diis)
+    hd = dfjk.DFJK(dev(Bp), nao)
+    out = hd.scf_uhf(dev(h), dev(S), na, nb, conv_tol=1e-10, diis_space=diis)
+    assert out["converged"] == ref["converged"] == True
+    e, eo = np.array(out["e_hist"]), ref["e_hist"]
+    assert len(e) == len(eo)
+    assert abs(e[0] - eo[0]) <= 1e-11 * abs(eo[0])
+    assert np.all(np.abs(e - eo) <= 1e-9 * np.abs(eo))
+    assert abs(e[-1] - eo[-1]) <= 1e-11 * abs(eo[-1])
+    for s, n in ((0, na), (1, nb)):
+        assert relerr(out["D"][s].cpu().numpy(), ref["D"][s]) <= 1e-7
+        assert relerr(out["mo_energy"][s].cpu().numpy(), ref["mo_energy"][s]) <= 1e-7
+        C = out["C"][s].cpu().numpy()
+        assert np.abs(C.T @ S @ C - np.eye(nao)).max() <= 1e-10
+        assert abs(np.trace(out["D"][s].cpu().numpy() @ S) - n) <= 1e-9
+    hd.close()
+
+
+def test_uhf_closed_shell_equals_rhf_on_the_device(dfjk):
+    cfg = gi.custom_config(48, 160, (5,), seed=3)
+    Bp = gi.fill_B_host(cfg) * 0.2
+    h, S = gi.core_hamiltonian(cfg), gi.overlap(cfg)
+    hd = dfjk.DFJK(dev(Bp), 48)
+    r = hd.scf_rhf(dev(h), dev(S), 5)
+    u = hd.scf_uhf(dev(h), dev(S), 5, 5)
+    assert r["converged"] and u["converged"] and len(r["e_hist"]) == len(u["e_hist"])
+    assert np.allclose(u["e_hist"], r["e_hist"], rtol=1e-11, atol=0)
+    assert relerr((u["D"][0] + u["D"][1]).cpu().numpy(), r["D"].cpu().numpy()) <= 1e-8
+    hd.close()
