@@ -166,3 +166,27 @@ def test_df_diag_parity(dfjk, nao, naux):
     torch.cuda.synchronize()
     assert relerr(diag.cpu().numpy(), oracle.df_diag(Bp, nao)) <= TOL
     h.close()
+
+
+def test_pair_is_the_orbital_derivative_of_get_jk_on_the_device(dfjk):
+    """SOSCF's use of the pair form: the first-order change of get_jk under
+    C -> C + eps V is 4 eps J_pair(C, V) and eps (K_pair + K_pair^T).  J and K are quadratic in C, so
+    the central difference of two get_jk calls is exact up to rounding -- a cross-check of the pair
+    kernels (full DMMA product, J from X) against the SYRK path that needs no oracle at all."""
+    nao, naux, nocc = 200, 30, 17
+    Bp = make_B(nao, naux, 9)
+    rng = np.random.default_rng(2)
+    C = gi.random_orbitals(nao, nocc, 3)
+    V = rng.standard_normal((nao, nocc))
+    eps = 1e-3
+    h = dfjk.DFJK(dev(Bp), nao)
+    Jp, Kp = h.get_jk(dev(C + eps * V))
+    Jm, Km = h.get_jk(dev(C - eps * V))
+    J1, K1 = h.get_jk_pair(dev(C), dev(V))
+    torch.cuda.synchronize()
+    dJ = ((Jp - Jm) / (2 * eps)).cpu().numpy()
+    dK = ((Kp - Km) / (2 * eps)).cpu().numpy()
+    K1n = K1.cpu().numpy()
+    assert relerr(dJ, 4.0 * J1.cpu().numpy()) <= 1e-9
+    assert relerr(dK, K1n + K1n.T) <= 1e-9
+    h.close()

@@ -194,3 +194,22 @@ def test_df_diag_pins():
     d1 = oracle.df_diag(Bp1, nao)
     ref = np.zeros((nao, nao)); ref[4, 2] = ref[2, 4] = 9.0
     assert np.array_equal(d1, ref)
+
+
+def test_pair_form_is_the_orbital_derivative_of_the_occupied_build():
+    """What the DF orbital Hessian of SOSCF contracts: for an orbital change
+    C -> C + eps V the restricted build changes, to first order, by the PAIR build of (C, V):
+        dJ = 4 eps J[C V^T],   dK = eps (K[C V^T] + K[C V^T]^T).
+    J and K are exactly quadratic in C, so a central difference gives the derivative up to rounding;
+    this pins oracle_jk_pair_slab against oracle_jk_slab (two different code paths)."""
+    nao, naux, nocc = 12, 9, 3
+    rng = np.random.default_rng(44)
+    Bp = rand_B(nao, naux, 5)
+    C = np.linalg.qr(rng.standard_normal((nao, nocc)))[0]
+    V = rng.standard_normal((nao, nocc))
+    eps = 1e-3
+    Jp, Kp, _ = oracle.get_jk(Bp, nao, [C + eps * V], [2.0])
+    Jm, Km, _ = oracle.get_jk(Bp, nao, [C - eps * V], [2.0])
+    J1, K1, _ = oracle.get_jk_pair(Bp, nao, C, V)
+    assert relerr((Jp - Jm) / (2 * eps), 4.0 * J1) < 1e-10
+    assert relerr((Kp[0] - Km[0]) / (2 * eps), K1 + K1.T) < 1e-10
