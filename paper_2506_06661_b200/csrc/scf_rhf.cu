@@ -1,6 +1,7 @@
 /*
- * scf_rhf.cu -- a closed-shell DF-SCF driver around the get_jk kernels (include/dfjk.h,
- * dfjk_scf_rhf).  The paper describes the loop in words only: the
+ * scf_rhf.cu -- the DF-SCF drivers around the get_jk kernels (include/dfjk.h: dfjk_scf_rhf,
+ * closed shell, and dfjk_scf_uhf, two spins -- one loop, scf_run, for both; SURVEY.md section 8f
+ * rank 4).  The paper describes the loop in words only: the
  * mean-field object iterates Fock build -> diagonalisation -> new density, DIIS being the default
  * accelerator (mf.kernel(dm0)), with get_jk(dm) -> (vj, vk)
  * as the expensive step.  Per iteration, all on the device:
@@ -16,7 +17,9 @@
  *                                                 dependency on it
  *     C (row-major), C_occ                        S5 (transpose of the column-major eigenvectors)
  *
- * The host reads back two scalars per iteration (E and max|e|) to decide convergence.
+ * Unrestricted: the same per spin block with D_s = C_s,occ C_s,occ^T, get_jk_u, F_s = hcore + J - K_s,
+ * E = sum_s 1/2 sum D_s o (hcore + F_s) and ONE DIIS over both blocks (B_ij = sum_s <e_s^i, e_s^j>).
+ * The host reads back a few scalars per iteration (E, max|e|, the new DIIS dots) to decide convergence.
  */
 #include "../../include/dfjk.h"
 #include "dfjk_internal.h"
