@@ -56,7 +56,7 @@ typedef struct dfjk_handle dfjk_handle;
  * dfjk_create -- bind a resident DF tensor and allocate the fixed workspace.
  *
  *   naux      number of auxiliary functions P (rows of B), >= 1
- *   nao       number of orbital basis functions, >= 1;  npair = nao*(nao+1)/2
+ *   nao       number of orbital basis functions, 1 <= nao <= 32640;  npair = nao*(nao+1)/2
  *   B_packed  DEVICE, naux*npair doubles:  B_packed[P*npair + mu*(mu+1)/2 + nu], mu >= nu
  *             (Eq. 1's T_{P,mu nu}; row-major lower triangle, R3/R4).
  *             BORROWED: never copied, never written, must stay valid and unchanged

@@ -144,7 +144,8 @@ extern "C" dfjk_handle *dfjk_create(int64_t naux, int64_t nao, const double *B_p
 {
     g_err[0] = 0;
     if (naux < 1 || nao < 1) { fail(DFJK_EINVAL, "dfjk_create: naux and nao must be >= 1"); return nullptr; }
-    if (nao > 46340) { fail(DFJK_EINVAL, "dfjk_create: nao too large"); return nullptr; }
+    /* 255 x 255 tiles of 128 keep every grid dimension below 65536 (one packed row is 4.3 GB there) */
+    if (nao > 32640) { fail(DFJK_EINVAL, "dfjk_create: nao > 32640 is not supported"); return nullptr; }
     if (!B_packed) { fail(DFJK_EINVAL, "dfjk_create: B_packed is NULL"); return nullptr; }
     if (((uintptr_t)B_packed & 15) != 0) { fail(DFJK_EINVAL, "dfjk_create: B_packed must be 16-byte aligned"); return nullptr; }
     int dev = 0;
