@@ -358,6 +358,7 @@ int get_jk_general_impl(dfjk_handle *h, const double *C1, const double *C2, int6
         int64_t pc = h->x_doubles / (nao * ldx);
         if (h->opt_k_chunk > 0 && h->opt_k_chunk < pc) pc = h->opt_k_chunk;
         if (pc > naux) pc = naux;
+        if (pc > 65535) pc = 65535;                /* K1U's grid.z */
         if (pc < 1) return fail(DFJK_ENOMEM, "%s: X workspace too small", who);
         const int nb = (int)((nao + 127) / 128);
         const int nsplit = h->opt_k_splits > 0 ? (int)h->opt_k_splits
