@@ -14,7 +14,8 @@
  * operands are row panels of X, so A (row-major) and B (col-major) fragments are read with
  * the same pattern; diagonal tiles load the panel once and use a triangular warp layout (the
  * 20 units of 32 x 16 that touch the lower triangle, dealt 3,3,3,3,2,2,2,2); block rows with
- * <= 64 valid rows use a 1 x 8 layout of 64 x 16 warp tiles, so no warp idles on ragged tiles.
+ * <= 64 valid rows use a 1 x 8 layout of 64 x 16 warp tiles (and, in the full product, block columns
+ * with <= 64 valid columns a 4 x 2 layout of 32 x 32), so no warp idles on ragged tiles.
  * The same kernel with FULL = true covers all nb x nb tiles with operands from two column
  * ranges of X (the non-symmetric product of the general-density entry points).
  * Splits: work item = (lower tile, split) with its own partial accumulator Kpart[split],
@@ -151,13 +152,16 @@ k2_syrk_lower_kernel(const double *__restrict__ X4, int64_t nao, int64_t np, int
      * costs 24 instead of 32 DMMAs per warp and k-group (the 2 x 4 layout would leave two warps idle
      * and the CTA would take as long as an off-diagonal one). */
     const bool tri = diag && !narrow;
+    /* full product only: a tile of the ragged last block COLUMN (<= 64 valid columns) would idle the
+     * warps of the right half: 4 (M) x 2 (N) warp tiles of 32 x 32 instead ("tall") */
+    const bool tall = FULL && !narrow && nao - nu0 <= 64;
     const int tr = (cw < 2 || cw == 4) ? 3 : (cw < 4 ? 2 : (cw < 7 ? 1 : 0));   /* 32-row strip */
     const int tc0 = (cw == 1 || cw == 3) ? 3 : (cw == 4 ? 6 : (cw == 6 ? 2 : 0)); /* first 16-col unit */
     const int wm = narrow ? 0 : cw >> 2, wn = narrow ? cw : cw & 3;
     const int wcols = narrow ? 16 : 32;          /* columns per warp tile (2 x 4 and 1 x 8 layouts) */
     const int lq = lane >> 2, lr = lane & 3;
-    const int row_w = tri ? 32 * tr : 64 * wm;   /* first row / column of this warp's tile */
-    const int col_w = tri ? 16 * tc0 : wcols * wn;
+    const int row_w = tri ? 32 * tr : (tall ? 32 * (cw >> 1) : 64 * wm);   /* first row / column of this warp's tile */
+    const int col_w = tri ? 16 * tc0 : (tall ? 32 * (cw & 1) : wcols * wn);
     /* skip warp tiles that lie outside the matrix or strictly above the diagonal */
     const bool warp_active = (mu0 + row_w < nao) && (nu0 + col_w < nao) &&
                              !(diag && !tri && col_w > row_w + 63);    /* diag is false when FULL */
@@ -175,7 +179,23 @@ k2_syrk_lower_kernel(const double *__restrict__ X4, int64_t nao, int64_t np, int
             const double *Xb = diag ? Xa : Xa + K2_OP_BYTES / 8;
             const double *a_base = Xa + (row_w + lq) * 4 + lr;
             const double *b_base = Xb + (col_w + lq) * 4 + lr;
-            if (tri) {
+            if (tall) {
+#pragma unroll
+                for (int q = 0; q < K2_KG; ++q) {
+                    if (q < n) {
+                        double a[4], b[4];
+#pragma unroll
+                        for (int mt = 0; mt < 4; ++mt) a[mt] = a_base[q * (K2_T * 4) + mt * 32];
+#pragma unroll
+                        for (int nt = 0; nt < 4; ++nt) b[nt] = b_base[q * (K2_T * 4) + nt * 32];
+#pragma unroll
+                        for (int mt = 0; mt < 4; ++mt)
+#pragma unroll
+                            for (int nt = 0; nt < 4; ++nt)
+                                dmma884(acc[mt * 4 + nt][0], acc[mt * 4 + nt][1], a[mt], b[nt]);
+                    }
+                }
+            } else if (tri) {
                 if (cw < 4) {
 #pragma unroll
                     for (int q = 0; q < K2_KG; ++q) {
@@ -269,7 +289,7 @@ k2_syrk_lower_kernel(const double *__restrict__ X4, int64_t nao, int64_t np, int
 #pragma unroll
     for (int mt = 0; mt < 8; ++mt) {
         const int64_t mu = mu0 + row_w + 8 * mt + lq;
-        if (mu >= nao) continue;
+        if (mu >= nao || (tall && mt >= 4)) continue;
 #pragma unroll
         for (int nt = 0; nt < 4; ++nt) {
             if (narrow && nt >= 2) continue;
