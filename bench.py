@@ -36,7 +36,7 @@ sys.path.insert(0, ROOT)
 
 import dfjk_inputs as gi  # noqa: E402
 
-FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12     # 37.2: SMs x FMA/clk/SM x 2 x max clock
+FP64_PEAK_FALLBACK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # only if the device cannot be queried
 HBM_FALLBACK_GBS = 6650.0
 
 
@@ -62,6 +62,26 @@ def measured_peaks():
             return json.load(f), "measured"
     except Exception:
         return {"hbm_gbs": HBM_FALLBACK_GBS}, "fallback"
+
+
+def fp64_peak(pkg):
+    """FP64 roofline denominator, read from the device: derived = SMs x 64 FMA/clk x 2 x peak SM
+    clock (dfjk_device_info), probe = the register-only DMMA loop (dfjk_probe_dmma_peak) measured in
+    this run; fractions are quoted against the smaller of the two, so that neither a different SKU
+    nor a capped box can flatter them."""
+    try:
+        info = pkg.device_info()
+        derived = info["fp64_peak_tflops"]
+    except Exception:
+        info, derived = {}, FP64_PEAK_FALLBACK_TFLOPS
+    probe = pkg.probe_fp64_peak()
+    used = min(derived, probe) if probe > 0 else derived
+    return {"peak": used, "derived_tflops": derived, "probe_tflops": probe,
+            "sm_count": info.get("sm_count"), "sm_clock_khz": info.get("sm_clock_khz"),
+            "source": f"min(derived, probe): derived = {info.get('sm_count')} SM x 64 FP64 FMA/clk x 2 x "
+                      f"{info.get('sm_clock_khz', 0) / 1e6:.3f} GHz (dfjk_device_info), probe = "
+                      "dfjk_probe_dmma_peak's register-only DMMA.8x8x4 loop measured in this run; "
+                      "sm_100a has no tcgen05 FP64 kind"}
 
 
 def max_over_ranks(x, dist=None, device="cpu"):
@@ -110,11 +130,11 @@ class ClockSampler:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
         self.proc.terminate()
         self.thread.join(timeout=2)
-        sm, mx, reasons = [], [], set()
+        sm, mx, pw, reasons = [], [], [], set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         for r in self.rows:
             try:
-                sm.append(float(r[0])); mx.append(float(r[1]))
+                sm.append(float(r[0])); mx.append(float(r[1])); pw.append(float(r[2]))
                 for n, v in zip(names, r[3:7]):
                     if v.lower().startswith("active"):
                         reasons.add(n)
@@ -122,6 +142,7 @@ class ClockSampler:
                 pass
         return {"sm_mhz": float(np.median(sm)) if sm else None,
                 "sm_max_mhz": max(mx) if mx else None, "samples": len(sm),
+                "power_w": float(np.median(pw)) if pw else None,
                 "reasons": sorted(reasons)}
 
 
@@ -173,28 +194,216 @@ def run_reference(args, cfg):
     print(json.dumps({
         "impl": "reference", "metric": "df_get_jk_gflops_fp64", "value": val, "unit": "GFLOP/s",
         "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": t * 1e3 * cfg.naux / rows, "higher_is_better": True, "scaling": "weak",
+        "ms_per_step": t * 1e3, "ms_per_step_scaled": t * 1e3 * cfg.naux / rows,
+        "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": workload_config(cfg, args),
         "cpu_baseline": {"value": val, "unit": "GFLOP/s", "cores": threads, "kind": "oracle",
                          "sample": sample},
         "e2e": {"value": val, "unit": "GFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
-        "note": "ms_per_step is the sample time scaled to all naux rows; flops are the algorithmic "
-                "count (4 naux npair + 3 naux nao^2 nocc), the oracle itself does the full-square work",
+        "note": "ms_per_step is the MEASURED time of one step = the oracle on the row sample; "
+                "ms_per_step_scaled extrapolates it to all naux rows (the oracle is linear in P); value "
+                "is a rate: algorithmic flops of the sample (4 npair + 3 nao^2 nocc per row) over the "
+                "measured time, the oracle itself does the full-square work",
     }))
 
 
-def workload_config(cfg, args):
+def workload_config(cfg, args, fused=True):
     origin = (f"BASELINE.json configs[{cfg.index - 1}]" if cfg.index <= 5 else
               "LRDF-shaped workload (PAPER.md:433-450, naux = nao/10; not a BASELINE config)")
+    passes = ("twice (K1's unpack, J2's axpy; d_P is read off the half-transformed X)" if fused else
+              "three times (J1 dot, J2 axpy, K1's unpack)")
     return {"workload": f"{origin} '{cfg.name}': nao={cfg.nao} "
                         f"naux={cfg.naux} nocc={'+'.join(map(str, cfg.nocc))} seed={cfg.seed}",
             "nao": cfg.nao, "naux": cfg.naux, "nocc": list(cfg.nocc),
             "b_bytes": cfg.b_bytes, "calls_per_step": 1,
-            "l2": "inputs larger than L2: every step streams the packed B "
-                  f"({cfg.b_bytes / 1e9:.1f} GB) three times" if cfg.b_bytes > (1 << 30) else
-                  "L2 flushed between steps (256 MB write)",
+            "l2": f"inputs larger than L2: every step streams the packed B ({cfg.b_bytes / 1e9:.1f} GB) {passes}"
+                  if cfg.b_bytes > (1 << 30) else "L2 flushed between steps (256 MB write)",
             "parallelism": f"replicas x{args.gpus}" if args.gpus > 1 else "single GPU"}
+
+
+class Workload:
+    """One config resident on the device: B generated in place, a handle, the call schedule."""
+
+    def __init__(self, pkg, cfg, dev, ncalls):
+        import torch
+        self.pkg, self.cfg, self.dev = pkg, cfg, dev
+        self.unrestricted = len(cfg.nocc) == 2
+        self.B = torch.empty(cfg.naux, cfg.npair, dtype=torch.float64, device=dev)
+        gi.fill_B_device(cfg, self.B)
+        self.h = pkg.DFJK(self.B, cfg.nao)
+        self.Cs_host = list(gi.orbital_sequence(cfg, ncalls))          # [call][set] numpy, host
+        self.Cs_dev = [[torch.from_numpy(C).to(dev) for C in sets] for sets in self.Cs_host]
+        self.flush = (None if cfg.b_bytes > (1 << 30)
+                      else torch.empty(256 << 20, dtype=torch.uint8, device=dev))
+
+    def step(self, k, **kw):
+        sets = self.Cs_dev[k % len(self.Cs_dev)]
+        if self.unrestricted:
+            return self.h.get_jk_u(sets[0], sets[1], **kw)
+        return self.h.get_jk(sets[0], **kw)
+
+    def close(self):
+        import torch
+        self.h.close()
+        del self.B, self.Cs_dev, self.flush
+        torch.cuda.empty_cache()
+
+
+def timed_steps(wl, first, steps, barrier, local, step_fn=None):
+    """`steps` steps bracketed by CUDA events on the launching stream, barrier + synchronize on both
+    sides, clocks sampled meanwhile.  Per-kernel event brackets are OFF here (they would sit inside
+    the timed region); kernel_breakdown() collects them from an untimed pass over the same calls."""
+    import torch
+    wl.h.set_option("time_kernels", 0)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+          for _ in range(steps)]
+    step_fn = step_fn or wl.step
+    launches0 = wl.h.launch_count
+    sampler = ClockSampler(local)
+    barrier()
+    sampler.start()
+    for k in range(steps):
+        if wl.flush is not None:
+            wl.flush.fill_(k & 0xFF)
+        ev[k][0].record()
+        step_fn(first + k)
+        ev[k][1].record()
+    barrier()
+    clocks = sampler.stop()
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    return step_ms, clocks, wl.h.launch_count - launches0
+
+
+def kernel_breakdown(wl, first, steps, **kw):
+    """Per-kernel CUDA-event times (ms per step) of the same calls, launched again OUTSIDE the
+    timed region with the library's event brackets on."""
+    import torch
+    wl.h.set_option("time_kernels", 1)
+    for k in range(steps):
+        wl.step(first + k, **kw)
+    torch.cuda.synchronize()
+    kt = {name: wl.h.kernel_time(name) for name in wl.pkg.KERNELS}
+    wl.h.set_option("time_kernels", 0)
+    return {n: (ms / steps, cnt) for n, (ms, cnt) in kt.items()}
+
+
+def j_and_k_summary(cfg, kt, peak, hbm, peak_src):
+    """J / K sub-records from a per-step kernel breakdown."""
+    k1, k2 = kt["K1"][0], kt["K2"][0]
+    j_ms = sum(kt[n][0] for n in ("J0", "J1", "J1R", "J2", "J3"))
+    k_ms = sum(kt[n][0] for n in ("K1", "K2", "K3"))
+    j2 = kt["J2"][0]
+    kf = flops_k1(cfg) + flops_k2(cfg)
+    return ({"ms": j_ms, "fused": True, "stream_ms": j2, "bytes": cfg.b_bytes,
+             "gbs": cfg.b_bytes / (j2 * 1e-3) / 1e9 if j2 > 0 else None,
+             "hbm_peak_gbs": hbm, "peak_source": peak_src,
+             "frac": cfg.b_bytes / (j2 * 1e-3) / 1e9 / hbm if j2 > 0 else None,
+             "d_from_x_ms": kt["J1"][0]},
+            {"ms": k_ms, "tflops": kf / (k_ms * 1e-3) / 1e12 if k_ms > 0 else None,
+             "frac_fp64_peak": kf / (k_ms * 1e-3) / 1e12 / peak if k_ms > 0 else None,
+             "k1_ms": k1, "k2_ms": k2,
+             "k1_tflops": flops_k1(cfg) / (k1 * 1e-3) / 1e12 if k1 > 0 else None,
+             "k2_tflops": flops_k2(cfg) / (k2 * 1e-3) / 1e12 if k2 > 0 else None})
+
+
+def two_pass_j(wl, first, n, hbm):
+    """north_star's J path as written -- two plain streaming passes over B (J1 dot, J2 axpy) -- timed
+    on J-only calls outside the timed region: 2|B| bytes over t_J1 + t_J2."""
+    wl.h.set_option("j_fused", 0)
+    kt = kernel_breakdown(wl, first, n, with_k=False)
+    wl.h.set_option("j_fused", 1)
+    t2 = kt["J1"][0] + kt["J2"][0]
+    gbs = 2 * wl.cfg.b_bytes / (t2 * 1e-3) / 1e9 if t2 > 0 else None
+    return {"stream_ms": t2, "bytes": 2 * wl.cfg.b_bytes, "gbs": gbs,
+            "frac": gbs / hbm if gbs else None}
+
+
+def other_workloads(pkg, wl4, args, dev, local, barrier, peak, hbm, peak_src):
+    """Short timed passes (3 warm-up + 3 steps each, same protocol) of the workloads the headline does
+    not cover, so that every number quoted in DESIGN.md is observed in the driver's own run:
+    the section-8f operations at cfg 4 (on the resident B), then BASELINE configs 3, 5, 2, 1 and the
+    LRDF shape."""
+    import torch
+    out = {}
+    W, K = 3, 3
+    cfg = wl4.cfg
+    nao, naux, nocc = cfg.nao, cfg.naux, cfg.nocc[0]
+    rng = np.random.default_rng(cfg.seed)
+
+    def timed(run, prep=None, warm=W, steps=K):
+        for _ in range(warm):
+            if prep:
+                prep()
+            run()
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        sampler = ClockSampler(local)
+        barrier()
+        sampler.start()
+        for k in range(steps):
+            if prep:
+                prep()
+            ev[k][0].record()
+            run()
+            ev[k][1].record()
+        barrier()
+        clocks = sampler.stop()
+        return float(np.median([a.elapsed_time(b) for a, b in ev])), clocks
+
+    # -- section 8f rank 1: the pair form (response-like density by its factors)
+    C1 = torch.from_numpy(rng.standard_normal((nao, nocc))).to(dev)
+    C2 = torch.from_numpy(rng.standard_normal((nao, nocc))).to(dev)
+    ms, clocks = timed(lambda: wl4.h.get_jk_pair(C1, C2))
+    fl = flops_j(cfg) + 2.0 * naux * nao ** 2 * (2 * nocc) + 2.0 * naux * nao ** 2 * nocc
+    out["cfg4_pair"] = {"op": f"dfjk_get_jk_pair ncol={nocc}", "ms_per_step": ms, "gflops": fl / ms / 1e6,
+                        "frac_fp64_peak": fl / ms / 1e9 / peak, "clocks": clocks}
+    # -- section 8f rank 3: Eq. 7's DF diagonal, one pass over B
+    ms, clocks = timed(lambda: wl4.h.get_df_diag())
+    out["cfg4_diag"] = {"op": "dfjk_get_df_diag (Eq. 7)", "ms_per_step": ms, "gbs": cfg.b_bytes / ms / 1e6,
+                        "frac_hbm": cfg.b_bytes / ms / 1e6 / hbm, "clocks": clocks}
+    # -- the north_star configuration of the whole step: J by two plain passes over B (j_fused = 0)
+    wl4.h.set_option("j_fused", 0)
+    ms, clocks = timed(lambda: wl4.step(0))
+    wl4.h.set_option("j_fused", 1)
+    out["cfg4_two_pass_j"] = {"op": "dfjk_get_jk with j_fused=0 (J1 dot + J2 axpy: B streamed three times)",
+                              "ms_per_step": ms, "gflops": flops_step(cfg) / ms / 1e6, "clocks": clocks}
+    # -- section 8f rank 2: building B in place (once: 1 warm-up + 1 timed, ~1 s each)
+    Mh = torch.from_numpy(gi.metric(cfg)).pin_memory()
+    Md = torch.empty(naux, naux, dtype=torch.float64, device=dev)
+
+    def prep():
+        Md.copy_(Mh, non_blocking=True)
+        gi.fill_B_device(cfg, wl4.B)                 # R is overwritten in place: regenerate it
+    ms, clocks = timed(lambda: pkg.build_b(Md, wl4.B, nao), prep, warm=1, steps=1)
+    fl = float(naux) ** 2 * cfg.npair + float(naux) ** 3 / 3.0
+    out["cfg4_build_b"] = {"op": "dfjk_build_b (Eq. 2-3, in place)", "ms_per_step": ms, "gflops": fl / ms / 1e6,
+                           "frac_fp64_peak": fl / ms / 1e9 / peak, "clocks": clocks}
+    del Md, Mh, C1, C2
+    wl4.close()
+
+    for cid in (3, 5, 2, 1, 6):
+        c = gi.CONFIGS[cid]
+        free, _ = torch.cuda.mem_get_info()
+        if free < c.b_bytes + (6 << 30):
+            out[f"cfg{cid}"] = {"skipped": f"needs {c.b_bytes / 1e9:.0f} GB of free device memory"}
+            continue
+        wl = Workload(pkg, c, dev, W + K)
+        for k in range(W):
+            wl.step(k)
+        step_ms, clocks, launches = timed_steps(wl, W, K, barrier, local)
+        kt = kernel_breakdown(wl, W, K)
+        j, kk = j_and_k_summary(c, kt, peak, hbm, peak_src)
+        ms = float(np.mean(step_ms))
+        rec = {"workload": workload_config(c, args)["workload"], "ms_per_step": ms, "step_ms": step_ms,
+               "gflops": flops_step(c) / ms / 1e6, "launches_per_step": launches / K,
+               "k_frac_fp64_peak": kk["frac_fp64_peak"], "k1_ms": kk["k1_ms"], "k2_ms": kk["k2_ms"],
+               "k1_tflops": kk["k1_tflops"], "k2_tflops": kk["k2_tflops"],
+               "j_ms": j["ms"], "j_gbs": j["gbs"], "clocks": clocks}
+        if c.b_bytes > (1 << 30):
+            rec["j_two_pass_gbs"] = two_pass_j(wl, W, 2, hbm)["gbs"]
+        out[f"cfg{cid}"] = rec
+        wl.close()
+    return out
 
 
 def run_ours(args, cfg):
@@ -220,28 +429,18 @@ def run_ours(args, cfg):
         torch.cuda.synchronize()
 
     pkg.lib()
-    fp64_probe = pkg.probe_fp64_peak() if rank == 0 else None     # measured FP64 pipe rate (untimed)
-    unrestricted = len(cfg.nocc) == 2
-    B = torch.empty(cfg.naux, cfg.npair, dtype=torch.float64, device=dev)
-    gi.fill_B_device(cfg, B)
-    h = pkg.DFJK(B, cfg.nao)
-    ncalls = args.warmup + args.steps
-    Cs_host = list(gi.orbital_sequence(cfg, ncalls))          # [call][set] numpy, host
-    Cs_dev = [[torch.from_numpy(C).to(dev) for C in sets] for sets in Cs_host]
-    flush = None if cfg.b_bytes > (1 << 30) else torch.empty(256 << 20, dtype=torch.uint8, device=dev)
-
-    def step(sets):
-        if unrestricted:
-            return h.get_jk_u(sets[0], sets[1])
-        return h.get_jk(sets[0])
-
+    pk = fp64_peak(pkg) if rank == 0 else None       # device-derived + measured FP64 pipe rate (untimed)
+    peaks, peak_src = measured_peaks()
+    hbm = float(peaks.get("hbm_gbs", HBM_FALLBACK_GBS))
+    wl = Workload(pkg, cfg, dev, args.warmup + args.steps)
+    h, unrestricted = wl.h, wl.unrestricted
     for k in range(args.warmup):
-        step(Cs_dev[k])
-    graph = None
+        wl.step(k)
+    step_fn = None
     if args.graph and not unrestricted:
-        # one CUDA-graph launch per step instead of 17 kernel launches (launch-bound small configs);
-        # the step's C_occ is copied into the captured input buffer inside the timed region
-        C_in = Cs_dev[0][0].clone()
+        # caller-side CUDA graph: one replay per step; the step's C_occ is copied into the captured
+        # input buffer inside the timed region
+        C_in = wl.Cs_dev[0][0].clone()
         Jg = torch.empty(cfg.nao, cfg.nao, dtype=torch.float64, device=dev)
         Kg = torch.empty_like(Jg)
         side = torch.cuda.Stream()
@@ -254,60 +453,20 @@ def run_ours(args, cfg):
             h.get_jk(C_in, out_j=Jg, out_k=Kg)
         launches_per_replay = h.launch_count - n0     # kernels inside one captured get_jk
 
-        def step(sets):                               # noqa: F811
-            C_in.copy_(sets[0])
+        def step_fn(k):
+            C_in.copy_(wl.Cs_dev[k][0])
             graph.replay()
-            return Jg, Kg
-        step(Cs_dev[0])
-    h.set_option("time_kernels", 0 if graph is not None else 1)
-    launches0 = h.launch_count
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
-          for _ in range(args.steps)]
-    sampler = ClockSampler(local)
-    barrier()
-    sampler.start()
-    for k in range(args.steps):
-        if flush is not None:
-            flush.fill_(k & 0xFF)
-        ev[k][0].record()
-        out = step(Cs_dev[args.warmup + k])
-        ev[k][1].record()
-    barrier()
-    clocks = sampler.stop()
-    launches = h.launch_count - launches0
-    step_ms = [a.elapsed_time(b) for a, b in ev]
-    total_ms = float(sum(step_ms))
-    if graph is not None:
-        # replays do not pass through the host-side counter / event brackets: count the captured
-        # kernels, and take the per-kernel times from the same steps launched plainly (untimed region)
-        launches = launches_per_replay * args.steps
-        h.set_option("time_kernels", 1)
-        for k in range(args.steps):
-            h.get_jk(Cs_dev[args.warmup + k][0])
-        torch.cuda.synchronize()
-    kt = {name: h.kernel_time(name) for name in pkg.KERNELS}
-    # the two plain streaming passes over B (north_star's J path), timed on J-only calls outside the
-    # timed region: 2|B| bytes over t_J1 + t_J2
-    h.set_option("j_fused", 0)
-    h.set_option("time_kernels", 1)
-    for k in range(min(args.steps, 3)):
-        sets = Cs_dev[args.warmup + k]
-        if unrestricted:
-            h.get_jk_u(sets[0], sets[1], with_k=False)
-        else:
-            h.get_jk(sets[0], with_k=False)
-    torch.cuda.synchronize()
-    t2 = (h.kernel_time("J1")[0] + h.kernel_time("J2")[0]) / min(args.steps, 3)
-    two_pass = {"stream_ms": t2, "bytes": 2 * cfg.b_bytes,
-                "gbs": 2 * cfg.b_bytes / (t2 * 1e-3) / 1e9 if t2 > 0 else None}
-    h.set_option("j_fused", 1)
-    h.set_option("time_kernels", 0)
-    total_ms = max_over_ranks(total_ms, dist, dev)
+        step_fn(0)
+    step_ms, clocks, launches = timed_steps(wl, args.warmup, args.steps, barrier, local, step_fn)
+    if step_fn is not None:
+        launches = launches_per_replay * args.steps   # replays bypass the host-side counter
+    total_ms = max_over_ranks(float(sum(step_ms)), dist, dev)
+    kt = kernel_breakdown(wl, args.warmup, args.steps)
+    two_pass = two_pass_j(wl, args.warmup, min(args.steps, 3), hbm)
 
     # ---- end to end through the host entry points
-    e2e = None
     if unrestricted:
-        Ch = [[torch.from_numpy(c).pin_memory() for c in s] for s in Cs_host]
+        Ch = [[torch.from_numpy(c).pin_memory() for c in s] for s in wl.Cs_host]
         Jh, Kah, Kbh = (torch.empty(cfg.nao, cfg.nao, dtype=torch.float64).pin_memory() for _ in range(3))
         h.get_jk_u_host(Ch[0][0], Ch[0][1], Jh, Kah, Kbh)
         barrier()
@@ -321,7 +480,7 @@ def run_ours(args, cfg):
                "api": "dfjk_get_jk_u_host (pinned host C_a, C_b in, pinned host J, K_a, K_b out; B resident)"}
     else:
         nocc = cfg.nocc[0]
-        Ch = [torch.from_numpy(s[0]).pin_memory() for s in Cs_host]
+        Ch = [torch.from_numpy(s[0]).pin_memory() for s in wl.Cs_host]
         Jh = torch.empty(cfg.nao, cfg.nao, dtype=torch.float64).pin_memory()
         Kh = torch.empty(cfg.nao, cfg.nao, dtype=torch.float64).pin_memory()
         h.get_jk_host(Ch[0], Jh, Kh)
@@ -340,13 +499,10 @@ def run_ours(args, cfg):
             dist.destroy_process_group()
         return
 
-    peaks, peak_src = measured_peaks()
+    peak = pk["peak"]
     ms_per_step = total_ms / args.steps
     value = whole_job_value(flops_step(cfg), args.steps, total_ms, world)
-    k1_ms, k1_n = kt["K1"]
-    k2_ms, k2_n = kt["K2"]
-    j_ms = sum(kt[n][0] for n in ("J0", "J1", "J1R", "J2", "J3")) / args.steps
-    k_ms = sum(kt[n][0] for n in ("K1", "K2", "K3")) / args.steps
+    k1_ms, k1_n = kt["K1"]                            # ms per step, launches in the breakdown pass
     # DRAM bytes of the dominant kernel from the committed ncu --set full capture
     # (profiles/traffic.csv), scaled from the captured launch's rows to the average launch
     traffic = None
@@ -359,59 +515,57 @@ def run_ours(args, cfg):
                     traffic = per_row * cfg.naux * args.steps / k1_n
     except Exception:
         pass
-    k1_tflops = flops_k1(cfg) * args.steps / (k1_ms * 1e-3) / 1e12 if k1_ms > 0 else 0.0
+    k1_tflops = flops_k1(cfg) / (k1_ms * 1e-3) / 1e12 if k1_ms > 0 else 0.0
     roofline = {"kernel": "k1_half_transform_kernel (X_P = B_P C, DMMA.8x8x4 on the FP64 pipe)",
-                "bound": "alu", "achieved": k1_tflops, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
-                "frac": k1_tflops / FP64_PEAK_TFLOPS, "traffic": traffic,
-                "peak_source": "148 SM x 64 FP64 FMA/clk x 2 x 1.965 GHz (DESIGN.md); peak_probe_tflops is "
-                               "dfjk_probe_dmma_peak's register-only DMMA loop measured in this run; "
-                               "sm_100a has no tcgen05 FP64 kind",
-                "peak_probe_tflops": fp64_probe, "launches": k1_n, "avg_launch_ms": k1_ms / max(k1_n, 1),
-                "flops_per_launch": flops_k1(cfg) * args.steps / max(k1_n, 1)}
-    hbm = float(peaks.get("hbm_gbs", HBM_FALLBACK_GBS))
-    # J inside a J+K call is fused (include/dfjk.h "j_fused"): d_P comes from the half-transformed X
-    # (kernel J1X, timed under the J1 id) and B is streamed once, by J2
-    j_stream_ms = kt["J2"][0] / args.steps
-    j_dx_ms = kt["J1"][0] / args.steps
-    k2_tflops = flops_k2(cfg) * args.steps / (k2_ms * 1e-3) / 1e12 if k2_ms > 0 else 0.0
+                "bound": "alu", "achieved": k1_tflops, "peak": peak, "unit": "TFLOP/s",
+                "frac": k1_tflops / peak, "traffic": traffic, "peak_source": pk["source"],
+                "peak_derived_tflops": pk["derived_tflops"], "peak_probe_tflops": pk["probe_tflops"],
+                "launches": k1_n, "avg_launch_ms": k1_ms * args.steps / max(k1_n, 1),
+                "flops_per_launch": flops_k1(cfg) * args.steps / max(k1_n, 1),
+                "timing": "CUDA events around each launch on the launching stream, collected from an untimed "
+                          "pass over the same calls (the timed steps carry no per-kernel brackets)"}
+    j, kk = j_and_k_summary(cfg, kt, peak, hbm, peak_src)
+    j["two_pass"] = two_pass
     out = {
         "metric": "df_get_jk_gflops_fp64", "value": value, "unit": "GFLOP/s", "n_gpus": world,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic", "config": workload_config(cfg, args), "clocks": clocks,
-        "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
-        "j": {"ms": j_ms, "fused": True, "stream_ms": j_stream_ms, "bytes": cfg.b_bytes,
-              "gbs": cfg.b_bytes / (j_stream_ms * 1e-3) / 1e9 if j_stream_ms > 0 else None,
-              "hbm_peak_gbs": hbm, "peak_source": peak_src,
-              "frac": cfg.b_bytes / (j_stream_ms * 1e-3) / 1e9 / hbm if j_stream_ms > 0 else None,
-              "d_from_x_ms": j_dx_ms, "two_pass": two_pass},
-        "k": {"ms": k_ms, "tflops": (flops_k1(cfg) + flops_k2(cfg)) / (k_ms * 1e-3) / 1e12 if k_ms > 0 else None,
-              "frac_fp64_peak": (flops_k1(cfg) + flops_k2(cfg)) / (k_ms * 1e-3) / 1e12 / FP64_PEAK_TFLOPS if k_ms > 0 else None,
-              "k1_ms": k1_ms / args.steps, "k2_ms": k2_ms / args.steps, "k2_tflops": k2_tflops},
+        "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "j": j, "k": kk,
         "step_ms": step_ms,
     }
-    if graph is not None:
+    if step_fn is not None:
         out["config"]["launch"] = "one CUDA-graph replay per step (+ a device copy of C_occ into the captured input)"
     if world == 1:
-        rows, t, threads = size_sample(cfg, 15.0)
+        if args.cpu_baseline_full:
+            rows, (t, threads) = cfg.naux, oracle_sample(cfg, cfg.naux)
+        else:
+            rows, t, threads = size_sample(cfg, 15.0)
         out["cpu_baseline"] = {
             "value": flops_step(cfg) / cfg.naux * rows / t / 1e9, "unit": "GFLOP/s", "cores": threads,
             "kind": "oracle", "seconds": t,
-            "sample": f"{rows} of {cfg.naux} auxiliary rows of cfg {cfg.index}, J and K, one call "
-                      "(algorithmic flop count; the oracle does the full-square work)"}
+            "sample": (f"all {cfg.naux} rows" if rows == cfg.naux else f"{rows} of {cfg.naux} auxiliary rows")
+                      + f" of cfg {cfg.index}, J and K, one call (algorithmic flop count; the oracle does the "
+                        "full-square work)"}
+        if cfg.index == 4 and not args.no_others and step_fn is None:
+            try:
+                out["other"] = other_workloads(pkg, wl, args, dev, local, barrier, peak, hbm, peak_src)
+            except Exception as e:                     # the headline line must survive
+                out["other"] = {"error": repr(e)}
     print(json.dumps(out))
     if dist is not None:
         dist.destroy_process_group()
 
 
 def run_extra(args, cfg):
-    """--op build_b | pair | dm | diag: the section-8f rows, timed alone with CUDA events (one JSON
+    """--op build_b | pair | dm | diag | scf: the section-8f rows, timed alone with CUDA events (one JSON
     line, same keys as the main line where they apply; no cpu_baseline / e2e legs)."""
     import torch
     import paper_2506_06661_b200 as pkg
     torch.cuda.set_device(0)
     dev = torch.device("cuda", 0)
     pkg.lib()
+    peak = fp64_peak(pkg)["peak"]
     B = torch.empty(cfg.naux, cfg.npair, dtype=torch.float64, device=dev)
     gi.fill_B_device(cfg, B)
     nao, naux, nocc = cfg.nao, cfg.naux, cfg.nocc[0]
@@ -485,10 +639,11 @@ def run_extra(args, cfg):
     if args.op == "scf":
         out["e_hist"] = res.get("e_hist")
         out["ms_per_iteration"] = t / 6
+        out["split_ms_per_iteration"] = res.get("timing")
     if args.op == "diag":
         out["gbs"] = cfg.b_bytes / (t * 1e-3) / 1e9
     else:
-        out["frac_fp64_peak"] = flops / (t * 1e-3) / 1e12 / FP64_PEAK_TFLOPS
+        out["frac_fp64_peak"] = flops / (t * 1e-3) / 1e12 / peak
     print(json.dumps(out))
 
 
@@ -501,6 +656,10 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--graph", action="store_true",
                     help="replay one captured CUDA graph per step (restricted configs; no per-kernel timing)")
+    ap.add_argument("--no-others", action="store_true",
+                    help="skip the short passes over the other configs / section-8f ops after the cfg-4 headline")
+    ap.add_argument("--cpu-baseline-full", action="store_true",
+                    help="time the oracle on ALL rows of the config instead of a ~15 s sample (cfg 4: ~90 s)")
     ap.add_argument("--op", default="get_jk", choices=["get_jk", "build_b", "pair", "dm", "diag", "scf"],
                     help="get_jk (default, the contract line) or one of the section-8f rows")
     args = ap.parse_args()

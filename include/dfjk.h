@@ -253,6 +253,13 @@ int dfjk_get_d(dfjk_handle *h, double *d_out, void *stream);
  *               instead of twice; 0 = always the two plain streaming passes over B (dot, then
  *               axpy).  Applies to dfjk_get_jk, dfjk_get_jk_u and dfjk_get_jk_pair (there
  *               <B_P, C1 C2^T> = <B_P C1, C2>); J-only calls and raw-dm calls always use two passes.
+ *   "graph"     1 (default) = dfjk_get_jk / dfjk_get_jk_u replay a CUDA graph of their own launch
+ *               sequence: the first call of a shape (orbital counts, requested outputs, options)
+ *               launches kernel by kernel, the second captures the sequence after the orbital
+ *               packing into a graph kept in the handle, later ones launch that graph (the call's
+ *               output pointers reach the finishing kernels through device memory).  Small problems
+ *               are bound by launch count, not by work.  0 = always launch kernel by kernel.  Not
+ *               used while "time_kernels" is on or while `stream` is itself being captured.
  */
 int dfjk_set_option(dfjk_handle *h, const char *name, int64_t value);
 
@@ -299,6 +306,23 @@ int dfjk_destroy(dfjk_handle *h);
  * (SMs x 64 FMA/clk x 2 x clock) that K's roofline fraction is quoted against.
  */
 int dfjk_probe_dmma_peak(double *tflops);
+
+/*
+ * dfjk_scf_timing -- where the time of the LAST dfjk_scf_rhf / dfjk_scf_uhf run on this handle went
+ * (HOST pointers, any may be NULL), measured with CUDA events on the run's stream: iterations done,
+ * total ms inside get_jk / get_jk_u, total ms inside the eigensolver (cuSOLVER Dsygvd, core guess
+ * included) and everything else (Fock, density, energy, DIIS error and extrapolation, host solves
+ * and read-backs).  DFJK_EINVAL if no SCF has run.  PAPER.md:258-262 (the SCF loop).
+ */
+int dfjk_scf_timing(const dfjk_handle *h, int64_t *iters, double *get_jk_ms, double *eig_ms, double *other_ms);
+
+/*
+ * dfjk_device_info -- measurement aid: what the roofline denominators are derived from, read from
+ * the CURRENT device (HOST pointers, any may be NULL): number of SMs, the peak SM clock in kHz
+ * (cudaDevAttrClockRate) and the L2 size in bytes.  Derived FP64 peak = sm_count x 64 FMA/clk x 2 x
+ * clock (DMMA.8x8x4 runs on the FP64 pipe).  Returns 0 or DFJK_ECUDA.
+ */
+int dfjk_device_info(int *sm_count, int *sm_clock_khz, int64_t *l2_bytes);
 
 /* dfjk_last_error -- thread-local text of the last failure ("" if none). */
 const char *dfjk_last_error(void);

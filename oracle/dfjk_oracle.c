@@ -45,7 +45,8 @@
  * the same way in tests/test_oracle_general_pins.py.  No function in this file is
  * "parity unpinned".
  *
- * Build: gcc -O2 -fopenmp -shared -fPIC (no -ffast-math; no reassociation).
+ * Build: gcc -O3 -march=x86-64-v3 -ffp-contract=off -fopenmp -shared -fPIC (no -ffast-math, no
+ * reassociation, no FMA contraction: bit-for-bit the results of a plain -O2 build).
  */
 #include <stdint.h>
 #include <stdlib.h>

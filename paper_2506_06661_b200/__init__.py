@@ -17,7 +17,7 @@ import os
 import subprocess
 from typing import Optional, Tuple
 
-__all__ = ["build", "lib", "build_b", "DFJK", "DFJKError", "SYMBOLS", "KERNELS", "LIB_PATH", "HEADER_PATH"]
+__all__ = ["build", "lib", "build_b", "device_info", "probe_fp64_peak", "DFJK", "DFJKError", "SYMBOLS", "KERNELS", "LIB_PATH", "HEADER_PATH"]
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libdfjk.so")
@@ -31,7 +31,7 @@ SYMBOLS = (
     "dfjk_version", "dfjk_launch_count", "dfjk_kernel_time",
     "dfjk_get_jk_pair", "dfjk_get_jk_dm", "dfjk_get_jk_dms", "dfjk_get_df_diag",
     "dfjk_build_b", "dfjk_scf_rhf", "dfjk_probe_dmma_peak",
-    "dfjk_get_jk_u_host", "dfjk_scf_uhf",
+    "dfjk_get_jk_u_host", "dfjk_scf_uhf", "dfjk_device_info", "dfjk_scf_timing",
 )
 
 # DFJK_KERNEL_* ids of include/dfjk.h
@@ -84,6 +84,11 @@ def lib() -> ctypes.CDLL:
     L.dfjk_scf_uhf.argtypes = [vp, vp, vp, i64, i64, i64, ctypes.c_double, i64, vp, vp, vp, vp, vp, vp,
                                ctypes.POINTER(ctypes.c_double), ctypes.POINTER(i64),
                                ctypes.POINTER(ci), vp]
+    L.dfjk_scf_timing.restype = ci
+    L.dfjk_scf_timing.argtypes = [vp, ctypes.POINTER(i64), ctypes.POINTER(ctypes.c_double),
+                                  ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]
+    L.dfjk_device_info.restype = ci
+    L.dfjk_device_info.argtypes = [ctypes.POINTER(ci), ctypes.POINTER(ci), ctypes.POINTER(i64)]
     L.dfjk_build_b.restype = ci
     L.dfjk_build_b.argtypes = [i64, i64, vp, vp, vp, vp]
     L.dfjk_get_df_diag.restype = ci
@@ -132,6 +137,15 @@ def probe_fp64_peak() -> float:
     v = ctypes.c_double(0.0)
     _check(lib().dfjk_probe_dmma_peak(ctypes.byref(v)), "dfjk_probe_dmma_peak")
     return v.value
+
+
+def device_info() -> dict:
+    """SM count, peak SM clock (kHz), L2 bytes of the current device, and the FP64 peak derived from
+    them (SMs x 64 FMA/clk x 2 x clock, TFLOP/s) -- the roofline denominators' raw material."""
+    sms, khz, l2 = ctypes.c_int(0), ctypes.c_int(0), ctypes.c_int64(0)
+    _check(lib().dfjk_device_info(ctypes.byref(sms), ctypes.byref(khz), ctypes.byref(l2)), "dfjk_device_info")
+    return {"sm_count": sms.value, "sm_clock_khz": khz.value, "l2_bytes": l2.value,
+            "fp64_peak_tflops": sms.value * 64 * 2 * khz.value * 1e3 / 1e12}
 
 
 def build_b(M, R_packed, nao: int, stream=None):
@@ -288,7 +302,7 @@ class DFJK:
                                       F.data_ptr(), e_hist, ctypes.byref(n_iter), ctypes.byref(conv), st),
                    "dfjk_scf_rhf")
         return dict(converged=bool(conv.value), e_hist=list(e_hist[:n_iter.value]), C=C,
-                    mo_energy=eps, D=D, F=F)
+                    mo_energy=eps, D=D, F=F, timing=self.scf_timing())
 
     def scf_uhf(self, hcore, S, nocc_a: int, nocc_b: int, max_iter: int = 50, conv_tol: float = 1e-10,
                 diis_space: int = 8, stream=None):
@@ -308,7 +322,16 @@ class DFJK:
                                       float(conv_tol), int(diis_space), C[0].data_ptr(), C[1].data_ptr(),
                                       eps[0].data_ptr(), eps[1].data_ptr(), D[0].data_ptr(), D[1].data_ptr(),
                                       e_hist, ctypes.byref(n_iter), ctypes.byref(conv), st), "dfjk_scf_uhf")
-        return dict(converged=bool(conv.value), e_hist=list(e_hist[:n_iter.value]), C=C, mo_energy=eps, D=D)
+        return dict(converged=bool(conv.value), e_hist=list(e_hist[:n_iter.value]), C=C, mo_energy=eps, D=D,
+                    timing=self.scf_timing())
+
+    def scf_timing(self) -> dict:
+        """ms per iteration of the last SCF run: get_jk, eigensolver (cuSOLVER Dsygvd), everything else."""
+        it, a, b, c = ctypes.c_int64(0), ctypes.c_double(0), ctypes.c_double(0), ctypes.c_double(0)
+        _check(lib().dfjk_scf_timing(self._h, ctypes.byref(it), ctypes.byref(a), ctypes.byref(b),
+                                     ctypes.byref(c)), "dfjk_scf_timing")
+        n = max(it.value, 1)
+        return {"iterations": it.value, "get_jk": a.value / n, "eigensolver": b.value / n, "glue": c.value / n}
 
     def get_df_diag(self, stream=None):
         """diag[mu][nu] = sum_P B_P[mu,nu]^2, the DF term of Eq. 7."""

@@ -347,13 +347,14 @@ int64_t build_b_workspace_doubles(int64_t naux)
 cudaError_t launch_build_b(int64_t naux, int64_t npair, double *M, double *T, double *ws,
                            long long *info, cudaStream_t st)
 {
-    static unsigned long long ok1 = 0, ok2 = 0, ok3 = 0;
-    ensure_dynamic_smem(chol_diag_kernel, NB * (NB + 1) * 8, ok1);
-    ensure_dynamic_smem(tri_inv_kernel, NB * NB * 8, ok2);
-    ensure_dynamic_smem(whiten_gemm_kernel, W_SMEM_BYTES, ok3);
+    static std::atomic<unsigned long long> ok1{0}, ok2{0}, ok3{0};
+    cudaError_t e = ensure_dynamic_smem(chol_diag_kernel, NB * (NB + 1) * 8, ok1);
+    if (e == cudaSuccess) e = ensure_dynamic_smem(tri_inv_kernel, NB * NB * 8, ok2);
+    if (e == cudaSuccess) e = ensure_dynamic_smem(whiten_gemm_kernel, W_SMEM_BYTES, ok3);
+    if (e != cudaSuccess) return e;
     const int64_t ldw = (naux + NB - 1) / NB * NB;
     double *Aw = ws, *panel = ws + ldw * ldw;
-    cudaError_t e = cudaMemsetAsync(Aw, 0, (size_t)(ldw * ldw) * sizeof(double), st);
+    e = cudaMemsetAsync(Aw, 0, (size_t)(ldw * ldw) * sizeof(double), st);
     if (e != cudaSuccess) return e;
     if (info) {
         e = cudaMemsetAsync(info, 0, sizeof(long long), st);

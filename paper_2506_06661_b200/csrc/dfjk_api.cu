@@ -44,9 +44,39 @@ int fail(int code, const char *fmt, ...)
             return fail(DFJK_ECUDA, "%s: %s", #expr, cudaGetErrorString(e_));            \
     } while (0)
 
+/* a launcher that reports failure (no tile shape, no shared-memory opt-in, bad launch) */
+#define DFJK_LAUNCH_TRY(expr)                                                            \
+    do {                                                                                 \
+        cudaError_t e_ = (expr);                                                         \
+        if (e_ != cudaSuccess)                                                           \
+            return fail(DFJK_ECUDA, "%s: %s", who, cudaGetErrorString(e_));              \
+    } while (0)
+
 int64_t round_up(int64_t x, int64_t m) { return (x + m - 1) / m * m; }
 
 }  // namespace
+
+#define DFJK_GRAPH_SLOTS 4
+
+namespace dfjk {
+/* split count that fills the SMs best: work items = ntile * s on sm_count SMs (one CTA each).
+ * Whole waves matter because a CTA's duration is fixed by its k range; a small penalty per
+ * split accounts for the read-modify-write of the partial tile. */
+int choose_splits(int ntile, int sm_count, int max_splits)
+{
+    int best = 1;
+    double best_score = -1.0;
+    for (int s = 1; s <= max_splits; ++s) {
+        const int items = ntile * s;
+        const int waves = (items + sm_count - 1) / sm_count;
+        const double score = (double)items / ((double)waves * sm_count) - 0.002 * s;
+        if (score > best_score) { best_score = score; best = s; }
+    }
+    return best;
+}
+
+}  // namespace dfjk
+using dfjk::choose_splits;
 
 struct dfjk_handle {
     int64_t naux, nao, npair;
@@ -74,6 +104,17 @@ struct dfjk_handle {
     cudaEvent_t *ev;     /* pairs: ev[2*i], ev[2*i+1] */
     int *ev_kind;        /* which kernel pair i brackets (DFJK_KERNEL_*) */
     int ev_cap, ev_used;
+    bool ev_overflow;    /* a launch went unrecorded (the ring could not grow): kernel_time reports it */
+    /* replayed launch sequences of get_jk / get_jk_u (see get_jk_impl) */
+    struct GraphSlot { bool seen; unsigned char key[64]; cudaGraphExec_t exec; int64_t launches; };
+    GraphSlot graphs[DFJK_GRAPH_SLOTS];
+    int graph_next;
+    int64_t opt_graph;
+    cudaStream_t cap_stream;
+    double **out_slots;  /* device: this call's output pointers (J, K_0, K_1), written by K0 */
+    /* the last SCF run's timing (dfjk_scf_timing) */
+    int64_t scf_iters;
+    double scf_get_jk_ms, scf_eig_ms, scf_total_ms;
     /* host-call resources (lazy) */
     cudaStream_t host_stream;
     double *hostC, *hostJ, *hostK, *hostC2, *hostK2;
@@ -87,41 +128,52 @@ void free_all(dfjk_handle *h)
     cudaFree(h->Jp_part); cudaFree(h->X); cudaFree(h->Kpart);
     cudaFree(h->hostC); cudaFree(h->hostJ); cudaFree(h->hostK); cudaFree(h->hostC2); cudaFree(h->hostK2);
     if (h->host_stream) cudaStreamDestroy(h->host_stream);
+    for (auto &g : h->graphs) if (g.exec) cudaGraphExecDestroy(g.exec);
+    if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
+    cudaFree(h->out_slots);
     for (int i = 0; i < 2 * h->ev_cap; ++i) cudaEventDestroy(h->ev[i]);
     delete[] h->ev;
     delete[] h->ev_kind;
 }
 
-/* bracket one kernel launch with events when "time_kernels" is on */
+/* the event ring of "time_kernels": (re)allocate to `cap` pairs, keeping the recorded ones */
+bool grow_events(dfjk_handle *h, int cap)
+{
+    cudaEvent_t *ev = new (std::nothrow) cudaEvent_t[2 * (size_t)cap];
+    int *kind = new (std::nothrow) int[cap];
+    if (!ev || !kind) { delete[] ev; delete[] kind; return false; }
+    for (int i = 0; i < 2 * h->ev_cap; ++i) ev[i] = h->ev[i];
+    for (int i = 0; i < h->ev_cap; ++i) kind[i] = h->ev_kind[i];
+    for (int i = 2 * h->ev_cap; i < 2 * cap; ++i)
+        if (cudaEventCreate(&ev[i]) != cudaSuccess) {
+            cudaGetLastError();
+            for (int j = 2 * h->ev_cap; j < i; ++j) cudaEventDestroy(ev[j]);
+            delete[] ev; delete[] kind;
+            return false;
+        }
+    delete[] h->ev; delete[] h->ev_kind;
+    h->ev = ev; h->ev_kind = kind; h->ev_cap = cap;
+    return true;
+}
+
+/* bracket one kernel launch with events when "time_kernels" is on; the ring grows on demand and a
+ * launch that could not be recorded raises ev_overflow (dfjk_kernel_time then fails loudly) */
 struct Timed {
     dfjk_handle *h; cudaStream_t st; int slot;
     Timed(dfjk_handle *h_, int kind, cudaStream_t st_) : h(h_), st(st_), slot(-1)
     {
         ++h->launches;
-        if (h->opt_time_kernels && h->ev_used < h->ev_cap) {
-            slot = h->ev_used++;
-            h->ev_kind[slot] = kind;
-            cudaEventRecord(h->ev[2 * slot], st);
+        if (!h->opt_time_kernels) return;
+        if (h->ev_used == h->ev_cap && !grow_events(h, h->ev_cap > 0 ? 2 * h->ev_cap : 1024)) {
+            h->ev_overflow = true;
+            return;
         }
+        slot = h->ev_used++;
+        h->ev_kind[slot] = kind;
+        cudaEventRecord(h->ev[2 * slot], st);
     }
     ~Timed() { if (slot >= 0) cudaEventRecord(h->ev[2 * slot + 1], st); }
 };
-
-/* split count that fills the SMs best: work items = ntile * s on sm_count SMs (one CTA each).
- * Whole waves matter because a CTA's duration is fixed by its k range; a small penalty per
- * split accounts for the read-modify-write of the partial tile. */
-int choose_splits(int ntile, int sm_count, int max_splits)
-{
-    int best = 1;
-    double best_score = -1.0;
-    for (int s = 1; s <= max_splits; ++s) {
-        const int items = ntile * s;
-        const int waves = (items + sm_count - 1) / sm_count;
-        const double score = (double)items / ((double)waves * sm_count) - 0.002 * s;
-        if (score > best_score) { best_score = score; best = s; }
-    }
-    return best;
-}
 
 int alloc_ws(dfjk_handle *h, double **p, int64_t ndoubles)
 {
@@ -163,6 +215,7 @@ extern "C" dfjk_handle *dfjk_create(int64_t naux, int64_t nao, const double *B_p
     memset(h, 0, sizeof *h);
     h->naux = naux; h->nao = nao; h->npair = nao * (nao + 1) / 2; h->B = B_packed; h->device = dev;
     h->opt_j_fused = 1;
+    h->opt_graph = 1;
     int v = 0;
     cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev); h->sm_count = v > 0 ? v : 148;
     cudaDeviceGetAttribute(&v, cudaDevAttrL2CacheSize, dev); h->l2_bytes = v;
@@ -196,6 +249,10 @@ extern "C" dfjk_handle *dfjk_create(int64_t naux, int64_t nao, const double *B_p
     if (rc == DFJK_OK) rc = alloc_ws(h, &h->Jp_part, h->j2_groups * h->npair);
     if (rc == DFJK_OK) rc = alloc_ws(h, &h->X, h->x_doubles);
     if (rc == DFJK_OK) rc = alloc_ws(h, &h->Kpart, 2LL * h->nsplit_alloc * nao * nao);
+    if (rc == DFJK_OK && cudaMalloc((void **)&h->out_slots, DFJK_OUT_SLOTS * sizeof(double *)) != cudaSuccess) {
+        h->out_slots = nullptr;
+        rc = fail(DFJK_ENOMEM, "dfjk_create: cudaMalloc of the output-pointer slots failed");
+    }
     if (rc != DFJK_OK) { free_all(h); delete h; return nullptr; }
     return h;
 }
@@ -220,22 +277,93 @@ extern "C" int dfjk_set_option(dfjk_handle *h, const char *name, int64_t value)
         h->opt_k_splits = value; return DFJK_OK;
     }
     if (!strcmp(name, "time_kernels")) {
-        if (value && !h->ev) {
-            const int cap = 16384;
-            h->ev = new (std::nothrow) cudaEvent_t[2 * cap];
-            h->ev_kind = new (std::nothrow) int[cap];
-            if (!h->ev || !h->ev_kind) return fail(DFJK_ENOMEM, "time_kernels: host allocation failed");
-            for (int i = 0; i < 2 * cap; ++i) DFJK_CUDA_TRY(cudaEventCreate(&h->ev[i]));
-            h->ev_cap = cap;
-        }
-        h->opt_time_kernels = value; h->ev_used = 0; return DFJK_OK;
+        if (value && !h->ev && !grow_events(h, 1024))
+            return fail(DFJK_ENOMEM, "time_kernels: could not create the event ring");
+        h->opt_time_kernels = value; h->ev_used = 0; h->ev_overflow = false; return DFJK_OK;
     }
     if (!strcmp(name, "j_fused")) { h->opt_j_fused = value != 0; return DFJK_OK; }
+    if (!strcmp(name, "graph")) { h->opt_graph = value != 0; return DFJK_OK; }
     return fail(DFJK_EINVAL, "dfjk_set_option: unknown option '%s'", name);
 }
 
 /* ------------------------------------------------------------------ one build */
 namespace {
+
+/* Everything of one get_jk after K0 (the orbital packing), enqueued on `st`.  With slots != NULL
+ * the finishing kernels take their output pointers from the device array K0 published them to
+ * (slot 0 = J, slot 1 + s = K_s) instead of from J / K[]: the sequence then depends on the CALL only
+ * through (nset, nocc, which outputs, options) and can be captured once and replayed. */
+int enqueue_jk_body(dfjk_handle *h, int nset, const int *nocc, const int *col0, int64_t ldc,
+                    const double *w, double *J, double *const *K, bool want_j, const bool *want_k,
+                    double *const *slots, cudaStream_t st, const char *who)
+{
+    const int64_t nao = h->nao, naux = h->naux, npair = h->npair;
+    bool any_k = false;
+    for (int s = 0; s < nset; ++s) any_k = any_k || want_k[s];
+    /* J and K in one call: d_P = <B_P, D> = sum_s w_s <X_P^s, C_s> is read off the half-transformed
+     * X that K1 writes anyway (J1X), so B is streamed once for J (J2) instead of twice */
+    const bool fused = want_j && any_k && h->opt_j_fused != 0;
+    if (want_j && !fused) {
+        { Timed t_(h, DFJK_KERNEL_J0, st); dfjk::launch_j0_build_dt(h->Ccat, ldc, nao, nset, col0, nocc, w, h->Dt, st); }
+        { Timed t_(h, DFJK_KERNEL_J1, st); dfjk::launch_j1_dot(h->B, naux, npair, h->Dt, h->d_part, h->sm_count, st); }
+        { Timed t_(h, DFJK_KERNEL_J1R, st); dfjk::launch_j1_reduce(h->d_part, h->nchunk, naux, h->d, st); }
+        { Timed t_(h, DFJK_KERNEL_J2, st); dfjk::launch_j2_axpy(h->B, naux, npair, h->d, h->Jp_part, h->j2_groups, st); }
+        { Timed t_(h, DFJK_KERNEL_J3, st); dfjk::launch_j3_unpack(h->Jp_part, h->j2_groups, npair, nao, J, slots ? slots + 0 : nullptr, st); }
+    }
+
+    if (any_k) {
+        int64_t pc = h->x_doubles / (nao * ldc);
+        if (h->opt_k_chunk > 0 && h->opt_k_chunk < pc) pc = h->opt_k_chunk;
+        if (pc > naux) pc = naux;
+        if (pc < 1) return fail(DFJK_ENOMEM, "%s: X workspace too small", who);
+        const int nsplit = h->opt_k_splits > 0 ? (int)h->opt_k_splits : h->nsplit_default;
+        int chunk = 0;
+        for (int64_t P0 = 0; P0 < naux; P0 += pc, ++chunk) {
+            const int64_t np = (P0 + pc <= naux) ? pc : naux - P0;
+            { Timed t_(h, DFJK_KERNEL_K1, st); DFJK_LAUNCH_TRY(dfjk::launch_k1_half_transform(h->B, naux, nao, npair, P0, np, h->Ccat, ldc, ldc, h->X, st)); }
+            if (fused) {
+                Timed t_(h, DFJK_KERNEL_J1, st);
+                dfjk::launch_j1x_dot(h->X, h->Ccat, nao, np, ldc, ldc, 0, nset, col0, nocc, w, P0, naux, h->d_part, st);
+            }
+            for (int s = 0; s < nset; ++s)
+                if (want_k[s]) {
+                    Timed t_(h, DFJK_KERNEL_K2, st);
+                    DFJK_LAUNCH_TRY(dfjk::launch_k2_syrk_lower(h->X, nao, np, ldc, col0[s], nocc[s],
+                                                               h->Kpart + (int64_t)s * h->nsplit_alloc * nao * nao,
+                                                               nsplit, chunk > 0, st));
+                }
+        }
+        for (int s = 0; s < nset; ++s)
+            if (want_k[s]) {
+                Timed t_(h, DFJK_KERNEL_K3, st);
+                dfjk::launch_k3_finish(h->Kpart + (int64_t)s * h->nsplit_alloc * nao * nao, nsplit,
+                                       nao, K[s], slots ? slots + 1 + s : nullptr, st);
+            }
+    }
+    if (fused) {
+        { Timed t_(h, DFJK_KERNEL_J1R, st); dfjk::launch_j1_reduce(h->d_part, dfjk::j1x_num_blocks(nao, ldc), naux, h->d, st); }
+        { Timed t_(h, DFJK_KERNEL_J2, st); dfjk::launch_j2_axpy(h->B, naux, npair, h->d, h->Jp_part, h->j2_groups, st); }
+        { Timed t_(h, DFJK_KERNEL_J3, st); dfjk::launch_j3_unpack(h->Jp_part, h->j2_groups, npair, nao, J, slots ? slots + 0 : nullptr, st); }
+    }
+    return DFJK_OK;
+}
+
+/* The launch sequence of a get_jk depends on the call only through its shape (sets, nocc, outputs,
+ * options): the second call with a shape already seen captures the body into a CUDA graph, later
+ * ones replay it -- one graph launch instead of 8-20 kernel launches, which is what bounds the small
+ * configs (cfg 1: 17 launches = 0.15 ms for 0.03 ms of work).  K0 stays a plain launch in front: it
+ * takes the call's C pointers and publishes the call's output pointers for the replayed K3 / J3. */
+struct GraphKey {
+    int nset, nocc[2];
+    bool want_j, want_k[2];
+    int64_t k_chunk, k_splits, j_fused;
+    bool operator==(const GraphKey &o) const
+    {
+        return nset == o.nset && nocc[0] == o.nocc[0] && nocc[1] == o.nocc[1] && want_j == o.want_j &&
+               want_k[0] == o.want_k[0] && want_k[1] == o.want_k[1] && k_chunk == o.k_chunk &&
+               k_splits == o.k_splits && j_fused == o.j_fused;
+    }
+};
 
 int get_jk_impl(dfjk_handle *h, int nset, const double *const *C, const int64_t *nocc64,
                 const double *w, double *J, double *const *K, cudaStream_t st, const char *who)
@@ -255,7 +383,7 @@ int get_jk_impl(dfjk_handle *h, int nset, const double *const *C, const int64_t 
     DFJK_CUDA_TRY(cudaGetDevice(&dev));
     if (dev != h->device) return fail(DFJK_EINVAL, "%s: handle belongs to device %d, current is %d", who, h->device, dev);
 
-    const int64_t nao = h->nao, naux = h->naux, npair = h->npair;
+    const int64_t nao = h->nao;
     int nocc[4], col0[4];
     int64_t ldc = 0;
     for (int s = 0; s < nset; ++s) {
@@ -263,56 +391,68 @@ int get_jk_impl(dfjk_handle *h, int nset, const double *const *C, const int64_t 
         col0[s] = (int)ldc;
         ldc += round_up(nocc64[s], 8);
     }
-    /* K0: zero-padded concatenation [C_0 | C_1], each set padded to a multiple of 8 columns */
-    { Timed t_(h, DFJK_KERNEL_K0, st); dfjk::launch_k0_pack_c(C, nocc, col0, nset, nao, ldc, h->Ccat, st); }
+    GraphKey key = {};
+    key.nset = nset; key.want_j = J != nullptr;
+    key.k_chunk = h->opt_k_chunk; key.k_splits = h->opt_k_splits; key.j_fused = h->opt_j_fused;
+    bool want_k[2] = {false, false};
+    for (int s = 0; s < nset; ++s) { key.nocc[s] = nocc[s]; key.want_k[s] = want_k[s] = K[s] != nullptr; }
 
-    /* J and K in one call: d_P = <B_P, D> = sum_s w_s <X_P^s, C_s> is read off the half-transformed
-     * X that K1 writes anyway (J1X), so B is streamed once for J (J2) instead of twice */
-    const bool fused = J && any_k && h->opt_j_fused != 0;
-    if (J && !fused) {
-        { Timed t_(h, DFJK_KERNEL_J0, st); dfjk::launch_j0_build_dt(h->Ccat, ldc, nao, nset, col0, nocc, w, h->Dt, st); }
-        { Timed t_(h, DFJK_KERNEL_J1, st); dfjk::launch_j1_dot(h->B, naux, npair, h->Dt, h->d_part, h->sm_count, st); }
-        { Timed t_(h, DFJK_KERNEL_J1R, st); dfjk::launch_j1_reduce(h->d_part, h->nchunk, naux, h->d, st); }
-        { Timed t_(h, DFJK_KERNEL_J2, st); dfjk::launch_j2_axpy(h->B, naux, npair, h->d, h->Jp_part, h->j2_groups, st); }
-        { Timed t_(h, DFJK_KERNEL_J3, st); dfjk::launch_j3_unpack(h->Jp_part, h->j2_groups, npair, nao, J, st); }
-        h->have_d = true;
-    }
-
-    if (any_k) {
-        int64_t pc = h->x_doubles / (nao * ldc);
-        if (h->opt_k_chunk > 0 && h->opt_k_chunk < pc) pc = h->opt_k_chunk;
-        if (pc > naux) pc = naux;
-        if (pc < 1) return fail(DFJK_ENOMEM, "%s: X workspace too small", who);
-        const int nsplit = h->opt_k_splits > 0 ? (int)h->opt_k_splits : h->nsplit_default;
-        int chunk = 0;
-        for (int64_t P0 = 0; P0 < naux; P0 += pc, ++chunk) {
-            const int64_t np = (P0 + pc <= naux) ? pc : naux - P0;
-            { Timed t_(h, DFJK_KERNEL_K1, st); dfjk::launch_k1_half_transform(h->B, naux, nao, npair, P0, np, h->Ccat, ldc, ldc, h->X, st); }
-            if (fused) {
-                Timed t_(h, DFJK_KERNEL_J1, st);
-                dfjk::launch_j1x_dot(h->X, h->Ccat, nao, np, ldc, ldc, 0, nset, col0, nocc, w, P0, naux, h->d_part, st);
-            }
-            for (int s = 0; s < nset; ++s)
-                if (K[s]) {
-                    Timed t_(h, DFJK_KERNEL_K2, st);
-                    dfjk::launch_k2_syrk_lower(h->X, nao, np, ldc, col0[s], nocc[s],
-                                               h->Kpart + (int64_t)s * h->nsplit_alloc * nao * nao,
-                                               nsplit, chunk > 0, st);
-                }
+    /* graph replay is for plain calls only: not while the per-kernel event brackets are on, and not
+     * inside someone else's capture (there the launches simply join the caller's graph) */
+    bool use_graph = h->opt_graph != 0 && h->opt_time_kernels == 0;
+    if (use_graph) {
+        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+        if (cudaStreamIsCapturing(st, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) {
+            cudaGetLastError();
+            use_graph = false;
         }
-        for (int s = 0; s < nset; ++s)
-            if (K[s]) {
-                Timed t_(h, DFJK_KERNEL_K3, st);
-                dfjk::launch_k3_finish(h->Kpart + (int64_t)s * h->nsplit_alloc * nao * nao, nsplit,
-                                       nao, K[s], st);
-            }
     }
-    if (fused) {
-        { Timed t_(h, DFJK_KERNEL_J1R, st); dfjk::launch_j1_reduce(h->d_part, dfjk::j1x_num_blocks(nao, ldc), naux, h->d, st); }
-        { Timed t_(h, DFJK_KERNEL_J2, st); dfjk::launch_j2_axpy(h->B, naux, npair, h->d, h->Jp_part, h->j2_groups, st); }
-        { Timed t_(h, DFJK_KERNEL_J3, st); dfjk::launch_j3_unpack(h->Jp_part, h->j2_groups, npair, nao, J, st); }
-        h->have_d = true;
+    dfjk_handle::GraphSlot *slot = nullptr;
+    if (use_graph) {
+        for (auto &g : h->graphs)
+            if (g.seen && *reinterpret_cast<const GraphKey *>(g.key) == key) { slot = &g; break; }
+        if (!slot) {
+            /* first call of this shape: remember it (round-robin over the slots), launch plainly */
+            slot = &h->graphs[h->graph_next];
+            h->graph_next = (h->graph_next + 1) % DFJK_GRAPH_SLOTS;
+            if (slot->exec) { cudaGraphExecDestroy(slot->exec); slot->exec = nullptr; }
+            static_assert(sizeof(GraphKey) <= sizeof(slot->key), "GraphSlot::key too small");
+            memcpy(slot->key, &key, sizeof key);
+            slot->seen = true;
+            slot = nullptr;
+        }
     }
+
+    /* K0: zero-padded concatenation [C_0 | C_1], each set padded to a multiple of 8 columns; it also
+     * publishes this call's output pointers (slot 0 = J, 1 + s = K_s) */
+    double *outs[DFJK_OUT_SLOTS] = {J, nset > 0 ? K[0] : nullptr, nset > 1 ? K[1] : nullptr, nullptr};
+    { Timed t_(h, DFJK_KERNEL_K0, st); dfjk::launch_k0_pack_c(C, nocc, col0, nset, nao, ldc, h->Ccat, outs, h->out_slots, st); }
+
+    if (slot && !slot->exec) {
+        /* second call of this shape: capture the body on the handle's own stream */
+        if (!h->cap_stream) DFJK_CUDA_TRY(cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking));
+        const int64_t launches0 = h->launches;
+        cudaGraph_t graph = nullptr;
+        DFJK_CUDA_TRY(cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeThreadLocal));
+        const int rc = enqueue_jk_body(h, nset, nocc, col0, ldc, w, nullptr, K, J != nullptr, want_k,
+                                       h->out_slots, h->cap_stream, who);
+        const cudaError_t ec = cudaStreamEndCapture(h->cap_stream, &graph);
+        slot->launches = h->launches - launches0;
+        h->launches = launches0;
+        if (rc != DFJK_OK) { if (graph) cudaGraphDestroy(graph); cudaGetLastError(); return rc; }
+        if (ec != cudaSuccess) { cudaGetLastError(); return fail(DFJK_ECUDA, "%s: stream capture: %s", who, cudaGetErrorString(ec)); }
+        const cudaError_t ei = cudaGraphInstantiate(&slot->exec, graph, 0);
+        cudaGraphDestroy(graph);
+        if (ei != cudaSuccess) { slot->exec = nullptr; cudaGetLastError(); return fail(DFJK_ECUDA, "%s: cudaGraphInstantiate: %s", who, cudaGetErrorString(ei)); }
+    }
+    if (slot) {
+        DFJK_CUDA_TRY(cudaGraphLaunch(slot->exec, st));
+        h->launches += slot->launches;
+    } else {
+        const int rc = enqueue_jk_body(h, nset, nocc, col0, ldc, w, J, K, J != nullptr, want_k, nullptr, st, who);
+        if (rc != DFJK_OK) return rc;
+    }
+    if (J) h->have_d = true;
     DFJK_CUDA_TRY(cudaGetLastError());
     return DFJK_OK;
 }
@@ -341,7 +481,7 @@ int get_jk_general_impl(dfjk_handle *h, const double *C1, const double *C2, int6
         { Timed t_(h, DFJK_KERNEL_J1, st); dfjk::launch_j1_dot(h->B, naux, npair, h->Dt, h->d_part, h->sm_count, st); }
         { Timed t_(h, DFJK_KERNEL_J1R, st); dfjk::launch_j1_reduce(h->d_part, h->nchunk, naux, h->d, st); }
         { Timed t_(h, DFJK_KERNEL_J2, st); dfjk::launch_j2_axpy(h->B, naux, npair, h->d, h->Jp_part, h->j2_groups, st); }
-        { Timed t_(h, DFJK_KERNEL_J3, st); dfjk::launch_j3_unpack(h->Jp_part, h->j2_groups, npair, nao, J, st); }
+        { Timed t_(h, DFJK_KERNEL_J3, st); dfjk::launch_j3_unpack(h->Jp_part, h->j2_groups, npair, nao, J, nullptr, st); }
         h->have_d = true;
     }
     if (K) {
@@ -354,7 +494,7 @@ int get_jk_general_impl(dfjk_handle *h, const double *C1, const double *C2, int6
         const int64_t w8 = round_up(ncol, 8);
         const int col0[2] = {0, (int)w8};
         const int64_t ldx = 2 * w8, ldc = raw ? w8 : ldx;
-        { Timed t_(h, DFJK_KERNEL_K0, st); dfjk::launch_k0_pack_c(Cp, nocc, col0, raw ? 1 : 2, nao, ldc, h->Ccat, st); }
+        { Timed t_(h, DFJK_KERNEL_K0, st); dfjk::launch_k0_pack_c(Cp, nocc, col0, raw ? 1 : 2, nao, ldc, h->Ccat, nullptr, nullptr, st); }
         int64_t pc = h->x_doubles / (nao * ldx);
         if (h->opt_k_chunk > 0 && h->opt_k_chunk < pc) pc = h->opt_k_chunk;
         if (pc > naux) pc = naux;
@@ -366,7 +506,7 @@ int get_jk_general_impl(dfjk_handle *h, const double *C1, const double *C2, int6
         int chunk = 0;
         for (int64_t P0 = 0; P0 < naux; P0 += pc, ++chunk) {
             const int64_t np = (P0 + pc <= naux) ? pc : naux - P0;
-            { Timed t_(h, DFJK_KERNEL_K1, st); dfjk::launch_k1_half_transform(h->B, naux, nao, npair, P0, np, h->Ccat, ldc, ldx, h->X, st); }
+            { Timed t_(h, DFJK_KERNEL_K1, st); DFJK_LAUNCH_TRY(dfjk::launch_k1_half_transform(h->B, naux, nao, npair, P0, np, h->Ccat, ldc, ldx, h->X, st)); }
             if (raw) { Timed t_(h, DFJK_KERNEL_K1, st); dfjk::launch_k1u_unpack(h->B, nao, npair, P0, np, ldx, w8, h->X, st); }
             if (fused) {
                 const double one = 1.0;
@@ -374,13 +514,13 @@ int get_jk_general_impl(dfjk_handle *h, const double *C1, const double *C2, int6
                 dfjk::launch_j1x_dot(h->X, h->Ccat, nao, np, ldx, ldc, w8, 1, col0, nocc, &one, P0, naux, h->d_part, st);
             }
             { Timed t_(h, DFJK_KERNEL_K2, st);
-              dfjk::launch_k2_gemm_full(h->X, nao, np, ldx, col0[0], col0[1], ncol, h->Kpart, nsplit, chunk > 0, st); }
+              DFJK_LAUNCH_TRY(dfjk::launch_k2_gemm_full(h->X, nao, np, ldx, col0[0], col0[1], ncol, h->Kpart, nsplit, chunk > 0, st)); }
         }
         { Timed t_(h, DFJK_KERNEL_K3, st); dfjk::launch_k3_sum(h->Kpart, nsplit, nao, K, st); }
         if (fused) {
             { Timed t_(h, DFJK_KERNEL_J1R, st); dfjk::launch_j1_reduce(h->d_part, dfjk::j1x_num_blocks(nao, ldc), naux, h->d, st); }
             { Timed t_(h, DFJK_KERNEL_J2, st); dfjk::launch_j2_axpy(h->B, naux, npair, h->d, h->Jp_part, h->j2_groups, st); }
-            { Timed t_(h, DFJK_KERNEL_J3, st); dfjk::launch_j3_unpack(h->Jp_part, h->j2_groups, npair, nao, J, st); }
+            { Timed t_(h, DFJK_KERNEL_J3, st); dfjk::launch_j3_unpack(h->Jp_part, h->j2_groups, npair, nao, J, nullptr, st); }
             h->have_d = true;
         }
     }
@@ -466,6 +606,41 @@ extern "C" int dfjk_probe_dmma_peak(double *tflops)
     cudaFree(sink);
     DFJK_CUDA_TRY(cudaGetLastError());
     *tflops = best;
+    return DFJK_OK;
+}
+
+namespace dfjk {
+ScfWorkspace scf_workspace(dfjk_handle *h)
+{
+    return ScfWorkspace{h->X, h->x_doubles, h->Kpart, h->nsplit_alloc, h->sm_count};
+}
+void scf_store_timing(dfjk_handle *h, int64_t iters, double get_jk_ms, double eig_ms, double total_ms)
+{
+    h->scf_iters = iters; h->scf_get_jk_ms = get_jk_ms; h->scf_eig_ms = eig_ms; h->scf_total_ms = total_ms;
+}
+}  // namespace dfjk
+
+extern "C" int dfjk_scf_timing(const dfjk_handle *h, int64_t *iters, double *get_jk_ms, double *eig_ms,
+                               double *other_ms)
+{
+    g_err[0] = 0;
+    if (!h) return fail(DFJK_EINVAL, "dfjk_scf_timing: NULL handle");
+    if (h->scf_iters <= 0) return fail(DFJK_EINVAL, "dfjk_scf_timing: no SCF has run on this handle");
+    if (iters) *iters = h->scf_iters;
+    if (get_jk_ms) *get_jk_ms = h->scf_get_jk_ms;
+    if (eig_ms) *eig_ms = h->scf_eig_ms;
+    if (other_ms) *other_ms = h->scf_total_ms - h->scf_get_jk_ms - h->scf_eig_ms;
+    return DFJK_OK;
+}
+
+extern "C" int dfjk_device_info(int *sm_count, int *sm_clock_khz, int64_t *l2_bytes)
+{
+    g_err[0] = 0;
+    int dev = 0, v = 0;
+    DFJK_CUDA_TRY(cudaGetDevice(&dev));
+    if (sm_count) { DFJK_CUDA_TRY(cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev)); *sm_count = v; }
+    if (sm_clock_khz) { DFJK_CUDA_TRY(cudaDeviceGetAttribute(&v, cudaDevAttrClockRate, dev)); *sm_clock_khz = v; }
+    if (l2_bytes) { DFJK_CUDA_TRY(cudaDeviceGetAttribute(&v, cudaDevAttrL2CacheSize, dev)); *l2_bytes = v; }
     return DFJK_OK;
 }
 
@@ -558,7 +733,7 @@ extern "C" int dfjk_get_df_diag(dfjk_handle *h, double *diag, void *stream)
     if (dev != h->device) return fail(DFJK_EINVAL, "dfjk_get_df_diag: handle belongs to device %d, current is %d", h->device, dev);
     cudaStream_t st = (cudaStream_t)stream;
     { Timed t_(h, DFJK_KERNEL_J2, st); dfjk::launch_j2_axpy(h->B, h->naux, h->npair, nullptr, h->Jp_part, h->j2_groups, st); }
-    { Timed t_(h, DFJK_KERNEL_J3, st); dfjk::launch_j3_unpack(h->Jp_part, h->j2_groups, h->npair, h->nao, diag, st); }
+    { Timed t_(h, DFJK_KERNEL_J3, st); dfjk::launch_j3_unpack(h->Jp_part, h->j2_groups, h->npair, h->nao, diag, nullptr, st); }
     DFJK_CUDA_TRY(cudaGetLastError());
     return DFJK_OK;
 }
@@ -573,6 +748,51 @@ extern "C" int dfjk_get_d(dfjk_handle *h, double *d_out, void *stream)
     return DFJK_OK;
 }
 
+namespace {
+
+/* Lazy resources of the host entry points: a stream and device staging buffers for C, J, K (and a
+ * second C, K for the unrestricted call), kept until destroy.  Nothing is published in the handle
+ * unless everything was obtained: a failed first call leaves the handle exactly as it was, and
+ * the device check comes first so the resources can never be bound to a foreign device. */
+int host_resources(dfjk_handle *h, bool second_set, const char *who)
+{
+    int dev = -1;
+    DFJK_CUDA_TRY(cudaGetDevice(&dev));
+    if (dev != h->device) return fail(DFJK_EINVAL, "%s: handle belongs to device %d, current is %d", who, h->device, dev);
+    const size_t bytes = (size_t)h->nao * h->nao * sizeof(double);
+    if (!h->host_stream) {
+        cudaStream_t s = nullptr;
+        double *p[3] = {nullptr, nullptr, nullptr};
+        cudaError_t e = cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking);
+        for (int i = 0; i < 3 && e == cudaSuccess; ++i) e = cudaMalloc((void **)&p[i], bytes);
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            for (double *q : p) cudaFree(q);
+            if (s) cudaStreamDestroy(s);
+            return fail(DFJK_ENOMEM, "%s: staging resources (3 x %zu bytes): %s", who, bytes, cudaGetErrorString(e));
+        }
+        h->hostC = p[0]; h->hostJ = p[1]; h->hostK = p[2];
+        h->ws_bytes += 3 * (int64_t)bytes;
+        h->host_stream = s;                       /* published last */
+    }
+    if (second_set && !h->hostC2) {
+        double *p[2] = {nullptr, nullptr};
+        cudaError_t e = cudaSuccess;
+        for (int i = 0; i < 2 && e == cudaSuccess; ++i) e = cudaMalloc((void **)&p[i], bytes);
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            for (double *q : p) cudaFree(q);
+            return fail(DFJK_ENOMEM, "%s: staging resources (2 x %zu bytes): %s", who, bytes, cudaGetErrorString(e));
+        }
+        h->hostK2 = p[1];
+        h->ws_bytes += 2 * (int64_t)bytes;
+        h->hostC2 = p[0];                         /* published last */
+    }
+    return DFJK_OK;
+}
+
+}  // namespace
+
 extern "C" int dfjk_get_jk_host(dfjk_handle *h, const double *C_occ_host, int64_t nocc,
                                 double *J_host, double *K_host)
 {
@@ -582,12 +802,7 @@ extern "C" int dfjk_get_jk_host(dfjk_handle *h, const double *C_occ_host, int64_
     if (nocc < 1 || nocc > h->nao) return fail(DFJK_EINVAL, "dfjk_get_jk_host: nocc outside [1, nao]");
     if (!J_host && !K_host) return fail(DFJK_EINVAL, "dfjk_get_jk_host: no output requested");
     const int64_t n2 = h->nao * h->nao;
-    if (!h->host_stream) {
-        /* first host call: staging buffers for C, J, K (kept until destroy) */
-        DFJK_CUDA_TRY(cudaStreamCreateWithFlags(&h->host_stream, cudaStreamNonBlocking));
-        if (alloc_ws(h, &h->hostC, n2) || alloc_ws(h, &h->hostJ, n2) || alloc_ws(h, &h->hostK, n2))
-            return DFJK_ENOMEM;
-    }
+    { const int rc0 = host_resources(h, false, "dfjk_get_jk_host"); if (rc0 != DFJK_OK) return rc0; }
     cudaStream_t st = h->host_stream;
     DFJK_CUDA_TRY(cudaMemcpyAsync(h->hostC, C_occ_host, (size_t)h->nao * nocc * 8, cudaMemcpyHostToDevice, st));
     const int rc = dfjk_get_jk(h, h->hostC, nocc, J_host ? h->hostJ : nullptr,
@@ -610,12 +825,7 @@ extern "C" int dfjk_get_jk_u_host(dfjk_handle *h, const double *C_a_host, int64_
         return fail(DFJK_EINVAL, "dfjk_get_jk_u_host: nocc outside [1, nao]");
     if (!J_host && !K_a_host && !K_b_host) return fail(DFJK_EINVAL, "dfjk_get_jk_u_host: no output requested");
     const int64_t n2 = h->nao * h->nao;
-    if (!h->host_stream) {
-        DFJK_CUDA_TRY(cudaStreamCreateWithFlags(&h->host_stream, cudaStreamNonBlocking));
-        if (alloc_ws(h, &h->hostC, n2) || alloc_ws(h, &h->hostJ, n2) || alloc_ws(h, &h->hostK, n2))
-            return DFJK_ENOMEM;
-    }
-    if (!h->hostC2 && (alloc_ws(h, &h->hostC2, n2) || alloc_ws(h, &h->hostK2, n2))) return DFJK_ENOMEM;
+    { const int rc0 = host_resources(h, true, "dfjk_get_jk_u_host"); if (rc0 != DFJK_OK) return rc0; }
     cudaStream_t st = h->host_stream;
     DFJK_CUDA_TRY(cudaMemcpyAsync(h->hostC, C_a_host, (size_t)h->nao * nocc_a * 8, cudaMemcpyHostToDevice, st));
     DFJK_CUDA_TRY(cudaMemcpyAsync(h->hostC2, C_b_host, (size_t)h->nao * nocc_b * 8, cudaMemcpyHostToDevice, st));
@@ -636,6 +846,9 @@ extern "C" int dfjk_kernel_time(dfjk_handle *h, int kernel, double *ms_total, in
     g_err[0] = 0;
     if (!h || !ms_total || !count) return fail(DFJK_EINVAL, "dfjk_kernel_time: NULL argument");
     if (kernel < 0 || kernel >= DFJK_KERNEL_COUNT) return fail(DFJK_EINVAL, "dfjk_kernel_time: bad kernel id");
+    if (h->ev_overflow)
+        return fail(DFJK_ENOMEM, "dfjk_kernel_time: the event ring could not grow, some launches since the last "
+                                 "set_option(time_kernels) were not recorded");
     double tot = 0.0;
     int64_t n = 0;
     for (int i = 0; i < h->ev_used; ++i) {

@@ -53,23 +53,28 @@ void launch_j2_axpy(const double *B, int64_t naux, int64_t npair, const double *
                     double *Jp_part, int64_t ngroup, cudaStream_t st);
 
 /* J3: J[mu][nu] = J[nu][mu] = sum_g Jp_part[g][mu(mu+1)/2+nu]. */
+/* Jslot != NULL: the kernel writes to *Jslot (a device-resident pointer published by K0) instead of J */
 void launch_j3_unpack(const double *Jp_part, int64_t ngroup, int64_t npair, int64_t nao,
-                      double *J, cudaStream_t st);
+                      double *J, double *const *Jslot, cudaStream_t st);
 
 /* ---------------------------------------------------------------- K path */
 
 /* K0: the zero-padded concatenation [C_0 | C_1 | ...] (every set padded to a multiple of 8
  * columns, ldc columns in total) in k-group-major layout
  *   Ccat4[(mu/4)*ldc*4 + c*4 + mu%4],  mu < round_up(nao, 32) (rows >= nao are zero). */
+#define DFJK_OUT_SLOTS 4
+/* outs != NULL: the kernel also copies the DFJK_OUT_SLOTS output pointers outs[] (J, K_0, K_1, ...) of
+ * this call to the device array out_slots, where K3 / J3 of a captured launch sequence find them. */
 void launch_k0_pack_c(const double *const *C, const int *nocc, const int *col0, int nset,
-                      int64_t nao, int64_t ldc, double *Ccat, cudaStream_t st);
+                      int64_t nao, int64_t ldc, double *Ccat, double *const *outs, double **out_slots,
+                      cudaStream_t st);
 
 /* K1: for P in [P0, P0+np), k = (P-P0)*ldc + i:
  *   X4[(k/4)*nao*4 + mu*4 + k%4] = sum_nu B_P(mu,nu) Ccat[nu][i]      (k-group-major X)
  * with k = (P-P0)*ldx + i: ldx >= ldc is X's row pitch (ldx > ldc leaves room for K1U's columns). */
-void launch_k1_half_transform(const double *B, int64_t naux, int64_t nao, int64_t npair,
-                              int64_t P0, int64_t np, const double *Ccat4, int64_t ldc, int64_t ldx,
-                              double *X4, cudaStream_t st);
+cudaError_t launch_k1_half_transform(const double *B, int64_t naux, int64_t nao, int64_t npair,
+                                     int64_t P0, int64_t np, const double *Ccat4, int64_t ldc, int64_t ldx,
+                                     double *X4, cudaStream_t st);
 
 /* K1U: X4 columns [col0, col0 + round_up(nao,4)) of the chunk = B_P unpacked (X_P = B_P . I). */
 void launch_k1u_unpack(const double *B, int64_t nao, int64_t npair, int64_t P0, int64_t np, int64_t ldx,
@@ -78,21 +83,22 @@ void launch_k1u_unpack(const double *B, int64_t nao, int64_t npair, int64_t P0, 
 /* K2: Kpart[split][mu][nu] (+)= sum_{k in split's share} X[mu][k] X[nu][k]
  * for mu-tile >= nu-tile (lower 128x128 tiles).  The set uses k = p*ldc + [col0, col0+round_up(ncol,4)),
  * p < np: K2's MMA k step is 4, so the 8-padding columns of Ccat beyond that are never read.  accumulate = 0 overwrites. */
-void launch_k2_syrk_lower(const double *X4, int64_t nao, int64_t np, int64_t ldc, int64_t col0,
-                          int64_t ncol, double *Kpart, int nsplit, int accumulate, cudaStream_t st);
+cudaError_t launch_k2_syrk_lower(const double *X4, int64_t nao, int64_t np, int64_t ldc, int64_t col0,
+                                 int64_t ncol, double *Kpart, int nsplit, int accumulate, cudaStream_t st);
 
 /* K2 general: Kpart[split][mu][nu] (+)= sum_k X[mu][k_a] X[nu][k_b] over ALL tiles, with
  * k_a = p*ldc + col0a + j, k_b = p*ldc + col0b + j, j < round_up(ncol,4): the product
  * sum_P (B_P C1)(B_P C2)^T of two column ranges of the same X chunk (not symmetric). */
-void launch_k2_gemm_full(const double *X4, int64_t nao, int64_t np, int64_t ldc, int64_t col0a,
-                         int64_t col0b, int64_t ncol, double *Kpart, int nsplit, int accumulate,
-                         cudaStream_t st);
+cudaError_t launch_k2_gemm_full(const double *X4, int64_t nao, int64_t np, int64_t ldc, int64_t col0a,
+                                int64_t col0b, int64_t ncol, double *Kpart, int nsplit, int accumulate,
+                                cudaStream_t st);
 
 /* K3 general: K[mu][nu] = sum_split Kpart[split][mu][nu] for every (mu, nu). */
 void launch_k3_sum(const double *Kpart, int nsplit, int64_t nao, double *K, cudaStream_t st);
 
 /* K3: K[mu][nu] = K[nu][mu] = sum_split Kpart[split][mu][nu], mu >= nu. */
-void launch_k3_finish(const double *Kpart, int nsplit, int64_t nao, double *K, cudaStream_t st);
+void launch_k3_finish(const double *Kpart, int nsplit, int64_t nao, double *K, double *const *Kslot,
+                      cudaStream_t st);
 
 /* ---------------------------------------------------------------- building B (Eq. 2-3) */
 
@@ -119,6 +125,13 @@ void launch_fp64_tile_gemm(const double *A, int64_t lda, const double *Bop, int6
 /* ---------------------------------------------------------------- SCF driver (scf_rhf.cu) */
 struct dfjk_handle;
 namespace dfjk {
+/* what the SCF driver borrows from the handle (dfjk_api.cu): the X workspace and the partial-K slots
+ * (idle between two get_jk calls) for its own DMMA products, and where it leaves its timing */
+struct ScfWorkspace { double *X; int64_t x_doubles; double *Kpart; int nsplit_alloc; int sm_count; };
+ScfWorkspace scf_workspace(dfjk_handle *h);
+void scf_store_timing(dfjk_handle *h, int64_t iters, double get_jk_ms, double eig_ms, double total_ms);
+/* split count that fills sm_count SMs best with ntile * s equal work items (dfjk_api.cu) */
+int choose_splits(int ntile, int sm_count, int max_splits);
 /* nspin = 1: restricted (get_jk), nspin = 2: unrestricted (get_jk_u); per-spin arguments are arrays */
 int scf_run(dfjk_handle *h, int64_t nao, int nspin, const double *hcore, const double *S,
             const int64_t *nocc, int64_t max_iter, double conv_tol, int64_t diis_space,

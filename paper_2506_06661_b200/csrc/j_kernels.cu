@@ -391,10 +391,13 @@ constexpr int J3_T = 32;
 
 __global__ void __launch_bounds__(256)
 j3_unpack_kernel(const double *__restrict__ Jp_part, int64_t ngroup, int64_t npair, int64_t nao,
-                 double *__restrict__ J)
+                 double *__restrict__ Jdirect, double *const *__restrict__ Jslot)
 {
     const int bi = blockIdx.y, bj = blockIdx.x;
     if (bj > bi) return;
+    /* Jslot != NULL: the output pointer of THIS call sits in device memory (written by K0), so that
+     * one captured launch sequence serves every call (dfjk_api.cu, "graph") */
+    double *__restrict__ J = Jslot ? *Jslot : Jdirect;
     __shared__ double t[J3_T][J3_T + 1];
     const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
     const int64_t mu0 = (int64_t)bi * J3_T, nu0 = (int64_t)bj * J3_T;
@@ -518,10 +521,10 @@ void launch_j2_axpy(const double *B, int64_t naux, int64_t npair, const double *
 }
 
 void launch_j3_unpack(const double *Jp_part, int64_t ngroup, int64_t npair, int64_t nao, double *J,
-                      cudaStream_t st)
+                      double *const *Jslot, cudaStream_t st)
 {
     const unsigned nb = (unsigned)((nao + J3_T - 1) / J3_T);
-    j3_unpack_kernel<<<dim3(nb, nb), 256, 0, st>>>(Jp_part, ngroup, npair, nao, J);
+    j3_unpack_kernel<<<dim3(nb, nb), 256, 0, st>>>(Jp_part, ngroup, npair, nao, J, Jslot);
 }
 
 }  // namespace dfjk

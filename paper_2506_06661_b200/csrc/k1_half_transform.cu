@@ -55,6 +55,25 @@ constexpr int K1_LDD = 36;                        /* 32 + shift + pad, 16-B mult
 constexpr int K1_LDT = 132;                       /* 128 + shift + pad, 16-B multiple */
 constexpr int K1_A_BYTES = K1_M * K1_LDD * 8;     /* 36864 >= 32 * K1_LDT * 8 = 33792 */
 constexpr int K1_SMEM_BUDGET = 220 * 1024;
+/* Every off-diagonal packed element is staged twice: in "row" form by the item of its row block and
+ * in "col" form by the item of its column block (the lower-numbered one).  The items of one P run
+ * at the same time on neighbouring CTAs and walk nu at the same pace, so the row-form read (stage
+ * nu/32) comes first and the col-form read (stage mu/32 > nu/32) second: the first is marked
+ * L2 evict_last, the second evict_first, and the items of a P are numbered from the LAST row block
+ * down so that the row-form reader never starts later than the col-form reader.  The second read
+ * then hits L2 instead of HBM (ncu r01e: K1 read 1.44 x |B| from DRAM without this). */
+#ifndef DFJK_K1_L2_HINTS
+#define DFJK_K1_L2_HINTS 1
+#endif
+#ifndef DFJK_K1_DESCENDING
+#define DFJK_K1_DESCENDING 1
+#endif
+
+/* row block of the r-th item of a P (r = item index within the P divided by the N tiles) */
+__device__ __forceinline__ int64_t k1_row_block(int r, int nib)
+{
+    return DFJK_K1_DESCENDING ? nib - 1 - r : r;
+}
 
 enum { K1_MODE_ROW = 0, K1_MODE_COL = 1, K1_MODE_GATHER = 2 };
 
@@ -97,7 +116,8 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int nk = (int)((nao + K1_KC - 1) / K1_KC);
-    const int items_per_p = (int)((nao + K1_M - 1) / K1_M) * ntiles_n;
+    const int nib = (int)((nao + K1_M - 1) / K1_M);
+    const int items_per_p = nib * ntiles_n;
 
     const uint32_t smem_base = smem_u32(smem_raw);
     const uint32_t bar_base = smem_base + Cfg::STAGES * Cfg::STAGE_BYTES;
@@ -116,13 +136,16 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
     if (warp < K1_PRODUCERS / 32) {
         /* ------------------------------------------------------------ producers */
         reg_dealloc<40>();
+#if DFJK_K1_L2_HINTS
+        const uint64_t pol_first = l2_policy_evict_last(), pol_second = l2_policy_evict_first();
+#endif
         int slot = 0;
         uint32_t phase = 1;                                /* parity of the "empty" phase to wait for */
         bool ring_full = false;                            /* all STAGES slots have been used once */
         for (int64_t item = blockIdx.x; item < nitems; item += gridDim.x) {
         const int64_t p = item / items_per_p;
         const int rem = (int)(item - p * items_per_p);
-        const int64_t mu0 = (int64_t)(rem / ntiles_n) * K1_M;
+        const int64_t mu0 = k1_row_block(rem / ntiles_n, nib) * K1_M;
         const int64_t n0 = (int64_t)(rem % ntiles_n) * Cfg::NW;
         const int64_t pb = (P0 + p) * npair;               /* index of B_P's first element in B */
         const int pbpar = (int)(pb & 1);
@@ -149,7 +172,11 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
                 const uint32_t nb = ok ? (uint32_t)(K1_KC + 2 * sft) * 8u : 0u;
                 my_bytes += nb;
                 if (my_bytes) mbar_arrive_expect_tx(bar, my_bytes); else mbar_arrive(bar);
+#if DFJK_K1_L2_HINTS
+                if (ok) bulk_g2s_hint(a_dst + tid * (K1_LDD * 8), B + (e - sft), nb, bar, pol_first);
+#else
                 if (ok) bulk_g2s(a_dst + tid * (K1_LDD * 8), B + (e - sft), nb, bar);
+#endif
             } else if (mode == K1_MODE_COL) {
                 /* thread t < 32 copies packed row nu0+t, columns mu0 .. mu0+rows_valid-1 */
                 const int64_t nu = nu0 + tid;
@@ -163,7 +190,11 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
                     for (int c = tid; c < K1_LDT; c += K1_PRODUCERS)
                         reinterpret_cast<double *>(smem_raw + slot * Cfg::STAGE_BYTES)[k * K1_LDT + c] = 0.0;
                 if (my_bytes) mbar_arrive_expect_tx(bar, my_bytes); else mbar_arrive(bar);
+#if DFJK_K1_L2_HINTS
+                if (ok) bulk_g2s_hint(a_dst + tid * (K1_LDT * 8), B + (e - sft), nb, bar, pol_second);
+#else
                 if (ok) bulk_g2s(a_dst + tid * (K1_LDT * 8), B + (e - sft), nb, bar);
+#endif
             } else {
                 /* element-wise gather into the "row" form (8-byte cp.async, zero fill outside) */
                 if (tid == 0) mbar_expect_tx(bar, c_bytes);
@@ -201,7 +232,7 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
         for (int64_t item = blockIdx.x; item < nitems; item += gridDim.x) {
         const int64_t p = item / items_per_p;
         const int rem = (int)(item - p * items_per_p);
-        const int64_t mu0 = (int64_t)(rem / ntiles_n) * K1_M;
+        const int64_t mu0 = k1_row_block(rem / ntiles_n, nib) * K1_M;
         const int64_t n0 = (int64_t)(rem % ntiles_n) * Cfg::NW;
         const int pbpar = (int)(((P0 + p) * npair) & 1);
         const bool last_p = P0 + p == naux - 1;
@@ -230,7 +261,6 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
                 const int a_gstep = colform ? 4 * K1_LDT : 4;        /* next k-group */
                 const int a_mstep = colform ? 8 : 8 * K1_LDD;        /* next 8 rows */
                 const double *b_base = Cs + lq * 4 + lr;
-#pragma unroll
                 if (!half) {
 #pragma unroll
                     for (int g = 0; g < K1_KG; ++g) {
@@ -305,11 +335,12 @@ k1u_unpack_kernel(const double *__restrict__ B, int64_t nao, int64_t npair, int6
 }
 
 template <int NT8>
-void k1_launch_t(const double *B, int64_t naux, int64_t nao, int64_t npair, int64_t P0, int64_t np,
-                 const double *Ccat4, int64_t ldc, int64_t ldx, int ntiles_n, double *X4, cudaStream_t st)
+cudaError_t k1_launch_t(const double *B, int64_t naux, int64_t nao, int64_t npair, int64_t P0, int64_t np,
+                        const double *Ccat4, int64_t ldc, int64_t ldx, int ntiles_n, double *X4, cudaStream_t st)
 {
-    static unsigned long long smem_ok = 0;
-    ensure_dynamic_smem(k1_half_transform_kernel<NT8>, K1Cfg<NT8>::SMEM_BYTES, smem_ok);
+    static std::atomic<unsigned long long> smem_ok{0};
+    cudaError_t e = ensure_dynamic_smem(k1_half_transform_kernel<NT8>, K1Cfg<NT8>::SMEM_BYTES, smem_ok);
+    if (e != cudaSuccess) return e;
     int dev = 0, sm_count = 0;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev);
@@ -319,25 +350,27 @@ void k1_launch_t(const double *B, int64_t naux, int64_t nao, int64_t npair, int6
     const unsigned grid = (unsigned)(nitems < sm_count ? nitems : sm_count);   /* persistent: 1 CTA / SM */
     k1_half_transform_kernel<NT8><<<grid, K1_THREADS, K1Cfg<NT8>::SMEM_BYTES, st>>>(
         B, naux, nao, npair, P0, Ccat4, ldc, ldx, ntiles_n, nitems, X4);
+    return cudaPeekAtLastError();
 }
 
 }  // namespace
 
-void launch_k1_half_transform(const double *B, int64_t naux, int64_t nao, int64_t npair, int64_t P0, int64_t np,
-                              const double *Ccat4, int64_t ldc, int64_t ldx, double *X4, cudaStream_t st)
+cudaError_t launch_k1_half_transform(const double *B, int64_t naux, int64_t nao, int64_t npair, int64_t P0,
+                                     int64_t np, const double *Ccat4, int64_t ldc, int64_t ldx, double *X4,
+                                     cudaStream_t st)
 {
     const int n8 = (int)(ldc / 8);
     const int ntiles_n = (n8 + 16) / 17;
     const int nt8 = (n8 + ntiles_n - 1) / ntiles_n;
     /* grid.y <= 65535: chunks are far smaller than that */
 #define DFJK_K1_CASE(N) \
-    case N: k1_launch_t<N>(B, naux, nao, npair, P0, np, Ccat4, ldc, ldx, ntiles_n, X4, st); break;
+    case N: return k1_launch_t<N>(B, naux, nao, npair, P0, np, Ccat4, ldc, ldx, ntiles_n, X4, st);
     switch (nt8) {
         DFJK_K1_CASE(1) DFJK_K1_CASE(2) DFJK_K1_CASE(3) DFJK_K1_CASE(4) DFJK_K1_CASE(5)
         DFJK_K1_CASE(6) DFJK_K1_CASE(7) DFJK_K1_CASE(8) DFJK_K1_CASE(9) DFJK_K1_CASE(10)
         DFJK_K1_CASE(11) DFJK_K1_CASE(12) DFJK_K1_CASE(13) DFJK_K1_CASE(14) DFJK_K1_CASE(15)
         DFJK_K1_CASE(16) DFJK_K1_CASE(17)
-    default: break;
+    default: return cudaErrorInvalidValue;      /* no tile shape for this width: never launch nothing silently */
     }
 #undef DFJK_K1_CASE
 }

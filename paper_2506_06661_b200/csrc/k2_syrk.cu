@@ -33,13 +33,19 @@ struct PackDesc {
     const double *C[4];
     int nocc[4];
     int col0[4];
+    double *out[DFJK_OUT_SLOTS];        /* this call's output pointers (J, K_0, K_1, ...) */
+    double **out_slots;                 /* device array they are published to, or NULL */
 };
 
-/* Ccat4[(mu/4)][c][mu%4], mu < nao16 (rows >= nao and padding columns are zero) */
+/* Ccat4[(mu/4)][c][mu%4], mu < nao16 (rows >= nao and padding columns are zero).  Thread 0 also
+ * publishes the call's output pointers to out_slots: the finishing kernels (K3, J3) of a captured
+ * launch sequence read them from there (stream order makes K0's write visible to them). */
 __global__ void k0_pack_c_kernel(PackDesc pd, int64_t nao, int64_t nao16, int64_t ldc,
                                  double *__restrict__ Ccat4)
 {
     const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx == 0 && pd.out_slots)
+        for (int i = 0; i < DFJK_OUT_SLOTS; ++i) pd.out_slots[i] = pd.out[i];
     if (idx >= nao16 * ldc) return;
     const int64_t mu = idx / ldc;
     const int c = (int)(idx % ldc);
@@ -74,10 +80,13 @@ k2_syrk_lower_kernel(const double *__restrict__ X4, int64_t nao, int64_t np, int
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     /* lower-triangle tile index -> (bi, bj), bi >= bj */
-    /* blockIdx.x = split (fastest), blockIdx.y = tile: the hardware dispatches CTAs in linear
-     * order, so the last block row -- the ragged, cheaper tiles -- runs last and the launch's
-     * tail is made of short CTAs */
-    const int t = blockIdx.y;
+    /* blockIdx.x = tile (fastest), blockIdx.y = split: the hardware dispatches CTAs in linear order, so
+     * the CTAs resident at any time belong to one or two splits and walk the SAME k range of X at the
+     * same pace -- a 128-row operand panel fetched from HBM by one CTA is an L2 hit for the other tiles
+     * of its block row / column (split-fastest order made co-resident CTAs read 13 different k ranges:
+     * 8.3 x the X chunk from DRAM, ncu r01e).  The last block row -- the ragged, cheaper tiles -- still
+     * comes last within every split, so the launch's tail is made of short CTAs. */
+    const int t = blockIdx.x;
     int bi, bj;
     if (FULL) {
         const int nb = (int)((nao + K2_T - 1) / K2_T);
@@ -90,7 +99,7 @@ k2_syrk_lower_kernel(const double *__restrict__ X4, int64_t nao, int64_t np, int
         bj = t - bi * (bi + 1) / 2;
     }
     const bool diag = !FULL && bi == bj;         /* both operands are the same panel */
-    const int split = blockIdx.x;
+    const int split = blockIdx.y;
     const int64_t mu0 = (int64_t)bi * K2_T, nu0 = (int64_t)bj * K2_T;
 
     /* this split's share of the k groups (4 columns each) of the set */
@@ -305,10 +314,12 @@ k2_syrk_lower_kernel(const double *__restrict__ X4, int64_t nao, int64_t np, int
 constexpr int K3_T = 32;
 
 __global__ void __launch_bounds__(256)
-k3_finish_kernel(const double *__restrict__ Kpart, int nsplit, int64_t nao, double *__restrict__ K)
+k3_finish_kernel(const double *__restrict__ Kpart, int nsplit, int64_t nao, double *__restrict__ Kdirect,
+                 double *const *__restrict__ Kslot)
 {
     const int bi = blockIdx.y, bj = blockIdx.x;
     if (bj > bi) return;
+    double *__restrict__ K = Kslot ? *Kslot : Kdirect;        /* see j3_unpack_kernel */
     __shared__ double t[K3_T][K3_T + 1];
     const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
     const int64_t mu0 = (int64_t)bi * K3_T, nu0 = (int64_t)bj * K3_T;
@@ -368,10 +379,12 @@ k3_sum_kernel(const double *__restrict__ Kpart, int nsplit, int64_t n2, double *
 }  // namespace
 
 void launch_k0_pack_c(const double *const *C, const int *nocc, const int *col0, int nset, int64_t nao,
-                      int64_t ldc, double *Ccat, cudaStream_t st)
+                      int64_t ldc, double *Ccat, double *const *outs, double **out_slots, cudaStream_t st)
 {
     PackDesc pd;
     pd.nset = nset;
+    for (int i = 0; i < DFJK_OUT_SLOTS; ++i) pd.out[i] = outs ? outs[i] : nullptr;
+    pd.out_slots = outs ? out_slots : nullptr;
     for (int s = 0; s < 4; ++s) {
         pd.C[s] = s < nset ? C[s] : nullptr;
         pd.nocc[s] = s < nset ? nocc[s] : 0;
@@ -382,34 +395,39 @@ void launch_k0_pack_c(const double *const *C, const int *nocc, const int *col0, 
     k0_pack_c_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(pd, nao, nao16, ldc, Ccat);
 }
 
-void launch_k2_syrk_lower(const double *X4, int64_t nao, int64_t np, int64_t ldc, int64_t col0,
-                          int64_t ncol, double *Kpart, int nsplit, int accumulate, cudaStream_t st)
+cudaError_t launch_k2_syrk_lower(const double *X4, int64_t nao, int64_t np, int64_t ldc, int64_t col0,
+                                 int64_t ncol, double *Kpart, int nsplit, int accumulate, cudaStream_t st)
 {
-    static unsigned long long smem_ok = 0;
-    ensure_dynamic_smem(k2_syrk_lower_kernel<false>, K2_SMEM_BYTES, smem_ok);
+    static std::atomic<unsigned long long> smem_ok{0};
+    const cudaError_t e = ensure_dynamic_smem(k2_syrk_lower_kernel<false>, K2_SMEM_BYTES, smem_ok);
+    if (e != cudaSuccess) return e;
     const int nb = (int)((nao + K2_T - 1) / K2_T);
     const int ntile = nb * (nb + 1) / 2;
     const int n4s = (int)((ncol + 3) / 4);              /* k step 4: Ccat's padding to 8 is not read */
-    k2_syrk_lower_kernel<false><<<dim3((unsigned)nsplit, (unsigned)ntile), K2_THREADS, K2_SMEM_BYTES, st>>>(
+    k2_syrk_lower_kernel<false><<<dim3((unsigned)ntile, (unsigned)nsplit), K2_THREADS, K2_SMEM_BYTES, st>>>(
         X4, nao, np, ldc / 4, col0 / 4, col0 / 4, n4s, Kpart, nsplit, accumulate);
+    return cudaPeekAtLastError();
 }
 
-void launch_k2_gemm_full(const double *X4, int64_t nao, int64_t np, int64_t ldc, int64_t col0a,
-                         int64_t col0b, int64_t ncol, double *Kpart, int nsplit, int accumulate,
-                         cudaStream_t st)
+cudaError_t launch_k2_gemm_full(const double *X4, int64_t nao, int64_t np, int64_t ldc, int64_t col0a,
+                                int64_t col0b, int64_t ncol, double *Kpart, int nsplit, int accumulate,
+                                cudaStream_t st)
 {
-    static unsigned long long smem_ok = 0;
-    ensure_dynamic_smem(k2_syrk_lower_kernel<true>, K2_SMEM_BYTES, smem_ok);
+    static std::atomic<unsigned long long> smem_ok{0};
+    const cudaError_t e = ensure_dynamic_smem(k2_syrk_lower_kernel<true>, K2_SMEM_BYTES, smem_ok);
+    if (e != cudaSuccess) return e;
     const int nb = (int)((nao + K2_T - 1) / K2_T);
     const int n4s = (int)((ncol + 3) / 4);
-    k2_syrk_lower_kernel<true><<<dim3((unsigned)nsplit, (unsigned)(nb * nb)), K2_THREADS, K2_SMEM_BYTES, st>>>(
+    k2_syrk_lower_kernel<true><<<dim3((unsigned)(nb * nb), (unsigned)nsplit), K2_THREADS, K2_SMEM_BYTES, st>>>(
         X4, nao, np, ldc / 4, col0a / 4, col0b / 4, n4s, Kpart, nsplit, accumulate);
+    return cudaPeekAtLastError();
 }
 
-void launch_k3_finish(const double *Kpart, int nsplit, int64_t nao, double *K, cudaStream_t st)
+void launch_k3_finish(const double *Kpart, int nsplit, int64_t nao, double *K, double *const *Kslot,
+                      cudaStream_t st)
 {
     const unsigned nb = (unsigned)((nao + K3_T - 1) / K3_T);
-    k3_finish_kernel<<<dim3(nb, nb), 256, 0, st>>>(Kpart, nsplit, nao, K);
+    k3_finish_kernel<<<dim3(nb, nb), 256, 0, st>>>(Kpart, nsplit, nao, K, Kslot);
 }
 
 double fp64_peak_probe_flops(int ctas, int iters) { return (double)ctas * 8.0 * iters * 16.0 * 512.0; }

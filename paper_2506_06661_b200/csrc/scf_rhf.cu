@@ -10,8 +10,11 @@
  *     F    = hcore + J - K                        S1 (elementwise)
  *     D    = 2 C_occ C_occ^T                      FP64 tile product
  *     E    = 1/2 sum D o (hcore + F)              S2 (two-stage deterministic reduction)
- *     e    = F D S - (F D S)^T                    two FP64 tile products + S3
- *     DIIS: B_ij = <e_i, e_j> (S2), the (m+1) x (m+1) system on the host, F_ext = sum c_i F_i (S4)
+ *     e    = F D S - (F D S)^T                    two DMMA products (S6 packs the operands into the
+ *                                                 k-group-major layout of the X workspace, then the
+ *                                                 full-product kernel of k2_syrk.cu and K3's sum) + S3
+ *     DIIS: B_im = <e_i, e_m> for all i in ONE launch pair (S2b), read back together with E and
+ *           max|e| in ONE host sync; the (m+1) x (m+1) system on the host, F_ext = sum c_i F_i (S4)
  *     F_ext C = S C eps                           cuSOLVER Dsygvd -- the one library step, loaded
  *                                                 with dlopen so libdfjk.so itself has no
  *                                                 dependency on it
@@ -30,6 +33,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <vector>
 
 namespace dfjk {
@@ -46,20 +50,22 @@ struct Cusolver {
                                       const double *, int *) = nullptr;
     cusolverStatus_t (*sygvd)(cusolverDnHandle_t, cusolverEigType_t, cusolverEigMode_t, cublasFillMode_t,
                               int, double *, int, double *, int, double *, double *, int, int *) = nullptr;
+    char why[256] = "";                 /* why loading failed (dlerror of the first name tried) */
     bool ok() const { return lib && create && destroy && set_stream && sygvd_bufsize && sygvd; }
 };
 
 Cusolver &cusolver()
 {
     static Cusolver cs;
-    static bool tried = false;
-    if (!tried) {
-        tried = true;
+    static std::once_flag once;
+    std::call_once(once, [] {
         const char *names[] = {"libcusolver.so.11", "libcusolver.so",
                                "/usr/local/cuda/lib64/libcusolver.so.11", "libcusolver.so.12"};
         for (const char *n : names) {
             cs.lib = dlopen(n, RTLD_NOW | RTLD_LOCAL);
             if (cs.lib) break;
+            const char *e = dlerror();          /* dlerror() clears itself: read it exactly once */
+            if (e && !cs.why[0]) snprintf(cs.why, sizeof cs.why, "%s", e);
         }
         if (cs.lib) {
             cs.create = (decltype(cs.create))dlsym(cs.lib, "cusolverDnCreate");
@@ -67,8 +73,9 @@ Cusolver &cusolver()
             cs.set_stream = (decltype(cs.set_stream))dlsym(cs.lib, "cusolverDnSetStream");
             cs.sygvd_bufsize = (decltype(cs.sygvd_bufsize))dlsym(cs.lib, "cusolverDnDsygvd_bufferSize");
             cs.sygvd = (decltype(cs.sygvd))dlsym(cs.lib, "cusolverDnDsygvd");
+            if (!cs.ok()) snprintf(cs.why, sizeof cs.why, "a cusolverDn symbol is missing");
         }
-    }
+    });
     return cs;
 }
 
@@ -135,6 +142,57 @@ __global__ void lincomb_kernel(Coefs cf, int64_t n2, double *__restrict__ out)
     out[i] = acc;
 }
 
+/* S6: operand packing for the DMMA product kernel of k2_syrk.cu, which reads both operands from one
+ * k-group-major array X4[(k/4)][row][k%4]:  X4 column c0 + k of row r = M[r][k], k < n (zero for the
+ * padding columns up to round_up(n, 4)).  One thread per (row, group of 4 columns): 32-byte store,
+ * consecutive threads own consecutive rows => contiguous stores. */
+__global__ void __launch_bounds__(256)
+pack_x4_kernel(const double *__restrict__ M, int64_t n, int64_t c0, double *__restrict__ X4)
+{
+    const int64_t r = (int64_t)blockIdx.x * 256 + threadIdx.x;
+    const int64_t g = blockIdx.y;
+    if (r >= n) return;
+    double v[4];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) v[q] = 4 * g + q < n ? M[r * n + 4 * g + q] : 0.0;
+    double2 *dst = reinterpret_cast<double2 *>(X4 + (((c0 >> 2) + g) * n + r) * 4);
+    dst[0] = make_double2(v[0], v[1]);
+    dst[1] = make_double2(v[2], v[3]);
+}
+
+/* S2b: all DIIS dots of one iteration at once: partial[(i*nspin + s)*RED_BLOCKS + b] = block b's
+ * share of <Ering_s[slot_i], Er_s>; dots_final sums blocks and spins in a fixed order. */
+struct DotArgs { const double *a[32]; const double *b[32]; int npairs; };
+
+__global__ void __launch_bounds__(RED_THREADS)
+dots_partial_kernel(DotArgs da, int64_t n, double *__restrict__ partial)
+{
+    __shared__ double sh[RED_THREADS];
+    const double *__restrict__ a = da.a[blockIdx.y];
+    const double *__restrict__ b = da.b[blockIdx.y];
+    double acc = 0.0;
+    for (int64_t i = (int64_t)blockIdx.x * RED_THREADS + threadIdx.x; i < n; i += (int64_t)RED_BLOCKS * RED_THREADS)
+        acc += a[i] * b[i];
+    sh[threadIdx.x] = acc;
+    __syncthreads();
+    for (int s = RED_THREADS / 2; s > 0; s >>= 1) {
+        if (threadIdx.x < s) sh[threadIdx.x] += sh[threadIdx.x + s];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) partial[(int64_t)blockIdx.y * RED_BLOCKS + blockIdx.x] = sh[0];
+}
+
+/* out[i] = sum_s sum_b partial[(i*nspin + s)][b], i < m */
+__global__ void dots_final_kernel(const double *__restrict__ partial, int m, int nspin, double *__restrict__ out)
+{
+    const int i = threadIdx.x;
+    if (i >= m) return;
+    double acc = 0.0;
+    for (int s = 0; s < nspin; ++s)
+        for (int b = 0; b < RED_BLOCKS; ++b) acc += partial[(int64_t)(i * nspin + s) * RED_BLOCKS + b];
+    out[i] = acc;
+}
+
 /* V holds the eigenvectors as columns of a column-major matrix: V[mu + i*n] = C[mu][i].
  * Writes C row-major (C[mu*n + i]) and the occupied block C_occ[mu*nocc + i], i < nocc. */
 __global__ void __launch_bounds__(256)
@@ -189,6 +247,15 @@ bool solve_dense(std::vector<double> &A, std::vector<double> &b, int n)
 
 }  // namespace
 
+namespace {
+void mark_end(std::vector<cudaEvent_t> &v, cudaStream_t st)
+{
+    if (v.size() != 1) return;                        /* the opening mark was never recorded */
+    cudaEvent_t e = nullptr;
+    if (cudaEventCreate(&e) == cudaSuccess) { cudaEventRecord(e, st); v.push_back(e); }
+}
+}  // namespace
+
 #define SCF_TRY(expr)                                                                      \
     do {                                                                                   \
         cudaError_t e_ = (expr);                                                           \
@@ -211,7 +278,7 @@ int scf_run(dfjk_handle *h, int64_t nao, int nspin, const double *hcore, const d
 {
     Cusolver &cs = cusolver();
     if (!cs.ok()) {
-        snprintf(err, errlen, "dfjk_scf: libcusolver could not be loaded (%s)", dlerror() ? dlerror() : "symbols missing");
+        snprintf(err, errlen, "dfjk_scf: libcusolver could not be loaded (%s)", cs.why[0] ? cs.why : "unknown reason");
         return DFJK_ECUDA;
     }
     const int64_t n2 = nao * nao;
@@ -224,6 +291,7 @@ int scf_run(dfjk_handle *h, int64_t nao, int nspin, const double *hcore, const d
     int lwork = 0;
     std::vector<double> Bmat((size_t)m_max * m_max, 0.0);
     std::vector<int> slot_of;                        /* history, oldest first: ring slot ids */
+    std::vector<cudaEvent_t> ev_jk, ev_eig, ev_total; /* timing: pairs (begin, end) */
     double e_prev = 0.0;
     *n_iter = 0;
     *converged = 0;
@@ -231,7 +299,7 @@ int scf_run(dfjk_handle *h, int64_t nao, int nspin, const double *hcore, const d
     /* workspace (doubles): per spin F, D, E(rr), C, K, C_occ, W and the DIIS rings; shared T1, T2, Va
      * (eigenvector / A copy), Sb (B copy), J, partials, scalars */
     const int64_t per_spin = 5 * n2 + nao * nao + nao + 2 * (int64_t)m_max * n2;
-    const int64_t total = nspin * per_spin + 5 * n2 + RED_BLOCKS + 8;
+    const int64_t total = nspin * per_spin + 5 * n2 + 33 * RED_BLOCKS + 32;
     double *F[2], *D[2], *Er[2], *C[2], *K[2], *Cocc[2], *W[2], *Fring[2], *Ering[2];
     double *T1, *T2, *Va, *Sb, *J, *part, *scal;
     const unsigned eb = (unsigned)((n2 + 255) / 256);
@@ -251,7 +319,7 @@ int scf_run(dfjk_handle *h, int64_t nao, int nspin, const double *hcore, const d
             Fring[s] = q; q += (int64_t)m_max * n2; Ering[s] = q; q += (int64_t)m_max * n2;
         }
         T1 = q; q += n2; T2 = q; q += n2; Va = q; q += n2; Sb = q; q += n2; J = q; q += n2;
-        part = q; q += RED_BLOCKS; scal = q;
+        part = q; q += 33 * RED_BLOCKS; scal = q;          /* scal[0..3] E, max|e| per spin; scal[4..] DIIS dots */
     }
     if (cs.sygvd_bufsize(sol, CUSOLVER_EIG_TYPE_1, CUSOLVER_EIG_MODE_VECTOR, CUBLAS_FILL_MODE_LOWER,
                          (int)nao, Va, (int)nao, Sb, (int)nao, W[0], &lwork) != CUSOLVER_STATUS_SUCCESS) {
@@ -265,12 +333,19 @@ int scf_run(dfjk_handle *h, int64_t nao, int nspin, const double *hcore, const d
     /* generalised symmetric eigenproblem A C = S C eps; a symmetric row-major matrix is its own
      * column-major image, the eigenvectors come back as columns of the column-major Va */
     {
+        auto mark_eig = [&]() {
+            cudaEvent_t e = nullptr;
+            if (cudaEventCreate(&e) == cudaSuccess) { cudaEventRecord(e, st); ev_eig.push_back(e); }
+        };
         auto diagonalise = [&](const double *A, int s) -> int {
             if (cudaMemcpyAsync(Va, A, (size_t)n2 * 8, cudaMemcpyDeviceToDevice, st) != cudaSuccess) return 1;
             if (cudaMemcpyAsync(Sb, S, (size_t)n2 * 8, cudaMemcpyDeviceToDevice, st) != cudaSuccess) return 1;
-            if (cs.sygvd(sol, CUSOLVER_EIG_TYPE_1, CUSOLVER_EIG_MODE_VECTOR, CUBLAS_FILL_MODE_LOWER, (int)nao,
-                         Va, (int)nao, Sb, (int)nao, W[s], work, lwork, dev_info) != CUSOLVER_STATUS_SUCCESS)
-                return 2;
+            mark_eig();
+            const cusolverStatus_t es = cs.sygvd(sol, CUSOLVER_EIG_TYPE_1, CUSOLVER_EIG_MODE_VECTOR,
+                                                 CUBLAS_FILL_MODE_LOWER, (int)nao, Va, (int)nao, Sb, (int)nao,
+                                                 W[s], work, lwork, dev_info);
+            mark_eig();
+            if (es != CUSOLVER_STATUS_SUCCESS) return 2;
             unpack_vectors_kernel<<<tgrid, 256, 0, st>>>(Va, nao, nocc[s], C[s], Cocc[s]);
             int info = 0;
             if (cudaMemcpyAsync(&info, dev_info, sizeof(int), cudaMemcpyDeviceToHost, st) != cudaSuccess) return 1;
@@ -286,6 +361,33 @@ int scf_run(dfjk_handle *h, int64_t nao, int nspin, const double *hcore, const d
             return e != cudaSuccess ? e : cudaStreamSynchronize(st);
         };
 
+        /* T = A Bs for a SYMMETRIC Bs (A Bs = A Bs^T): both operands packed side by side into the X
+         * workspace, one full DMMA product over all tiles with k = nao, splits summed by K3's kernel */
+        const ScfWorkspace wsx = scf_workspace(h);
+        const int64_t w4 = (nao + 3) / 4 * 4;
+        const int nbt = (int)((nao + 127) / 128);
+        const int psplit = choose_splits(nbt * nbt, wsx.sm_count, wsx.nsplit_alloc < 8 ? wsx.nsplit_alloc : 8);
+        const dim3 pgrid((unsigned)((nao + 255) / 256), (unsigned)(w4 / 4));
+        auto product_sym = [&](const double *A, const double *Bs, double *T) -> cudaError_t {
+            pack_x4_kernel<<<pgrid, 256, 0, st>>>(A, nao, 0, wsx.X);
+            pack_x4_kernel<<<pgrid, 256, 0, st>>>(Bs, nao, w4, wsx.X);
+            const cudaError_t e = launch_k2_gemm_full(wsx.X, nao, 1, 2 * w4, 0, w4, nao, wsx.Kpart, psplit, 0, st);
+            if (e != cudaSuccess) return e;
+            launch_k3_sum(wsx.Kpart, psplit, nao, T, st);
+            return cudaSuccess;
+        };
+        if (wsx.x_doubles < 2 * w4 * nao) {
+            snprintf(err, errlen, "dfjk_scf: X workspace too small for the DIIS products");
+            rc = DFJK_ENOMEM;
+            goto done;
+        }
+        /* timing (dfjk_scf_timing): event pairs around every get_jk and every Dsygvd */
+        auto mark = [&](std::vector<cudaEvent_t> &v) {
+            cudaEvent_t e = nullptr;
+            if (cudaEventCreate(&e) == cudaSuccess) { cudaEventRecord(e, st); v.push_back(e); }
+        };
+        mark(ev_total);
+
         for (int s = 0; s < nspin; ++s) {                               /* 0. core guess, both spins */
             const int dr = diagonalise(hcore, s);
             if (dr != 0) {
@@ -295,9 +397,11 @@ int scf_run(dfjk_handle *h, int64_t nao, int nspin, const double *hcore, const d
             }
         }
         for (int64_t k = 0; k < max_iter; ++k) {
+            mark(ev_jk);
             rc = nspin == 1 ? dfjk_get_jk(h, Cocc[0], nocc[0], J, K[0], (void *)st)
                             : dfjk_get_jk_u(h, Cocc[0], nocc[0], Cocc[1], nocc[1], J, K[0], K[1], (void *)st);
             if (rc != DFJK_OK) { snprintf(err, errlen, "%s", dfjk_last_error()); goto done; }
+            mark(ev_jk);
             /* the new (F, e) pair goes into the ring slot of the entry it evicts (or a fresh one) */
             int slot;
             if ((int)slot_of.size() < m_max) slot = (int)slot_of.size();
@@ -306,13 +410,30 @@ int scf_run(dfjk_handle *h, int64_t nao, int nspin, const double *hcore, const d
                 fock_kernel<<<eb, 256, 0, st>>>(hcore, J, K[s], n2, F[s]);
                 launch_fp64_tile_gemm(Cocc[s], nocc[s], Cocc[s], 1, nocc[s], D[s], nao, nao, nao, nocc[s], dw, 0.0, 0, st);
                 reduce(1, D[s], hcore, F[s], 0.5, scal + s);            /* E_s = 1/2 sum D_s o (h + F_s) */
-                launch_fp64_tile_gemm(F[s], nao, D[s], nao, 1, T1, nao, nao, nao, nao, 1.0, 0.0, 0, st);   /* F D */
-                launch_fp64_tile_gemm(T1, nao, S, nao, 1, T2, nao, nao, nao, nao, 1.0, 0.0, 0, st);        /* F D S */
+                SCF_TRY(product_sym(F[s], D[s], T1));                   /* F D   (D symmetric) */
+                SCF_TRY(product_sym(T1, S, T2));                        /* F D S (S symmetric) */
                 antisym_kernel<<<eb, 256, 0, st>>>(T2, nao, Er[s]);     /* e_s = F D S - S D F */
                 reduce(2, Er[s], nullptr, nullptr, 1.0, scal + 2 + s);  /* max |e_s| */
             }
-            double hs[4] = {0.0, 0.0, 0.0, 0.0};
-            SCF_TRY(read_scalars(hs, 4));
+            /* the DIIS dots of this iteration against the history it WOULD have (oldest entry dropped
+             * when the ring is full, the new error last), all in one launch pair, so that E, max|e| and
+             * the dots come back in ONE host sync */
+            std::vector<int> hist(slot_of);
+            if ((int)hist.size() == m_max) hist.erase(hist.begin());
+            const int m = (int)hist.size() + 1;
+            {
+                DotArgs da;
+                da.npairs = m * nspin;
+                for (int i = 0; i < m; ++i)
+                    for (int s = 0; s < nspin; ++s) {
+                        da.a[i * nspin + s] = i + 1 < m ? Ering[s] + (int64_t)hist[i] * n2 : Er[s];
+                        da.b[i * nspin + s] = Er[s];
+                    }
+                dots_partial_kernel<<<dim3(RED_BLOCKS, (unsigned)da.npairs), RED_THREADS, 0, st>>>(da, n2, part);
+                dots_final_kernel<<<1, 32, 0, st>>>(part, m, nspin, scal + 4);
+            }
+            double hs[4 + 16] = {0.0};
+            SCF_TRY(read_scalars(hs, 4 + m));
             const double E = nspin == 1 ? hs[0] : hs[0] + hs[1];
             const double emax = nspin == 1 ? hs[2] : std::fmax(hs[2], hs[3]);
             e_hist[k] = E;
@@ -335,16 +456,7 @@ int scf_run(dfjk_handle *h, int64_t nao, int nspin, const double *hcore, const d
                 SCF_TRY(cudaMemcpyAsync(Ering[s] + (int64_t)slot * n2, Er[s], (size_t)n2 * 8, cudaMemcpyDeviceToDevice, st));
                 SCF_TRY(cudaMemcpyAsync(Fring[s] + (int64_t)slot * n2, F[s], (size_t)n2 * 8, cudaMemcpyDeviceToDevice, st));
             }
-            const int m = (int)slot_of.size();
-            /* B_im = sum_s <e_s^i, e_s^m>: one dot per launch pair, read back (m <= 16 per iteration) */
-            for (int i = 0; i < m; ++i) {
-                for (int s = 0; s < nspin; ++s)
-                    reduce(0, Ering[s] + (int64_t)slot_of[i] * n2, Er[s], nullptr, 1.0, scal + 4 + s);
-                double v[2] = {0.0, 0.0};
-                SCF_TRY(cudaMemcpyAsync(v, scal + 4, nspin * sizeof(double), cudaMemcpyDeviceToHost, st));
-                SCF_TRY(cudaStreamSynchronize(st));
-                Bmat[i * m_max + (m - 1)] = Bmat[(m - 1) * m_max + i] = nspin == 1 ? v[0] : v[0] + v[1];
-            }
+            for (int i = 0; i < m; ++i) Bmat[i * m_max + (m - 1)] = Bmat[(m - 1) * m_max + i] = hs[4 + i];
             std::vector<double> A((size_t)(m + 1) * (m + 1), 0.0), rhs(m + 1, 0.0);
             for (int i = 0; i < m; ++i) {
                 for (int j = 0; j < m; ++j) A[i * (m + 1) + j] = Bmat[i * m_max + j];
@@ -380,6 +492,24 @@ int scf_run(dfjk_handle *h, int64_t nao, int nspin, const double *hcore, const d
         SCF_TRY(cudaGetLastError());
     }
 done:
+    {
+        /* where the time went: sums over the (begin, end) event pairs; the run has synchronised */
+        mark_end(ev_total, st);
+        cudaStreamSynchronize(st);
+        auto total = [](std::vector<cudaEvent_t> &v) {
+            double t = 0.0;
+            for (size_t i = 0; i + 1 < v.size(); i += 2) {
+                float ms = 0.f;
+                if (cudaEventElapsedTime(&ms, v[i], v[i + 1]) == cudaSuccess) t += ms;
+            }
+            for (cudaEvent_t e : v) cudaEventDestroy(e);
+            v.clear();
+            return t;
+        };
+        const double t_jk = total(ev_jk), t_eig = total(ev_eig), t_all = total(ev_total);
+        cudaGetLastError();
+        if (rc == DFJK_OK) scf_store_timing(h, *n_iter, t_jk, t_eig, t_all);
+    }
     if (sol) cs.destroy(sol);
     cudaFree(ws);
     cudaFree(work);

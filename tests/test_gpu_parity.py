@@ -59,7 +59,7 @@ def test_baseline_configs_all_calls(dfjk, cfg_id):
     Bp = gi.fill_B_host(cfg)
     Bd = dev(Bp)
     h = dfjk.DFJK(Bd, cfg.nao)
-    for call in range(min(cfg.calls, 3)):
+    for call in range(cfg.calls):                 # every call of the schedule (cfg 2: 10 fresh C_occ)
         C = gi.orbitals(cfg, call)[0]
         J, K = h.get_jk(dev(C))
         d = h.get_d()
@@ -299,4 +299,101 @@ def test_cuda_graph_capture_and_replay(dfjk):
         Jo, Ko, _ = oracle.get_jk(Bp, cfg.nao, [C], [2.0])
         assert relerr(J.cpu().numpy(), Jo) <= TOL and relerr(K.cpu().numpy(), Ko[0]) <= TOL
     del g
+    h.close()
+
+
+def test_internal_graph_replay_matches_plain_launches(dfjk):
+    """The handle's own CUDA graph ("graph" option, default on): the first call of a shape launches
+    kernel by kernel, the second captures, later ones replay.  Every call gets FRESH orbital and
+    output tensors (the replay must not remember pointers), interleaved with other shapes, and must
+    equal the graph-free handle bit for bit and the oracle to tolerance."""
+    nao, naux = 150, 19
+    Bp, _ = rand_case(nao, naux, (7,), seed=31)
+    Bd = dev(Bp)
+    h, hp = dfjk.DFJK(Bd, nao), dfjk.DFJK(Bd, nao)
+    hp.set_option("graph", 0)
+    n0 = h.launch_count
+    for it in range(6):
+        nocc = 7 if it != 3 else 11                     # another shape in between (its own slot)
+        C = gi.random_orbitals(nao, nocc, 400 + it)
+        J, K = h.get_jk(dev(C))
+        Jp, Kp = hp.get_jk(dev(C))
+        d, dp = h.get_d(), hp.get_d()
+        Jonly = h.get_jk(dev(C), with_k=False)[0]       # a third shape (J only)
+        torch.cuda.synchronize()
+        assert torch.equal(J, Jp) and torch.equal(K, Kp) and torch.equal(d, dp), it
+        Jo, Ko, do = oracle.get_jk(Bp, nao, [C], [2.0])
+        assert relerr(J.cpu().numpy(), Jo) <= TOL and relerr(K.cpu().numpy(), Ko[0]) <= TOL
+        assert relerr(Jonly.cpu().numpy(), Jo) <= TOL and relerr(d.cpu().numpy(), do) <= TOL
+    # the launch counter counts replayed kernels too: J+K calls cost the same on both handles, the
+    # extra J-only calls on h add to it
+    assert h.launch_count - n0 > hp.launch_count
+    # unrestricted replay
+    Ca, Cb = gi.random_orbitals(nao, 9, 1), gi.random_orbitals(nao, 5, 2)
+    for it in range(3):
+        J, Ka, Kb = h.get_jk_u(dev(Ca), dev(Cb))
+        Jp, Kap, Kbp = hp.get_jk_u(dev(Ca), dev(Cb))
+        torch.cuda.synchronize()
+        assert torch.equal(J, Jp) and torch.equal(Ka, Kap) and torch.equal(Kb, Kbp)
+    Jo, Kao, Kbo = oracle.get_jk_unrestricted(Bp, nao, Ca, Cb)
+    assert relerr(J.cpu().numpy(), Jo) <= TOL and relerr(Ka.cpu().numpy(), Kao) <= TOL
+    assert relerr(Kb.cpu().numpy(), Kbo) <= TOL
+    h.close(); hp.close()
+
+
+def test_two_handles_from_two_host_threads(dfjk):
+    """Two host threads, each with its own handle and stream, first use of every kernel racing on
+    the shared-memory opt-in (k_common.cuh ensure_dynamic_smem) and on the thread-local error text."""
+    import threading
+    shapes = [(131, 14, 9, 77), (197, 11, 141, 78)]       # different NT8 instantiations of K1
+    cases = [rand_case(nao, naux, (nocc,), seed=seed) for nao, naux, nocc, seed in shapes]
+    results, errors = [None, None], []
+    start = threading.Barrier(2)
+
+    def work(i):
+        try:
+            nao = shapes[i][0]
+            Bp, (C,) = cases[i]
+            torch.cuda.set_device(0)
+            s = torch.cuda.Stream()
+            with torch.cuda.stream(s):
+                h = dfjk.DFJK(dev(Bp), nao)
+                start.wait(timeout=60)
+                outs = []
+                for _ in range(4):
+                    J, K = h.get_jk(dev(C))
+                    outs.append((J, K))
+                s.synchronize()
+                results[i] = [(J.cpu().numpy(), K.cpu().numpy()) for J, K in outs]
+                h.close()
+        except Exception as e:          # noqa: BLE001
+            errors.append((i, repr(e)))
+
+    ts = [threading.Thread(target=work, args=(i,)) for i in range(2)]
+    for t in ts:
+        t.start()
+    for t in ts:
+        t.join(300)
+    assert not errors, errors
+    for i, (nao, naux, nocc, seed) in enumerate(shapes):
+        Bp, (C,) = cases[i]
+        Jo, Ko, _ = oracle.get_jk(Bp, nao, [C], [2.0])
+        for J, K in results[i]:
+            assert relerr(J, Jo) <= TOL and relerr(K, Ko[0]) <= TOL
+
+
+def test_kernel_timing_ring_grows(dfjk):
+    """More than the initial 1024 event pairs: the ring grows instead of silently dropping launches."""
+    nao = 40
+    Bp, (C,) = rand_case(nao, 6, (3,), seed=9)
+    h = dfjk.DFJK(dev(Bp), nao)
+    h.set_option("k_chunk", 1)                            # 6 chunks -> ~25 launches per call
+    h.set_option("time_kernels", 1)
+    Cd = dev(C)
+    n0 = h.launch_count
+    for _ in range(60):
+        h.get_jk(Cd)
+    torch.cuda.synchronize()
+    total = sum(h.kernel_time(k)[1] for k in dfjk.KERNELS)
+    assert total == h.launch_count - n0 and total > 1024
     h.close()
