@@ -56,17 +56,27 @@ constexpr int K1_LDT = 132;                       /* 128 + shift + pad, 16-B mul
 constexpr int K1_A_BYTES = K1_M * K1_LDD * 8;     /* 36864 >= 32 * K1_LDT * 8 = 33792 */
 constexpr int K1_SMEM_BUDGET = 220 * 1024;
 /* Every off-diagonal packed element is staged twice: in "row" form by the item of its row block and
- * in "col" form by the item of its column block (the lower-numbered one).  The items of one P run
- * at the same time on neighbouring CTAs and walk nu at the same pace, so the row-form read (stage
- * nu/32) comes first and the col-form read (stage mu/32 > nu/32) second: the first is marked
- * L2 evict_last, the second evict_first, and the items of a P are numbered from the LAST row block
- * down so that the row-form reader never starts later than the col-form reader.  The second read
- * then hits L2 instead of HBM (ncu r01e: K1 read 1.44 x |B| from DRAM without this). */
+ * in "col" form by the item of its column block.  The nib items of one P run at the same time on
+ * neighbouring CTAs, so the two reads can be made to COINCIDE: item i does not walk nu from 0 up but
+ * visits the 128-wide column blocks j in the round-robin tournament order j = (s - i) mod nib,
+ * s = 0 .. nib-1.  At step s the pair (i, j) with i + j == s (mod nib) work on each other's block:
+ * i stages B_P[block i, block j] while j stages B_P[block j, block i] -- the same packed elements, at
+ * the same time.  Whichever read arrives second is an L2 hit (or joins the first one's miss), so B
+ * comes from HBM once per build instead of 1.44 times (ncu r01e; 1.33 with eviction hints only).
+ * DFJK_K1_L2_HINTS (off) marks row-form reads evict_last and col-form reads evict_first, which is
+ * what helped the sequential walk (DFJK_K1_PAIRED=0, items of a P numbered from the last block down
+ * so the row-form reader never starts late). */
+#ifndef DFJK_K1_PAIRED
+#define DFJK_K1_PAIRED 1
+#endif
 #ifndef DFJK_K1_L2_HINTS
-#define DFJK_K1_L2_HINTS 1
+#define DFJK_K1_L2_HINTS 0
 #endif
 #ifndef DFJK_K1_DESCENDING
-#define DFJK_K1_DESCENDING 1
+#define DFJK_K1_DESCENDING 0
+#endif
+#ifndef DFJK_K1_X_EVICT_FIRST
+#define DFJK_K1_X_EVICT_FIRST 0
 #endif
 
 /* row block of the r-th item of a P (r = item index within the P divided by the N tiles) */
@@ -137,7 +147,13 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
         /* ------------------------------------------------------------ producers */
         reg_dealloc<40>();
 #if DFJK_K1_L2_HINTS
+#if DFJK_K1_L2_HINTS == 2
+        const uint64_t pol_first = l2_policy_evict_last(), pol_second = l2_policy_evict_last();
+#elif DFJK_K1_L2_HINTS == 3
+        const uint64_t pol_first = l2_policy_evict_first(), pol_second = l2_policy_evict_first();
+#else
         const uint64_t pol_first = l2_policy_evict_last(), pol_second = l2_policy_evict_first();
+#endif
 #endif
         int slot = 0;
         uint32_t phase = 1;                                /* parity of the "empty" phase to wait for */
@@ -156,7 +172,12 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
         const uint32_t c_bytes = K1_KG * (uint32_t)ncols * 32u;
         int64_t rows_valid = nao - mu0;
         if (rows_valid > K1_M) rows_valid = K1_M;
-        for (int kc = 0; kc < nk; ++kc) {
+        const int rbi = (int)(mu0 / K1_M);
+        for (int sstep = 0; sstep < nib; ++sstep) {
+        /* column block of this step: the tournament partner (paired) or simply the next one */
+        const int jb = DFJK_K1_PAIRED ? (sstep >= rbi ? sstep - rbi : sstep - rbi + nib) : sstep;
+        const int kc_end = (jb + 1) * (K1_M / K1_KC) < nk ? (jb + 1) * (K1_M / K1_KC) : nk;
+        for (int kc = jb * (K1_M / K1_KC); kc < kc_end; ++kc) {
             if (ring_full) mbar_wait(empty_bar(slot), phase);
             const int64_t nu0 = (int64_t)kc * K1_KC;
             const uint32_t a_dst = smem_base + slot * Cfg::STAGE_BYTES;
@@ -221,6 +242,7 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
             }
             if (++slot == Cfg::STAGES) { slot = 0; phase ^= 1; ring_full = true; }
         }
+        }   /* column blocks */
         }   /* items */
     } else {
         /* ------------------------------------------------------------ consumers */
@@ -250,7 +272,11 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
 #pragma unroll
             for (int nt = 0; nt < NT8; ++nt) acc[mt][nt][0] = acc[mt][nt][1] = 0.0;
 
-        for (int kc = 0; kc < nk; ++kc) {
+        const int rbi = (int)(mu0 / K1_M);
+        for (int sstep = 0; sstep < nib; ++sstep) {
+        const int jb = DFJK_K1_PAIRED ? (sstep >= rbi ? sstep - rbi : sstep - rbi + nib) : sstep;
+        const int kc_end = (jb + 1) * (K1_M / K1_KC) < nk ? (jb + 1) * (K1_M / K1_KC) : nk;
+        for (int kc = jb * (K1_M / K1_KC); kc < kc_end; ++kc) {
             mbar_wait(full_bar(slot), phase);
             if (warp_active) {
                 const double *As = reinterpret_cast<const double *>(smem_raw + slot * Cfg::STAGE_BYTES);
@@ -287,8 +313,12 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
             if (lane == 0) mbar_arrive(empty_bar(slot));
             if (++slot == Cfg::STAGES) { slot = 0; phase ^= 1; }
         }
+        }   /* column blocks */
 
         if (warp_active) {
+#if DFJK_K1_X_EVICT_FIRST
+            const uint64_t pol_x = l2_policy_evict_first();
+#endif
 #pragma unroll
             for (int mt = 0; mt < 2; ++mt) {
                 const int64_t mu = mu0 + row_w + 8 * mt + lq;
@@ -299,7 +329,12 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
                     if (col < ldc) {
                         const int64_t k = p * ldx + col;       /* ldx >= ldc: X row pitch */
                         double *dst = X4 + ((k >> 2) * nao + mu) * 4 + (k & 3);
+#if DFJK_K1_X_EVICT_FIRST
+                        asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1, %2}, %3;"
+                                     ::"l"(dst), "d"(acc[mt][nt][0]), "d"(acc[mt][nt][1]), "l"(pol_x) : "memory");
+#else
                         *reinterpret_cast<double2 *>(dst) = make_double2(acc[mt][nt][0], acc[mt][nt][1]);
+#endif
                     }
                 }
             }
