@@ -244,7 +244,8 @@ int dfjk_get_d(dfjk_handle *h, double *d_out, void *stream);
  * return DFJK_EINVAL.  Known names:
  *   "k_chunk"   number of auxiliary rows whose half-transformed X stays in the
  *               L2-sized workspace between the K1 and K2 kernels (0 = automatic)
- *   "k_splits"  number of partial-K accumulators the SYRK is split over (0 = automatic)
+ *   "k_splits"  number of partial-K accumulators the SYRK is split over / the largest number of
+ *               slabs the panel-synchronous kernel may use (0 = automatic)
  *   "time_kernels"  1 = bracket every kernel launch with CUDA events on the call's stream
  *               (read back with dfjk_kernel_time); setting it (to 0 or 1) clears the record
  *   "j_fused"   1 (default) = in a call that builds J and K together, the fitting coefficients
@@ -253,6 +254,12 @@ int dfjk_get_d(dfjk_handle *h, double *d_out, void *stream);
  *               instead of twice; 0 = always the two plain streaming passes over B (dot, then
  *               axpy).  Applies to dfjk_get_jk, dfjk_get_jk_u and dfjk_get_jk_pair (there
  *               <B_P, C1 C2^T> = <B_P C1, C2>); J-only calls and raw-dm calls always use two passes.
+ *   "k2_panel"  which K2 kernel forms K += X X^T: 0 = one CTA per (tile, contiguous k range) with a
+ *               partial K per range; 1 = panel-synchronous (the k range is cut into short panels,
+ *               items (panel, tile) are dealt dynamically to persistent CTAs and added in panel
+ *               order into L2-resident slabs, so that X is read from HBM once instead of ~8 times);
+ *               2 (default) = 1 when the X chunk is larger than L2, else 0.
+ *   "k2_panel_kb"  target size in KB of one k panel of X for "k2_panel" (default 32768)
  *   "graph"     1 (default) = dfjk_get_jk / dfjk_get_jk_u replay a CUDA graph of their own launch
  *               sequence: the first call of a shape (orbital counts, requested outputs, options)
  *               launches kernel by kernel, the second captures the sequence after the orbital

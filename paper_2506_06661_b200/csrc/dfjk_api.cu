@@ -96,7 +96,8 @@ struct dfjk_handle {
     int nsplit_alloc, nsplit_default;
     int64_t ws_bytes;
     /* options */
-    int64_t opt_k_chunk, opt_k_splits, opt_j_fused;
+    int64_t opt_k_chunk, opt_k_splits, opt_j_fused, opt_k2_panel, opt_k2_panel_kb;
+    int *k2work;         /* 1 + nsplit_alloc * nb^2 ints: item counter and per-(slab, tile) counters of K2P */
     bool have_d;
     /* instrumentation: launch counter and optional per-kernel CUDA-event timing */
     int64_t launches;
@@ -125,7 +126,7 @@ namespace {
 void free_all(dfjk_handle *h)
 {
     cudaFree(h->Ccat); cudaFree(h->Dt); cudaFree(h->d_part); cudaFree(h->d);
-    cudaFree(h->Jp_part); cudaFree(h->X); cudaFree(h->Kpart);
+    cudaFree(h->Jp_part); cudaFree(h->X); cudaFree(h->Kpart); cudaFree(h->k2work);
     cudaFree(h->hostC); cudaFree(h->hostJ); cudaFree(h->hostK); cudaFree(h->hostC2); cudaFree(h->hostK2);
     if (h->host_stream) cudaStreamDestroy(h->host_stream);
     for (auto &g : h->graphs) if (g.exec) cudaGraphExecDestroy(g.exec);
@@ -216,6 +217,8 @@ extern "C" dfjk_handle *dfjk_create(int64_t naux, int64_t nao, const double *B_p
     h->naux = naux; h->nao = nao; h->npair = nao * (nao + 1) / 2; h->B = B_packed; h->device = dev;
     h->opt_j_fused = 1;
     h->opt_graph = 1;
+    h->opt_k2_panel = 2;             /* automatic */
+    h->opt_k2_panel_kb = 32768;
     int v = 0;
     cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev); h->sm_count = v > 0 ? v : 148;
     cudaDeviceGetAttribute(&v, cudaDevAttrL2CacheSize, dev); h->l2_bytes = v;
@@ -249,6 +252,10 @@ extern "C" dfjk_handle *dfjk_create(int64_t naux, int64_t nao, const double *B_p
     if (rc == DFJK_OK) rc = alloc_ws(h, &h->Jp_part, h->j2_groups * h->npair);
     if (rc == DFJK_OK) rc = alloc_ws(h, &h->X, h->x_doubles);
     if (rc == DFJK_OK) rc = alloc_ws(h, &h->Kpart, 2LL * h->nsplit_alloc * nao * nao);
+    if (rc == DFJK_OK && cudaMalloc((void **)&h->k2work, sizeof(int) * (size_t)(1 + h->nsplit_alloc * nb * nb)) != cudaSuccess) {
+        h->k2work = nullptr;
+        rc = fail(DFJK_ENOMEM, "dfjk_create: cudaMalloc of the K2 work counters failed");
+    }
     if (rc == DFJK_OK && cudaMalloc((void **)&h->out_slots, DFJK_OUT_SLOTS * sizeof(double *)) != cudaSuccess) {
         h->out_slots = nullptr;
         rc = fail(DFJK_ENOMEM, "dfjk_create: cudaMalloc of the output-pointer slots failed");
@@ -283,6 +290,14 @@ extern "C" int dfjk_set_option(dfjk_handle *h, const char *name, int64_t value)
     }
     if (!strcmp(name, "j_fused")) { h->opt_j_fused = value != 0; return DFJK_OK; }
     if (!strcmp(name, "graph")) { h->opt_graph = value != 0; return DFJK_OK; }
+    if (!strcmp(name, "k2_panel")) {
+        if (value > 2) return fail(DFJK_EINVAL, "k2_panel must be 0, 1 or 2");
+        h->opt_k2_panel = value; return DFJK_OK;
+    }
+    if (!strcmp(name, "k2_panel_kb")) {
+        if (value < 64) return fail(DFJK_EINVAL, "k2_panel_kb must be >= 64");
+        h->opt_k2_panel_kb = value; return DFJK_OK;
+    }
     return fail(DFJK_EINVAL, "dfjk_set_option: unknown option '%s'", name);
 }
 
@@ -316,7 +331,21 @@ int enqueue_jk_body(dfjk_handle *h, int nset, const int *nocc, const int *col0, 
         if (h->opt_k_chunk > 0 && h->opt_k_chunk < pc) pc = h->opt_k_chunk;
         if (pc > naux) pc = naux;
         if (pc < 1) return fail(DFJK_ENOMEM, "%s: X workspace too small", who);
-        const int nsplit = h->opt_k_splits > 0 ? (int)h->opt_k_splits : h->nsplit_default;
+        /* K2P pays a read-modify-write per item to keep the k window of X inside L2; an X chunk that
+         * fits in L2 whole has nothing to gain from it (and small problems are all overhead) */
+        const bool panel = h->opt_k2_panel == 1 || (h->opt_k2_panel == 2 && pc * nao * ldc * 8 > h->l2_bytes);
+        const int nbk = (int)((nao + 127) / 128);
+        /* K2P: panel length and slab count per set, planned from the first (largest) chunk; the old
+         * split kernel: one partial per k-split */
+        int nsplit[2] = {0, 0}, pstages[2] = {0, 0};
+        for (int s = 0; s < nset; ++s) {
+            if (panel)
+                dfjk::k2p_plan(nao, pc * ((nocc[s] + 3) / 4), nbk * (nbk + 1) / 2, h->sm_count,
+                               h->opt_k_splits > 0 ? (int)h->opt_k_splits : h->nsplit_alloc,
+                               h->opt_k2_panel_kb << 10, &pstages[s], &nsplit[s]);
+            else
+                nsplit[s] = h->opt_k_splits > 0 ? (int)h->opt_k_splits : h->nsplit_default;
+        }
         int chunk = 0;
         for (int64_t P0 = 0; P0 < naux; P0 += pc, ++chunk) {
             const int64_t np = (P0 + pc <= naux) ? pc : naux - P0;
@@ -328,15 +357,19 @@ int enqueue_jk_body(dfjk_handle *h, int nset, const int *nocc, const int *col0, 
             for (int s = 0; s < nset; ++s)
                 if (want_k[s]) {
                     Timed t_(h, DFJK_KERNEL_K2, st);
-                    DFJK_LAUNCH_TRY(dfjk::launch_k2_syrk_lower(h->X, nao, np, ldc, col0[s], nocc[s],
-                                                               h->Kpart + (int64_t)s * h->nsplit_alloc * nao * nao,
-                                                               nsplit, chunk > 0, st));
+                    double *Kp = h->Kpart + (int64_t)s * h->nsplit_alloc * nao * nao;
+                    if (panel)
+                        DFJK_LAUNCH_TRY(dfjk::launch_k2p_syrk_lower(h->X, nao, np, ldc, col0[s], nocc[s], Kp, pstages[s],
+                                                                    nsplit[s], chunk > 0, h->k2work, h->sm_count, st));
+                    else
+                        DFJK_LAUNCH_TRY(dfjk::launch_k2_syrk_lower(h->X, nao, np, ldc, col0[s], nocc[s], Kp,
+                                                                   nsplit[s], chunk > 0, st));
                 }
         }
         for (int s = 0; s < nset; ++s)
             if (want_k[s]) {
                 Timed t_(h, DFJK_KERNEL_K3, st);
-                dfjk::launch_k3_finish(h->Kpart + (int64_t)s * h->nsplit_alloc * nao * nao, nsplit,
+                dfjk::launch_k3_finish(h->Kpart + (int64_t)s * h->nsplit_alloc * nao * nao, nsplit[s],
                                        nao, K[s], slots ? slots + 1 + s : nullptr, st);
             }
     }
@@ -356,9 +389,10 @@ int enqueue_jk_body(dfjk_handle *h, int nset, const int *nocc, const int *col0, 
 struct GraphKey {
     int nset, nocc[2];
     bool want_j, want_k[2];
-    int64_t k_chunk, k_splits, j_fused;
+    int64_t k_chunk, k_splits, j_fused, k2_panel, k2_panel_kb;
     bool operator==(const GraphKey &o) const
     {
+        if (k2_panel != o.k2_panel || k2_panel_kb != o.k2_panel_kb) return false;
         return nset == o.nset && nocc[0] == o.nocc[0] && nocc[1] == o.nocc[1] && want_j == o.want_j &&
                want_k[0] == o.want_k[0] && want_k[1] == o.want_k[1] && k_chunk == o.k_chunk &&
                k_splits == o.k_splits && j_fused == o.j_fused;
@@ -394,6 +428,7 @@ int get_jk_impl(dfjk_handle *h, int nset, const double *const *C, const int64_t 
     GraphKey key = {};
     key.nset = nset; key.want_j = J != nullptr;
     key.k_chunk = h->opt_k_chunk; key.k_splits = h->opt_k_splits; key.j_fused = h->opt_j_fused;
+    key.k2_panel = h->opt_k2_panel; key.k2_panel_kb = h->opt_k2_panel_kb;
     bool want_k[2] = {false, false};
     for (int s = 0; s < nset; ++s) { key.nocc[s] = nocc[s]; key.want_k[s] = want_k[s] = K[s] != nullptr; }
 
@@ -501,8 +536,14 @@ int get_jk_general_impl(dfjk_handle *h, const double *C1, const double *C2, int6
         if (pc > 65535) pc = 65535;                /* K1U's grid.z */
         if (pc < 1) return fail(DFJK_ENOMEM, "%s: X workspace too small", who);
         const int nb = (int)((nao + 127) / 128);
-        const int nsplit = h->opt_k_splits > 0 ? (int)h->opt_k_splits
-                                               : choose_splits(nb * nb, h->sm_count, h->nsplit_alloc);
+        const bool panel = h->opt_k2_panel == 1 || (h->opt_k2_panel == 2 && pc * nao * ldx * 8 > h->l2_bytes);
+        int nsplit = h->opt_k_splits > 0 ? (int)h->opt_k_splits
+                                         : choose_splits(nb * nb, h->sm_count, h->nsplit_alloc);
+        int pstages = 0;
+        if (panel)
+            dfjk::k2p_plan(nao, pc * ((ncol + 3) / 4), nb * nb, h->sm_count,
+                           h->opt_k_splits > 0 ? (int)h->opt_k_splits : h->nsplit_alloc,
+                           h->opt_k2_panel_kb << 10, &pstages, &nsplit);
         int chunk = 0;
         for (int64_t P0 = 0; P0 < naux; P0 += pc, ++chunk) {
             const int64_t np = (P0 + pc <= naux) ? pc : naux - P0;
@@ -514,7 +555,11 @@ int get_jk_general_impl(dfjk_handle *h, const double *C1, const double *C2, int6
                 dfjk::launch_j1x_dot(h->X, h->Ccat, nao, np, ldx, ldc, w8, 1, col0, nocc, &one, P0, naux, h->d_part, st);
             }
             { Timed t_(h, DFJK_KERNEL_K2, st);
-              DFJK_LAUNCH_TRY(dfjk::launch_k2_gemm_full(h->X, nao, np, ldx, col0[0], col0[1], ncol, h->Kpart, nsplit, chunk > 0, st)); }
+              if (panel)
+                  DFJK_LAUNCH_TRY(dfjk::launch_k2p_gemm_full(h->X, nao, np, ldx, col0[0], col0[1], ncol, h->Kpart, pstages,
+                                                             nsplit, chunk > 0, h->k2work, h->sm_count, st));
+              else
+                  DFJK_LAUNCH_TRY(dfjk::launch_k2_gemm_full(h->X, nao, np, ldx, col0[0], col0[1], ncol, h->Kpart, nsplit, chunk > 0, st)); }
         }
         { Timed t_(h, DFJK_KERNEL_K3, st); dfjk::launch_k3_sum(h->Kpart, nsplit, nao, K, st); }
         if (fused) {

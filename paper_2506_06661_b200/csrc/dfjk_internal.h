@@ -93,6 +93,22 @@ cudaError_t launch_k2_gemm_full(const double *X4, int64_t nao, int64_t np, int64
                                 int64_t col0b, int64_t ncol, double *Kpart, int nsplit, int accumulate,
                                 cudaStream_t st);
 
+/* K2P: the same two products, panel-synchronous (k2_syrk.cu, k2p_kernel): the k range of the chunk is
+ * cut into npanel panels, items (panel, tile) are dealt dynamically to one persistent CTA per SM and
+ * added into slab (panel % nslab) of Kpart in panel order.  k2p_plan picks npanel / nslab from the
+ * shape of the build's FIRST chunk (ng = np * ceil(ncol / 4) k-groups, ntile tiles, panel_bytes of X
+ * per panel) as a panel length in stages of k = 32; every chunk is then cut at that length.  `work` is a
+ * device array of 1 + nslab * ntile ints (zeroed by the launcher).  The slab count must be the same
+ * for every chunk of a build (accumulate != 0 continues the slabs of the previous chunk). */
+void k2p_plan(int64_t nao, int64_t ng, int ntile, int sm_count, int max_slabs, int64_t panel_bytes,
+              int *panel_stages, int *nslab);
+cudaError_t launch_k2p_syrk_lower(const double *X4, int64_t nao, int64_t np, int64_t ldc, int64_t col0,
+                                  int64_t ncol, double *Kpart, int panel_stages, int nslab, int accumulate,
+                                  int *work, int sm_count, cudaStream_t st);
+cudaError_t launch_k2p_gemm_full(const double *X4, int64_t nao, int64_t np, int64_t ldc, int64_t col0a,
+                                 int64_t col0b, int64_t ncol, double *Kpart, int panel_stages, int nslab,
+                                 int accumulate, int *work, int sm_count, cudaStream_t st);
+
 /* K3 general: K[mu][nu] = sum_split Kpart[split][mu][nu] for every (mu, nu). */
 void launch_k3_sum(const double *Kpart, int nsplit, int64_t nao, double *K, cudaStream_t st);
 

@@ -331,6 +331,361 @@ k2_syrk_lower_kernel(const double *__restrict__ X4, int64_t nao, int64_t np, int
     }
 }
 
+/* ------------------------------------------------------------------ K2P: panel-synchronous K2 */
+/* The same product with the k range cut into short PANELS and the work dealt out dynamically:
+ * item = (panel p, tile t), tile fastest, claimed in order from a global counter by persistent
+ * CTAs (one per SM).  The CTAs working at any moment therefore sit on one or two neighbouring
+ * panels -- a k window of X a few MB wide that stays in L2 while every tile of the block row /
+ * column that needs it comes by (k2_syrk_lower_kernel hands each CTA a long contiguous k range:
+ * co-resident CTAs read 13 different ranges and X comes from HBM 8.3 times, ncu r01e).  The price
+ * is that a tile's accumulator no longer lives in one CTA's registers for the whole range: item
+ * (p, t) adds its 128 x 128 partial into slab p % S of Kpart, after item (p - S, t) has (a per
+ * (slab, tile) counter in global memory, release/acquire; items are claimed in order and never
+ * wait on later ones, so the wait cannot deadlock and in practice never spins).  The slabs are
+ * L2-resident (S x nao^2 doubles) and summed in the fixed order K3 uses => deterministic.
+ * The producer lane runs ahead through item boundaries (the stage ring never drains), warp
+ * layouts per tile are those of k2_syrk_lower_kernel. */
+struct K2PArgs {
+    const double *X4;
+    int64_t nao, np, ldc4, col04, col04b;
+    int n4s;
+    double *Kpart;            /* S slabs of nao x nao */
+    int nslab, accumulate, npanel, ntile, nb;
+    int *work;                /* [0]: item counter; [1 + slab * ntile + tile]: items completed */
+};
+
+constexpr int K2P_THREADS = 128 + 32 * K2_CONSUMER_WARPS;     /* producer warpgroup + 8 consumer warps */
+constexpr int K2P_SMEM_BYTES = K2_STAGES * K2_STAGE_BYTES + 2 * K2_STAGES * 8 + 4 * 8 + 2 * 8 + 16;
+
+__device__ __forceinline__ int ld_acquire_gpu(const int *p)
+{
+    int v;
+    asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_release_gpu(int *p, int v)
+{
+    asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+
+template <bool FULL>
+__device__ __forceinline__ void k2p_decode(int t, int nb, int &bi, int &bj)
+{
+    if (FULL) {
+        bi = t / nb;
+        bj = t - bi * nb;
+    } else {
+        bi = (int)((sqrtf(8.0f * (float)t + 1.0f) - 1.0f) * 0.5f);
+        while (bi * (bi + 1) / 2 > t) --bi;
+        while ((bi + 1) * (bi + 2) / 2 <= t) ++bi;
+        bj = t - bi * (bi + 1) / 2;
+    }
+}
+
+/* row[8 nt + {0,1}] (+)= acc[nt][{0,1}], nt < NNT, columns nu_first + 8 nt + {0,1} < nao: all loads
+ * of the row are issued before the first store */
+template <int NNT>
+__device__ __forceinline__ void k2p_add_row(const double (*acc)[2], double *row, int64_t nu_first,
+                                            int64_t nao, bool overwrite, bool vec)
+{
+    double v0[NNT], v1[NNT];
+#pragma unroll
+    for (int nt = 0; nt < NNT; ++nt) v0[nt] = v1[nt] = 0.0;
+    if (!overwrite) {
+        if (vec) {
+#pragma unroll
+            for (int nt = 0; nt < NNT; ++nt)
+                if (nu_first + 8 * nt < nao) {
+                    const double2 t = __ldcg(reinterpret_cast<const double2 *>(row + 8 * nt));
+                    v0[nt] = t.x; v1[nt] = t.y;
+                }
+        } else {
+#pragma unroll
+            for (int nt = 0; nt < NNT; ++nt) {
+                if (nu_first + 8 * nt < nao) v0[nt] = __ldcg(row + 8 * nt);
+                if (nu_first + 8 * nt + 1 < nao) v1[nt] = __ldcg(row + 8 * nt + 1);
+            }
+        }
+    }
+#pragma unroll
+    for (int nt = 0; nt < NNT; ++nt) {
+        const double r0 = v0[nt] + acc[nt][0], r1 = v1[nt] + acc[nt][1];
+        if (vec) {
+            if (nu_first + 8 * nt < nao)                  /* nao and nu even: the pair is inside */
+                *reinterpret_cast<double2 *>(row + 8 * nt) = make_double2(r0, r1);
+        } else {
+            if (nu_first + 8 * nt < nao) row[8 * nt] = r0;
+            if (nu_first + 8 * nt + 1 < nao) row[8 * nt + 1] = r1;
+        }
+    }
+}
+
+template <bool FULL>
+__global__ void __launch_bounds__(K2P_THREADS, 1)
+k2p_kernel(const K2PArgs a)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int64_t nao = a.nao;
+    const int64_t ng = a.np * a.n4s;                      /* k groups (4 columns each) of the set */
+    const int nitems = a.npanel * a.ntile;
+
+    const uint32_t smem_base = smem_u32(smem_raw);
+    const uint32_t bar_base = smem_base + K2_STAGES * K2_STAGE_BYTES;
+    auto full_bar = [&](int s) { return bar_base + 8u * s; };
+    auto empty_bar = [&](int s) { return bar_base + 8u * (K2_STAGES + s); };
+    auto item_full = [&](int s) { return bar_base + 8u * (2 * K2_STAGES + s); };
+    auto item_empty = [&](int s) { return bar_base + 8u * (2 * K2_STAGES + 2 + s); };
+    volatile int *item_id = reinterpret_cast<volatile int *>(smem_raw + K2_STAGES * K2_STAGE_BYTES + 8 * (2 * K2_STAGES + 4));
+    if (tid == 0) {
+        for (int s = 0; s < K2_STAGES; ++s) {
+            mbar_init(full_bar(s), 1);
+            mbar_init(empty_bar(s), K2_CONSUMER_WARPS);
+        }
+        for (int s = 0; s < 2; ++s) {
+            mbar_init(item_full(s), 1);
+            mbar_init(item_empty(s), K2_CONSUMER_WARPS);
+        }
+        mbar_fence_init();
+    }
+    __syncthreads();
+
+    if (warp < 4) {
+        /* ------------------------------------------------------------ producer (one lane of the
+         * first warpgroup, which gives its registers to the consumers) */
+        reg_dealloc<40>();
+        if (warp == 0 && lane == 0) {
+            int st = 0;                                   /* stages issued so far (ring position) */
+            for (int ir = 0;; ++ir) {
+                const int item = atomicAdd(a.work, 1);
+                const int is = ir & 1;
+                if (ir >= 2) mbar_wait(item_empty(is), ((ir >> 1) - 1) & 1);
+                item_id[is] = item < nitems ? item : -1;
+                mbar_arrive(item_full(is));
+                if (item >= nitems) break;
+                const int p = item / a.ntile, t = item - p * a.ntile;
+                int bi, bj;
+                k2p_decode<FULL>(t, a.nb, bi, bj);
+                const bool diag = !FULL && bi == bj;
+                const int64_t mu0 = (int64_t)bi * K2_T, nu0 = (int64_t)bj * K2_T;
+                const int64_t rows_a = (nao - mu0 < K2_T) ? nao - mu0 : K2_T;
+                const int64_t rows_b = (nao - nu0 < K2_T) ? nao - nu0 : K2_T;
+                const int64_t gbeg = ng * p / a.npanel, gend = ng * (p + 1) / a.npanel;
+                const int nk = (int)((gend - gbeg + K2_KG - 1) / K2_KG);
+                for (int kc = 0; kc < nk; ++kc, ++st) {
+                    const int slot = st % K2_STAGES;
+                    const int round = st / K2_STAGES;
+                    if (round > 0) mbar_wait(empty_bar(slot), (round - 1) & 1);
+                    const int64_t g0 = gbeg + K2_KG * (int64_t)kc;
+                    const int n = (int)((gend - g0 < K2_KG) ? gend - g0 : K2_KG);
+                    const uint32_t bytes = (uint32_t)(n * 32 * (rows_a + (diag ? 0 : rows_b)));
+                    mbar_arrive_expect_tx(full_bar(slot), bytes);
+                    const uint32_t dst = smem_base + slot * K2_STAGE_BYTES;
+                    for (int q = 0; q < n; ++q) {
+                        const int64_t g = g0 + q;
+                        const int64_t kg = (g / a.n4s) * a.ldc4 + a.col04 + g % a.n4s;   /* k-group in X4 */
+                        const double *src = a.X4 + kg * nao * 4;
+                        bulk_g2s(dst + q * (K2_T * 32), src + mu0 * 4, (uint32_t)(rows_a * 32), full_bar(slot));
+                        if (!diag) {
+                            const double *srcb = FULL ? src + (a.col04b - a.col04) * nao * 4 : src;
+                            bulk_g2s(dst + K2_OP_BYTES + q * (K2_T * 32), srcb + nu0 * 4,
+                                     (uint32_t)(rows_b * 32), full_bar(slot));
+                        }
+                    }
+                }
+            }
+        }
+        return;
+    }
+
+    /* ---------------------------------------------------------------- consumers (two warpgroups) */
+    reg_alloc<232>();
+    const int cw = warp - 4;
+    const int lq = lane >> 2, lr = lane & 3;
+    /* warp tile of the triangular layout (see k2_syrk_lower_kernel) */
+    const int tr = (cw < 2 || cw == 4) ? 3 : (cw < 4 ? 2 : (cw < 7 ? 1 : 0));
+    const int tc0 = (cw == 1 || cw == 3) ? 3 : (cw == 4 ? 6 : (cw == 6 ? 2 : 0));
+    int st = 0;
+    for (int ir = 0;; ++ir) {
+        const int is = ir & 1;
+        mbar_wait(item_full(is), (ir >> 1) & 1);
+        const int item = item_id[is];
+        __syncwarp();
+        if (lane == 0) mbar_arrive(item_empty(is));
+        if (item < 0) break;
+        const int p = item / a.ntile, t = item - p * a.ntile;
+        int bi, bj;
+        k2p_decode<FULL>(t, a.nb, bi, bj);
+        const bool diag = !FULL && bi == bj;
+        const int64_t mu0 = (int64_t)bi * K2_T, nu0 = (int64_t)bj * K2_T;
+        const int64_t gbeg = ng * p / a.npanel, gend = ng * (p + 1) / a.npanel;
+        const int nk = (int)((gend - gbeg + K2_KG - 1) / K2_KG);
+        const bool narrow = nao - mu0 <= 64;
+        const bool tri = diag && !narrow;
+        const bool tall = FULL && !narrow && nao - nu0 <= 64;
+        const int wm = narrow ? 0 : cw >> 2, wn = narrow ? cw : cw & 3;
+        const int wcols = narrow ? 16 : 32;
+        const int row_w = tri ? 32 * tr : (tall ? 32 * (cw >> 1) : 64 * wm);
+        const int col_w = tri ? 16 * tc0 : (tall ? 32 * (cw & 1) : wcols * wn);
+        const bool warp_active = (mu0 + row_w < nao) && (nu0 + col_w < nao) &&
+                                 !(diag && !tri && col_w > row_w + 63);
+        double acc[32][2];
+#pragma unroll
+        for (int q = 0; q < 32; ++q) acc[q][0] = acc[q][1] = 0.0;
+
+        for (int kc = 0; kc < nk; ++kc, ++st) {
+            const int slot = st % K2_STAGES;
+            mbar_wait(full_bar(slot), (st / K2_STAGES) & 1);
+            if (warp_active) {
+                const int64_t g0 = gbeg + K2_KG * (int64_t)kc;
+                const int n = (int)((gend - g0 < K2_KG) ? gend - g0 : K2_KG);
+                const double *Xa = reinterpret_cast<const double *>(smem_raw + slot * K2_STAGE_BYTES);
+                const double *Xb = diag ? Xa : Xa + K2_OP_BYTES / 8;
+                const double *a_base = Xa + (row_w + lq) * 4 + lr;
+                const double *b_base = Xb + (col_w + lq) * 4 + lr;
+                if (tall) {
+#pragma unroll
+                    for (int q = 0; q < K2_KG; ++q) {
+                        if (q < n) {
+                            double av[4], bv[4];
+#pragma unroll
+                            for (int mt = 0; mt < 4; ++mt) av[mt] = a_base[q * (K2_T * 4) + mt * 32];
+#pragma unroll
+                            for (int nt = 0; nt < 4; ++nt) bv[nt] = b_base[q * (K2_T * 4) + nt * 32];
+#pragma unroll
+                            for (int mt = 0; mt < 4; ++mt)
+#pragma unroll
+                                for (int nt = 0; nt < 4; ++nt)
+                                    dmma884(acc[mt * 4 + nt][0], acc[mt * 4 + nt][1], av[mt], bv[nt]);
+                        }
+                    }
+                } else if (tri) {
+                    if (cw < 4) {
+#pragma unroll
+                        for (int q = 0; q < K2_KG; ++q) {
+                            if (q < n) {
+                                double av[4], bv[6];
+#pragma unroll
+                                for (int mt = 0; mt < 4; ++mt) av[mt] = a_base[q * (K2_T * 4) + mt * 32];
+#pragma unroll
+                                for (int nt = 0; nt < 6; ++nt) bv[nt] = b_base[q * (K2_T * 4) + nt * 32];
+#pragma unroll
+                                for (int mt = 0; mt < 4; ++mt)
+#pragma unroll
+                                    for (int nt = 0; nt < 6; ++nt)
+                                        dmma884(acc[mt * 6 + nt][0], acc[mt * 6 + nt][1], av[mt], bv[nt]);
+                            }
+                        }
+                    } else {
+#pragma unroll
+                        for (int q = 0; q < K2_KG; ++q) {
+                            if (q < n) {
+                                double av[4], bv[4];
+#pragma unroll
+                                for (int mt = 0; mt < 4; ++mt) av[mt] = a_base[q * (K2_T * 4) + mt * 32];
+#pragma unroll
+                                for (int nt = 0; nt < 4; ++nt) bv[nt] = b_base[q * (K2_T * 4) + nt * 32];
+#pragma unroll
+                                for (int mt = 0; mt < 4; ++mt)
+#pragma unroll
+                                    for (int nt = 0; nt < 4; ++nt)
+                                        dmma884(acc[mt * 6 + nt][0], acc[mt * 6 + nt][1], av[mt], bv[nt]);
+                            }
+                        }
+                    }
+                } else if (!narrow) {
+#pragma unroll
+                    for (int q = 0; q < K2_KG; ++q) {
+                        if (q < n) {
+                            double av[8], bv[4];
+#pragma unroll
+                            for (int mt = 0; mt < 8; ++mt) av[mt] = a_base[q * (K2_T * 4) + mt * 32];
+#pragma unroll
+                            for (int nt = 0; nt < 4; ++nt) bv[nt] = b_base[q * (K2_T * 4) + nt * 32];
+#pragma unroll
+                            for (int mt = 0; mt < 8; ++mt)
+#pragma unroll
+                                for (int nt = 0; nt < 4; ++nt)
+                                    dmma884(acc[mt * 4 + nt][0], acc[mt * 4 + nt][1], av[mt], bv[nt]);
+                        }
+                    }
+                } else {
+#pragma unroll
+                    for (int q = 0; q < K2_KG; ++q) {
+                        if (q < n) {
+                            double av[8], bv[2];
+#pragma unroll
+                            for (int mt = 0; mt < 8; ++mt) av[mt] = a_base[q * (K2_T * 4) + mt * 32];
+#pragma unroll
+                            for (int nt = 0; nt < 2; ++nt) bv[nt] = b_base[q * (K2_T * 4) + nt * 32];
+#pragma unroll
+                            for (int mt = 0; mt < 8; ++mt)
+#pragma unroll
+                                for (int nt = 0; nt < 2; ++nt)
+                                    dmma884(acc[mt * 4 + nt][0], acc[mt * 4 + nt][1], av[mt], bv[nt]);
+                        }
+                    }
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(empty_bar(slot));
+        }
+
+        /* ---- add the partial into slab p % S, after item (p - S, t) has */
+        const int slab = p % a.nslab, seq = p / a.nslab;
+        int *flag = a.work + 1 + slab * a.ntile + t;
+        const bool overwrite = seq == 0 && !a.accumulate;
+        if (warp_active) {
+            if (seq > 0) {
+                if (lane == 0) while (ld_acquire_gpu(flag) < seq) { }
+                __syncwarp();
+                (void)ld_acquire_gpu(flag);              /* every lane orders its loads after the flag */
+            }
+            double *Kp = a.Kpart + (int64_t)slab * nao * nao;
+            /* The adds are batched: all loads of a batch (one 8-row MMA row of the warp tile, 4-6
+             * column pairs) are issued before the first store, so an item pays a handful of L2 round
+             * trips instead of one per element (a plain load-add-store loop cost ~20 us per item: the
+             * compiler must keep each load behind the previous store).  16-byte accesses when the row
+             * pitch allows (nao even), else element-wise. */
+            const bool vec = (nao & 1) == 0;
+            const int64_t nu_first = nu0 + col_w + 2 * lr;
+            double *row0 = Kp + (mu0 + row_w + lq) * nao + nu_first;
+            if (tri) {
+                if (cw < 4) {
+#pragma unroll
+                    for (int mt = 0; mt < 4; ++mt)
+                        if (mu0 + row_w + 8 * mt + lq < nao)
+                            k2p_add_row<6>(&acc[mt * 6], row0 + 8 * mt * nao, nu_first, nao, overwrite, vec);
+                } else {
+#pragma unroll
+                    for (int mt = 0; mt < 4; ++mt)
+                        if (mu0 + row_w + 8 * mt + lq < nao)
+                            k2p_add_row<4>(&acc[mt * 6], row0 + 8 * mt * nao, nu_first, nao, overwrite, vec);
+                }
+            } else if (narrow) {
+#pragma unroll
+                for (int mt = 0; mt < 8; ++mt)
+                    if (mu0 + row_w + 8 * mt + lq < nao)
+                        k2p_add_row<2>(&acc[mt * 4], row0 + 8 * mt * nao, nu_first, nao, overwrite, vec);
+            } else if (tall) {
+#pragma unroll
+                for (int mt = 0; mt < 4; ++mt)
+                    if (mu0 + row_w + 8 * mt + lq < nao)
+                        k2p_add_row<4>(&acc[mt * 4], row0 + 8 * mt * nao, nu_first, nao, overwrite, vec);
+            } else {
+#pragma unroll
+                for (int mt = 0; mt < 8; ++mt)
+                    if (mu0 + row_w + 8 * mt + lq < nao)
+                        k2p_add_row<4>(&acc[mt * 4], row0 + 8 * mt * nao, nu_first, nao, overwrite, vec);
+            }
+            __threadfence();
+        }
+        /* all eight consumer warps (the idle ones too) meet, then one thread publishes the item */
+        asm volatile("bar.sync 1, %0;" ::"n"(32 * K2_CONSUMER_WARPS) : "memory");
+        if (cw == 0 && lane == 0) st_release_gpu(flag, seq + 1);
+    }
+}
+
 /* ------------------------------------------------------------------ K3 */
 constexpr int K3_T = 32;
 
@@ -444,6 +799,71 @@ cudaError_t launch_k2_gemm_full(const double *X4, int64_t nao, int64_t np, int64
     k2_syrk_lower_kernel<true><<<grid, K2_THREADS, K2_SMEM_BYTES, st>>>(
         X4, nao, np, ldc / 4, col0a / 4, col0b / 4, n4s, Kpart, nsplit, accumulate);
     return cudaPeekAtLastError();
+}
+
+/* panel length (stages of k = 32) and slab count of the panel-synchronous K2, see k2p_kernel;
+ * planned once per build from its first (largest) chunk */
+void k2p_plan(int64_t nao, int64_t ng, int ntile, int sm_count, int max_slabs, int64_t panel_bytes,
+              int *panel_stages, int *nslab)
+{
+    const int64_t stages_total = (ng + K2_KG - 1) / K2_KG;
+    /* L2: one panel of X (all nao rows) is about panel_bytes */
+    int64_t len = panel_bytes / (nao * 32 * K2_KG);
+    /* balance: at least ~30 items per SM when the problem is big enough for that */
+    const int64_t len_bal = stages_total * ntile / (30LL * sm_count);
+    if (len > len_bal) len = len_bal;
+    if (len < 8) len = 8;                                 /* the 128 KB read-modify-write must amortise */
+    if (len > stages_total) len = stages_total > 0 ? stages_total : 1;
+    const int64_t np_ = (stages_total + len - 1) / len;
+    /* slabs: the chain of read-modify-writes of one (slab, tile) must be short beside an item;
+     * ~3 us per add, items of len x 4.2 us, sm_count / ntile items of a tile in flight at once */
+    int64_t s_ = (2LL * sm_count * 3 * 10 + (int64_t)ntile * len * 42 - 1) / ((int64_t)ntile * len * 42);
+    if (s_ < 1) s_ = 1;
+    if (s_ > max_slabs) s_ = max_slabs;
+    if (s_ > np_) s_ = np_ > 0 ? np_ : 1;
+    *panel_stages = (int)len;
+    *nslab = (int)s_;
+}
+
+template <bool FULL>
+cudaError_t k2p_launch(const double *X4, int64_t nao, int64_t np, int64_t ldc, int64_t col0a, int64_t col0b,
+                       int64_t ncol, double *Kpart, int panel_stages, int nslab, int accumulate, int *work,
+                       int sm_count, cudaStream_t st)
+{
+    static std::atomic<unsigned long long> smem_ok{0};
+    cudaError_t e = ensure_dynamic_smem(k2p_kernel<FULL>, K2P_SMEM_BYTES, smem_ok);
+    if (e != cudaSuccess) return e;
+    K2PArgs a;
+    a.X4 = X4; a.nao = nao; a.np = np; a.ldc4 = ldc / 4; a.col04 = col0a / 4; a.col04b = col0b / 4;
+    a.n4s = (int)((ncol + 3) / 4);
+    const int64_t stages_total = (np * a.n4s + K2_KG - 1) / K2_KG;
+    const int npanel = (int)((stages_total + panel_stages - 1) / panel_stages);
+    a.Kpart = Kpart; a.nslab = nslab; a.accumulate = accumulate; a.npanel = npanel;
+    a.nb = (int)((nao + K2_T - 1) / K2_T);
+    a.ntile = FULL ? a.nb * a.nb : a.nb * (a.nb + 1) / 2;
+    a.work = work;
+    e = cudaMemsetAsync(work, 0, sizeof(int) * (size_t)(1 + nslab * a.ntile), st);
+    if (e != cudaSuccess) return e;
+    const int64_t nitems = (int64_t)npanel * a.ntile;
+    const unsigned grid = (unsigned)(nitems < sm_count ? nitems : sm_count);
+    k2p_kernel<FULL><<<grid, K2P_THREADS, K2P_SMEM_BYTES, st>>>(a);
+    return cudaPeekAtLastError();
+}
+
+cudaError_t launch_k2p_syrk_lower(const double *X4, int64_t nao, int64_t np, int64_t ldc, int64_t col0,
+                                  int64_t ncol, double *Kpart, int panel_stages, int nslab, int accumulate,
+                                  int *work, int sm_count, cudaStream_t st)
+{
+    return k2p_launch<false>(X4, nao, np, ldc, col0, col0, ncol, Kpart, panel_stages, nslab, accumulate, work,
+                             sm_count, st);
+}
+
+cudaError_t launch_k2p_gemm_full(const double *X4, int64_t nao, int64_t np, int64_t ldc, int64_t col0a,
+                                 int64_t col0b, int64_t ncol, double *Kpart, int panel_stages, int nslab,
+                                 int accumulate, int *work, int sm_count, cudaStream_t st)
+{
+    return k2p_launch<true>(X4, nao, np, ldc, col0a, col0b, ncol, Kpart, panel_stages, nslab, accumulate, work,
+                            sm_count, st);
 }
 
 void launch_k3_finish(const double *Kpart, int nsplit, int64_t nao, double *K, double *const *Kslot,

@@ -56,8 +56,10 @@ def test_pair_parity(dfjk, nao, naux, ncol):
     C1, C2 = rng.standard_normal((nao, ncol)), rng.standard_normal((nao, ncol))
     h = dfjk.DFJK(dev(Bp), nao)
     Jo, Ko, do = oracle.get_jk_pair(Bp, nao, C1, C2)
-    for fused in (1, 0):             # d_P read off X = B_P C1 (default), or by a pass over B
-        h.set_option("j_fused", fused)
+    h.set_option("k2_panel_kb", 64)
+    for fused, k2_panel in ((1, 0), (0, 0), (1, 1)):   # d_P read off X = B_P C1 (default) or by a pass
+        h.set_option("j_fused", fused)                  # over B; both full-product K2 kernels
+        h.set_option("k2_panel", k2_panel)
         J, K = h.get_jk_pair(dev(C1), dev(C2))
         d = h.get_d()
         torch.cuda.synchronize()
@@ -72,11 +74,14 @@ def test_dm_parity(dfjk, nao, naux):
     Bp = make_B(nao, naux, 300 + nao)
     dm = np.random.default_rng(nao).standard_normal((nao, nao))       # neither symmetric nor PSD
     h = dfjk.DFJK(dev(Bp), nao)
-    J, K = h.get_jk_dm(dev(dm))
-    torch.cuda.synchronize()
     Jo, Ko, _ = oracle.get_jk_dm(Bp, nao, dm)
-    assert relerr(J.cpu().numpy(), Jo) <= TOL
-    assert relerr(K.cpu().numpy(), Ko) <= TOL
+    h.set_option("k2_panel_kb", 64)
+    for k2_panel in (0, 1):
+        h.set_option("k2_panel", k2_panel)
+        J, K = h.get_jk_dm(dev(dm))
+        torch.cuda.synchronize()
+        assert relerr(J.cpu().numpy(), Jo) <= TOL
+        assert relerr(K.cpu().numpy(), Ko) <= TOL
     h.close()
 
 

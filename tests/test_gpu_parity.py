@@ -84,9 +84,10 @@ def test_baseline_configs_all_calls(dfjk, cfg_id):
     (257, 6, 31),
     (300, 40, 300),     # nocc = nao, three N tiles
 ])
-def test_ragged_shapes(dfjk, nao, naux, nocc):
+@pytest.mark.parametrize("k2_panel", [0, 1])       # both K2 kernels (the default picks by size)
+def test_ragged_shapes(dfjk, nao, naux, nocc, k2_panel):
     Bp, (C,) = rand_case(nao, naux, (nocc,), seed=nao + naux)
-    J, K, d = run_restricted(dfjk, Bp, nao, C)
+    J, K, d = run_restricted(dfjk, Bp, nao, C, k2_panel=k2_panel, k2_panel_kb=64)
     Jo, Ko, do = oracle.get_jk(Bp, nao, [C], [2.0])
     assert relerr(d, do) <= TOL
     assert relerr(J, Jo) <= TOL
@@ -102,7 +103,10 @@ def test_non_orthonormal_orbitals(dfjk):
 
 
 @pytest.mark.parametrize("opts", [dict(k_chunk=1), dict(k_chunk=3), dict(k_chunk=4, k_splits=1),
-                                  dict(k_chunk=7, k_splits=2), dict(j_fused=0), dict(j_fused=0, k_chunk=5)])
+                                  dict(k_chunk=7, k_splits=2), dict(j_fused=0), dict(j_fused=0, k_chunk=5),
+                                  dict(k2_panel=1), dict(k2_panel=1, k_chunk=3, k_splits=1),
+                                  dict(k2_panel=1, k_chunk=7, k_splits=2, k2_panel_kb=64),
+                                  dict(k2_panel=1, k2_panel_kb=64, graph=0)])
 def test_chunk_and_split_options(dfjk, opts):
     Bp, (C,) = rand_case(260, 23, (13,), seed=3)
     J, K, _ = run_restricted(dfjk, Bp, 260, C, **opts)
@@ -110,12 +114,14 @@ def test_chunk_and_split_options(dfjk, opts):
     assert relerr(J, Jo) <= TOL and relerr(K, Ko[0]) <= TOL
 
 
-@pytest.mark.parametrize("fused", [1, 0])
-def test_unrestricted(dfjk, fused):
+@pytest.mark.parametrize("fused,k2_panel", [(1, 0), (0, 0), (1, 1)])
+def test_unrestricted(dfjk, fused, k2_panel):
     nao, naux = 210, 33
     Bp, (Ca, Cb) = rand_case(nao, naux, (19, 14), seed=8)
     h = dfjk.DFJK(dev(Bp), nao)
     h.set_option("j_fused", fused)      # d_P from the half-transformed X (default) or by a pass over B
+    h.set_option("k2_panel", k2_panel)
+    h.set_option("k2_panel_kb", 64)
     J, Ka, Kb = h.get_jk_u(dev(Ca), dev(Cb))
     d = h.get_d()
     torch.cuda.synchronize()
@@ -250,13 +256,15 @@ def test_seeded_shape_fuzz(dfjk):
         if kind == 0:
             nocc = int(rng.integers(1, nao + 1))
             Bp, (C,) = rand_case(nao, naux, (nocc,), seed=1000 + case, orthonormal=bool(case & 1))
-            J, K, d = run_restricted(dfjk, Bp, nao, C)
+            J, K, d = run_restricted(dfjk, Bp, nao, C, k2_panel=(case // 3) % 2, k2_panel_kb=64)
             Jo, Ko, do = oracle.get_jk(Bp, nao, [C], [2.0])
             errs = [relerr(d, do), relerr(J, Jo), relerr(K, Ko[0])]
         elif kind == 1:
             na, nb = int(rng.integers(1, nao + 1)), int(rng.integers(1, nao + 1))
             Bp, (Ca, Cb) = rand_case(nao, naux, (na, nb), seed=1000 + case)
             h = dfjk.DFJK(dev(Bp), nao)
+            h.set_option("k2_panel", (case // 3) % 2)
+            h.set_option("k2_panel_kb", 64)
             J, Ka, Kb = h.get_jk_u(dev(Ca), dev(Cb))
             torch.cuda.synchronize()
             Jo, Kao, Kbo = oracle.get_jk_unrestricted(Bp, nao, Ca, Cb)
@@ -266,6 +274,8 @@ def test_seeded_shape_fuzz(dfjk):
             ncol = int(rng.integers(1, nao + 1))
             Bp, (C1, C2) = rand_case(nao, naux, (ncol, ncol), seed=1000 + case, orthonormal=False)
             h = dfjk.DFJK(dev(Bp), nao)
+            h.set_option("k2_panel", (case // 3) % 2)
+            h.set_option("k2_panel_kb", 64)
             J, K = h.get_jk_pair(dev(C1), dev(C2))
             torch.cuda.synchronize()
             Jo, Ko, _ = oracle.get_jk_pair(Bp, nao, C1, C2)
