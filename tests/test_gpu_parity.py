@@ -401,7 +401,7 @@ def test_kernel_timing_ring_grows(dfjk):
     h.set_option("time_kernels", 1)
     Cd = dev(C)
     n0 = h.launch_count
-    for _ in range(60):
+    for _ in range(100):
         h.get_jk(Cd)
     torch.cuda.synchronize()
     total = sum(h.kernel_time(k)[1] for k in dfjk.KERNELS)
