@@ -332,8 +332,10 @@ int enqueue_jk_body(dfjk_handle *h, int nset, const int *nocc, const int *col0, 
         if (pc > naux) pc = naux;
         if (pc < 1) return fail(DFJK_ENOMEM, "%s: X workspace too small", who);
         /* K2P pays a read-modify-write per item to keep the k window of X inside L2; an X chunk that
-         * fits in L2 whole has nothing to gain from it (and small problems are all overhead) */
-        const bool panel = h->opt_k2_panel == 1 || (h->opt_k2_panel == 2 && pc * nao * ldc * 8 > h->l2_bytes);
+         * fits in L2 whole has nothing to gain from it (and small problems are all overhead), and the
+         * slab it adds into (nao^2 doubles) must itself stay in L2 beside the window */
+        const bool panel = h->opt_k2_panel == 1 ||
+                           (h->opt_k2_panel == 2 && pc * nao * ldc * 8 > h->l2_bytes && nao * nao * 8 * 3 <= h->l2_bytes);
         const int nbk = (int)((nao + 127) / 128);
         /* K2P: panel length and slab count per set, planned from the first (largest) chunk; the old
          * split kernel: one partial per k-split */
@@ -536,7 +538,8 @@ int get_jk_general_impl(dfjk_handle *h, const double *C1, const double *C2, int6
         if (pc > 65535) pc = 65535;                /* K1U's grid.z */
         if (pc < 1) return fail(DFJK_ENOMEM, "%s: X workspace too small", who);
         const int nb = (int)((nao + 127) / 128);
-        const bool panel = h->opt_k2_panel == 1 || (h->opt_k2_panel == 2 && pc * nao * ldx * 8 > h->l2_bytes);
+        const bool panel = h->opt_k2_panel == 1 ||
+                           (h->opt_k2_panel == 2 && pc * nao * ldx * 8 > h->l2_bytes && nao * nao * 8 * 3 <= h->l2_bytes);
         int nsplit = h->opt_k_splits > 0 ? (int)h->opt_k_splits
                                          : choose_splits(nb * nb, h->sm_count, h->nsplit_alloc);
         int pstages = 0;

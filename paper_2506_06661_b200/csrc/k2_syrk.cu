@@ -176,6 +176,7 @@ k2_syrk_lower_kernel(const double *__restrict__ X4, int64_t nao, int64_t np, int
      * rows would leave the lower four warps idle: it is covered 1 (M) x 8 (N) with 64 x 16 warp
      * tiles instead, so all eight warps share the work ("narrow"; CTA-uniform). */
     const bool narrow = nao - mu0 <= 64;
+    const int nmt_narrow = nao - mu0 <= 32 ? 4 : 8;      /* 8-row MMA rows of a narrow warp tile in use */
     /* A full-height diagonal tile needs only its lower triangle: 20 units of 32 x 16 touch it.  They
      * are dealt 3,3,3,3,2,2,2,2 to the eight warps as 32 x 48 / 32 x 32 warp tiles ("tri"), so the tile
      * costs 24 instead of 32 DMMAs per warp and k-group (the 2 x 4 layout would leave two warps idle
@@ -281,14 +282,16 @@ k2_syrk_lower_kernel(const double *__restrict__ X4, int64_t nao, int64_t np, int
                     if (q < n) {
                         double a[8], b[2];
 #pragma unroll
-                        for (int mt = 0; mt < 8; ++mt) a[mt] = a_base[q * (K2_T * 4) + mt * 32];
+                        for (int mt = 0; mt < 8; ++mt) a[mt] = mt < nmt_narrow ? a_base[q * (K2_T * 4) + mt * 32] : 0.0;
 #pragma unroll
                         for (int nt = 0; nt < 2; ++nt) b[nt] = b_base[q * (K2_T * 4) + nt * 32];
 #pragma unroll
                         for (int mt = 0; mt < 8; ++mt)
+                            if (mt < nmt_narrow) {       /* <= 32 valid rows: 4 of the 8 MMA rows */
 #pragma unroll
-                            for (int nt = 0; nt < 2; ++nt)
-                                dmma884(acc[mt * 4 + nt][0], acc[mt * 4 + nt][1], a[mt], b[nt]);
+                                for (int nt = 0; nt < 2; ++nt)
+                                    dmma884(acc[mt * 4 + nt][0], acc[mt * 4 + nt][1], a[mt], b[nt]);
+                            }
                     }
                 }
             }
@@ -382,40 +385,51 @@ __device__ __forceinline__ void k2p_decode(int t, int nb, int &bi, int &bj)
     }
 }
 
-/* row[8 nt + {0,1}] (+)= acc[nt][{0,1}], nt < NNT, columns nu_first + 8 nt + {0,1} < nao: all loads
- * of the row are issued before the first store */
-template <int NNT>
-__device__ __forceinline__ void k2p_add_row(const double (*acc)[2], double *row, int64_t nu_first,
-                                            int64_t nao, bool overwrite, bool vec)
+/* NR rows (8 apart) of the warp tile at once:  row_r[8 nt + {0,1}] (+)= acc[r * AST + nt][{0,1}],
+ * nt < NNT, for the rows r with mu_first + 8 r < nao and the columns nu_first + 8 nt + {0,1} < nao.
+ * ALL loads of the NR rows are issued before the first store: one L2 round trip per batch. */
+template <int NNT, int NR, int AST>
+__device__ __forceinline__ void k2p_add_rows(const double (*acc)[2], double *row, int64_t mu_first,
+                                             int64_t nu_first, int64_t nao, bool overwrite, bool vec)
 {
-    double v0[NNT], v1[NNT];
+    double v0[NR][NNT], v1[NR][NNT];
 #pragma unroll
-    for (int nt = 0; nt < NNT; ++nt) v0[nt] = v1[nt] = 0.0;
+    for (int r = 0; r < NR; ++r)
+#pragma unroll
+        for (int nt = 0; nt < NNT; ++nt) v0[r][nt] = v1[r][nt] = 0.0;
     if (!overwrite) {
-        if (vec) {
 #pragma unroll
-            for (int nt = 0; nt < NNT; ++nt)
-                if (nu_first + 8 * nt < nao) {
-                    const double2 t = __ldcg(reinterpret_cast<const double2 *>(row + 8 * nt));
-                    v0[nt] = t.x; v1[nt] = t.y;
-                }
-        } else {
+        for (int r = 0; r < NR; ++r) {
+            if (mu_first + 8 * r >= nao) continue;
+            const double *rp = row + (int64_t)8 * r * nao;
 #pragma unroll
             for (int nt = 0; nt < NNT; ++nt) {
-                if (nu_first + 8 * nt < nao) v0[nt] = __ldcg(row + 8 * nt);
-                if (nu_first + 8 * nt + 1 < nao) v1[nt] = __ldcg(row + 8 * nt + 1);
+                if (vec) {
+                    if (nu_first + 8 * nt < nao) {
+                        const double2 t = __ldcg(reinterpret_cast<const double2 *>(rp + 8 * nt));
+                        v0[r][nt] = t.x; v1[r][nt] = t.y;
+                    }
+                } else {
+                    if (nu_first + 8 * nt < nao) v0[r][nt] = __ldcg(rp + 8 * nt);
+                    if (nu_first + 8 * nt + 1 < nao) v1[r][nt] = __ldcg(rp + 8 * nt + 1);
+                }
             }
         }
     }
 #pragma unroll
-    for (int nt = 0; nt < NNT; ++nt) {
-        const double r0 = v0[nt] + acc[nt][0], r1 = v1[nt] + acc[nt][1];
-        if (vec) {
-            if (nu_first + 8 * nt < nao)                  /* nao and nu even: the pair is inside */
-                *reinterpret_cast<double2 *>(row + 8 * nt) = make_double2(r0, r1);
-        } else {
-            if (nu_first + 8 * nt < nao) row[8 * nt] = r0;
-            if (nu_first + 8 * nt + 1 < nao) row[8 * nt + 1] = r1;
+    for (int r = 0; r < NR; ++r) {
+        if (mu_first + 8 * r >= nao) continue;
+        double *rp = row + (int64_t)8 * r * nao;
+#pragma unroll
+        for (int nt = 0; nt < NNT; ++nt) {
+            const double r0 = v0[r][nt] + acc[r * AST + nt][0], r1 = v1[r][nt] + acc[r * AST + nt][1];
+            if (vec) {
+                if (nu_first + 8 * nt < nao)              /* nao and nu even: the pair is inside */
+                    *reinterpret_cast<double2 *>(rp + 8 * nt) = make_double2(r0, r1);
+            } else {
+                if (nu_first + 8 * nt < nao) rp[8 * nt] = r0;
+                if (nu_first + 8 * nt + 1 < nao) rp[8 * nt + 1] = r1;
+            }
         }
     }
 }
@@ -521,6 +535,7 @@ k2p_kernel(const K2PArgs a)
         const int64_t gbeg = ng * p / a.npanel, gend = ng * (p + 1) / a.npanel;
         const int nk = (int)((gend - gbeg + K2_KG - 1) / K2_KG);
         const bool narrow = nao - mu0 <= 64;
+        const int nmt_narrow = nao - mu0 <= 32 ? 4 : 8;  /* 8-row MMA rows of a narrow warp tile in use */
         const bool tri = diag && !narrow;
         const bool tall = FULL && !narrow && nao - nu0 <= 64;
         const int wm = narrow ? 0 : cw >> 2, wn = narrow ? cw : cw & 3;
@@ -615,14 +630,16 @@ k2p_kernel(const K2PArgs a)
                         if (q < n) {
                             double av[8], bv[2];
 #pragma unroll
-                            for (int mt = 0; mt < 8; ++mt) av[mt] = a_base[q * (K2_T * 4) + mt * 32];
+                            for (int mt = 0; mt < 8; ++mt) av[mt] = mt < nmt_narrow ? a_base[q * (K2_T * 4) + mt * 32] : 0.0;
 #pragma unroll
                             for (int nt = 0; nt < 2; ++nt) bv[nt] = b_base[q * (K2_T * 4) + nt * 32];
 #pragma unroll
                             for (int mt = 0; mt < 8; ++mt)
+                                if (mt < nmt_narrow) {   /* <= 32 valid rows: 4 of the 8 MMA rows */
 #pragma unroll
-                                for (int nt = 0; nt < 2; ++nt)
-                                    dmma884(acc[mt * 4 + nt][0], acc[mt * 4 + nt][1], av[mt], bv[nt]);
+                                    for (int nt = 0; nt < 2; ++nt)
+                                        dmma884(acc[mt * 4 + nt][0], acc[mt * 4 + nt][1], av[mt], bv[nt]);
+                                }
                         }
                     }
                 }
@@ -650,33 +667,21 @@ k2p_kernel(const K2PArgs a)
             const bool vec = (nao & 1) == 0;
             const int64_t nu_first = nu0 + col_w + 2 * lr;
             double *row0 = Kp + (mu0 + row_w + lq) * nao + nu_first;
+            const int64_t mu_first = mu0 + row_w + lq;
             if (tri) {
                 if (cw < 4) {
-#pragma unroll
-                    for (int mt = 0; mt < 4; ++mt)
-                        if (mu0 + row_w + 8 * mt + lq < nao)
-                            k2p_add_row<6>(&acc[mt * 6], row0 + 8 * mt * nao, nu_first, nao, overwrite, vec);
+                    k2p_add_rows<6, 2, 6>(&acc[0], row0, mu_first, nu_first, nao, overwrite, vec);
+                    k2p_add_rows<6, 2, 6>(&acc[12], row0 + 16 * nao, mu_first + 16, nu_first, nao, overwrite, vec);
                 } else {
-#pragma unroll
-                    for (int mt = 0; mt < 4; ++mt)
-                        if (mu0 + row_w + 8 * mt + lq < nao)
-                            k2p_add_row<4>(&acc[mt * 6], row0 + 8 * mt * nao, nu_first, nao, overwrite, vec);
+                    k2p_add_rows<4, 4, 6>(&acc[0], row0, mu_first, nu_first, nao, overwrite, vec);
                 }
             } else if (narrow) {
-#pragma unroll
-                for (int mt = 0; mt < 8; ++mt)
-                    if (mu0 + row_w + 8 * mt + lq < nao)
-                        k2p_add_row<2>(&acc[mt * 4], row0 + 8 * mt * nao, nu_first, nao, overwrite, vec);
+                k2p_add_rows<2, 8, 4>(&acc[0], row0, mu_first, nu_first, nao, overwrite, vec);
             } else if (tall) {
-#pragma unroll
-                for (int mt = 0; mt < 4; ++mt)
-                    if (mu0 + row_w + 8 * mt + lq < nao)
-                        k2p_add_row<4>(&acc[mt * 4], row0 + 8 * mt * nao, nu_first, nao, overwrite, vec);
+                k2p_add_rows<4, 4, 4>(&acc[0], row0, mu_first, nu_first, nao, overwrite, vec);
             } else {
-#pragma unroll
-                for (int mt = 0; mt < 8; ++mt)
-                    if (mu0 + row_w + 8 * mt + lq < nao)
-                        k2p_add_row<4>(&acc[mt * 4], row0 + 8 * mt * nao, nu_first, nao, overwrite, vec);
+                k2p_add_rows<4, 4, 4>(&acc[0], row0, mu_first, nu_first, nao, overwrite, vec);
+                k2p_add_rows<4, 4, 4>(&acc[16], row0 + 32 * nao, mu_first + 32, nu_first, nao, overwrite, vec);
             }
             __threadfence();
         }
