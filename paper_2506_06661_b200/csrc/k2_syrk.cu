@@ -683,9 +683,10 @@ k2p_kernel(const K2PArgs a)
                 k2p_add_rows<4, 4, 4>(&acc[0], row0, mu_first, nu_first, nao, overwrite, vec);
                 k2p_add_rows<4, 4, 4>(&acc[16], row0 + 32 * nao, mu_first + 32, nu_first, nao, overwrite, vec);
             }
-            __threadfence();
         }
-        /* all eight consumer warps (the idle ones too) meet, then one thread publishes the item */
+        /* all eight consumer warps (the idle ones too) meet, then one thread publishes the item: the
+         * barrier orders every warp's stores before the gpu-scope release store (release is cumulative
+         * over what the barrier made visible to the releasing thread), no per-thread fence needed */
         asm volatile("bar.sync 1, %0;" ::"n"(32 * K2_CONSUMER_WARPS) : "memory");
         if (cw == 0 && lane == 0) st_release_gpu(flag, seq + 1);
     }
