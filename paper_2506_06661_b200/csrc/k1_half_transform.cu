@@ -61,29 +61,9 @@ constexpr int K1_SMEM_BUDGET = 220 * 1024;
  * visits the 128-wide column blocks j in the round-robin tournament order j = (s - i) mod nib,
  * s = 0 .. nib-1.  At step s the pair (i, j) with i + j == s (mod nib) work on each other's block:
  * i stages B_P[block i, block j] while j stages B_P[block j, block i] -- the same packed elements, at
- * the same time.  Whichever read arrives second is an L2 hit (or joins the first one's miss), so B
- * comes from HBM once per build instead of 1.44 times (ncu r01e; 1.33 with eviction hints only).
- * DFJK_K1_L2_HINTS (off) marks row-form reads evict_last and col-form reads evict_first, which is
- * what helped the sequential walk (DFJK_K1_PAIRED=0, items of a P numbered from the last block down
- * so the row-form reader never starts late). */
-#ifndef DFJK_K1_PAIRED
-#define DFJK_K1_PAIRED 1
-#endif
-#ifndef DFJK_K1_L2_HINTS
-#define DFJK_K1_L2_HINTS 0
-#endif
-#ifndef DFJK_K1_DESCENDING
-#define DFJK_K1_DESCENDING 0
-#endif
-#ifndef DFJK_K1_X_EVICT_FIRST
-#define DFJK_K1_X_EVICT_FIRST 0
-#endif
-
-/* row block of the r-th item of a P (r = item index within the P divided by the N tiles) */
-__device__ __forceinline__ int64_t k1_row_block(int r, int nib)
-{
-    return DFJK_K1_DESCENDING ? nib - 1 - r : r;
-}
+ * (nearly) the same time, so whichever read arrives second is an L2 hit.  B comes from HBM 1.22
+ * times per build at nao = 1600 and 1.01 times at nao = 800 instead of 1.44 (ncu r01e / r02).
+ * L2 eviction hints on top of this made it worse. */
 
 enum { K1_MODE_ROW = 0, K1_MODE_COL = 1, K1_MODE_GATHER = 2 };
 
@@ -146,22 +126,13 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
     if (warp < K1_PRODUCERS / 32) {
         /* ------------------------------------------------------------ producers */
         reg_dealloc<40>();
-#if DFJK_K1_L2_HINTS
-#if DFJK_K1_L2_HINTS == 2
-        const uint64_t pol_first = l2_policy_evict_last(), pol_second = l2_policy_evict_last();
-#elif DFJK_K1_L2_HINTS == 3
-        const uint64_t pol_first = l2_policy_evict_first(), pol_second = l2_policy_evict_first();
-#else
-        const uint64_t pol_first = l2_policy_evict_last(), pol_second = l2_policy_evict_first();
-#endif
-#endif
         int slot = 0;
         uint32_t phase = 1;                                /* parity of the "empty" phase to wait for */
         bool ring_full = false;                            /* all STAGES slots have been used once */
         for (int64_t item = blockIdx.x; item < nitems; item += gridDim.x) {
         const int64_t p = item / items_per_p;
         const int rem = (int)(item - p * items_per_p);
-        const int64_t mu0 = k1_row_block(rem / ntiles_n, nib) * K1_M;
+        const int64_t mu0 = (int64_t)(rem / ntiles_n) * K1_M;
         const int64_t n0 = (int64_t)(rem % ntiles_n) * Cfg::NW;
         const int64_t pb = (P0 + p) * npair;               /* index of B_P's first element in B */
         const int pbpar = (int)(pb & 1);
@@ -174,8 +145,8 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
         if (rows_valid > K1_M) rows_valid = K1_M;
         const int rbi = (int)(mu0 / K1_M);
         for (int sstep = 0; sstep < nib; ++sstep) {
-        /* column block of this step: the tournament partner (paired) or simply the next one */
-        const int jb = DFJK_K1_PAIRED ? (sstep >= rbi ? sstep - rbi : sstep - rbi + nib) : sstep;
+        /* column block of this step: the tournament partner */
+        const int jb = sstep >= rbi ? sstep - rbi : sstep - rbi + nib;
         const int kc_end = (jb + 1) * (K1_M / K1_KC) < nk ? (jb + 1) * (K1_M / K1_KC) : nk;
         for (int kc = jb * (K1_M / K1_KC); kc < kc_end; ++kc) {
             if (ring_full) mbar_wait(empty_bar(slot), phase);
@@ -193,11 +164,7 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
                 const uint32_t nb = ok ? (uint32_t)(K1_KC + 2 * sft) * 8u : 0u;
                 my_bytes += nb;
                 if (my_bytes) mbar_arrive_expect_tx(bar, my_bytes); else mbar_arrive(bar);
-#if DFJK_K1_L2_HINTS
-                if (ok) bulk_g2s_hint(a_dst + tid * (K1_LDD * 8), B + (e - sft), nb, bar, pol_first);
-#else
                 if (ok) bulk_g2s(a_dst + tid * (K1_LDD * 8), B + (e - sft), nb, bar);
-#endif
             } else if (mode == K1_MODE_COL) {
                 /* thread t < 32 copies packed row nu0+t, columns mu0 .. mu0+rows_valid-1 */
                 const int64_t nu = nu0 + tid;
@@ -211,11 +178,7 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
                     for (int c = tid; c < K1_LDT; c += K1_PRODUCERS)
                         reinterpret_cast<double *>(smem_raw + slot * Cfg::STAGE_BYTES)[k * K1_LDT + c] = 0.0;
                 if (my_bytes) mbar_arrive_expect_tx(bar, my_bytes); else mbar_arrive(bar);
-#if DFJK_K1_L2_HINTS
-                if (ok) bulk_g2s_hint(a_dst + tid * (K1_LDT * 8), B + (e - sft), nb, bar, pol_second);
-#else
                 if (ok) bulk_g2s(a_dst + tid * (K1_LDT * 8), B + (e - sft), nb, bar);
-#endif
             } else {
                 /* element-wise gather into the "row" form (8-byte cp.async, zero fill outside) */
                 if (tid == 0) mbar_expect_tx(bar, c_bytes);
@@ -254,7 +217,7 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
         for (int64_t item = blockIdx.x; item < nitems; item += gridDim.x) {
         const int64_t p = item / items_per_p;
         const int rem = (int)(item - p * items_per_p);
-        const int64_t mu0 = k1_row_block(rem / ntiles_n, nib) * K1_M;
+        const int64_t mu0 = (int64_t)(rem / ntiles_n) * K1_M;
         const int64_t n0 = (int64_t)(rem % ntiles_n) * Cfg::NW;
         const int pbpar = (int)(((P0 + p) * npair) & 1);
         const bool last_p = P0 + p == naux - 1;
@@ -274,7 +237,7 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
 
         const int rbi = (int)(mu0 / K1_M);
         for (int sstep = 0; sstep < nib; ++sstep) {
-        const int jb = DFJK_K1_PAIRED ? (sstep >= rbi ? sstep - rbi : sstep - rbi + nib) : sstep;
+        const int jb = sstep >= rbi ? sstep - rbi : sstep - rbi + nib;
         const int kc_end = (jb + 1) * (K1_M / K1_KC) < nk ? (jb + 1) * (K1_M / K1_KC) : nk;
         for (int kc = jb * (K1_M / K1_KC); kc < kc_end; ++kc) {
             mbar_wait(full_bar(slot), phase);
@@ -316,9 +279,6 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
         }   /* column blocks */
 
         if (warp_active) {
-#if DFJK_K1_X_EVICT_FIRST
-            const uint64_t pol_x = l2_policy_evict_first();
-#endif
 #pragma unroll
             for (int mt = 0; mt < 2; ++mt) {
                 const int64_t mu = mu0 + row_w + 8 * mt + lq;
@@ -329,12 +289,7 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
                     if (col < ldc) {
                         const int64_t k = p * ldx + col;       /* ldx >= ldc: X row pitch */
                         double *dst = X4 + ((k >> 2) * nao + mu) * 4 + (k & 3);
-#if DFJK_K1_X_EVICT_FIRST
-                        asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1, %2}, %3;"
-                                     ::"l"(dst), "d"(acc[mt][nt][0]), "d"(acc[mt][nt][1]), "l"(pol_x) : "memory");
-#else
                         *reinterpret_cast<double2 *>(dst) = make_double2(acc[mt][nt][0], acc[mt][nt][1]);
-#endif
                     }
                 }
             }

@@ -58,12 +58,6 @@ __global__ void k0_pack_c_kernel(PackDesc pd, int64_t nao, int64_t nao16, int64_
 }
 
 /* ------------------------------------------------------------------ K2 */
-#ifndef DFJK_K2_TILE_FASTEST
-#define DFJK_K2_TILE_FASTEST 0
-#endif
-#ifndef DFJK_K2_ROTATE
-#define DFJK_K2_ROTATE 0
-#endif
 constexpr int K2_T = 128;
 constexpr int K2_KG = 8;                              /* k-groups (of 4) per stage: k = 32 */
 constexpr int K2_STAGES = 3;
@@ -86,17 +80,12 @@ k2_syrk_lower_kernel(const double *__restrict__ X4, int64_t nao, int64_t np, int
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     /* lower-triangle tile index -> (bi, bj), bi >= bj */
-    /* blockIdx.x = tile (fastest), blockIdx.y = split: the hardware dispatches CTAs in linear order, so
-     * the CTAs resident at any time belong to one or two splits and walk the SAME k range of X at the
-     * same pace -- a 128-row operand panel fetched from HBM by one CTA is an L2 hit for the other tiles
-     * of its block row / column (split-fastest order made co-resident CTAs read 13 different k ranges:
-     * 8.3 x the X chunk from DRAM, ncu r01e).  The last block row -- the ragged, cheaper tiles -- still
-     * comes last within every split, so the launch's tail is made of short CTAs. */
-#if DFJK_K2_TILE_FASTEST
-    const int t = blockIdx.x;
-#else
+    /* blockIdx.x = split (fastest), blockIdx.y = tile: the hardware dispatches CTAs in linear
+     * order, so the last block row -- the ragged, cheaper tiles -- runs last and the launch's
+     * tail is made of short CTAs.  (Tile-fastest order shares k ranges between co-resident CTAs --
+     * X from HBM 3.5 instead of 8.3 times -- but was 5.7 % slower; the panel-synchronous kernel
+     * below is the real answer to the re-reads.) */
     const int t = blockIdx.y;
-#endif
     int bi, bj;
     if (FULL) {
         const int nb = (int)((nao + K2_T - 1) / K2_T);
@@ -109,22 +98,13 @@ k2_syrk_lower_kernel(const double *__restrict__ X4, int64_t nao, int64_t np, int
         bj = t - bi * (bi + 1) / 2;
     }
     const bool diag = !FULL && bi == bj;         /* both operands are the same panel */
-#if DFJK_K2_TILE_FASTEST
-    const int split = blockIdx.y;
-#else
     const int split = blockIdx.x;
-#endif
     const int64_t mu0 = (int64_t)bi * K2_T, nu0 = (int64_t)bj * K2_T;
 
     /* this split's share of the k groups (4 columns each) of the set */
     const int64_t ng = np * n4s;
     const int64_t gbeg = ng * split / nsplit, gend = ng * (split + 1) / nsplit;
     const int nk = (int)((gend - gbeg + K2_KG - 1) / K2_KG);
-    /* The tiles of one split walk the same k range at the same pace.  Started at the same k they
-     * would all ask the same few L2 slices for the same 4 KB panels at the same instant; each tile
-     * therefore starts its (cyclic) walk bi + bj stages in, which spreads the tiles that share a
-     * panel over neighbouring stages: same L2 reuse a few microseconds apart, no hot slice. */
-    const int rot = DFJK_K2_ROTATE && nk > 0 ? (bi + bj) % nk : 0;
 
     const uint32_t smem_base = smem_u32(smem_raw);
     const uint32_t bar_base = smem_base + K2_STAGES * K2_STAGE_BYTES;
@@ -148,8 +128,7 @@ k2_syrk_lower_kernel(const double *__restrict__ X4, int64_t nao, int64_t np, int
                 const int slot = kc % K2_STAGES;
                 const int round = kc / K2_STAGES;
                 if (round > 0) mbar_wait(empty_bar(slot), (round - 1) & 1);
-                const int kk = kc + rot < nk ? kc + rot : kc + rot - nk;
-                const int64_t g0 = gbeg + K2_KG * (int64_t)kk;
+                const int64_t g0 = gbeg + K2_KG * (int64_t)kc;
                 const int n = (int)((gend - g0 < K2_KG) ? gend - g0 : K2_KG);
                 const uint32_t bytes = (uint32_t)(n * 32 * (rows_a + (diag ? 0 : rows_b)));
                 mbar_arrive_expect_tx(full_bar(slot), bytes);
@@ -203,8 +182,7 @@ k2_syrk_lower_kernel(const double *__restrict__ X4, int64_t nao, int64_t np, int
         const int slot = kc % K2_STAGES;
         mbar_wait(full_bar(slot), (kc / K2_STAGES) & 1);
         if (warp_active) {
-            const int kk = kc + rot < nk ? kc + rot : kc + rot - nk;
-            const int64_t g0 = gbeg + K2_KG * (int64_t)kk;
+            const int64_t g0 = gbeg + K2_KG * (int64_t)kc;
             const int n = (int)((gend - g0 < K2_KG) ? gend - g0 : K2_KG);
             const double *Xa = reinterpret_cast<const double *>(smem_raw + slot * K2_STAGE_BYTES);
             const double *Xb = diag ? Xa : Xa + K2_OP_BYTES / 8;
@@ -786,8 +764,7 @@ cudaError_t launch_k2_syrk_lower(const double *X4, int64_t nao, int64_t np, int6
     const int nb = (int)((nao + K2_T - 1) / K2_T);
     const int ntile = nb * (nb + 1) / 2;
     const int n4s = (int)((ncol + 3) / 4);              /* k step 4: Ccat's padding to 8 is not read */
-    const dim3 grid = DFJK_K2_TILE_FASTEST ? dim3((unsigned)ntile, (unsigned)nsplit) : dim3((unsigned)nsplit, (unsigned)ntile);
-    k2_syrk_lower_kernel<false><<<grid, K2_THREADS, K2_SMEM_BYTES, st>>>(
+    k2_syrk_lower_kernel<false><<<dim3((unsigned)nsplit, (unsigned)ntile), K2_THREADS, K2_SMEM_BYTES, st>>>(
         X4, nao, np, ldc / 4, col0 / 4, col0 / 4, n4s, Kpart, nsplit, accumulate);
     return cudaPeekAtLastError();
 }
@@ -801,8 +778,7 @@ cudaError_t launch_k2_gemm_full(const double *X4, int64_t nao, int64_t np, int64
     if (e != cudaSuccess) return e;
     const int nb = (int)((nao + K2_T - 1) / K2_T);
     const int n4s = (int)((ncol + 3) / 4);
-    const dim3 grid = DFJK_K2_TILE_FASTEST ? dim3((unsigned)(nb * nb), (unsigned)nsplit) : dim3((unsigned)nsplit, (unsigned)(nb * nb));
-    k2_syrk_lower_kernel<true><<<grid, K2_THREADS, K2_SMEM_BYTES, st>>>(
+    k2_syrk_lower_kernel<true><<<dim3((unsigned)nsplit, (unsigned)(nb * nb)), K2_THREADS, K2_SMEM_BYTES, st>>>(
         X4, nao, np, ldc / 4, col0a / 4, col0b / 4, n4s, Kpart, nsplit, accumulate);
     return cudaPeekAtLastError();
 }
