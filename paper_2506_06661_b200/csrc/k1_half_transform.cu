@@ -73,6 +73,9 @@ __device__ __forceinline__ int k1_mode(int64_t mu0, int64_t nu0, int64_t nao, bo
     if (nu0 + K1_KC - 1 <= mu0) return K1_MODE_ROW;            /* every nu <= every mu */
     if (nu0 >= mu0 + K1_M - 1 && !(last_p && nu0 + K1_KC >= nao))
         return K1_MODE_COL;                                    /* every nu >= every mu */
+#ifdef DFJK_EXP_NOGATHER
+    return K1_MODE_ROW;
+#endif
     return K1_MODE_GATHER;    /* crosses the diagonal (or would read past the end of B) */
 }
 
@@ -81,13 +84,21 @@ __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
     asm volatile("mbarrier.expect_tx.relaxed.cta.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
 
+#ifdef DFJK_K1_DBG
+__device__ long long k1_dbg[148 * 8 * 4];
+#endif
+
 template <int NT8>
 struct K1Cfg {
     static constexpr int NW = 8 * NT8;
     static constexpr int C_BYTES = K1_KC * NW * 8;
     static constexpr int STAGE_BYTES = K1_A_BYTES + C_BYTES;
     static constexpr int STAGES_RAW = K1_SMEM_BUDGET / STAGE_BYTES;
+#ifdef DFJK_K1_MAXSTAGES
+    static constexpr int STAGES = STAGES_RAW > DFJK_K1_MAXSTAGES ? DFJK_K1_MAXSTAGES : STAGES_RAW;
+#else
     static constexpr int STAGES = STAGES_RAW > 8 ? 8 : STAGES_RAW;
+#endif
     static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 2 * STAGES * 8 + 16;
 };
 
@@ -214,6 +225,9 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
         const int lq = lane >> 2, lr = lane & 3;
         int slot = 0;
         uint32_t phase = 0;
+#ifdef DFJK_K1_DBG
+        long long dbg_wait = 0, dbg_n = 0, dbg_slow = 0, dbg_t0 = clock64();
+#endif
         for (int64_t item = blockIdx.x; item < nitems; item += gridDim.x) {
         const int64_t p = item / items_per_p;
         const int rem = (int)(item - p * items_per_p);
@@ -240,7 +254,16 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
         const int jb = sstep >= rbi ? sstep - rbi : sstep - rbi + nib;
         const int kc_end = (jb + 1) * (K1_M / K1_KC) < nk ? (jb + 1) * (K1_M / K1_KC) : nk;
         for (int kc = jb * (K1_M / K1_KC); kc < kc_end; ++kc) {
+#ifdef DFJK_K1_DBG
+            {
+                const long long t0 = clock64();
+                mbar_wait(full_bar(slot), phase);
+                const long long dt = clock64() - t0;
+                dbg_wait += dt; ++dbg_n; if (dt > 200) ++dbg_slow;
+            }
+#else
             mbar_wait(full_bar(slot), phase);
+#endif
             if (warp_active) {
                 const double *As = reinterpret_cast<const double *>(smem_raw + slot * Cfg::STAGE_BYTES);
                 const double *Cs = As + K1_A_BYTES / 8;
@@ -278,7 +301,11 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
         }
         }   /* column blocks */
 
+#ifdef DFJK_EXP_NOEPI
+        if (warp_active && acc[0][0][0] == 123.456) {
+#else
         if (warp_active) {
+#endif
 #pragma unroll
             for (int mt = 0; mt < 2; ++mt) {
                 const int64_t mu = mu0 + row_w + 8 * mt + lq;
@@ -295,6 +322,12 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
             }
         }
         }   /* items */
+#ifdef DFJK_K1_DBG
+        if (lane == 0 && blockIdx.x < 148) {
+            long long *d = k1_dbg + (blockIdx.x * 8 + cw) * 4;
+            d[0] = dbg_wait; d[1] = dbg_n; d[2] = dbg_slow; d[3] = clock64() - dbg_t0;
+        }
+#endif
     }
 }
 
@@ -344,6 +377,10 @@ cudaError_t k1_launch_t(const double *B, int64_t naux, int64_t nao, int64_t npai
 }
 
 }  // namespace
+
+#ifdef DFJK_K1_DBG
+extern "C" int dfjk_dbg_k1(long long *out) { return (int)cudaMemcpyFromSymbol(out, k1_dbg, sizeof(long long) * 148 * 8 * 4); }
+#endif
 
 cudaError_t launch_k1_half_transform(const double *B, int64_t naux, int64_t nao, int64_t npair, int64_t P0,
                                      int64_t np, const double *Ccat4, int64_t ldc, int64_t ldx, double *X4,

@@ -124,6 +124,8 @@ k2_syrk_lower_kernel(const double *__restrict__ X4, int64_t nao, int64_t np, int
         if (lane == 0) {
             const int64_t rows_a = (nao - mu0 < K2_T) ? nao - mu0 : K2_T;
             const int64_t rows_b = (nao - nu0 < K2_T) ? nao - nu0 : K2_T;
+            int64_t gp = gbeg / n4s;                      /* (g / n4s, g % n4s), kept incrementally */
+            int gi = (int)(gbeg - gp * n4s);
             for (int kc = 0; kc < nk; ++kc) {
                 const int slot = kc % K2_STAGES;
                 const int round = kc / K2_STAGES;
@@ -134,8 +136,8 @@ k2_syrk_lower_kernel(const double *__restrict__ X4, int64_t nao, int64_t np, int
                 mbar_arrive_expect_tx(full_bar(slot), bytes);
                 const uint32_t dst = smem_base + slot * K2_STAGE_BYTES;
                 for (int q = 0; q < n; ++q) {
-                    const int64_t g = g0 + q;
-                    const int64_t kg = (g / n4s) * ldc4 + col04 + g % n4s;     /* k-group in X4 */
+                    const int64_t kg = gp * ldc4 + col04 + gi;                 /* k-group in X4 */
+                    if (++gi == n4s) { gi = 0; ++gp; }
                     const double *src = X4 + kg * nao * 4;
                     bulk_g2s(dst + q * (K2_T * 32), src + mu0 * 4, (uint32_t)(rows_a * 32), full_bar(slot));
                     if (!diag) {
@@ -336,7 +338,7 @@ struct K2PArgs {
 };
 
 constexpr int K2P_THREADS = 128 + 32 * K2_CONSUMER_WARPS;     /* producer warpgroup + 8 consumer warps */
-constexpr int K2P_SMEM_BYTES = K2_STAGES * K2_STAGE_BYTES + 2 * K2_STAGES * 8 + 4 * 8 + 2 * 8 + 16;
+constexpr int K2P_SMEM_BYTES = K2_STAGES * K2_STAGE_BYTES + 2 * K2_STAGES * 8 + 6 * 8 + 2 * 8 + 16;
 
 __device__ __forceinline__ int ld_acquire_gpu(const int *p)
 {
@@ -363,54 +365,48 @@ __device__ __forceinline__ void k2p_decode(int t, int nb, int &bi, int &bj)
     }
 }
 
+/* fire-and-forget FP64 add at L2 (SASS RED.E.ADD.F64): no load, no round trip */
+__device__ __forceinline__ void red_add_f64(double *p, double v)
+{
+    asm volatile("red.relaxed.gpu.global.add.f64 [%0], %1;" ::"l"(p), "d"(v) : "memory");
+}
+
 /* NR rows (8 apart) of the warp tile at once:  row_r[8 nt + {0,1}] (+)= acc[r * AST + nt][{0,1}],
  * nt < NNT, for the rows r with mu_first + 8 r < nao and the columns nu_first + 8 nt + {0,1} < nao.
- * ALL loads of the NR rows are issued before the first store: one L2 round trip per batch. */
+ * The first item of a (slab, tile) stores, every later one adds with `red` at L2: the consumers
+ * never wait for a slab line to come back, and since the items of one (slab, tile) are chained by
+ * its release/acquire counter each address still receives its adds in panel order => the sum is
+ * the same on every run.  (The load-add-store version idled the FP64 pipe ~3 us per item.) */
 template <int NNT, int NR, int AST>
 __device__ __forceinline__ void k2p_add_rows(const double (*acc)[2], double *row, int64_t mu_first,
                                              int64_t nu_first, int64_t nao, bool overwrite, bool vec)
 {
-    double v0[NR][NNT], v1[NR][NNT];
-#pragma unroll
-    for (int r = 0; r < NR; ++r)
-#pragma unroll
-        for (int nt = 0; nt < NNT; ++nt) v0[r][nt] = v1[r][nt] = 0.0;
-    if (!overwrite) {
-#pragma unroll
-        for (int r = 0; r < NR; ++r) {
-            if (mu_first + 8 * r >= nao) continue;
-            const double *rp = row + (int64_t)8 * r * nao;
-#pragma unroll
-            for (int nt = 0; nt < NNT; ++nt) {
-                if (vec) {
-                    if (nu_first + 8 * nt < nao) {
-                        const double2 t = __ldcg(reinterpret_cast<const double2 *>(rp + 8 * nt));
-                        v0[r][nt] = t.x; v1[r][nt] = t.y;
-                    }
-                } else {
-                    if (nu_first + 8 * nt < nao) v0[r][nt] = __ldcg(rp + 8 * nt);
-                    if (nu_first + 8 * nt + 1 < nao) v1[r][nt] = __ldcg(rp + 8 * nt + 1);
-                }
-            }
-        }
-    }
 #pragma unroll
     for (int r = 0; r < NR; ++r) {
         if (mu_first + 8 * r >= nao) continue;
         double *rp = row + (int64_t)8 * r * nao;
 #pragma unroll
         for (int nt = 0; nt < NNT; ++nt) {
-            const double r0 = v0[r][nt] + acc[r * AST + nt][0], r1 = v1[r][nt] + acc[r * AST + nt][1];
-            if (vec) {
-                if (nu_first + 8 * nt < nao)              /* nao and nu even: the pair is inside */
-                    *reinterpret_cast<double2 *>(rp + 8 * nt) = make_double2(r0, r1);
+            const double r0 = acc[r * AST + nt][0], r1 = acc[r * AST + nt][1];
+            if (overwrite) {
+                if (vec) {
+                    if (nu_first + 8 * nt < nao)              /* nao and nu even: the pair is inside */
+                        *reinterpret_cast<double2 *>(rp + 8 * nt) = make_double2(r0, r1);
+                } else {
+                    if (nu_first + 8 * nt < nao) rp[8 * nt] = r0;
+                    if (nu_first + 8 * nt + 1 < nao) rp[8 * nt + 1] = r1;
+                }
             } else {
-                if (nu_first + 8 * nt < nao) rp[8 * nt] = r0;
-                if (nu_first + 8 * nt + 1 < nao) rp[8 * nt + 1] = r1;
+                if (nu_first + 8 * nt < nao) red_add_f64(rp + 8 * nt, r0);
+                if (nu_first + 8 * nt + 1 < nao) red_add_f64(rp + 8 * nt + 1, r1);
             }
         }
     }
 }
+
+#ifdef DFJK_K2_DBG
+__device__ long long k2_dbg[148 * 8 * 8];
+#endif
 
 template <bool FULL>
 __global__ void __launch_bounds__(K2P_THREADS, 1)
@@ -428,7 +424,8 @@ k2p_kernel(const K2PArgs a)
     auto empty_bar = [&](int s) { return bar_base + 8u * (K2_STAGES + s); };
     auto item_full = [&](int s) { return bar_base + 8u * (2 * K2_STAGES + s); };
     auto item_empty = [&](int s) { return bar_base + 8u * (2 * K2_STAGES + 2 + s); };
-    volatile int *item_id = reinterpret_cast<volatile int *>(smem_raw + K2_STAGES * K2_STAGE_BYTES + 8 * (2 * K2_STAGES + 4));
+    auto item_done = [&](int s) { return bar_base + 8u * (2 * K2_STAGES + 4 + s); };
+    volatile int *item_id = reinterpret_cast<volatile int *>(smem_raw + K2_STAGES * K2_STAGE_BYTES + 8 * (2 * K2_STAGES + 6));
     if (tid == 0) {
         for (int s = 0; s < K2_STAGES; ++s) {
             mbar_init(full_bar(s), 1);
@@ -436,7 +433,8 @@ k2p_kernel(const K2PArgs a)
         }
         for (int s = 0; s < 2; ++s) {
             mbar_init(item_full(s), 1);
-            mbar_init(item_empty(s), K2_CONSUMER_WARPS);
+            mbar_init(item_empty(s), K2_CONSUMER_WARPS + 1);       /* consumers + the releaser */
+            mbar_init(item_done(s), K2_CONSUMER_WARPS);
         }
         mbar_fence_init();
     }
@@ -464,6 +462,10 @@ k2p_kernel(const K2PArgs a)
                 const int64_t rows_b = (nao - nu0 < K2_T) ? nao - nu0 : K2_T;
                 const int64_t gbeg = ng * p / a.npanel, gend = ng * (p + 1) / a.npanel;
                 const int nk = (int)((gend - gbeg + K2_KG - 1) / K2_KG);
+                /* (gp, gi) = (g / n4s, g % n4s) of the running k-group g, kept incrementally: the lane
+                 * must issue a stage faster than the consumers eat it (2048 cycles on a 32-row tile) */
+                int64_t gp = gbeg / a.n4s;
+                int gi = (int)(gbeg - gp * a.n4s);
                 for (int kc = 0; kc < nk; ++kc, ++st) {
                     const int slot = st % K2_STAGES;
                     const int round = st / K2_STAGES;
@@ -474,8 +476,8 @@ k2p_kernel(const K2PArgs a)
                     mbar_arrive_expect_tx(full_bar(slot), bytes);
                     const uint32_t dst = smem_base + slot * K2_STAGE_BYTES;
                     for (int q = 0; q < n; ++q) {
-                        const int64_t g = g0 + q;
-                        const int64_t kg = (g / a.n4s) * a.ldc4 + a.col04 + g % a.n4s;   /* k-group in X4 */
+                        const int64_t kg = gp * a.ldc4 + a.col04 + gi;                   /* k-group in X4 */
+                        if (++gi == a.n4s) { gi = 0; ++gp; }
                         const double *src = a.X4 + kg * nao * 4;
                         bulk_g2s(dst + q * (K2_T * 32), src + mu0 * 4, (uint32_t)(rows_a * 32), full_bar(slot));
                         if (!diag) {
@@ -485,6 +487,21 @@ k2p_kernel(const K2PArgs a)
                         }
                     }
                 }
+            }
+        } else if (warp == 1 && lane == 0) {
+            /* ---------------------------------------------------------- releaser: publishes an item
+             * once all eight consumer warps have issued its adds (item_done).  The consumers arrive and
+             * go straight on to the next item; the gpu-scope release below is cumulative over what the
+             * mbarrier made visible to this thread, i.e. it waits for the adds, not the consumers. */
+            for (int ir = 0;; ++ir) {
+                const int is = ir & 1;
+                mbar_wait(item_full(is), (ir >> 1) & 1);
+                const int item = item_id[is];
+                mbar_arrive(item_empty(is));
+                if (item < 0) break;
+                const int p = item / a.ntile, t = item - p * a.ntile;
+                mbar_wait(item_done(is), (ir >> 1) & 1);
+                st_release_gpu(a.work + 1 + (p % a.nslab) * a.ntile + t, p / a.nslab + 1);
             }
         }
         return;
@@ -498,9 +515,16 @@ k2p_kernel(const K2PArgs a)
     const int tr = (cw < 2 || cw == 4) ? 3 : (cw < 4 ? 2 : (cw < 7 ? 1 : 0));
     const int tc0 = (cw == 1 || cw == 3) ? 3 : (cw == 4 ? 6 : (cw == 6 ? 2 : 0));
     int st = 0;
+#ifdef DFJK_K2_DBG
+    long long dbg[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    const long long dbg_t0 = clock64();
+#define DBG_T(i, stmt) { const long long t0_ = clock64(); stmt; dbg[i] += clock64() - t0_; }
+#else
+#define DBG_T(i, stmt) { stmt; }
+#endif
     for (int ir = 0;; ++ir) {
         const int is = ir & 1;
-        mbar_wait(item_full(is), (ir >> 1) & 1);
+        DBG_T(0, mbar_wait(item_full(is), (ir >> 1) & 1));
         const int item = item_id[is];
         __syncwarp();
         if (lane == 0) mbar_arrive(item_empty(is));
@@ -528,7 +552,10 @@ k2p_kernel(const K2PArgs a)
 
         for (int kc = 0; kc < nk; ++kc, ++st) {
             const int slot = st % K2_STAGES;
-            mbar_wait(full_bar(slot), (st / K2_STAGES) & 1);
+            DBG_T(1, mbar_wait(full_bar(slot), (st / K2_STAGES) & 1));
+#ifdef DFJK_K2_DBG
+            ++dbg[2];
+#endif
             if (warp_active) {
                 const int64_t g0 = gbeg + K2_KG * (int64_t)kc;
                 const int n = (int)((gend - g0 < K2_KG) ? gend - g0 : K2_KG);
@@ -630,18 +657,19 @@ k2p_kernel(const K2PArgs a)
         const int slab = p % a.nslab, seq = p / a.nslab;
         int *flag = a.work + 1 + slab * a.ntile + t;
         const bool overwrite = seq == 0 && !a.accumulate;
+#ifdef DFJK_K2_DBG
+        const long long dbg_ta = clock64();
+        ++dbg[6];
+#endif
         if (warp_active) {
             if (seq > 0) {
-                if (lane == 0) while (ld_acquire_gpu(flag) < seq) { }
+                DBG_T(3, if (lane == 0) while (ld_acquire_gpu(flag) < seq) { }
                 __syncwarp();
-                (void)ld_acquire_gpu(flag);              /* every lane orders its loads after the flag */
+                (void)ld_acquire_gpu(flag));              /* every lane orders its adds after the flag */
             }
             double *Kp = a.Kpart + (int64_t)slab * nao * nao;
-            /* The adds are batched: all loads of a batch (one 8-row MMA row of the warp tile, 4-6
-             * column pairs) are issued before the first store, so an item pays a handful of L2 round
-             * trips instead of one per element (a plain load-add-store loop cost ~20 us per item: the
-             * compiler must keep each load behind the previous store).  16-byte accesses when the row
-             * pitch allows (nao even), else element-wise. */
+            /* first item of the (slab, tile): 16-byte stores when the row pitch allows (nao even);
+             * later ones: `red` adds, ordered behind the previous item by the flag (k2p_add_rows) */
             const bool vec = (nao & 1) == 0;
             const int64_t nu_first = nu0 + col_w + 2 * lr;
             double *row0 = Kp + (mu0 + row_w + lq) * nao + nu_first;
@@ -662,12 +690,17 @@ k2p_kernel(const K2PArgs a)
                 k2p_add_rows<4, 4, 4>(&acc[16], row0 + 32 * nao, mu_first + 32, nu_first, nao, overwrite, vec);
             }
         }
-        /* all eight consumer warps (the idle ones too) meet, then one thread publishes the item: the
-         * barrier orders every warp's stores before the gpu-scope release store (release is cumulative
-         * over what the barrier made visible to the releasing thread), no per-thread fence needed */
-        asm volatile("bar.sync 1, %0;" ::"n"(32 * K2_CONSUMER_WARPS) : "memory");
-        if (cw == 0 && lane == 0) st_release_gpu(flag, seq + 1);
+        /* every consumer warp (the idle ones too) reports its adds issued and moves on; the releaser
+         * warp publishes the item (no CTA-wide barrier, no consumer waits for the adds to land) */
+        __syncwarp();
+        DBG_T(5, if (lane == 0) mbar_arrive(item_done(is)));
     }
+#ifdef DFJK_K2_DBG
+    if (lane == 0 && blockIdx.x < 148) {
+        dbg[7] = clock64() - dbg_t0;
+        for (int i = 0; i < 8; ++i) k2_dbg[(blockIdx.x * 8 + cw) * 8 + i] = dbg[i];
+    }
+#endif
 }
 
 /* ------------------------------------------------------------------ K3 */
@@ -738,6 +771,10 @@ k3_sum_kernel(const double *__restrict__ Kpart, int nsplit, int64_t n2, double *
 
 }  // namespace
 
+#ifdef DFJK_K2_DBG
+extern "C" int dfjk_dbg_k2(long long *out) { return (int)cudaMemcpyFromSymbol(out, k2_dbg, sizeof(long long) * 148 * 8 * 8); }
+#endif
+
 void launch_k0_pack_c(const double *const *C, const int *nocc, const int *col0, int nset, int64_t nao,
                       int64_t ldc, double *Ccat, double *const *outs, double **out_slots, cudaStream_t st)
 {
@@ -792,7 +829,10 @@ void k2p_plan(int64_t nao, int64_t ng, int ntile, int sm_count, int max_slabs, i
     /* L2: one panel of X (all nao rows) is about panel_bytes */
     int64_t len = panel_bytes / (nao * 32 * K2_KG);
     /* balance: at least ~30 items per SM when the problem is big enough for that */
-    const int64_t len_bal = stages_total * ntile / (30LL * sm_count);
+#ifndef DFJK_K2P_ITEMS_PER_SM
+#define DFJK_K2P_ITEMS_PER_SM 30
+#endif
+    const int64_t len_bal = stages_total * ntile / ((int64_t)DFJK_K2P_ITEMS_PER_SM * sm_count);
     if (len > len_bal) len = len_bal;
     if (len < 8) len = 8;                                 /* the 128 KB read-modify-write must amortise */
     if (len > stages_total) len = stages_total > 0 ? stages_total : 1;
