@@ -401,17 +401,24 @@ j3_unpack_kernel(const double *__restrict__ Jp_part, int64_t ngroup, int64_t npa
     __shared__ double t[J3_T][J3_T + 1];
     const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
     const int64_t mu0 = (int64_t)bi * J3_T, nu0 = (int64_t)bj * J3_T;
+    /* the four rows of a thread are summed side by side, eight groups per round, so that 32 loads are
+     * in flight at once (one row after the other was a chain of L2 round trips: 29 us at nao = 290);
+     * each element still adds its groups in ascending order */
+    const double *src[4];
+    double v[4];
 #pragma unroll
     for (int r = 0; r < 4; ++r) {
-        const int row = ty + 8 * r;
-        const int64_t mu = mu0 + row, nu = nu0 + tx;
-        double v = 0.0;
-        if (mu < nao && nu <= mu) {
-            const int64_t pair = mu * (mu + 1) / 2 + nu;
-            for (int64_t g = 0; g < ngroup; ++g) v += Jp_part[g * npair + pair];
-        }
-        t[row][tx] = v;
+        const int64_t mu = mu0 + ty + 8 * r, nu = nu0 + tx;
+        src[r] = (mu < nao && nu <= mu) ? Jp_part + mu * (mu + 1) / 2 + nu : nullptr;
+        v[r] = 0.0;
     }
+#pragma unroll 8
+    for (int g = 0; g < (int)ngroup; ++g)
+#pragma unroll
+        for (int r = 0; r < 4; ++r)
+            if (src[r]) v[r] += src[r][(int64_t)g * npair];
+#pragma unroll
+    for (int r = 0; r < 4; ++r) t[ty + 8 * r][tx] = v[r];
     __syncthreads();
 #pragma unroll
     for (int r = 0; r < 4; ++r) {

@@ -65,18 +65,16 @@ constexpr int K1_SMEM_BUDGET = 220 * 1024;
  * times per build at nao = 1600 and 1.01 times at nao = 800 instead of 1.44 (ncu r01e / r02).
  * L2 eviction hints on top of this made it worse. */
 
-enum { K1_MODE_ROW = 0, K1_MODE_COL = 1, K1_MODE_GATHER = 2 };
+enum { K1_MODE_ROW = 0, K1_MODE_COL = 1, K1_MODE_GATHER = 2, K1_MODE_DIAG = 3 };
 
 /* which form stage kc of row block mu0 takes; identical on producer and consumer side */
 __device__ __forceinline__ int k1_mode(int64_t mu0, int64_t nu0, int64_t nao, bool last_p)
 {
-    if (nu0 + K1_KC - 1 <= mu0) return K1_MODE_ROW;            /* every nu <= every mu */
-    if (nu0 >= mu0 + K1_M - 1 && !(last_p && nu0 + K1_KC >= nao))
-        return K1_MODE_COL;                                    /* every nu >= every mu */
-#ifdef DFJK_EXP_NOGATHER
-    return K1_MODE_ROW;
-#endif
-    return K1_MODE_GATHER;    /* crosses the diagonal (or would read past the end of B) */
+    if (nu0 < mu0) return K1_MODE_ROW;                         /* every nu <= every mu (32 | 128 aligned) */
+    if (nu0 < mu0 + K1_M)                                      /* inside the diagonal block */
+        return nu0 + K1_KC <= nao ? K1_MODE_DIAG : K1_MODE_GATHER;   /* (ragged last stage: zero fill) */
+    if (!(last_p && nu0 + K1_KC >= nao)) return K1_MODE_COL;   /* every nu >= every mu */
+    return K1_MODE_GATHER;                                     /* a bulk copy would read past the end of B */
 }
 
 __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
@@ -190,6 +188,53 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
                         reinterpret_cast<double *>(smem_raw + slot * Cfg::STAGE_BYTES)[k * K1_LDT + c] = 0.0;
                 if (my_bytes) mbar_arrive_expect_tx(bar, my_bytes); else mbar_arrive(bar);
                 if (ok) bulk_g2s(a_dst + tid * (K1_LDT * 8), B + (e - sft), nb, bar);
+            } else if (mode == K1_MODE_DIAG) {
+                /* A stage inside the diagonal block, R0 = nu0 - mu0 in {0, 32, 64, 96}: three bands of rows.
+                 *   m <  R0      : every nu > mu -> "col" form, 32 copies of R0 doubles (packed rows nu0+k),
+                 *                  pitch R0 + 4, at the start of the stage buffer (it ends below row R0 of
+                 *                  the "row" form: 32 (R0 + 4) 8 <= R0 36 8)
+                 *   m >= R0 + 32 : every nu < mu -> "row" form, one copy of 32 doubles per row
+                 *   the 32 x 32 block on the diagonal: element-wise (8-byte cp.async, zero fill outside)
+                 * so 1024 instead of 4096 gathered elements per stage (they cost 16 % of K1 at nao = 290). */
+                const int R0 = (int)(nu0 - mu0);
+                uint32_t nbytes = tid == 0 ? c_bytes : 0u;
+                if (tid >= R0 + K1_KC) {
+                    const int64_t mu = mu0 + tid;
+                    if (mu < nao) {
+                        const int64_t e = pb + mu * (mu + 1) / 2 + nu0;
+                        const int sft = (int)(e & 1);
+                        const uint32_t nb = (uint32_t)(K1_KC + 2 * sft) * 8u;
+                        nbytes += nb;
+                        mbar_expect_tx(bar, nbytes);
+                        bulk_g2s(a_dst + tid * (K1_LDD * 8), B + (e - sft), nb, bar);
+                        nbytes = 0;
+                    }
+                } else if (tid < K1_KC && R0 > 0) {           /* nu0 + 31 < nao in this mode */
+                    const int64_t nu = nu0 + tid;
+                    const int64_t e = pb + nu * (nu + 1) / 2 + mu0;
+                    const int sft = (int)(e & 1);
+                    const uint32_t nb = (uint32_t)((R0 + sft + 1) & ~1) * 8u;
+                    nbytes += nb;
+                    mbar_expect_tx(bar, nbytes);
+                    bulk_g2s(a_dst + tid * ((R0 + 4) * 8), B + (e - sft), nb, bar);
+                    nbytes = 0;
+                }
+                if (nbytes) mbar_expect_tx(bar, nbytes);       /* thread 0 without a copy of its own */
+                {
+                    const int k = tid & 31;
+                    const int64_t nu = nu0 + k;
+                    const int64_t tri_nu = nu * (nu + 1) / 2;
+#pragma unroll
+                    for (int r = 0; r < K1_KC / 4; ++r) {
+                        const int m = R0 + 4 * r + (tid >> 5);
+                        const int64_t mu = mu0 + m;
+                        const bool ok = nu < nao && mu < nao;
+                        const int64_t off = mu >= nu ? mu * (mu + 1) / 2 + nu : tri_nu + mu;
+                        const int sd = (((m & 3) == 1 || (m & 3) == 2) ? 1 : 0) ^ pbpar;
+                        cp_async8(a_dst + (m * K1_LDD + k + sd) * 8, ok ? Bp + off : Bp, ok);
+                    }
+                }
+                cp_async_mbar_arrive_noinc(bar);
             } else {
                 /* element-wise gather into the "row" form (8-byte cp.async, zero fill outside) */
                 if (tid == 0) mbar_expect_tx(bar, c_bytes);
@@ -267,10 +312,14 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
             if (warp_active) {
                 const double *As = reinterpret_cast<const double *>(smem_raw + slot * Cfg::STAGE_BYTES);
                 const double *Cs = As + K1_A_BYTES / 8;
-                const bool colform = k1_mode(mu0, (int64_t)kc * K1_KC, nao, last_p) == K1_MODE_COL;
-                const double *a_base = colform ? As + lr * K1_LDT + row_w + lq + st_shift
+                /* "col" form: COL stages, and the rows above the diagonal of a DIAG stage (pitch R0 + 4) */
+                const int mode = k1_mode(mu0, (int64_t)kc * K1_KC, nao, last_p);
+                const int R0 = (int)((int64_t)kc * K1_KC - mu0);
+                const bool colform = mode == K1_MODE_COL || (mode == K1_MODE_DIAG && row_w < R0);
+                const int ldt = mode == K1_MODE_COL ? K1_LDT : R0 + 4;
+                const double *a_base = colform ? As + lr * ldt + row_w + lq + st_shift
                                                : As + (row_w + lq) * K1_LDD + lr + sd_shift;
-                const int a_gstep = colform ? 4 * K1_LDT : 4;        /* next k-group */
+                const int a_gstep = colform ? 4 * ldt : 4;           /* next k-group */
                 const int a_mstep = colform ? 8 : 8 * K1_LDD;        /* next 8 rows */
                 const double *b_base = Cs + lq * 4 + lr;
                 if (!half) {

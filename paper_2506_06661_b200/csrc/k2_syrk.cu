@@ -67,6 +67,67 @@ constexpr int K2_CONSUMER_WARPS = 8;
 constexpr int K2_THREADS = 32 * (1 + K2_CONSUMER_WARPS);
 constexpr int K2_SMEM_BYTES = K2_STAGES * K2_STAGE_BYTES + 2 * K2_STAGES * 8 + 16;
 
+/* Triangular layout of a full-height DIAGONAL tile: the lower triangle in units of 16 x 16 (2 x 2
+ * MMA tiles), strip r (rows 16r .. 16r+15) holding the units c = 0 .. r -- 36 units = 144 MMA tiles
+ * where the square has 256 (an earlier 32 x 16 unit layout issued 192).  Warps 0-3 take five units
+ * each, all in one strip (strip 7 - cw, c = 0 .. 4: a 16 x 80 warp tile); warps 4-7 take the other
+ * sixteen, four each, as listed below.  The two warps of a sub-partition (cw, cw + 4) hold 5 + 4. */
+__device__ __forceinline__ void tri_unit(int j, int u, int &r, int &c)      /* j = cw - 4, u < 4 */
+{
+    /* j = 0: (7,5) (7,6) (7,7) (0,0);  1: (6,5) (6,6) (1,0) (1,1);  2: (5,5) (2,0) (2,1) (2,2);  3: (3,0..3) */
+    const unsigned rows = j == 0 ? 0x0777u : (j == 1 ? 0x1166u : (j == 2 ? 0x2225u : 0x3333u));
+    const unsigned cols = j == 0 ? 0x0765u : (j == 1 ? 0x1065u : (j == 2 ? 0x2105u : 0x3210u));
+    r = (int)((rows >> (4 * u)) & 15u);
+    c = (int)((cols >> (4 * u)) & 15u);
+}
+
+/* one stage (n <= 8 k-groups) of a diagonal tile for a warp of the wide kind (cw < 4): acc[mt * 10 + nt] */
+__device__ __forceinline__ void tri_stage_wide(double (*acc)[2], const double *a_base, const double *b_base, int n)
+{
+#pragma unroll
+    for (int q = 0; q < K2_KG; ++q) {
+        if (q < n) {
+            double a[2], b[10];
+#pragma unroll
+            for (int mt = 0; mt < 2; ++mt) a[mt] = a_base[q * (K2_T * 4) + mt * 32];
+#pragma unroll
+            for (int nt = 0; nt < 10; ++nt) b[nt] = b_base[q * (K2_T * 4) + nt * 32];
+#pragma unroll
+            for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+                for (int nt = 0; nt < 10; ++nt)
+                    dmma884(acc[mt * 10 + nt][0], acc[mt * 10 + nt][1], a[mt], b[nt]);
+        }
+    }
+}
+
+/* ... and of the unit kind (cw >= 4): four 16 x 16 units at ua[u] / ub[u] (offsets in doubles into the
+ * panel, lane part included): acc[4 u + 2 mt + nt] */
+__device__ __forceinline__ void tri_stage_units(double (*acc)[2], const double *X, const int (&ua)[4],
+                                                const int (&ub)[4], int n)
+{
+#pragma unroll
+    for (int q = 0; q < K2_KG; ++q) {
+        if (q < n) {
+            double a[4][2], b[4][2];
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+#pragma unroll
+                for (int t = 0; t < 2; ++t) {
+                    a[u][t] = X[ua[u] + q * (K2_T * 4) + t * 32];
+                    b[u][t] = X[ub[u] + q * (K2_T * 4) + t * 32];
+                }
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+#pragma unroll
+                for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+                    for (int nt = 0; nt < 2; ++nt)
+                        dmma884(acc[4 * u + 2 * mt + nt][0], acc[4 * u + 2 * mt + nt][1], a[u][mt], b[u][nt]);
+        }
+    }
+}
+
 /* FULL == false: the SYRK above (one column range, lower tiles only).
  * FULL == true : the general product  Kpart += X[:, range a] X[:, range b]^T  over ALL nb x nb
  *                tiles (K[C1 C2^T] = sum_P (B_P C1)(B_P C2)^T is not symmetric); blockIdx.y is the
@@ -158,25 +219,31 @@ k2_syrk_lower_kernel(const double *__restrict__ X4, int64_t nao, int64_t np, int
      * tiles instead, so all eight warps share the work ("narrow"; CTA-uniform). */
     const bool narrow = nao - mu0 <= 64;
     const int nmt_narrow = nao - mu0 <= 32 ? 4 : 8;      /* 8-row MMA rows of a narrow warp tile in use */
-    /* A full-height diagonal tile needs only its lower triangle: 20 units of 32 x 16 touch it.  They
-     * are dealt 3,3,3,3,2,2,2,2 to the eight warps as 32 x 48 / 32 x 32 warp tiles ("tri"), so the tile
-     * costs 24 instead of 32 DMMAs per warp and k-group (the 2 x 4 layout would leave two warps idle
-     * and the CTA would take as long as an off-diagonal one). */
+    /* A full-height diagonal tile needs only its lower triangle: see tri_unit() ("tri"; the 2 x 4
+     * layout would leave two warps idle and the CTA would take as long as an off-diagonal one). */
     const bool tri = diag && !narrow;
     /* full product only: a tile of the ragged last block COLUMN (<= 64 valid columns) would idle the
      * warps of the right half: 4 (M) x 2 (N) warp tiles of 32 x 32 instead ("tall") */
     const bool tall = FULL && !narrow && nao - nu0 <= 64;
-    const int tr = (cw < 2 || cw == 4) ? 3 : (cw < 4 ? 2 : (cw < 7 ? 1 : 0));   /* 32-row strip */
-    const int tc0 = (cw == 1 || cw == 3) ? 3 : (cw == 4 ? 6 : (cw == 6 ? 2 : 0)); /* first 16-col unit */
     const int wm = narrow ? 0 : cw >> 2, wn = narrow ? cw : cw & 3;
     const int wcols = narrow ? 16 : 32;          /* columns per warp tile (2 x 4 and 1 x 8 layouts) */
     const int lq = lane >> 2, lr = lane & 3;
-    const int row_w = tri ? 32 * tr : (tall ? 32 * (cw >> 1) : 64 * wm);   /* first row / column of this warp's tile */
-    const int col_w = tri ? 16 * tc0 : (tall ? 32 * (cw & 1) : wcols * wn);
+    const int row_w = tri ? 16 * (7 - (cw & 3)) : (tall ? 32 * (cw >> 1) : 64 * wm);   /* first row / column of this warp's tile */
+    const int col_w = tri ? 0 : (tall ? 32 * (cw & 1) : wcols * wn);
+    int ua[4] = {0, 0, 0, 0}, ub[4] = {0, 0, 0, 0};       /* tri, cw >= 4: the four units' panel offsets */
+    if (tri && cw >= 4) {
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            int r, c;
+            tri_unit(cw - 4, u, r, c);
+            ua[u] = (16 * r + lq) * 4 + lr;
+            ub[u] = (16 * c + lq) * 4 + lr;
+        }
+    }
     /* skip warp tiles that lie outside the matrix or strictly above the diagonal */
-    const bool warp_active = (mu0 + row_w < nao) && (nu0 + col_w < nao) &&
-                             !(diag && !tri && col_w > row_w + 63);    /* diag is false when FULL */
-    double acc[32][2];                           /* [mt*4+nt] (8 x 4, or 8 x 2 narrow); tri: [mt*6+nt] (4 x 6) */
+    const bool warp_active = tri || ((mu0 + row_w < nao) && (nu0 + col_w < nao) &&
+                                     !(diag && col_w > row_w + 63));   /* diag is false when FULL */
+    double acc[32][2];                           /* [mt*4+nt] (8 x 4, or 8 x 2 narrow); tri: see tri_stage_* */
 #pragma unroll
     for (int t = 0; t < 32; ++t) acc[t][0] = acc[t][1] = 0.0;
 
@@ -207,39 +274,8 @@ k2_syrk_lower_kernel(const double *__restrict__ X4, int64_t nao, int64_t np, int
                     }
                 }
             } else if (tri) {
-                if (cw < 4) {
-#pragma unroll
-                    for (int q = 0; q < K2_KG; ++q) {
-                        if (q < n) {
-                            double a[4], b[6];
-#pragma unroll
-                            for (int mt = 0; mt < 4; ++mt) a[mt] = a_base[q * (K2_T * 4) + mt * 32];
-#pragma unroll
-                            for (int nt = 0; nt < 6; ++nt) b[nt] = b_base[q * (K2_T * 4) + nt * 32];
-#pragma unroll
-                            for (int mt = 0; mt < 4; ++mt)
-#pragma unroll
-                                for (int nt = 0; nt < 6; ++nt)
-                                    dmma884(acc[mt * 6 + nt][0], acc[mt * 6 + nt][1], a[mt], b[nt]);
-                        }
-                    }
-                } else {
-#pragma unroll
-                    for (int q = 0; q < K2_KG; ++q) {
-                        if (q < n) {
-                            double a[4], b[4];
-#pragma unroll
-                            for (int mt = 0; mt < 4; ++mt) a[mt] = a_base[q * (K2_T * 4) + mt * 32];
-#pragma unroll
-                            for (int nt = 0; nt < 4; ++nt) b[nt] = b_base[q * (K2_T * 4) + nt * 32];
-#pragma unroll
-                            for (int mt = 0; mt < 4; ++mt)
-#pragma unroll
-                                for (int nt = 0; nt < 4; ++nt)
-                                    dmma884(acc[mt * 6 + nt][0], acc[mt * 6 + nt][1], a[mt], b[nt]);
-                        }
-                    }
-                }
+                if (cw < 4) tri_stage_wide(acc, a_base, b_base, n);
+                else tri_stage_units(acc, Xa, ua, ub, n);
             } else if (!narrow) {
 #pragma unroll
                 for (int q = 0; q < K2_KG; ++q) {
@@ -283,18 +319,37 @@ k2_syrk_lower_kernel(const double *__restrict__ X4, int64_t nao, int64_t np, int
     if (!warp_active) return;
     double *Kp = Kpart + (int64_t)split * nao * nao;
     if (tri) {
-        const int ntw = cw < 4 ? 6 : 4;
+        if (cw < 4) {
 #pragma unroll
-        for (int mt = 0; mt < 4; ++mt) {
-            const int64_t mu = mu0 + row_w + 8 * mt + lq;
-            if (mu >= nao) continue;
+            for (int mt = 0; mt < 2; ++mt) {
+                const int64_t mu = mu0 + row_w + 8 * mt + lq;
+                if (mu >= nao) continue;
 #pragma unroll
-            for (int nt = 0; nt < 6; ++nt) {
-                if (nt >= ntw) continue;
-                const int64_t nu = nu0 + col_w + 8 * nt + 2 * lr;
-                double *dst = Kp + mu * nao + nu;
-                if (nu < nao) dst[0] = accumulate ? dst[0] + acc[mt * 6 + nt][0] : acc[mt * 6 + nt][0];
-                if (nu + 1 < nao) dst[1] = accumulate ? dst[1] + acc[mt * 6 + nt][1] : acc[mt * 6 + nt][1];
+                for (int nt = 0; nt < 10; ++nt) {
+                    const int64_t nu = nu0 + 8 * nt + 2 * lr;
+                    double *dst = Kp + mu * nao + nu;
+                    if (nu < nao) dst[0] = accumulate ? dst[0] + acc[mt * 10 + nt][0] : acc[mt * 10 + nt][0];
+                    if (nu + 1 < nao) dst[1] = accumulate ? dst[1] + acc[mt * 10 + nt][1] : acc[mt * 10 + nt][1];
+                }
+            }
+        } else {
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                int r, c;
+                tri_unit(cw - 4, u, r, c);
+#pragma unroll
+                for (int mt = 0; mt < 2; ++mt) {
+                    const int64_t mu = mu0 + 16 * r + 8 * mt + lq;
+                    if (mu >= nao) continue;
+#pragma unroll
+                    for (int nt = 0; nt < 2; ++nt) {
+                        const int64_t nu = nu0 + 16 * c + 8 * nt + 2 * lr;
+                        double *dst = Kp + mu * nao + nu;
+                        const int t = 4 * u + 2 * mt + nt;
+                        if (nu < nao) dst[0] = accumulate ? dst[0] + acc[t][0] : acc[t][0];
+                        if (nu + 1 < nao) dst[1] = accumulate ? dst[1] + acc[t][1] : acc[t][1];
+                    }
+                }
             }
         }
         return;
@@ -511,9 +566,16 @@ k2p_kernel(const K2PArgs a)
     reg_alloc<232>();
     const int cw = warp - 4;
     const int lq = lane >> 2, lr = lane & 3;
-    /* warp tile of the triangular layout (see k2_syrk_lower_kernel) */
-    const int tr = (cw < 2 || cw == 4) ? 3 : (cw < 4 ? 2 : (cw < 7 ? 1 : 0));
-    const int tc0 = (cw == 1 || cw == 3) ? 3 : (cw == 4 ? 6 : (cw == 6 ? 2 : 0));
+    /* this warp's units of the triangular layout (tri_unit) */
+    int ua[4] = {0, 0, 0, 0}, ub[4] = {0, 0, 0, 0}, ur[4] = {0, 0, 0, 0}, uc[4] = {0, 0, 0, 0};
+    if (cw >= 4) {
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            tri_unit(cw - 4, u, ur[u], uc[u]);
+            ua[u] = (16 * ur[u] + lq) * 4 + lr;
+            ub[u] = (16 * uc[u] + lq) * 4 + lr;
+        }
+    }
     int st = 0;
 #ifdef DFJK_K2_DBG
     long long dbg[8] = {0, 0, 0, 0, 0, 0, 0, 0};
@@ -542,10 +604,10 @@ k2p_kernel(const K2PArgs a)
         const bool tall = FULL && !narrow && nao - nu0 <= 64;
         const int wm = narrow ? 0 : cw >> 2, wn = narrow ? cw : cw & 3;
         const int wcols = narrow ? 16 : 32;
-        const int row_w = tri ? 32 * tr : (tall ? 32 * (cw >> 1) : 64 * wm);
-        const int col_w = tri ? 16 * tc0 : (tall ? 32 * (cw & 1) : wcols * wn);
-        const bool warp_active = (mu0 + row_w < nao) && (nu0 + col_w < nao) &&
-                                 !(diag && !tri && col_w > row_w + 63);
+        const int row_w = tri ? 16 * (7 - (cw & 3)) : (tall ? 32 * (cw >> 1) : 64 * wm);
+        const int col_w = tri ? 0 : (tall ? 32 * (cw & 1) : wcols * wn);
+        const bool warp_active = tri || ((mu0 + row_w < nao) && (nu0 + col_w < nao) &&
+                                         !(diag && col_w > row_w + 63));
         double acc[32][2];
 #pragma unroll
         for (int q = 0; q < 32; ++q) acc[q][0] = acc[q][1] = 0.0;
@@ -580,39 +642,8 @@ k2p_kernel(const K2PArgs a)
                         }
                     }
                 } else if (tri) {
-                    if (cw < 4) {
-#pragma unroll
-                        for (int q = 0; q < K2_KG; ++q) {
-                            if (q < n) {
-                                double av[4], bv[6];
-#pragma unroll
-                                for (int mt = 0; mt < 4; ++mt) av[mt] = a_base[q * (K2_T * 4) + mt * 32];
-#pragma unroll
-                                for (int nt = 0; nt < 6; ++nt) bv[nt] = b_base[q * (K2_T * 4) + nt * 32];
-#pragma unroll
-                                for (int mt = 0; mt < 4; ++mt)
-#pragma unroll
-                                    for (int nt = 0; nt < 6; ++nt)
-                                        dmma884(acc[mt * 6 + nt][0], acc[mt * 6 + nt][1], av[mt], bv[nt]);
-                            }
-                        }
-                    } else {
-#pragma unroll
-                        for (int q = 0; q < K2_KG; ++q) {
-                            if (q < n) {
-                                double av[4], bv[4];
-#pragma unroll
-                                for (int mt = 0; mt < 4; ++mt) av[mt] = a_base[q * (K2_T * 4) + mt * 32];
-#pragma unroll
-                                for (int nt = 0; nt < 4; ++nt) bv[nt] = b_base[q * (K2_T * 4) + nt * 32];
-#pragma unroll
-                                for (int mt = 0; mt < 4; ++mt)
-#pragma unroll
-                                    for (int nt = 0; nt < 4; ++nt)
-                                        dmma884(acc[mt * 6 + nt][0], acc[mt * 6 + nt][1], av[mt], bv[nt]);
-                            }
-                        }
-                    }
+                    if (cw < 4) tri_stage_wide(acc, a_base, b_base, n);
+                    else tri_stage_units(acc, Xa, ua, ub, n);
                 } else if (!narrow) {
 #pragma unroll
                     for (int q = 0; q < K2_KG; ++q) {
@@ -676,10 +707,13 @@ k2p_kernel(const K2PArgs a)
             const int64_t mu_first = mu0 + row_w + lq;
             if (tri) {
                 if (cw < 4) {
-                    k2p_add_rows<6, 2, 6>(&acc[0], row0, mu_first, nu_first, nao, overwrite, vec);
-                    k2p_add_rows<6, 2, 6>(&acc[12], row0 + 16 * nao, mu_first + 16, nu_first, nao, overwrite, vec);
+                    k2p_add_rows<10, 2, 10>(&acc[0], row0, mu_first, nu_first, nao, overwrite, vec);
                 } else {
-                    k2p_add_rows<4, 4, 6>(&acc[0], row0, mu_first, nu_first, nao, overwrite, vec);
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        const int64_t mu_u = mu0 + 16 * ur[u] + lq, nu_u = nu0 + 16 * uc[u] + 2 * lr;
+                        k2p_add_rows<2, 2, 2>(&acc[4 * u], Kp + mu_u * nao + nu_u, mu_u, nu_u, nao, overwrite, vec);
+                    }
                 }
             } else if (narrow) {
                 k2p_add_rows<2, 8, 4>(&acc[0], row0, mu_first, nu_first, nao, overwrite, vec);
@@ -716,15 +750,22 @@ k3_finish_kernel(const double *__restrict__ Kpart, int nsplit, int64_t nao, doub
     __shared__ double t[K3_T][K3_T + 1];
     const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
     const int64_t mu0 = (int64_t)bi * K3_T, nu0 = (int64_t)bj * K3_T;
+    /* four rows side by side, eight splits per round: 32 loads in flight (see j3_unpack_kernel) */
+    const double *src[4];
+    double v[4];
 #pragma unroll
     for (int r = 0; r < 4; ++r) {
-        const int row = ty + 8 * r;
-        const int64_t mu = mu0 + row, nu = nu0 + tx;
-        double v = 0.0;
-        if (mu < nao && nu <= mu)
-            for (int s = 0; s < nsplit; ++s) v += Kpart[(int64_t)s * nao * nao + mu * nao + nu];
-        t[row][tx] = v;
+        const int64_t mu = mu0 + ty + 8 * r, nu = nu0 + tx;
+        src[r] = (mu < nao && nu <= mu) ? Kpart + mu * nao + nu : nullptr;
+        v[r] = 0.0;
     }
+#pragma unroll 8
+    for (int s = 0; s < nsplit; ++s)
+#pragma unroll
+        for (int r = 0; r < 4; ++r)
+            if (src[r]) v[r] += src[r][(int64_t)s * nao * nao];
+#pragma unroll
+    for (int r = 0; r < 4; ++r) t[ty + 8 * r][tx] = v[r];
     __syncthreads();
 #pragma unroll
     for (int r = 0; r < 4; ++r) {
@@ -765,6 +806,7 @@ k3_sum_kernel(const double *__restrict__ Kpart, int nsplit, int64_t n2, double *
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n2) return;
     double v = 0.0;
+#pragma unroll 8
     for (int s = 0; s < nsplit; ++s) v += Kpart[(int64_t)s * n2 + i];
     K[i] = v;
 }
