@@ -68,11 +68,12 @@ constexpr int K1_SMEM_BUDGET = 220 * 1024;
 enum { K1_MODE_ROW = 0, K1_MODE_COL = 1, K1_MODE_GATHER = 2, K1_MODE_DIAG = 3 };
 
 /* which form stage kc of row block mu0 takes; identical on producer and consumer side */
-__device__ __forceinline__ int k1_mode(int64_t mu0, int64_t nu0, int64_t nao, bool last_p)
+__device__ __forceinline__ int k1_mode(int64_t mu0, int64_t nu0, int64_t nao, bool last_p, bool multi)
 {
     if (nu0 < mu0) return K1_MODE_ROW;                         /* every nu <= every mu (32 | 128 aligned) */
     if (nu0 < mu0 + K1_M)                                      /* inside the diagonal block */
-        return nu0 + K1_KC <= nao ? K1_MODE_DIAG : K1_MODE_GATHER;   /* (ragged last stage: zero fill) */
+        return (nu0 + K1_KC <= nao && !multi) ? K1_MODE_DIAG : K1_MODE_GATHER;   /* (ragged last stage: zero
+                                                                  fill; a ragged item stacks several P) */
     if (!(last_p && nu0 + K1_KC >= nao)) return K1_MODE_COL;   /* every nu >= every mu */
     return K1_MODE_GATHER;                                     /* a bulk copy would read past the end of B */
 }
@@ -100,23 +101,72 @@ struct K1Cfg {
     static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 2 * STAGES * 8 + 16;
 };
 
+/* Work items.  A plain item is (p, row block, column tile): 128 rows of one B_P.  A ragged last row
+ * block with r <= 64 valid rows would be a low-intensity item (the whole C tile staged for a quarter
+ * of the MMAs: its stages outrun the 3-4 stage ring, 4.5 % of K1 at nao = 800), so its rows are
+ * batched over G = 2, 4 or 8 consecutive P (r <= 64, 32, 16): a RAGGED item stacks the r rows of G
+ * different B_P into one 128-row tile -- slot pp = m >> rshift of the tile holds P = p + pp, its row
+ * m & (rpad - 1) is mu0 + that -- against the one C tile they all share.  Items are numbered per group
+ * of G auxiliary indices: the G (nib - 1) ntiles_n plain items first (p-major, so the items of one P
+ * still run side by side for the tournament order), then the group's ntiles_n ragged items. */
+struct K1Item {
+    int64_t p, mu0, n0;      /* first (or only) auxiliary index relative to P0, first row, first column */
+    int np_item, rshift;     /* P slots in use (1 for a plain item), log2(rows per slot) (7: plain) */
+};
+
+__device__ __forceinline__ K1Item k1_decode(int64_t item, int nib, int ntiles_n, int rag_g, int64_t np, int nw)
+{
+    K1Item it;
+    if (rag_g == 0) {
+        const int per_p = nib * ntiles_n;
+        it.p = item / per_p;
+        const int rem = (int)(item - it.p * per_p);
+        it.mu0 = (int64_t)(rem / ntiles_n) * K1_M;
+        it.n0 = (int64_t)(rem % ntiles_n) * nw;
+        it.np_item = 1;
+        it.rshift = 7;
+        return it;
+    }
+    const int nfull = nib - 1;
+    const int per_group = (rag_g * nfull + 1) * ntiles_n;
+    const int64_t grp = item / per_group;
+    const int w = (int)(item - grp * per_group);
+    const int64_t left = np - grp * rag_g;                    /* auxiliary indices from this group on */
+    const int gg = left < rag_g ? (int)left : rag_g;
+    const int nf = gg * nfull * ntiles_n;
+    if (w < nf) {
+        const int pl = w / (nfull * ntiles_n), rem = w - pl * (nfull * ntiles_n);
+        it.p = grp * rag_g + pl;
+        it.mu0 = (int64_t)(rem / ntiles_n) * K1_M;
+        it.n0 = (int64_t)(rem % ntiles_n) * nw;
+        it.np_item = 1;
+        it.rshift = 7;
+    } else {
+        it.p = grp * rag_g;
+        it.mu0 = (int64_t)nfull * K1_M;
+        it.n0 = (int64_t)(w - nf) * nw;
+        it.np_item = gg;
+        it.rshift = rag_g == 2 ? 6 : (rag_g == 4 ? 5 : 4);
+    }
+    return it;
+}
+
 /* PERSISTENT: the grid is one CTA per SM; CTA b processes the work items b, b + gridDim.x, ...
- * (item = (p, row block, column tile), p slowest) with the mbarrier ring running THROUGH item
- * boundaries: while the consumers write one item's X tile, the producers are already filling the
- * stages of the next one.  Producers and consumers walk the same item sequence independently.
+ * with the mbarrier ring running THROUGH item boundaries: while the consumers write one item's X
+ * tile, the producers are already filling the stages of the next one.  Producers and consumers walk
+ * the same item sequence independently.
  * (One CTA per item cost a pipeline fill + drain per 25-50 stages: 16 % of K1 at nao = 290.) */
 template <int NT8>
 __global__ void __launch_bounds__(K1_THREADS, 1)
 k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao, int64_t npair, int64_t P0,
-                         const double *__restrict__ Ccat4, int64_t ldc, int64_t ldx, int ntiles_n,
-                         int64_t nitems, double *__restrict__ X4)
+                         int64_t np, const double *__restrict__ Ccat4, int64_t ldc, int64_t ldx, int ntiles_n,
+                         int rag_g, int64_t nitems, double *__restrict__ X4)
 {
     using Cfg = K1Cfg<NT8>;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int nk = (int)((nao + K1_KC - 1) / K1_KC);
     const int nib = (int)((nao + K1_M - 1) / K1_M);
-    const int items_per_p = nib * ntiles_n;
 
     const uint32_t smem_base = smem_u32(smem_raw);
     const uint32_t bar_base = smem_base + Cfg::STAGES * Cfg::STAGE_BYTES;
@@ -139,19 +189,21 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
         uint32_t phase = 1;                                /* parity of the "empty" phase to wait for */
         bool ring_full = false;                            /* all STAGES slots have been used once */
         for (int64_t item = blockIdx.x; item < nitems; item += gridDim.x) {
-        const int64_t p = item / items_per_p;
-        const int rem = (int)(item - p * items_per_p);
-        const int64_t mu0 = (int64_t)(rem / ntiles_n) * K1_M;
-        const int64_t n0 = (int64_t)(rem % ntiles_n) * Cfg::NW;
-        const int64_t pb = (P0 + p) * npair;               /* index of B_P's first element in B */
-        const int pbpar = (int)(pb & 1);
-        const bool last_p = P0 + p == naux - 1;
-        const double *__restrict__ Bp = B + pb;
+        const K1Item it = k1_decode(item, nib, ntiles_n, rag_g, np, Cfg::NW);
+        const int64_t mu0 = it.mu0, n0 = it.n0;
+        const bool multi = it.rshift != 7;
+        const int64_t pb = (P0 + it.p) * npair;            /* index of B_P's first element in B */
+        const bool last_p = P0 + it.p == naux - 1;
         int64_t ncols = ldc - n0;                          /* valid columns of this N tile */
         if (ncols > Cfg::NW) ncols = Cfg::NW;
         const uint32_t c_bytes = K1_KG * (uint32_t)ncols * 32u;
         int64_t rows_valid = nao - mu0;
         if (rows_valid > K1_M) rows_valid = K1_M;
+        /* "row" form: thread t stages tile row t = packed row mu_t of slot t >> rshift */
+        const int pp_t = tid >> it.rshift;
+        const int64_t mu_t = mu0 + (tid & ((1 << it.rshift) - 1));
+        const bool ok_t = mu_t < nao && pp_t < it.np_item;
+        const int64_t erow = pb + pp_t * npair + mu_t * (mu_t + 1) / 2;      /* element (mu_t, 0) of that P */
         const int rbi = (int)(mu0 / K1_M);
         for (int sstep = 0; sstep < nib; ++sstep) {
         /* column block of this step: the tournament partner */
@@ -162,18 +214,16 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
             const int64_t nu0 = (int64_t)kc * K1_KC;
             const uint32_t a_dst = smem_base + slot * Cfg::STAGE_BYTES;
             const uint32_t bar = full_bar(slot);
-            const int mode = k1_mode(mu0, nu0, nao, last_p);
+            const int mode = k1_mode(mu0, nu0, nao, last_p, multi);
             uint32_t my_bytes = tid == 0 ? c_bytes : 0u;
             if (mode == K1_MODE_ROW) {
-                /* thread t copies packed row mu0+t, columns nu0 .. nu0+31 (+ alignment slack) */
-                const int64_t mu = mu0 + tid;
-                const bool ok = mu < nao;
-                const int64_t e = pb + mu * (mu + 1) / 2 + nu0;
+                /* columns nu0 .. nu0+31 of the thread's packed row (+ alignment slack) */
+                const int64_t e = erow + nu0;
                 const int sft = (int)(e & 1);
-                const uint32_t nb = ok ? (uint32_t)(K1_KC + 2 * sft) * 8u : 0u;
+                const uint32_t nb = ok_t ? (uint32_t)(K1_KC + 2 * sft) * 8u : 0u;
                 my_bytes += nb;
                 if (my_bytes) mbar_arrive_expect_tx(bar, my_bytes); else mbar_arrive(bar);
-                if (ok) bulk_g2s(a_dst + tid * (K1_LDD * 8), B + (e - sft), nb, bar);
+                if (ok_t) bulk_g2s(a_dst + tid * (K1_LDD * 8), B + (e - sft), nb, bar);
             } else if (mode == K1_MODE_COL) {
                 /* thread t < 32 copies packed row nu0+t, columns mu0 .. mu0+rows_valid-1 */
                 const int64_t nu = nu0 + tid;
@@ -189,7 +239,8 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
                 if (my_bytes) mbar_arrive_expect_tx(bar, my_bytes); else mbar_arrive(bar);
                 if (ok) bulk_g2s(a_dst + tid * (K1_LDT * 8), B + (e - sft), nb, bar);
             } else if (mode == K1_MODE_DIAG) {
-                /* A stage inside the diagonal block, R0 = nu0 - mu0 in {0, 32, 64, 96}: three bands of rows.
+                /* A stage inside the diagonal block of a plain item, R0 = nu0 - mu0 in {0, 32, 64, 96}:
+                 * three bands of rows.
                  *   m <  R0      : every nu > mu -> "col" form, 32 copies of R0 doubles (packed rows nu0+k),
                  *                  pitch R0 + 4, at the start of the stage buffer (it ends below row R0 of
                  *                  the "row" form: 32 (R0 + 4) 8 <= R0 36 8)
@@ -197,30 +248,27 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
                  *   the 32 x 32 block on the diagonal: element-wise (8-byte cp.async, zero fill outside)
                  * so 1024 instead of 4096 gathered elements per stage (they cost 16 % of K1 at nao = 290). */
                 const int R0 = (int)(nu0 - mu0);
-                uint32_t nbytes = tid == 0 ? c_bytes : 0u;
                 if (tid >= R0 + K1_KC) {
-                    const int64_t mu = mu0 + tid;
-                    if (mu < nao) {
-                        const int64_t e = pb + mu * (mu + 1) / 2 + nu0;
+                    if (ok_t) {
+                        const int64_t e = erow + nu0;
                         const int sft = (int)(e & 1);
                         const uint32_t nb = (uint32_t)(K1_KC + 2 * sft) * 8u;
-                        nbytes += nb;
-                        mbar_expect_tx(bar, nbytes);
+                        mbar_expect_tx(bar, my_bytes + nb);
                         bulk_g2s(a_dst + tid * (K1_LDD * 8), B + (e - sft), nb, bar);
-                        nbytes = 0;
+                        my_bytes = 0;
                     }
                 } else if (tid < K1_KC && R0 > 0) {           /* nu0 + 31 < nao in this mode */
                     const int64_t nu = nu0 + tid;
                     const int64_t e = pb + nu * (nu + 1) / 2 + mu0;
                     const int sft = (int)(e & 1);
                     const uint32_t nb = (uint32_t)((R0 + sft + 1) & ~1) * 8u;
-                    nbytes += nb;
-                    mbar_expect_tx(bar, nbytes);
+                    mbar_expect_tx(bar, my_bytes + nb);
                     bulk_g2s(a_dst + tid * ((R0 + 4) * 8), B + (e - sft), nb, bar);
-                    nbytes = 0;
+                    my_bytes = 0;
                 }
-                if (nbytes) mbar_expect_tx(bar, nbytes);       /* thread 0 without a copy of its own */
+                if (my_bytes) mbar_expect_tx(bar, my_bytes);   /* thread 0 without a copy of its own */
                 {
+                    const int pbpar = (int)(pb & 1);
                     const int k = tid & 31;
                     const int64_t nu = nu0 + k;
                     const int64_t tri_nu = nu * (nu + 1) / 2;
@@ -231,12 +279,13 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
                         const bool ok = nu < nao && mu < nao;
                         const int64_t off = mu >= nu ? mu * (mu + 1) / 2 + nu : tri_nu + mu;
                         const int sd = (((m & 3) == 1 || (m & 3) == 2) ? 1 : 0) ^ pbpar;
-                        cp_async8(a_dst + (m * K1_LDD + k + sd) * 8, ok ? Bp + off : Bp, ok);
+                        cp_async8(a_dst + (m * K1_LDD + k + sd) * 8, ok ? B + pb + off : B, ok);
                     }
                 }
                 cp_async_mbar_arrive_noinc(bar);
             } else {
-                /* element-wise gather into the "row" form (8-byte cp.async, zero fill outside) */
+                /* element-wise gather into the "row" form (8-byte cp.async, zero fill outside); tile row
+                 * m belongs to slot m >> rshift (a plain item has one slot) */
                 if (tid == 0) mbar_expect_tx(bar, c_bytes);
                 const int k = tid & 31;
                 const int64_t nu = nu0 + k;
@@ -244,11 +293,13 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
 #pragma unroll 4
                 for (int r = 0; r < K1_M / 4; ++r) {
                     const int m = 4 * r + (tid >> 5);
-                    const int64_t mu = mu0 + m;
-                    const bool ok = nu < nao && mu < nao;
+                    const int pp = m >> it.rshift;
+                    const int64_t mu = mu0 + (m & ((1 << it.rshift) - 1));
+                    const bool ok = nu < nao && mu < nao && pp < it.np_item;
+                    const int64_t pbm = pb + pp * npair;
                     const int64_t off = mu >= nu ? mu * (mu + 1) / 2 + nu : tri_nu + mu;
-                    const int sd = (((m & 3) == 1 || (m & 3) == 2) ? 1 : 0) ^ pbpar;
-                    cp_async8(a_dst + (m * K1_LDD + k + sd) * 8, ok ? Bp + off : Bp, ok);
+                    const int sd = (((m & 3) == 1 || (m & 3) == 2) ? 1 : 0) ^ (int)(pbm & 1);
+                    cp_async8(a_dst + (m * K1_LDD + k + sd) * 8, ok ? B + pbm + off : B, ok);
                 }
                 cp_async_mbar_arrive_noinc(bar);
             }
@@ -266,7 +317,8 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
     } else {
         /* ------------------------------------------------------------ consumers */
         reg_alloc<232>();
-        const int cw = warp - K1_PRODUCERS / 32;           /* 0..7: rows 16*cw .. 16*cw+15 */
+        const int cw = warp - K1_PRODUCERS / 32;           /* 0..7: tile rows 16*cw .. 16*cw+15 */
+        const int row_w = 16 * cw;
         const int lq = lane >> 2, lr = lane & 3;
         int slot = 0;
         uint32_t phase = 0;
@@ -274,17 +326,16 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
         long long dbg_wait = 0, dbg_n = 0, dbg_slow = 0, dbg_t0 = clock64();
 #endif
         for (int64_t item = blockIdx.x; item < nitems; item += gridDim.x) {
-        const int64_t p = item / items_per_p;
-        const int rem = (int)(item - p * items_per_p);
-        const int64_t mu0 = (int64_t)(rem / ntiles_n) * K1_M;
-        const int64_t n0 = (int64_t)(rem % ntiles_n) * Cfg::NW;
-        const int pbpar = (int)(((P0 + p) * npair) & 1);
-        const bool last_p = P0 + p == naux - 1;
-        /* a ragged last row block with <= 64 valid rows: each warp takes 8 rows instead of 16, so
-         * all eight warps share it (otherwise the upper four would idle) */
-        const bool half = nao - mu0 <= 64;
-        const int row_w = half ? 8 * cw : 16 * cw;
-        const bool warp_active = mu0 + row_w < nao;
+        const K1Item it = k1_decode(item, nib, ntiles_n, rag_g, np, Cfg::NW);
+        const int64_t mu0 = it.mu0, n0 = it.n0;
+        const bool multi = it.rshift != 7;
+        /* this warp's 16 tile rows lie in one slot: auxiliary index pw, rows mu_w .. mu_w + 15 */
+        const int pp_w = row_w >> it.rshift;
+        const int64_t pw = it.p + pp_w;
+        const int64_t mu_w = mu0 + (row_w & ((1 << it.rshift) - 1));
+        const bool warp_active = mu_w < nao && pp_w < it.np_item;
+        const int pbpar = (int)(((P0 + pw) * npair) & 1);
+        const bool last_p = P0 + it.p == naux - 1;
         /* per-lane alignment shifts of the two tile forms (see K1_LDD / K1_LDT) */
         const int sd_shift = (((lq & 3) == 1 || (lq & 3) == 2) ? 1 : 0) ^ pbpar;
         const int st_shift = ((lr == 1 || lr == 2) ? 1 : 0) ^ pbpar;
@@ -313,7 +364,7 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
                 const double *As = reinterpret_cast<const double *>(smem_raw + slot * Cfg::STAGE_BYTES);
                 const double *Cs = As + K1_A_BYTES / 8;
                 /* "col" form: COL stages, and the rows above the diagonal of a DIAG stage (pitch R0 + 4) */
-                const int mode = k1_mode(mu0, (int64_t)kc * K1_KC, nao, last_p);
+                const int mode = k1_mode(mu0, (int64_t)kc * K1_KC, nao, last_p, multi);
                 const int R0 = (int)((int64_t)kc * K1_KC - mu0);
                 const bool colform = mode == K1_MODE_COL || (mode == K1_MODE_DIAG && row_w < R0);
                 const int ldt = mode == K1_MODE_COL ? K1_LDT : R0 + 4;
@@ -322,25 +373,15 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
                 const int a_gstep = colform ? 4 * ldt : 4;           /* next k-group */
                 const int a_mstep = colform ? 8 : 8 * K1_LDD;        /* next 8 rows */
                 const double *b_base = Cs + lq * 4 + lr;
-                if (!half) {
 #pragma unroll
-                    for (int g = 0; g < K1_KG; ++g) {
-                        const double a0 = a_base[g * a_gstep];
-                        const double a1 = a_base[g * a_gstep + a_mstep];
+                for (int g = 0; g < K1_KG; ++g) {
+                    const double a0 = a_base[g * a_gstep];
+                    const double a1 = a_base[g * a_gstep + a_mstep];
 #pragma unroll
-                        for (int nt = 0; nt < NT8; ++nt) {
-                            const double b = b_base[g * (Cfg::NW * 4) + nt * 32];
-                            dmma884(acc[0][nt][0], acc[0][nt][1], a0, b);
-                            dmma884(acc[1][nt][0], acc[1][nt][1], a1, b);
-                        }
-                    }
-                } else {
-#pragma unroll
-                    for (int g = 0; g < K1_KG; ++g) {
-                        const double a0 = a_base[g * a_gstep];
-#pragma unroll
-                        for (int nt = 0; nt < NT8; ++nt)
-                            dmma884(acc[0][nt][0], acc[0][nt][1], a0, b_base[g * (Cfg::NW * 4) + nt * 32]);
+                    for (int nt = 0; nt < NT8; ++nt) {
+                        const double b = b_base[g * (Cfg::NW * 4) + nt * 32];
+                        dmma884(acc[0][nt][0], acc[0][nt][1], a0, b);
+                        dmma884(acc[1][nt][0], acc[1][nt][1], a1, b);
                     }
                 }
             }
@@ -350,20 +391,16 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
         }
         }   /* column blocks */
 
-#ifdef DFJK_EXP_NOEPI
-        if (warp_active && acc[0][0][0] == 123.456) {
-#else
         if (warp_active) {
-#endif
 #pragma unroll
             for (int mt = 0; mt < 2; ++mt) {
-                const int64_t mu = mu0 + row_w + 8 * mt + lq;
-                if (mu >= nao || (half && mt == 1)) continue;
+                const int64_t mu = mu_w + 8 * mt + lq;
+                if (mu >= nao) continue;
 #pragma unroll
                 for (int nt = 0; nt < NT8; ++nt) {
                     const int64_t col = n0 + 8 * nt + 2 * lr;          /* even */
                     if (col < ldc) {
-                        const int64_t k = p * ldx + col;       /* ldx >= ldc: X row pitch */
+                        const int64_t k = pw * ldx + col;      /* ldx >= ldc: X row pitch */
                         double *dst = X4 + ((k >> 2) * nao + mu) * 4 + (k & 3);
                         *reinterpret_cast<double2 *>(dst) = make_double2(acc[mt][nt][0], acc[mt][nt][1]);
                     }
@@ -418,10 +455,19 @@ cudaError_t k1_launch_t(const double *B, int64_t naux, int64_t nao, int64_t npai
     cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev);
     if (sm_count <= 0) sm_count = 148;
     const int64_t nib = (nao + K1_M - 1) / K1_M;
-    const int64_t nitems = nib * ntiles_n * np;
+    /* a ragged last row block with <= 64 rows is batched over G auxiliary indices (see K1Item) */
+    const int64_t rlast = nao - (nib - 1) * K1_M;
+    const int rag_g = rlast <= 16 ? 8 : (rlast <= 32 ? 4 : (rlast <= 64 ? 2 : 0));
+    int64_t nitems;
+    if (rag_g == 0) {
+        nitems = nib * ntiles_n * np;
+    } else {
+        const int64_t ngroups = (np + rag_g - 1) / rag_g, gl = np - (ngroups - 1) * rag_g;
+        nitems = (ngroups - 1) * (rag_g * (nib - 1) + 1) * ntiles_n + (gl * (nib - 1) + 1) * ntiles_n;
+    }
     const unsigned grid = (unsigned)(nitems < sm_count ? nitems : sm_count);   /* persistent: 1 CTA / SM */
     k1_half_transform_kernel<NT8><<<grid, K1_THREADS, K1Cfg<NT8>::SMEM_BYTES, st>>>(
-        B, naux, nao, npair, P0, Ccat4, ldc, ldx, ntiles_n, nitems, X4);
+        B, naux, nao, npair, P0, np, Ccat4, ldc, ldx, ntiles_n, rag_g, nitems, X4);
     return cudaPeekAtLastError();
 }
 
