@@ -392,18 +392,22 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
         }   /* column blocks */
 
         if (warp_active) {
+            /* X4[(k >> 2)][mu][k & 3], k = pw ldx + n0 + 8 nt + 2 lr: ldx and n0 are multiples of 8, so the
+             * k-group is kb + 2 nt + (lr >> 1) and the store of column tile nt sits 8 nao doubles after
+             * the one of nt - 1 (per-store 64-bit index arithmetic cost 1.6 % of K1 at nao = 800) */
+            const int64_t kb = (pw * ldx + n0) >> 2;
+            const int nt_valid = (int)((ldc - n0) >> 3);           /* column tiles inside ldc */
+            double *dst0 = X4 + ((kb + (lr >> 1)) * nao + mu_w + lq) * 4 + 2 * (lr & 1);
+            const int64_t nt_step = 8 * nao;
 #pragma unroll
             for (int mt = 0; mt < 2; ++mt) {
-                const int64_t mu = mu_w + 8 * mt + lq;
-                if (mu >= nao) continue;
+                if (mu_w + 8 * mt + lq >= nao) continue;
+                double *dst = dst0 + 32 * mt;
 #pragma unroll
                 for (int nt = 0; nt < NT8; ++nt) {
-                    const int64_t col = n0 + 8 * nt + 2 * lr;          /* even */
-                    if (col < ldc) {
-                        const int64_t k = pw * ldx + col;      /* ldx >= ldc: X row pitch */
-                        double *dst = X4 + ((k >> 2) * nao + mu) * 4 + (k & 3);
+                    if (nt < nt_valid)
                         *reinterpret_cast<double2 *>(dst) = make_double2(acc[mt][nt][0], acc[mt][nt][1]);
-                    }
+                    dst += nt_step;
                 }
             }
         }
@@ -481,6 +485,7 @@ cudaError_t launch_k1_half_transform(const double *B, int64_t naux, int64_t nao,
                                      int64_t np, const double *Ccat4, int64_t ldc, int64_t ldx, double *X4,
                                      cudaStream_t st)
 {
+    if (ldc % 8 != 0 || ldx % 8 != 0) return cudaErrorInvalidValue;   /* the kernel's X addressing relies on it */
     const int n8 = (int)(ldc / 8);
     const int ntiles_n = (n8 + 16) / 17;
     const int nt8 = (n8 + ntiles_n - 1) / ntiles_n;
