@@ -68,7 +68,7 @@ constexpr int K1_SMEM_BUDGET = 220 * 1024;
 enum { K1_MODE_ROW = 0, K1_MODE_COL = 1, K1_MODE_GATHER = 2, K1_MODE_DIAG = 3 };
 
 /* which form stage kc of row block mu0 takes; identical on producer and consumer side */
-__device__ __forceinline__ int k1_mode(int64_t mu0, int64_t nu0, int64_t nao, bool last_p, bool multi)
+__device__ __forceinline__ int k1_mode(int mu0, int nu0, int nao, bool last_p, bool multi)
 {
     if (nu0 < mu0) return K1_MODE_ROW;                         /* every nu <= every mu (32 | 128 aligned) */
     if (nu0 < mu0 + K1_M)                                      /* inside the diagonal block */
@@ -214,7 +214,7 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
             const int64_t nu0 = (int64_t)kc * K1_KC;
             const uint32_t a_dst = smem_base + slot * Cfg::STAGE_BYTES;
             const uint32_t bar = full_bar(slot);
-            const int mode = k1_mode(mu0, nu0, nao, last_p, multi);
+            const int mode = k1_mode((int)mu0, kc * K1_KC, (int)nao, last_p, multi);
             uint32_t my_bytes = tid == 0 ? c_bytes : 0u;
             if (mode == K1_MODE_ROW) {
                 /* columns nu0 .. nu0+31 of the thread's packed row (+ alignment slack) */
@@ -364,8 +364,8 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
                 const double *As = reinterpret_cast<const double *>(smem_raw + slot * Cfg::STAGE_BYTES);
                 const double *Cs = As + K1_A_BYTES / 8;
                 /* "col" form: COL stages, and the rows above the diagonal of a DIAG stage (pitch R0 + 4) */
-                const int mode = k1_mode(mu0, (int64_t)kc * K1_KC, nao, last_p, multi);
-                const int R0 = (int)((int64_t)kc * K1_KC - mu0);
+                const int mode = k1_mode((int)mu0, kc * K1_KC, (int)nao, last_p, multi);
+                const int R0 = kc * K1_KC - (int)mu0;
                 const bool colform = mode == K1_MODE_COL || (mode == K1_MODE_DIAG && row_w < R0);
                 const int ldt = mode == K1_MODE_COL ? K1_LDT : R0 + 4;
                 const double *a_base = colform ? As + lr * ldt + row_w + lq + st_shift

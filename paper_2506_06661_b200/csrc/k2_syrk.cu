@@ -483,12 +483,12 @@ k2p_kernel(const K2PArgs a)
     volatile int *item_id = reinterpret_cast<volatile int *>(smem_raw + K2_STAGES * K2_STAGE_BYTES + 8 * (2 * K2_STAGES + 6));
     if (tid == 0) {
         for (int s = 0; s < K2_STAGES; ++s) {
-            mbar_init(full_bar(s), 1);
+            mbar_init(full_bar(s), 4);                            /* the four producer lanes */
             mbar_init(empty_bar(s), K2_CONSUMER_WARPS);
         }
         for (int s = 0; s < 2; ++s) {
             mbar_init(item_full(s), 1);
-            mbar_init(item_empty(s), K2_CONSUMER_WARPS + 1);       /* consumers + the releaser */
+            mbar_init(item_empty(s), K2_CONSUMER_WARPS + 3);       /* consumers + producers 1-3 */
             mbar_init(item_done(s), K2_CONSUMER_WARPS);
         }
         mbar_fence_init();
@@ -496,67 +496,97 @@ k2p_kernel(const K2PArgs a)
     __syncthreads();
 
     if (warp < 4) {
-        /* ------------------------------------------------------------ producer (one lane of the
-         * first warpgroup, which gives its registers to the consumers) */
+        /* ------------------------------------------------------------ producers: lane 0 of each warp
+         * of the first warpgroup (which gives its registers to the consumers).  Producer w issues the
+         * k-groups q = w and w + 4 of every stage, so each of the four sub-partitions carries a quarter
+         * of the copy-issuing instructions: with ONE producer lane its ~640 instructions per stage took
+         * issue slots from the two consumer warps of its sub-partition exactly when their DMMAs were due,
+         * that sub-partition ran 270 cycles per stage behind and the other three waited for it at the
+         * full barrier.  Producer 0 also claims the items; producer 1 also publishes finished ones. */
         reg_dealloc<40>();
-        if (warp == 0 && lane == 0) {
+        if (lane == 0) {
+            const int w = warp;
             int st = 0;                                   /* stages issued so far (ring position) */
+            bool pending = false;                         /* producer 1: an item waits to be published */
+            int pend_is = 0, pend_val = 0;
+            uint32_t pend_phase = 0;
+            int *pend_flag = nullptr;
             for (int ir = 0;; ++ir) {
-                const int item = atomicAdd(a.work, 1);
                 const int is = ir & 1;
-                if (ir >= 2) mbar_wait(item_empty(is), ((ir >> 1) - 1) & 1);
-                item_id[is] = item < nitems ? item : -1;
-                mbar_arrive(item_full(is));
-                if (item >= nitems) break;
+                int item;
+                if (w == 0) {
+                    item = atomicAdd(a.work, 1);
+                    if (item >= nitems) item = -1;
+                    if (ir >= 2) mbar_wait(item_empty(is), ((ir >> 1) - 1) & 1);
+                    item_id[is] = item;
+                    mbar_arrive(item_full(is));
+                } else {
+                    mbar_wait(item_full(is), (ir >> 1) & 1);
+                    item = item_id[is];
+                    mbar_arrive(item_empty(is));
+                }
+                if (item < 0) break;
                 const int p = item / a.ntile, t = item - p * a.ntile;
                 int bi, bj;
                 k2p_decode<FULL>(t, a.nb, bi, bj);
                 const bool diag = !FULL && bi == bj;
                 const int64_t mu0 = (int64_t)bi * K2_T, nu0 = (int64_t)bj * K2_T;
-                const int64_t rows_a = (nao - mu0 < K2_T) ? nao - mu0 : K2_T;
-                const int64_t rows_b = (nao - nu0 < K2_T) ? nao - nu0 : K2_T;
+                const uint32_t bytes_a = (uint32_t)(((nao - mu0 < K2_T) ? nao - mu0 : K2_T) * 32);
+                const uint32_t bytes_b = (uint32_t)(((nao - nu0 < K2_T) ? nao - nu0 : K2_T) * 32);
                 const int64_t gbeg = ng * p / a.npanel, gend = ng * (p + 1) / a.npanel;
                 const int nk = (int)((gend - gbeg + K2_KG - 1) / K2_KG);
-                /* (gp, gi) = (g / n4s, g % n4s) of the running k-group g, kept incrementally: the lane
-                 * must issue a stage faster than the consumers eat it (2048 cycles on a 32-row tile) */
-                int64_t gp = gbeg / a.n4s;
-                int gi = (int)(gbeg - gp * a.n4s);
+                /* this lane's k-groups are gbeg + w, + 4, + 8, ...: the index inside its P (gi) and the
+                 * source pointers are kept incrementally, no division in the stage loop */
+                int64_t g = gbeg + w;
+                const int64_t gp = g / a.n4s;
+                int gi = (int)(g - gp * a.n4s);
+                const int64_t gstride = nao * 4;                              /* doubles per k-group */
+                const double *src_a = a.X4 + (gp * a.ldc4 + a.col04 + gi) * gstride + mu0 * 4;
+                const double *src_b = a.X4 + (gp * a.ldc4 + (FULL ? a.col04b : a.col04) + gi) * gstride + nu0 * 4;
+                const int64_t wrap_skip = (a.ldc4 - a.n4s) * gstride;         /* past the other columns of a P */
                 for (int kc = 0; kc < nk; ++kc, ++st) {
                     const int slot = st % K2_STAGES;
                     const int round = st / K2_STAGES;
+                    if (w == 1 && pending && mbar_test_wait(item_done(pend_is), pend_phase)) {
+                        st_release_gpu(pend_flag, pend_val);
+                        pending = false;
+                    }
                     if (round > 0) mbar_wait(empty_bar(slot), (round - 1) & 1);
-                    const int64_t g0 = gbeg + K2_KG * (int64_t)kc;
-                    const int n = (int)((gend - g0 < K2_KG) ? gend - g0 : K2_KG);
-                    const uint32_t bytes = (uint32_t)(n * 32 * (rows_a + (diag ? 0 : rows_b)));
-                    mbar_arrive_expect_tx(full_bar(slot), bytes);
                     const uint32_t dst = smem_base + slot * K2_STAGE_BYTES;
-                    for (int q = 0; q < n; ++q) {
-                        const int64_t kg = gp * a.ldc4 + a.col04 + gi;                   /* k-group in X4 */
-                        if (++gi == a.n4s) { gi = 0; ++gp; }
-                        const double *src = a.X4 + kg * nao * 4;
-                        bulk_g2s(dst + q * (K2_T * 32), src + mu0 * 4, (uint32_t)(rows_a * 32), full_bar(slot));
-                        if (!diag) {
-                            const double *srcb = FULL ? src + (a.col04b - a.col04) * nao * 4 : src;
-                            bulk_g2s(dst + K2_OP_BYTES + q * (K2_T * 32), srcb + nu0 * 4,
-                                     (uint32_t)(rows_b * 32), full_bar(slot));
+                    const int mine = (g < gend ? 1 : 0) + (g + 4 < gend ? 1 : 0);     /* my groups in this stage */
+                    if (mine) mbar_arrive_expect_tx(full_bar(slot), (uint32_t)mine * (bytes_a + (diag ? 0u : bytes_b)));
+                    else mbar_arrive(full_bar(slot));
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        if (g < gend) {
+                            const int q = w + 4 * h;
+                            bulk_g2s(dst + q * (K2_T * 32), src_a, bytes_a, full_bar(slot));
+                            if (!diag) bulk_g2s(dst + K2_OP_BYTES + q * (K2_T * 32), src_b, bytes_b, full_bar(slot));
                         }
+                        g += 4; gi += 4;
+                        src_a += 4 * gstride; src_b += 4 * gstride;
+                        while (gi >= a.n4s) { gi -= a.n4s; src_a += wrap_skip; src_b += wrap_skip; }
                     }
                 }
+                if (w == 1) {
+                    /* the item just issued is published once its consumers report their adds issued
+                     * (item_done): polled from the stage loop of the NEXT item, never waited for while
+                     * stages remain to be issued; the gpu-scope release is cumulative over what the
+                     * mbarrier made visible to this thread, i.e. it orders the adds, not the consumers */
+                    if (pending) {
+                        mbar_wait(item_done(pend_is), pend_phase);
+                        st_release_gpu(pend_flag, pend_val);
+                    }
+                    pending = true;
+                    pend_is = is;
+                    pend_phase = (uint32_t)((ir >> 1) & 1);
+                    pend_flag = a.work + 1 + (p % a.nslab) * a.ntile + t;
+                    pend_val = p / a.nslab + 1;
+                }
             }
-        } else if (warp == 1 && lane == 0) {
-            /* ---------------------------------------------------------- releaser: publishes an item
-             * once all eight consumer warps have issued its adds (item_done).  The consumers arrive and
-             * go straight on to the next item; the gpu-scope release below is cumulative over what the
-             * mbarrier made visible to this thread, i.e. it waits for the adds, not the consumers. */
-            for (int ir = 0;; ++ir) {
-                const int is = ir & 1;
-                mbar_wait(item_full(is), (ir >> 1) & 1);
-                const int item = item_id[is];
-                mbar_arrive(item_empty(is));
-                if (item < 0) break;
-                const int p = item / a.ntile, t = item - p * a.ntile;
-                mbar_wait(item_done(is), (ir >> 1) & 1);
-                st_release_gpu(a.work + 1 + (p % a.nslab) * a.ntile + t, p / a.nslab + 1);
+            if (w == 1 && pending) {
+                mbar_wait(item_done(pend_is), pend_phase);
+                st_release_gpu(pend_flag, pend_val);
             }
         }
         return;
@@ -614,9 +644,17 @@ k2p_kernel(const K2PArgs a)
 
         for (int kc = 0; kc < nk; ++kc, ++st) {
             const int slot = st % K2_STAGES;
-            DBG_T(1, mbar_wait(full_bar(slot), (st / K2_STAGES) & 1));
 #ifdef DFJK_K2_DBG
-            ++dbg[2];
+            {
+                const long long t0_ = clock64();
+                mbar_wait(full_bar(slot), (st / K2_STAGES) & 1);
+                const long long dt_ = clock64() - t0_;
+                dbg[1] += dt_;
+                if (kc < 3) dbg[4] += dt_;
+                ++dbg[2];
+            }
+#else
+            mbar_wait(full_bar(slot), (st / K2_STAGES) & 1);
 #endif
             if (warp_active) {
                 const int64_t g0 = gbeg + K2_KG * (int64_t)kc;
@@ -689,7 +727,6 @@ k2p_kernel(const K2PArgs a)
         int *flag = a.work + 1 + slab * a.ntile + t;
         const bool overwrite = seq == 0 && !a.accumulate;
 #ifdef DFJK_K2_DBG
-        const long long dbg_ta = clock64();
         ++dbg[6];
 #endif
         if (warp_active) {
