@@ -14,11 +14,14 @@
  *       transposed tile, "col" form); each is one 1-D bulk copy (cp.async.bulk -> UBLKCP)
  *       issued by one producer thread.  Packed rows are only 8-byte aligned: a copy whose
  *       source index is odd starts one element early and the consumer reads that row with
- *       a +1 column shift, which is a per-lane constant (see K1_LDD/K1_LDT).  Only the
- *       stages that cross the diagonal (4 of 50 at nao=1600) gather element-wise with
- *       8-byte cp.async (max/min addressing, zero fill).  An earlier version gathered every
- *       stage with cp.async: the 4096 LDGSTS per stage cost 7 % of K1 through the LSU.
+ *       a +1 column shift, which is a per-lane constant (see K1_LDD/K1_LDT).  The four
+ *       stages inside the diagonal block mix the two forms band by band and gather only the
+ *       32 x 32 block that sits on the diagonal element-wise (8-byte cp.async, max/min
+ *       addressing, zero fill; see K1_MODE_DIAG).  An earlier version gathered every stage
+ *       with cp.async: the 4096 LDGSTS per stage cost 7 % of K1 through the LSU.
  *       Every packed element is read twice per call (K1 is compute-bound: ~65 flop/B).
+ *     - a ragged last row block (<= 64 rows) is batched over 2/4/8 auxiliary indices into one
+ *       full 128-row item (see K1Item).
  *     - C tile: Ccat is kept k-group-major ([nu/4][ldc][4]), so the 8 x NW x 4 tile of a
  *       stage is eight contiguous bulk copies completing on the same mbarrier.
  *   two consumer warpgroups (8 warps, 232 registers after setmaxnreg.inc)
@@ -83,9 +86,6 @@ __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
     asm volatile("mbarrier.expect_tx.relaxed.cta.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
 
-#ifdef DFJK_K1_DBG
-__device__ long long k1_dbg[148 * 8 * 4];
-#endif
 
 template <int NT8>
 struct K1Cfg {
@@ -93,11 +93,7 @@ struct K1Cfg {
     static constexpr int C_BYTES = K1_KC * NW * 8;
     static constexpr int STAGE_BYTES = K1_A_BYTES + C_BYTES;
     static constexpr int STAGES_RAW = K1_SMEM_BUDGET / STAGE_BYTES;
-#ifdef DFJK_K1_MAXSTAGES
-    static constexpr int STAGES = STAGES_RAW > DFJK_K1_MAXSTAGES ? DFJK_K1_MAXSTAGES : STAGES_RAW;
-#else
     static constexpr int STAGES = STAGES_RAW > 8 ? 8 : STAGES_RAW;
-#endif
     static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 2 * STAGES * 8 + 16;
 };
 
@@ -322,9 +318,6 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
         const int lq = lane >> 2, lr = lane & 3;
         int slot = 0;
         uint32_t phase = 0;
-#ifdef DFJK_K1_DBG
-        long long dbg_wait = 0, dbg_n = 0, dbg_slow = 0, dbg_t0 = clock64();
-#endif
         for (int64_t item = blockIdx.x; item < nitems; item += gridDim.x) {
         const K1Item it = k1_decode(item, nib, ntiles_n, rag_g, np, Cfg::NW);
         const int64_t mu0 = it.mu0, n0 = it.n0;
@@ -350,16 +343,7 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
         const int jb = sstep >= rbi ? sstep - rbi : sstep - rbi + nib;
         const int kc_end = (jb + 1) * (K1_M / K1_KC) < nk ? (jb + 1) * (K1_M / K1_KC) : nk;
         for (int kc = jb * (K1_M / K1_KC); kc < kc_end; ++kc) {
-#ifdef DFJK_K1_DBG
-            {
-                const long long t0 = clock64();
-                mbar_wait(full_bar(slot), phase);
-                const long long dt = clock64() - t0;
-                dbg_wait += dt; ++dbg_n; if (dt > 200) ++dbg_slow;
-            }
-#else
             mbar_wait(full_bar(slot), phase);
-#endif
             if (warp_active) {
                 const double *As = reinterpret_cast<const double *>(smem_raw + slot * Cfg::STAGE_BYTES);
                 const double *Cs = As + K1_A_BYTES / 8;
@@ -412,12 +396,6 @@ k1_half_transform_kernel(const double *__restrict__ B, int64_t naux, int64_t nao
             }
         }
         }   /* items */
-#ifdef DFJK_K1_DBG
-        if (lane == 0 && blockIdx.x < 148) {
-            long long *d = k1_dbg + (blockIdx.x * 8 + cw) * 4;
-            d[0] = dbg_wait; d[1] = dbg_n; d[2] = dbg_slow; d[3] = clock64() - dbg_t0;
-        }
-#endif
     }
 }
 
@@ -477,9 +455,6 @@ cudaError_t k1_launch_t(const double *B, int64_t naux, int64_t nao, int64_t npai
 
 }  // namespace
 
-#ifdef DFJK_K1_DBG
-extern "C" int dfjk_dbg_k1(long long *out) { return (int)cudaMemcpyFromSymbol(out, k1_dbg, sizeof(long long) * 148 * 8 * 4); }
-#endif
 
 cudaError_t launch_k1_half_transform(const double *B, int64_t naux, int64_t nao, int64_t npair, int64_t P0,
                                      int64_t np, const double *Ccat4, int64_t ldc, int64_t ldx, double *X4,

@@ -13,7 +13,7 @@
  * warp tile 64 x 32 = 8 x 4 DMMA.8x8x4 accumulators, 12 shared loads per 32 MMAs.  Both
  * operands are row panels of X, so A (row-major) and B (col-major) fragments are read with
  * the same pattern; diagonal tiles load the panel once and use a triangular warp layout (the
- * 20 units of 32 x 16 that touch the lower triangle, dealt 3,3,3,3,2,2,2,2); block rows with
+ * 36 units of 16 x 16 that touch the lower triangle, five or four per warp: tri_unit); block rows with
  * <= 64 valid rows use a 1 x 8 layout of 64 x 16 warp tiles (and, in the full product, block columns
  * with <= 64 valid columns a 4 x 2 layout of 32 x 32), so no warp idles on ragged tiles.
  * The same kernel with FULL = true covers all nb x nb tiles with operands from two column
@@ -381,8 +381,10 @@ k2_syrk_lower_kernel(const double *__restrict__ X4, int64_t nao, int64_t np, int
  * (slab, tile) counter in global memory, release/acquire; items are claimed in order and never
  * wait on later ones, so the wait cannot deadlock and in practice never spins).  The slabs are
  * L2-resident (S x nao^2 doubles) and summed in the fixed order K3 uses => deterministic.
- * The producer lane runs ahead through item boundaries (the stage ring never drains), warp
- * layouts per tile are those of k2_syrk_lower_kernel. */
+ * The adds are `red.add.f64` at L2, ordered by that counter (each address receives them in panel
+ * order), so no consumer waits for a slab line.  Four producer lanes, one per sub-partition, run
+ * ahead through item boundaries (the stage ring never drains); warp layouts per tile are those of
+ * k2_syrk_lower_kernel. */
 struct K2PArgs {
     const double *X4;
     int64_t nao, np, ldc4, col04, col04b;
@@ -459,9 +461,6 @@ __device__ __forceinline__ void k2p_add_rows(const double (*acc)[2], double *row
     }
 }
 
-#ifdef DFJK_K2_DBG
-__device__ long long k2_dbg[148 * 8 * 8];
-#endif
 
 template <bool FULL>
 __global__ void __launch_bounds__(K2P_THREADS, 1)
@@ -607,16 +606,9 @@ k2p_kernel(const K2PArgs a)
         }
     }
     int st = 0;
-#ifdef DFJK_K2_DBG
-    long long dbg[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-    const long long dbg_t0 = clock64();
-#define DBG_T(i, stmt) { const long long t0_ = clock64(); stmt; dbg[i] += clock64() - t0_; }
-#else
-#define DBG_T(i, stmt) { stmt; }
-#endif
     for (int ir = 0;; ++ir) {
         const int is = ir & 1;
-        DBG_T(0, mbar_wait(item_full(is), (ir >> 1) & 1));
+        mbar_wait(item_full(is), (ir >> 1) & 1);
         const int item = item_id[is];
         __syncwarp();
         if (lane == 0) mbar_arrive(item_empty(is));
@@ -644,18 +636,7 @@ k2p_kernel(const K2PArgs a)
 
         for (int kc = 0; kc < nk; ++kc, ++st) {
             const int slot = st % K2_STAGES;
-#ifdef DFJK_K2_DBG
-            {
-                const long long t0_ = clock64();
-                mbar_wait(full_bar(slot), (st / K2_STAGES) & 1);
-                const long long dt_ = clock64() - t0_;
-                dbg[1] += dt_;
-                if (kc < 3) dbg[4] += dt_;
-                ++dbg[2];
-            }
-#else
             mbar_wait(full_bar(slot), (st / K2_STAGES) & 1);
-#endif
             if (warp_active) {
                 const int64_t g0 = gbeg + K2_KG * (int64_t)kc;
                 const int n = (int)((gend - g0 < K2_KG) ? gend - g0 : K2_KG);
@@ -726,14 +707,11 @@ k2p_kernel(const K2PArgs a)
         const int slab = p % a.nslab, seq = p / a.nslab;
         int *flag = a.work + 1 + slab * a.ntile + t;
         const bool overwrite = seq == 0 && !a.accumulate;
-#ifdef DFJK_K2_DBG
-        ++dbg[6];
-#endif
         if (warp_active) {
             if (seq > 0) {
-                DBG_T(3, if (lane == 0) while (ld_acquire_gpu(flag) < seq) { }
+                if (lane == 0) while (ld_acquire_gpu(flag) < seq) { }
                 __syncwarp();
-                (void)ld_acquire_gpu(flag));              /* every lane orders its adds after the flag */
+                (void)ld_acquire_gpu(flag);              /* every lane orders its adds after the flag */
             }
             double *Kp = a.Kpart + (int64_t)slab * nao * nao;
             /* first item of the (slab, tile): 16-byte stores when the row pitch allows (nao even);
@@ -761,17 +739,11 @@ k2p_kernel(const K2PArgs a)
                 k2p_add_rows<4, 4, 4>(&acc[16], row0 + 32 * nao, mu_first + 32, nu_first, nao, overwrite, vec);
             }
         }
-        /* every consumer warp (the idle ones too) reports its adds issued and moves on; the releaser
-         * warp publishes the item (no CTA-wide barrier, no consumer waits for the adds to land) */
+        /* every consumer warp (the idle ones too) reports its adds issued and moves on; producer 1
+         * publishes the item (no CTA-wide barrier, no consumer waits for the adds to land) */
         __syncwarp();
-        DBG_T(5, if (lane == 0) mbar_arrive(item_done(is)));
+        if (lane == 0) mbar_arrive(item_done(is));
     }
-#ifdef DFJK_K2_DBG
-    if (lane == 0 && blockIdx.x < 148) {
-        dbg[7] = clock64() - dbg_t0;
-        for (int i = 0; i < 8; ++i) k2_dbg[(blockIdx.x * 8 + cw) * 8 + i] = dbg[i];
-    }
-#endif
 }
 
 /* ------------------------------------------------------------------ K3 */
@@ -850,9 +822,6 @@ k3_sum_kernel(const double *__restrict__ Kpart, int nsplit, int64_t n2, double *
 
 }  // namespace
 
-#ifdef DFJK_K2_DBG
-extern "C" int dfjk_dbg_k2(long long *out) { return (int)cudaMemcpyFromSymbol(out, k2_dbg, sizeof(long long) * 148 * 8 * 8); }
-#endif
 
 void launch_k0_pack_c(const double *const *C, const int *nocc, const int *col0, int nset, int64_t nao,
                       int64_t ldc, double *Ccat, double *const *outs, double **out_slots, cudaStream_t st)
@@ -908,10 +877,7 @@ void k2p_plan(int64_t nao, int64_t ng, int ntile, int sm_count, int max_slabs, i
     /* L2: one panel of X (all nao rows) is about panel_bytes */
     int64_t len = panel_bytes / (nao * 32 * K2_KG);
     /* balance: at least ~30 items per SM when the problem is big enough for that */
-#ifndef DFJK_K2P_ITEMS_PER_SM
-#define DFJK_K2P_ITEMS_PER_SM 30
-#endif
-    const int64_t len_bal = stages_total * ntile / ((int64_t)DFJK_K2P_ITEMS_PER_SM * sm_count);
+    const int64_t len_bal = stages_total * ntile / (30LL * sm_count);
     if (len > len_bal) len = len_bal;
     if (len < 8) len = 8;                                 /* the 128 KB read-modify-write must amortise */
     if (len > stages_total) len = stages_total > 0 ? stages_total : 1;
