@@ -57,6 +57,9 @@ int64_t round_up(int64_t x, int64_t m) { return (x + m - 1) / m * m; }
 }  // namespace
 
 #define DFJK_GRAPH_SLOTS 4
+#ifndef DFJK_K2P_MIN_NB
+#define DFJK_K2P_MIN_NB 6   /* K2P needs enough tiles per panel: below 21 lower tiles the split kernel wins */
+#endif
 
 namespace dfjk {
 /* split count that fills the SMs best: work items = ntile * s on sm_count SMs (one CTA each).
@@ -75,8 +78,25 @@ int choose_splits(int ntile, int sm_count, int max_splits)
     return best;
 }
 
+/* The lower-triangle split kernel: tiles are cut in proportion to their cost, s is the count of a
+ * full off-diagonal tile and a CTA then lasts ~1/s of a tile; minimise waves / s (small penalty per
+ * split for the partials K3 has to add). */
+int choose_splits_lower(int64_t nao, int sm_count, int max_splits)
+{
+    int best = 1;
+    double best_time = 1e300;
+    for (int s = 1; s <= max_splits; ++s) {
+        const int64_t items = k2_lower_items(nao, s);
+        const int64_t waves = (items + sm_count - 1) / sm_count;
+        const double t = (double)waves / s * (1.0 + 0.002 * s);
+        if (t < best_time) { best_time = t; best = s; }
+    }
+    return best;
+}
+
 }  // namespace dfjk
 using dfjk::choose_splits;
+using dfjk::choose_splits_lower;
 
 struct dfjk_handle {
     int64_t naux, nao, npair;
@@ -94,6 +114,9 @@ struct dfjk_handle {
     double *Kpart;       /* 2 x nsplit_alloc x nao x nao */
     int64_t nchunk, j2_groups, x_doubles;
     int nsplit_alloc, nsplit_default;
+    int nsplit_weighted; /* split kernel with per-tile split counts in proportion to tile cost (k2_tile_splits):
+                            the count of a full tile, 0 if there are more lower tiles than SMs */
+    int64_t opt_k2_weighted;
     int64_t ws_bytes;
     /* options */
     int64_t opt_k_chunk, opt_k_splits, opt_j_fused, opt_k2_panel, opt_k2_panel_kb;
@@ -218,6 +241,7 @@ extern "C" dfjk_handle *dfjk_create(int64_t naux, int64_t nao, const double *B_p
     h->opt_j_fused = 1;
     h->opt_graph = 1;
     h->opt_k2_panel = 2;             /* automatic */
+    h->opt_k2_weighted = 2;          /* automatic */
     h->opt_k2_panel_kb = 32768;
     int v = 0;
     cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev); h->sm_count = v > 0 ? v : 148;
@@ -234,9 +258,19 @@ extern "C" dfjk_handle *dfjk_create(int64_t naux, int64_t nao, const double *B_p
     h->x_doubles = xd;
     const int nb = (int)((nao + 127) / 128);
     h->nsplit_default = choose_splits(nb * (nb + 1) / 2, h->sm_count, 32);
+    /* small problems (fewer lower tiles than SMs, X chunk L2-resident): ONE wave, balanced tile by tile;
+     * up to 64 splits of a full tile while the 2 x nsplit_alloc partial-K slots stay below 512 MB */
+    h->nsplit_weighted = 0;
+    if (nb * (nb + 1) / 2 <= h->sm_count) {
+        int max_s = (int)((512LL << 20) / (2 * nao * nao * 8));
+        if (max_s > 64) max_s = 64;
+        if (max_s < 8) max_s = 8;
+        h->nsplit_weighted = choose_splits_lower(nao, h->sm_count, max_s);
+    }
     /* partial-K slots: what the two automatic choices (lower tiles; all tiles for the general
      * product) need, at least 8 for the "k_splits" option -- 2*32 slots would be 8 GB at nao=4000 */
     h->nsplit_alloc = h->nsplit_default;
+    if (h->nsplit_weighted > h->nsplit_alloc) h->nsplit_alloc = h->nsplit_weighted;
     if (choose_splits(nb * nb, h->sm_count, 32) > h->nsplit_alloc)
         h->nsplit_alloc = choose_splits(nb * nb, h->sm_count, 32);
     if (h->nsplit_alloc < 8) h->nsplit_alloc = 8;
@@ -294,6 +328,10 @@ extern "C" int dfjk_set_option(dfjk_handle *h, const char *name, int64_t value)
         if (value > 2) return fail(DFJK_EINVAL, "k2_panel must be 0, 1 or 2");
         h->opt_k2_panel = value; return DFJK_OK;
     }
+    if (!strcmp(name, "k2_weighted")) {
+        if (value > 2) return fail(DFJK_EINVAL, "k2_weighted must be 0, 1 or 2");
+        h->opt_k2_weighted = value; return DFJK_OK;
+    }
     if (!strcmp(name, "k2_panel_kb")) {
         if (value < 64) return fail(DFJK_EINVAL, "k2_panel_kb must be >= 64");
         h->opt_k2_panel_kb = value; return DFJK_OK;
@@ -334,9 +372,15 @@ int enqueue_jk_body(dfjk_handle *h, int nset, const int *nocc, const int *col0, 
         /* K2P pays a read-modify-write per item to keep the k window of X inside L2; an X chunk that
          * fits in L2 whole has nothing to gain from it (and small problems are all overhead), and the
          * slab it adds into (nao^2 doubles) must itself stay in L2 beside the window */
-        const bool panel = h->opt_k2_panel == 1 ||
-                           (h->opt_k2_panel == 2 && pc * nao * ldc * 8 > h->l2_bytes && nao * nao * 8 * 3 <= h->l2_bytes);
         const int nbk = (int)((nao + 127) / 128);
+        const bool panel = h->opt_k2_panel == 1 ||
+                           (h->opt_k2_panel == 2 && pc * nao * ldc * 8 > h->l2_bytes && nao * nao * 8 * 3 <= h->l2_bytes &&
+                            nbk >= DFJK_K2P_MIN_NB);
+        /* the split kernel balances a single wave tile by tile when the chunk of X it re-reads stays in
+         * L2 (tiles then cut the k range at different places: no two CTAs stream the same lines together) */
+        const bool weighted = !panel && h->nsplit_weighted > 0 && h->opt_k_splits == 0 &&
+                              (h->opt_k2_weighted == 1 ||
+                               (h->opt_k2_weighted == 2 && pc * nao * ldc * 8 * 10 <= h->l2_bytes * 7));
         /* K2P: panel length and slab count per set, planned from the first (largest) chunk; the old
          * split kernel: one partial per k-split */
         int nsplit[2] = {0, 0}, pstages[2] = {0, 0};
@@ -346,7 +390,7 @@ int enqueue_jk_body(dfjk_handle *h, int nset, const int *nocc, const int *col0, 
                                h->opt_k_splits > 0 ? (int)h->opt_k_splits : h->nsplit_alloc,
                                h->opt_k2_panel_kb << 10, &pstages[s], &nsplit[s]);
             else
-                nsplit[s] = h->opt_k_splits > 0 ? (int)h->opt_k_splits : h->nsplit_default;
+                nsplit[s] = h->opt_k_splits > 0 ? (int)h->opt_k_splits : (weighted ? h->nsplit_weighted : h->nsplit_default);
         }
         int chunk = 0;
         for (int64_t P0 = 0; P0 < naux; P0 += pc, ++chunk) {
@@ -365,13 +409,13 @@ int enqueue_jk_body(dfjk_handle *h, int nset, const int *nocc, const int *col0, 
                                                                     nsplit[s], chunk > 0, h->k2work, h->sm_count, st));
                     else
                         DFJK_LAUNCH_TRY(dfjk::launch_k2_syrk_lower(h->X, nao, np, ldc, col0[s], nocc[s], Kp,
-                                                                   nsplit[s], chunk > 0, st));
+                                                                   nsplit[s], weighted ? 1 : 0, chunk > 0, st));
                 }
         }
         for (int s = 0; s < nset; ++s)
             if (want_k[s]) {
                 Timed t_(h, DFJK_KERNEL_K3, st);
-                dfjk::launch_k3_finish(h->Kpart + (int64_t)s * h->nsplit_alloc * nao * nao, nsplit[s],
+                dfjk::launch_k3_finish(h->Kpart + (int64_t)s * h->nsplit_alloc * nao * nao, nsplit[s], weighted ? 1 : 0,
                                        nao, K[s], slots ? slots + 1 + s : nullptr, st);
             }
     }
@@ -391,10 +435,10 @@ int enqueue_jk_body(dfjk_handle *h, int nset, const int *nocc, const int *col0, 
 struct GraphKey {
     int nset, nocc[2];
     bool want_j, want_k[2];
-    int64_t k_chunk, k_splits, j_fused, k2_panel, k2_panel_kb;
+    int64_t k_chunk, k_splits, j_fused, k2_panel, k2_panel_kb, k2_weighted;
     bool operator==(const GraphKey &o) const
     {
-        if (k2_panel != o.k2_panel || k2_panel_kb != o.k2_panel_kb) return false;
+        if (k2_panel != o.k2_panel || k2_panel_kb != o.k2_panel_kb || k2_weighted != o.k2_weighted) return false;
         return nset == o.nset && nocc[0] == o.nocc[0] && nocc[1] == o.nocc[1] && want_j == o.want_j &&
                want_k[0] == o.want_k[0] && want_k[1] == o.want_k[1] && k_chunk == o.k_chunk &&
                k_splits == o.k_splits && j_fused == o.j_fused;
@@ -430,7 +474,7 @@ int get_jk_impl(dfjk_handle *h, int nset, const double *const *C, const int64_t 
     GraphKey key = {};
     key.nset = nset; key.want_j = J != nullptr;
     key.k_chunk = h->opt_k_chunk; key.k_splits = h->opt_k_splits; key.j_fused = h->opt_j_fused;
-    key.k2_panel = h->opt_k2_panel; key.k2_panel_kb = h->opt_k2_panel_kb;
+    key.k2_panel = h->opt_k2_panel; key.k2_panel_kb = h->opt_k2_panel_kb; key.k2_weighted = h->opt_k2_weighted;
     bool want_k[2] = {false, false};
     for (int s = 0; s < nset; ++s) { key.nocc[s] = nocc[s]; key.want_k[s] = want_k[s] = K[s] != nullptr; }
 

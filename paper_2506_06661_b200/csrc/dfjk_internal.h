@@ -84,7 +84,8 @@ void launch_k1u_unpack(const double *B, int64_t nao, int64_t npair, int64_t P0, 
  * for mu-tile >= nu-tile (lower 128x128 tiles).  The set uses k = p*ldc + [col0, col0+round_up(ncol,4)),
  * p < np: K2's MMA k step is 4, so the 8-padding columns of Ccat beyond that are never read.  accumulate = 0 overwrites. */
 cudaError_t launch_k2_syrk_lower(const double *X4, int64_t nao, int64_t np, int64_t ldc, int64_t col0,
-                                 int64_t ncol, double *Kpart, int nsplit, int accumulate, cudaStream_t st);
+                                 int64_t ncol, double *Kpart, int nsplit, int weighted, int accumulate,
+                                 cudaStream_t st);
 
 /* K2 general: Kpart[split][mu][nu] (+)= sum_k X[mu][k_a] X[nu][k_b] over ALL tiles, with
  * k_a = p*ldc + col0a + j, k_b = p*ldc + col0b + j, j < round_up(ncol,4): the product
@@ -113,7 +114,7 @@ cudaError_t launch_k2p_gemm_full(const double *X4, int64_t nao, int64_t np, int6
 void launch_k3_sum(const double *Kpart, int nsplit, int64_t nao, double *K, cudaStream_t st);
 
 /* K3: K[mu][nu] = K[nu][mu] = sum_split Kpart[split][mu][nu], mu >= nu. */
-void launch_k3_finish(const double *Kpart, int nsplit, int64_t nao, double *K, double *const *Kslot,
+void launch_k3_finish(const double *Kpart, int nsplit, int weighted, int64_t nao, double *K, double *const *Kslot,
                       cudaStream_t st);
 
 /* ---------------------------------------------------------------- building B (Eq. 2-3) */
@@ -148,6 +149,10 @@ ScfWorkspace scf_workspace(dfjk_handle *h);
 void scf_store_timing(dfjk_handle *h, int64_t iters, double get_jk_ms, double eig_ms, double total_ms);
 /* split count that fills sm_count SMs best with ntile * s equal work items (dfjk_api.cu) */
 int choose_splits(int ntile, int sm_count, int max_splits);
+/* split count (of a full off-diagonal tile) of the lower-triangle split kernel, whose tiles get
+ * splits in proportion to their cost (k2_tile_splits); k2_lower_items counts the CTAs that do work */
+int choose_splits_lower(int64_t nao, int sm_count, int max_splits);
+int64_t k2_lower_items(int64_t nao, int nsplit);
 /* nspin = 1: restricted (get_jk), nspin = 2: unrestricted (get_jk_u); per-spin arguments are arrays */
 int scf_run(dfjk_handle *h, int64_t nao, int nspin, const double *hcore, const double *S,
             const int64_t *nocc, int64_t max_iter, double conv_tol, int64_t diis_space,

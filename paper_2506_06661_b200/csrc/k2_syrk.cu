@@ -67,6 +67,23 @@ constexpr int K2_CONSUMER_WARPS = 8;
 constexpr int K2_THREADS = 32 * (1 + K2_CONSUMER_WARPS);
 constexpr int K2_SMEM_BYTES = K2_STAGES * K2_STAGE_BYTES + 2 * K2_STAGES * 8 + 16;
 
+/* Lower tiles are not equally expensive: a full-height diagonal tile issues 9/16 of the MMAs of an
+ * off-diagonal one, a block row with <= 64 (<= 32) valid rows a half (a quarter), its diagonal tile
+ * half of that again.  The split kernel therefore cuts the k range of a tile into a number of splits
+ * PROPORTIONAL to its cost -- nsplit is the count of a full off-diagonal tile -- so that all CTAs of
+ * the single wave runs about equally long; with the same count for every tile a launch took as long
+ * as its off-diagonal CTAs while the others idled (44 % of the SM-time at nao = 290).  Used while
+ * there are fewer lower tiles than SMs ("weighted"): with many waves the equal split does better
+ * (the cheap last block row runs last and shortens the tail: nao = 4000, 61.7 vs 63.1 ms). */
+__host__ __device__ inline int k2_tile_splits(int bi, int bj, int64_t nao, int nsplit)
+{
+    const int64_t rows = nao - (int64_t)bi * K2_T;
+    int c16 = bi == bj ? 9 : 16;                             /* cost in sixteenths of a full tile */
+    if (rows <= 64) c16 = (rows <= 32 ? 4 : 8) / (bi == bj ? 2 : 1);
+    const int s = (nsplit * c16 + 8) / 16;
+    return s < 1 ? 1 : s;
+}
+
 /* Triangular layout of a full-height DIAGONAL tile: the lower triangle in units of 16 x 16 (2 x 2
  * MMA tiles), strip r (rows 16r .. 16r+15) holding the units c = 0 .. r -- 36 units = 144 MMA tiles
  * where the square has 256 (an earlier 32 x 16 unit layout issued 192).  Warps 0-3 take five units
@@ -136,7 +153,7 @@ template <bool FULL>
 __global__ void __launch_bounds__(K2_THREADS, 1)
 k2_syrk_lower_kernel(const double *__restrict__ X4, int64_t nao, int64_t np, int64_t ldc4,
                      int64_t col04, int64_t col04b, int n4s, double *__restrict__ Kpart, int nsplit,
-                     int accumulate)
+                     int weighted, int accumulate)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -160,6 +177,10 @@ k2_syrk_lower_kernel(const double *__restrict__ X4, int64_t nao, int64_t np, int
     }
     const bool diag = !FULL && bi == bj;         /* both operands are the same panel */
     const int split = blockIdx.x;
+    if (!FULL && weighted) {                     /* this tile's own split count (k2_tile_splits) */
+        nsplit = k2_tile_splits(bi, bj, nao, nsplit);
+        if (split >= nsplit) return;
+    }
     const int64_t mu0 = (int64_t)bi * K2_T, nu0 = (int64_t)bj * K2_T;
 
     /* this split's share of the k groups (4 columns each) of the set */
@@ -546,9 +567,19 @@ k2p_kernel(const K2PArgs a)
                 for (int kc = 0; kc < nk; ++kc, ++st) {
                     const int slot = st % K2_STAGES;
                     const int round = st / K2_STAGES;
-                    if (w == 1 && pending && mbar_test_wait(item_done(pend_is), pend_phase)) {
-                        st_release_gpu(pend_flag, pend_val);
-                        pending = false;
+                    if (w == 1 && pending) {
+                        /* keep an eye on item_done while waiting for the slot: a finished item must be
+                         * published at once, the next item of its (slab, tile) chain may be waiting for
+                         * it in another CTA (published only between stages, the chains of a 21-tile
+                         * problem cost 13 % of K2 in flag waits) */
+                        while (true) {
+                            if (mbar_test_wait(item_done(pend_is), pend_phase)) {
+                                st_release_gpu(pend_flag, pend_val);
+                                pending = false;
+                                break;
+                            }
+                            if (round == 0 || mbar_try_wait_for(empty_bar(slot), (round - 1) & 1, 200)) break;
+                        }
                     }
                     if (round > 0) mbar_wait(empty_bar(slot), (round - 1) & 1);
                     const uint32_t dst = smem_base + slot * K2_STAGE_BYTES;
@@ -750,11 +781,13 @@ k2p_kernel(const K2PArgs a)
 constexpr int K3_T = 32;
 
 __global__ void __launch_bounds__(256)
-k3_finish_kernel(const double *__restrict__ Kpart, int nsplit, int64_t nao, double *__restrict__ Kdirect,
-                 double *const *__restrict__ Kslot)
+k3_finish_kernel(const double *__restrict__ Kpart, int nsplit, int weighted, int64_t nao,
+                 double *__restrict__ Kdirect, double *const *__restrict__ Kslot)
 {
     const int bi = blockIdx.y, bj = blockIdx.x;
     if (bj > bi) return;
+    /* partials of the split kernel: as many as the 128 x 128 tile around this block was cut into */
+    if (weighted) nsplit = k2_tile_splits(bi / (K2_T / K3_T), bj / (K2_T / K3_T), nao, nsplit);
     double *__restrict__ K = Kslot ? *Kslot : Kdirect;        /* see j3_unpack_kernel */
     __shared__ double t[K3_T][K3_T + 1];
     const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
@@ -841,7 +874,8 @@ void launch_k0_pack_c(const double *const *C, const int *nocc, const int *col0, 
 }
 
 cudaError_t launch_k2_syrk_lower(const double *X4, int64_t nao, int64_t np, int64_t ldc, int64_t col0,
-                                 int64_t ncol, double *Kpart, int nsplit, int accumulate, cudaStream_t st)
+                                 int64_t ncol, double *Kpart, int nsplit, int weighted, int accumulate,
+                                 cudaStream_t st)
 {
     static std::atomic<unsigned long long> smem_ok{0};
     const cudaError_t e = ensure_dynamic_smem(k2_syrk_lower_kernel<false>, K2_SMEM_BYTES, smem_ok);
@@ -850,7 +884,7 @@ cudaError_t launch_k2_syrk_lower(const double *X4, int64_t nao, int64_t np, int6
     const int ntile = nb * (nb + 1) / 2;
     const int n4s = (int)((ncol + 3) / 4);              /* k step 4: Ccat's padding to 8 is not read */
     k2_syrk_lower_kernel<false><<<dim3((unsigned)nsplit, (unsigned)ntile), K2_THREADS, K2_SMEM_BYTES, st>>>(
-        X4, nao, np, ldc / 4, col0 / 4, col0 / 4, n4s, Kpart, nsplit, accumulate);
+        X4, nao, np, ldc / 4, col0 / 4, col0 / 4, n4s, Kpart, nsplit, weighted, accumulate);
     return cudaPeekAtLastError();
 }
 
@@ -864,7 +898,7 @@ cudaError_t launch_k2_gemm_full(const double *X4, int64_t nao, int64_t np, int64
     const int nb = (int)((nao + K2_T - 1) / K2_T);
     const int n4s = (int)((ncol + 3) / 4);
     k2_syrk_lower_kernel<true><<<dim3((unsigned)nsplit, (unsigned)(nb * nb)), K2_THREADS, K2_SMEM_BYTES, st>>>(
-        X4, nao, np, ldc / 4, col0a / 4, col0b / 4, n4s, Kpart, nsplit, accumulate);
+        X4, nao, np, ldc / 4, col0a / 4, col0b / 4, n4s, Kpart, nsplit, 0, accumulate);
     return cudaPeekAtLastError();
 }
 
@@ -933,11 +967,21 @@ cudaError_t launch_k2p_gemm_full(const double *X4, int64_t nao, int64_t np, int6
                             sm_count, st);
 }
 
-void launch_k3_finish(const double *Kpart, int nsplit, int64_t nao, double *K, double *const *Kslot,
+int64_t k2_lower_items(int64_t nao, int nsplit)
+{
+    const int nb = (int)((nao + K2_T - 1) / K2_T);
+    /* rows 0 .. nb-2 are full height: bi off-diagonal tiles and one diagonal tile each */
+    int64_t items = 0;
+    for (int bi = 0; bi < nb; ++bi)
+        items += (int64_t)bi * k2_tile_splits(bi, 0, nao, nsplit) + k2_tile_splits(bi, bi, nao, nsplit);
+    return items;
+}
+
+void launch_k3_finish(const double *Kpart, int nsplit, int weighted, int64_t nao, double *K, double *const *Kslot,
                       cudaStream_t st)
 {
     const unsigned nb = (unsigned)((nao + K3_T - 1) / K3_T);
-    k3_finish_kernel<<<dim3(nb, nb), 256, 0, st>>>(Kpart, nsplit, nao, K, Kslot);
+    k3_finish_kernel<<<dim3(nb, nb), 256, 0, st>>>(Kpart, nsplit, weighted, nao, K, Kslot);
 }
 
 double fp64_peak_probe_flops(int ctas, int iters) { return (double)ctas * 8.0 * iters * 16.0 * 512.0; }
