@@ -107,6 +107,12 @@ def run_config(cfg_id, calls=(0,)):
             assert relerr(J2.cpu().numpy(), got[call][0]) <= 1e-12
             assert relerr(d2.cpu().numpy(), got[call][2]) <= 1e-12
             del J2, d2
+            # the same call again: every reduction has a fixed order (K2P's slab adds are `red` operations
+            # chained by a release/acquire counter per (slab, tile) over 148 CTAs) => bit for bit
+            rep = h.get_jk_u(Cd[0], Cd[1]) if unrestricted else h.get_jk(Cd[0])
+            torch.cuda.synchronize()
+            assert all(torch.equal(a, b) for a, b in zip(rep, out)), "repeat call differs bitwise"
+            del rep
         del out
 
     rows = sample_rows(cfg.nao)

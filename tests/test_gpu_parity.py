@@ -83,6 +83,11 @@ def test_baseline_configs_all_calls(dfjk, cfg_id):
     (200, 21, 140),     # nocc > 136: two N tiles in K1
     (257, 6, 31),
     (300, 40, 300),     # nocc = nao, three N tiles
+    (150, 11, 10),      # ragged last block of 22 rows: K1 batches it over 4 P, naux not a multiple of 4
+    (190, 7, 12),       # 62 rows: batched over 2 P, odd naux (the last ragged item holds one P)
+    (280, 9, 20),       # 24 rows after two full blocks
+    (400, 13, 30),      # 16 rows after three full blocks: batched over 8 P
+    (96, 5, 40),        # a single row block of 96 rows: not batched
 ])
 @pytest.mark.parametrize("k2_panel", [0, 1])       # both K2 kernels (the default picks by size)
 def test_ragged_shapes(dfjk, nao, naux, nocc, k2_panel):
@@ -112,6 +117,41 @@ def test_chunk_and_split_options(dfjk, opts):
     J, K, _ = run_restricted(dfjk, Bp, 260, C, **opts)
     Jo, Ko, _ = oracle.get_jk(Bp, 260, [C], [2.0])
     assert relerr(J, Jo) <= TOL and relerr(K, Ko[0]) <= TOL
+
+
+@pytest.mark.parametrize("nao,naux,nocc", [(290, 60, 25), (48, 40, 5), (400, 30, 33)])
+def test_weighted_splits(dfjk, nao, naux, nocc):
+    """The split kernel with per-tile split counts (k2_weighted = 1) and with one count for all tiles
+    (0) against the oracle; the automatic choice must be one of the two, bit for bit."""
+    Bp, (C,) = rand_case(nao, naux, (nocc,), seed=7 * nao + nocc)
+    Jo, Ko, _ = oracle.get_jk(Bp, nao, [C], [2.0])
+    res = {}
+    for w in (0, 1, 2):
+        J, K, _ = run_restricted(dfjk, Bp, nao, C, k2_panel=0, k2_weighted=w)
+        assert relerr(J, Jo) <= TOL and relerr(K, Ko[0]) <= TOL, w
+        assert np.array_equal(K, K.T)
+        res[w] = K
+    assert np.array_equal(res[2], res[0]) or np.array_equal(res[2], res[1])
+
+
+def test_panel_kernel_repeatable(dfjk):
+    """K2P with many short panels and few slabs: the slab adds of one (slab, tile) are chained across
+    CTAs by a release/acquire counter, so repeat calls must agree bit for bit."""
+    nao, naux, nocc = 260, 300, 20
+    Bp, (C,) = rand_case(nao, naux, (nocc,), seed=99)
+    h = dfjk.DFJK(dev(Bp), nao)
+    h.set_option("k2_panel", 1)
+    h.set_option("k2_panel_kb", 64)
+    Cd = dev(C)
+    ref = h.get_jk(Cd)
+    torch.cuda.synchronize()
+    Jo, Ko, _ = oracle.get_jk(Bp, nao, [C], [2.0])
+    assert relerr(ref[1].cpu().numpy(), Ko[0]) <= TOL
+    for _ in range(5):
+        again = h.get_jk(Cd)
+        torch.cuda.synchronize()
+        assert torch.equal(again[0], ref[0]) and torch.equal(again[1], ref[1])
+    h.close()
 
 
 @pytest.mark.parametrize("fused,k2_panel", [(1, 0), (0, 0), (1, 1)])
