@@ -68,8 +68,8 @@ constexpr int K2_THREADS = 32 * (1 + K2_CONSUMER_WARPS);
 constexpr int K2_SMEM_BYTES = K2_STAGES * K2_STAGE_BYTES + 2 * K2_STAGES * 8 + 16;
 
 /* Lower tiles are not equally expensive: a full-height diagonal tile issues 9/16 of the MMAs of an
- * off-diagonal one, a block row with <= 64 (<= 32) valid rows a half (a quarter), its diagonal tile
- * half of that again.  The split kernel therefore cuts the k range of a tile into a number of splits
+ * off-diagonal one, a ragged last block row its share of valid MMA rows (rect_stage_full / _narrow), its
+ * diagonal tile half of that when it has <= 64 rows.  The split kernel therefore cuts the k range of a tile into a number of splits
  * PROPORTIONAL to its cost -- nsplit is the count of a full off-diagonal tile -- so that all CTAs of
  * the single wave runs about equally long; with the same count for every tile a launch took as long
  * as its off-diagonal CTAs while the others idled (44 % of the SM-time at nao = 290).  Used while
@@ -79,7 +79,9 @@ __host__ __device__ inline int k2_tile_splits(int bi, int bj, int64_t nao, int n
 {
     const int64_t rows = nao - (int64_t)bi * K2_T;
     int c16 = bi == bj ? 9 : 16;                             /* cost in sixteenths of a full tile */
-    if (rows <= 64) c16 = (rows <= 16 ? 2 : (rows <= 32 ? 4 : 8)) / (bi == bj ? 2 : 1);
+    if (rows <= 64) c16 = (rows <= 16 ? 2 : (rows <= 32 ? 4 : 8)) / (bi == bj ? 2 : 1);   /* 1 x 8 layout */
+    else if (rows < K2_T && bi != bj) c16 = 8 + 2 * (int)((rows - 64 + 15) / 16);      /* 2 x 4: ragged lower warp row */
+    if (c16 < 1) c16 = 1;
     const int s = (nsplit * c16 + 8) / 16;
     return s < 1 ? 1 : s;
 }
@@ -145,28 +147,48 @@ __device__ __forceinline__ void tri_stage_units(double (*acc)[2], const double *
     }
 }
 
-/* one stage of a NARROW tile (a block row with <= 64 valid rows, 1 x 8 warp layout): NMT of the eight
- * 8-row MMA rows of the 64 x 16 warp tile hold valid rows.  A template parameter, not a runtime bound:
- * with `if (mt < nmt)` around the (non-volatile) MMA the compiler is free to issue it anyway and select
- * the result, and did (7.5 % more DMMAs at nao = 800). */
-template <int NMT>
-__device__ __forceinline__ void narrow_stage(double (*acc)[2], const double *a_base, const double *b_base, int n)
+/* one stage (n <= 8 k-groups) of a rectangular warp tile of NMT x NNT MMA tiles: acc[mt * 4 + nt].
+ * The tile shape is a TEMPLATE parameter, never a runtime bound: with `if (mt < nmt)` around the
+ * (non-volatile) MMA the compiler is free to issue it anyway and select the result, and did (7.5 % more
+ * DMMAs at nao = 800, visible only in ncu's op count). */
+template <int NMT, int NNT>
+__device__ __forceinline__ void rect_stage(double (*acc)[2], const double *a_base, const double *b_base, int n)
 {
 #pragma unroll
     for (int q = 0; q < K2_KG; ++q) {
         if (q < n) {
-            double a[NMT], b[2];
+            double a[NMT], b[NNT];
 #pragma unroll
             for (int mt = 0; mt < NMT; ++mt) a[mt] = a_base[q * (K2_T * 4) + mt * 32];
 #pragma unroll
-            for (int nt = 0; nt < 2; ++nt) b[nt] = b_base[q * (K2_T * 4) + nt * 32];
+            for (int nt = 0; nt < NNT; ++nt) b[nt] = b_base[q * (K2_T * 4) + nt * 32];
 #pragma unroll
             for (int mt = 0; mt < NMT; ++mt)
 #pragma unroll
-                for (int nt = 0; nt < 2; ++nt)
+                for (int nt = 0; nt < NNT; ++nt)
                     dmma884(acc[mt * 4 + nt][0], acc[mt * 4 + nt][1], a[mt], b[nt]);
         }
     }
+}
+
+/* ... with the number of valid 8-row MMA rows of the warp tile chosen at run time (warp-uniform), from
+ * a SHORT list: ragged block rows cost what they hold in steps of 16 rows (2 x 4 layout: 2, 4, 6 or 8 MMA
+ * rows in the lower warp row) or 16 / 32 / 64 rows (1 x 8 layout).  One instantiation per MMA row count
+ * (8 + 8 unrolled loops) cost more in instruction fetch than it saved: cfg 4 K2 +1.5 %, cfg 2 +21 %. */
+__device__ __forceinline__ void rect_stage_full(int nmt, double (*acc)[2], const double *a_base,
+                                                const double *b_base, int n)
+{
+    if (nmt > 6) rect_stage<8, 4>(acc, a_base, b_base, n);
+    else if (nmt > 4) rect_stage<6, 4>(acc, a_base, b_base, n);
+    else if (nmt > 2) rect_stage<4, 4>(acc, a_base, b_base, n);
+    else rect_stage<2, 4>(acc, a_base, b_base, n);
+}
+__device__ __forceinline__ void rect_stage_narrow(int nmt, double (*acc)[2], const double *a_base,
+                                                  const double *b_base, int n)
+{
+    if (nmt > 4) rect_stage<8, 2>(acc, a_base, b_base, n);
+    else if (nmt > 2) rect_stage<4, 2>(acc, a_base, b_base, n);
+    else rect_stage<2, 2>(acc, a_base, b_base, n);
 }
 
 /* FULL == false: the SYRK above (one column range, lower tiles only).
@@ -263,7 +285,7 @@ k2_syrk_lower_kernel(const double *__restrict__ X4, int64_t nao, int64_t np, int
      * rows would leave the lower four warps idle: it is covered 1 (M) x 8 (N) with 64 x 16 warp
      * tiles instead, so all eight warps share the work ("narrow"; CTA-uniform). */
     const bool narrow = nao - mu0 <= 64;
-    const int nmt_narrow = nao - mu0 <= 16 ? 2 : (nao - mu0 <= 32 ? 4 : 8);   /* MMA rows of a narrow warp tile in use */
+
     /* A full-height diagonal tile needs only its lower triangle: see tri_unit() ("tri"; the 2 x 4
      * layout would leave two warps idle and the CTA would take as long as an off-diagonal one). */
     const bool tri = diag && !narrow;
@@ -274,6 +296,8 @@ k2_syrk_lower_kernel(const double *__restrict__ X4, int64_t nao, int64_t np, int
     const int wcols = narrow ? 16 : 32;          /* columns per warp tile (2 x 4 and 1 x 8 layouts) */
     const int lq = lane >> 2, lr = lane & 3;
     const int row_w = tri ? 16 * (7 - (cw & 3)) : (tall ? 32 * (cw >> 1) : 64 * wm);   /* first row / column of this warp's tile */
+    /* valid 8-row MMA rows of a rectangular (2 x 4 or 1 x 8) warp tile: ragged block rows in steps of 8 */
+    const int nmt_w = (int)((nao - mu0 - row_w + 7) / 8 < 8 ? (nao - mu0 - row_w + 7) / 8 : 8);
     const int col_w = tri ? 0 : (tall ? 32 * (cw & 1) : wcols * wn);
     int ua[4] = {0, 0, 0, 0}, ub[4] = {0, 0, 0, 0};       /* tri, cw >= 4: the four units' panel offsets */
     if (tri && cw >= 4) {
@@ -303,46 +327,14 @@ k2_syrk_lower_kernel(const double *__restrict__ X4, int64_t nao, int64_t np, int
             const double *a_base = Xa + (row_w + lq) * 4 + lr;
             const double *b_base = Xb + (col_w + lq) * 4 + lr;
             if (tall) {
-#pragma unroll
-                for (int q = 0; q < K2_KG; ++q) {
-                    if (q < n) {
-                        double a[4], b[4];
-#pragma unroll
-                        for (int mt = 0; mt < 4; ++mt) a[mt] = a_base[q * (K2_T * 4) + mt * 32];
-#pragma unroll
-                        for (int nt = 0; nt < 4; ++nt) b[nt] = b_base[q * (K2_T * 4) + nt * 32];
-#pragma unroll
-                        for (int mt = 0; mt < 4; ++mt)
-#pragma unroll
-                            for (int nt = 0; nt < 4; ++nt)
-                                dmma884(acc[mt * 4 + nt][0], acc[mt * 4 + nt][1], a[mt], b[nt]);
-                    }
-                }
+                rect_stage<4, 4>(acc, a_base, b_base, n);
             } else if (tri) {
                 if (cw < 4) tri_stage_wide(acc, a_base, b_base, n);
                 else tri_stage_units(acc, Xa, ua, ub, n);
             } else if (!narrow) {
-#pragma unroll
-                for (int q = 0; q < K2_KG; ++q) {
-                    if (q < n) {
-                        double a[8], b[4];
-#pragma unroll
-                        for (int mt = 0; mt < 8; ++mt) a[mt] = a_base[q * (K2_T * 4) + mt * 32];
-#pragma unroll
-                        for (int nt = 0; nt < 4; ++nt) b[nt] = b_base[q * (K2_T * 4) + nt * 32];
-#pragma unroll
-                        for (int mt = 0; mt < 8; ++mt)
-#pragma unroll
-                            for (int nt = 0; nt < 4; ++nt)
-                                dmma884(acc[mt * 4 + nt][0], acc[mt * 4 + nt][1], a[mt], b[nt]);
-                    }
-                }
-            } else if (nmt_narrow == 2) {
-                narrow_stage<2>(acc, a_base, b_base, n);
-            } else if (nmt_narrow == 4) {
-                narrow_stage<4>(acc, a_base, b_base, n);
+                rect_stage_full(nmt_w, acc, a_base, b_base, n);
             } else {
-                narrow_stage<8>(acc, a_base, b_base, n);
+                rect_stage_narrow(nmt_w, acc, a_base, b_base, n);
             }
         }
         __syncwarp();
@@ -664,12 +656,13 @@ k2p_kernel(const K2PArgs a)
         const int64_t gbeg = ng * p / a.npanel, gend = ng * (p + 1) / a.npanel;
         const int nk = (int)((gend - gbeg + K2_KG - 1) / K2_KG);
         const bool narrow = nao - mu0 <= 64;
-        const int nmt_narrow = nao - mu0 <= 16 ? 2 : (nao - mu0 <= 32 ? 4 : 8);   /* MMA rows of a narrow warp tile in use */
+    
         const bool tri = diag && !narrow;
         const bool tall = FULL && !narrow && nao - nu0 <= 64;
         const int wm = narrow ? 0 : cw >> 2, wn = narrow ? cw : cw & 3;
         const int wcols = narrow ? 16 : 32;
         const int row_w = tri ? 16 * (7 - (cw & 3)) : (tall ? 32 * (cw >> 1) : 64 * wm);
+        const int nmt_w = (int)((nao - mu0 - row_w + 7) / 8 < 8 ? (nao - mu0 - row_w + 7) / 8 : 8);   /* valid MMA rows */
         const int col_w = tri ? 0 : (tall ? 32 * (cw & 1) : wcols * wn);
         const bool warp_active = tri || ((mu0 + row_w < nao) && (nu0 + col_w < nao) &&
                                          !(diag && col_w > row_w + 63));
@@ -688,46 +681,14 @@ k2p_kernel(const K2PArgs a)
                 const double *a_base = Xa + (row_w + lq) * 4 + lr;
                 const double *b_base = Xb + (col_w + lq) * 4 + lr;
                 if (tall) {
-#pragma unroll
-                    for (int q = 0; q < K2_KG; ++q) {
-                        if (q < n) {
-                            double av[4], bv[4];
-#pragma unroll
-                            for (int mt = 0; mt < 4; ++mt) av[mt] = a_base[q * (K2_T * 4) + mt * 32];
-#pragma unroll
-                            for (int nt = 0; nt < 4; ++nt) bv[nt] = b_base[q * (K2_T * 4) + nt * 32];
-#pragma unroll
-                            for (int mt = 0; mt < 4; ++mt)
-#pragma unroll
-                                for (int nt = 0; nt < 4; ++nt)
-                                    dmma884(acc[mt * 4 + nt][0], acc[mt * 4 + nt][1], av[mt], bv[nt]);
-                        }
-                    }
+                    rect_stage<4, 4>(acc, a_base, b_base, n);
                 } else if (tri) {
                     if (cw < 4) tri_stage_wide(acc, a_base, b_base, n);
                     else tri_stage_units(acc, Xa, ua, ub, n);
                 } else if (!narrow) {
-#pragma unroll
-                    for (int q = 0; q < K2_KG; ++q) {
-                        if (q < n) {
-                            double av[8], bv[4];
-#pragma unroll
-                            for (int mt = 0; mt < 8; ++mt) av[mt] = a_base[q * (K2_T * 4) + mt * 32];
-#pragma unroll
-                            for (int nt = 0; nt < 4; ++nt) bv[nt] = b_base[q * (K2_T * 4) + nt * 32];
-#pragma unroll
-                            for (int mt = 0; mt < 8; ++mt)
-#pragma unroll
-                                for (int nt = 0; nt < 4; ++nt)
-                                    dmma884(acc[mt * 4 + nt][0], acc[mt * 4 + nt][1], av[mt], bv[nt]);
-                        }
-                    }
-                } else if (nmt_narrow == 2) {
-                    narrow_stage<2>(acc, a_base, b_base, n);
-                } else if (nmt_narrow == 4) {
-                    narrow_stage<4>(acc, a_base, b_base, n);
+                    rect_stage_full(nmt_w, acc, a_base, b_base, n);
                 } else {
-                    narrow_stage<8>(acc, a_base, b_base, n);
+                    rect_stage_narrow(nmt_w, acc, a_base, b_base, n);
                 }
             }
             __syncwarp();
