@@ -259,7 +259,9 @@ j1_dot_kernel(const double *__restrict__ B, int64_t naux, int64_t npair,
  * d_part[blockIdx.x][P] (deterministic; J1R adds the blocks). */
 constexpr int J1X_PB = 16;            /* P per CTA */
 constexpr int J1X_PARTS = 256 / J1X_PB;
-constexpr int J1X_TILES = 8;          /* tiles of 256 units per CTA */
+constexpr int J1X_TILES = 1;          /* tiles of 256 units per CTA: swept on B200 at cfg 4, PB x TILES = 16 x 8:
+                                         2.10 ms, 16 x 2: 1.50, 8 x 1: 1.41, 16 x 1: 1.29 ms (6.7 TB/s) -- short CTAs,
+                                         many in flight; J1R then adds 425 instead of 53 partials per P */
 
 __global__ void __launch_bounds__(256)
 j1x_dot_kernel(const double *__restrict__ X4, const double *__restrict__ Ccat4, int64_t nao, int64_t np,
@@ -312,14 +314,27 @@ j1x_dot_kernel(const double *__restrict__ X4, const double *__restrict__ Ccat4, 
     }
 }
 
-__global__ void j1_reduce_kernel(const double *__restrict__ d_part, int64_t nchunk, int64_t naux,
-                                 double *__restrict__ d)
+/* d[P] = sum_c d_part[c][P]: 32 P x 8 groups per CTA, group g adds the chunks c = g, g + 8, ... (loads
+ * pipelined), the eight group sums are added in order: a fixed order, as everywhere */
+__global__ void __launch_bounds__(256)
+j1_reduce_kernel(const double *__restrict__ d_part, int64_t nchunk, int64_t naux, double *__restrict__ d)
 {
-    const int64_t P = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (P >= naux) return;
+    __shared__ double gs[8][33];
+    const int pl = threadIdx.x & 31, g = threadIdx.x >> 5;
+    const int64_t P = (int64_t)blockIdx.x * 32 + pl;
     double acc = 0.0;
-    for (int64_t c = 0; c < nchunk; ++c) acc += d_part[c * naux + P];
-    d[P] = acc;
+    if (P < naux) {
+#pragma unroll 8
+        for (int c = g; c < (int)nchunk; c += 8) acc += d_part[(int64_t)c * naux + P];
+    }
+    gs[g][pl] = acc;
+    __syncthreads();
+    if (g == 0 && P < naux) {
+        double v = gs[0][pl];
+#pragma unroll
+        for (int q = 1; q < 8; ++q) v += gs[q][pl];
+        d[P] = v;
+    }
 }
 
 /* ------------------------------------------------------------------ J2 */
@@ -498,7 +513,7 @@ void launch_j1x_dot(const double *X4, const double *Ccat4, int64_t nao, int64_t 
 
 void launch_j1_reduce(const double *d_part, int64_t nchunk, int64_t naux, double *d, cudaStream_t st)
 {
-    j1_reduce_kernel<<<(unsigned)((naux + 127) / 128), 128, 0, st>>>(d_part, nchunk, naux, d);
+    j1_reduce_kernel<<<(unsigned)((naux + 31) / 32), 256, 0, st>>>(d_part, nchunk, naux, d);
 }
 
 int64_t j2_num_groups(int64_t naux, int64_t npair, int sm_count)
