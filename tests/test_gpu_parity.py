@@ -154,6 +154,30 @@ def test_panel_kernel_repeatable(dfjk):
     h.close()
 
 
+def test_panel_kernel_stress_all_sms(dfjk):
+    """K2P with every SM busy (nao = 900: 36 tiles, hundreds of short panels, one or two slabs): ten
+    calls must agree bit for bit with each other (the cross-CTA chains of `red` adds are ordered by
+    release/acquire counters) and, up to summation order, with the split kernel."""
+    cfg = gi.custom_config(900, 700, (70,), seed=123)
+    B = torch.empty(cfg.naux, cfg.npair, dtype=torch.float64, device="cuda")
+    gi.fill_B_device(cfg, B)
+    C = dev(gi.random_orbitals(cfg.nao, 70, 5))
+    h = dfjk.DFJK(B, cfg.nao)
+    h.set_option("k2_panel", 0)
+    _, Ksplit = h.get_jk(C, with_j=False)
+    h.set_option("k2_panel", 1)
+    h.set_option("k2_panel_kb", 1024)
+    _, Kref = h.get_jk(C, with_j=False)
+    torch.cuda.synchronize()
+    assert relerr(Kref.cpu().numpy(), Ksplit.cpu().numpy()) <= 1e-13
+    assert torch.equal(Kref, Kref.T)
+    for _ in range(10):
+        _, K = h.get_jk(C, with_j=False)
+        torch.cuda.synchronize()
+        assert torch.equal(K, Kref)
+    h.close()
+
+
 @pytest.mark.parametrize("fused,k2_panel", [(1, 0), (0, 0), (1, 1)])
 def test_unrestricted(dfjk, fused, k2_panel):
     nao, naux = 210, 33
