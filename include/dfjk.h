@@ -258,8 +258,8 @@ int dfjk_get_d(dfjk_handle *h, double *d_out, void *stream);
  *               partial K per range; 1 = panel-synchronous (the k range is cut into short panels,
  *               items (panel, tile) are dealt dynamically to persistent CTAs and added in panel
  *               order into L2-resident slabs, so that X is read from HBM once instead of ~8 times);
- *               2 (default) = 1 when the X chunk is larger than L2, a slab (nao^2 doubles) is
- *               at most a third of it and there are at least 21 lower tiles (nao > 640), else 0.
+ *               2 (default) = 1 when the X chunk is larger than L2 and there are at least 21
+ *               lower tiles (nao > 640), else 0.
  *   "k2_panel_kb"  target size in KB of one k panel of X for "k2_panel" (default 32768)
  *   "k2_weighted"  split counts of the "k2_panel" = 0 kernel: 0 = the same for every lower tile; 1 = in
  *               proportion to the tile's cost (diagonal and ragged tiles are cheaper), so that the

@@ -369,13 +369,13 @@ int enqueue_jk_body(dfjk_handle *h, int nset, const int *nocc, const int *col0, 
         if (h->opt_k_chunk > 0 && h->opt_k_chunk < pc) pc = h->opt_k_chunk;
         if (pc > naux) pc = naux;
         if (pc < 1) return fail(DFJK_ENOMEM, "%s: X workspace too small", who);
-        /* K2P pays a read-modify-write per item to keep the k window of X inside L2; an X chunk that
-         * fits in L2 whole has nothing to gain from it (and small problems are all overhead), and the
-         * slab it adds into (nao^2 doubles) must itself stay in L2 beside the window */
+        /* K2P pays an add per item to keep the k window of X inside L2; an X chunk that fits in L2
+         * whole has nothing to gain from it, and small problems are all overhead.  The slab it adds
+         * into need NOT stay in L2 since the adds are `red` operations (nobody waits for the line):
+         * nao = 4000, a 128 MB slab: 61.0 ms against the split kernel's 62.5 */
         const int nbk = (int)((nao + 127) / 128);
         const bool panel = h->opt_k2_panel == 1 ||
-                           (h->opt_k2_panel == 2 && pc * nao * ldc * 8 > h->l2_bytes && nao * nao * 8 * 3 <= h->l2_bytes &&
-                            nbk >= DFJK_K2P_MIN_NB);
+                           (h->opt_k2_panel == 2 && pc * nao * ldc * 8 > h->l2_bytes && nbk >= DFJK_K2P_MIN_NB);
         /* the split kernel balances a single wave tile by tile when the chunk of X it re-reads stays in
          * L2 (tiles then cut the k range at different places: no two CTAs stream the same lines together) */
         const bool weighted = !panel && h->nsplit_weighted > 0 && h->opt_k_splits == 0 &&
@@ -583,7 +583,7 @@ int get_jk_general_impl(dfjk_handle *h, const double *C1, const double *C2, int6
         if (pc < 1) return fail(DFJK_ENOMEM, "%s: X workspace too small", who);
         const int nb = (int)((nao + 127) / 128);
         const bool panel = h->opt_k2_panel == 1 ||
-                           (h->opt_k2_panel == 2 && pc * nao * ldx * 8 > h->l2_bytes && nao * nao * 8 * 3 <= h->l2_bytes);
+                           (h->opt_k2_panel == 2 && pc * nao * ldx * 8 > h->l2_bytes && nb >= DFJK_K2P_MIN_NB - 1);
         int nsplit = h->opt_k_splits > 0 ? (int)h->opt_k_splits
                                          : choose_splits(nb * nb, h->sm_count, h->nsplit_alloc);
         int pstages = 0;
