@@ -15,11 +15,14 @@
  * the same pattern; diagonal tiles load the panel once and use a triangular warp layout (the
  * 36 units of 16 x 16 that touch the lower triangle, five or four per warp: tri_unit); block rows with
  * <= 64 valid rows use a 1 x 8 layout of 64 x 16 warp tiles (and, in the full product, block columns
- * with <= 64 valid columns a 4 x 2 layout of 32 x 32), so no warp idles on ragged tiles.
+ * with <= 64 valid columns a 4 x 2 layout of 32 x 32), so no warp idles on ragged tiles; the number
+ * of valid 8-row MMA rows of a ragged warp tile is a template parameter (rect_stage).
  * The same kernel with FULL = true covers all nb x nb tiles with operands from two column
  * ranges of X (the non-symmetric product of the general-density entry points).
  * Splits: work item = (lower tile, split) with its own partial accumulator Kpart[split],
- * read-modify-written by exactly one CTA per launch => deterministic, no atomics.
+ * read-modify-written by exactly one CTA per launch => deterministic, no atomics; small problems
+ * cut each tile in proportion to its cost (k2_tile_splits).
+ * Larger problems (>= 21 lower tiles, X chunk beyond L2) run the panel-synchronous K2P kernel below.
  */
 #include "dfjk_internal.h"
 #include "k_common.cuh"
