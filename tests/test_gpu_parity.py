@@ -154,6 +154,28 @@ def test_panel_kernel_repeatable(dfjk):
     h.close()
 
 
+@pytest.mark.parametrize("nao,naux,nocc,chunk", [(656, 301, 57, 77), (736, 203, 140, 50), (1000, 150, 90, 0)])
+def test_midsize_ragged_multichunk(dfjk, nao, naux, nocc, chunk):
+    """Mid-size shapes against the full oracle: a 16-row (656), 96-row (736) and 104-row (1000) last
+    block, chunks whose length is not a multiple of K1's batching group (partial last groups in every
+    chunk), two N tiles (nocc 140), both K2 kernels, unrestricted on top of the restricted call."""
+    Bp, (C,) = rand_case(nao, naux, (nocc,), seed=nao + 3)
+    Jo, Ko, _ = oracle.get_jk(Bp, nao, [C], [2.0])
+    for k2_panel in (0, 1):
+        J, K, _ = run_restricted(dfjk, Bp, nao, C, k_chunk=chunk, k2_panel=k2_panel, k2_panel_kb=512)
+        assert relerr(J, Jo) <= TOL and relerr(K, Ko[0]) <= TOL, k2_panel
+        assert np.array_equal(K, K.T)
+    Cb = gi.random_orbitals(nao, nocc - 7, 4242)
+    h = dfjk.DFJK(dev(Bp), nao)
+    h.set_option("k_chunk", chunk)
+    Ju, Ka, Kb = h.get_jk_u(dev(C), dev(Cb))
+    torch.cuda.synchronize()
+    Juo, Kao, Kbo = oracle.get_jk_unrestricted(Bp, nao, C, Cb)
+    assert relerr(Ju.cpu().numpy(), Juo) <= TOL
+    assert relerr(Ka.cpu().numpy(), Kao) <= TOL and relerr(Kb.cpu().numpy(), Kbo) <= TOL
+    h.close()
+
+
 def test_panel_kernel_stress_all_sms(dfjk):
     """K2P with every SM busy (nao = 900: 36 tiles, hundreds of short panels, one or two slabs): ten
     calls must agree bit for bit with each other (the cross-CTA chains of `red` adds are ordered by
