@@ -223,6 +223,47 @@ int dfjk_build_b(int64_t naux, int64_t nao, double *M, double *R_packed, int64_t
 int dfjk_get_df_diag(dfjk_handle *h, double *diag, void *stream);
 
 /*
+ * dfjk_df_diag_noalloc -- the same Eq. 7 diagonal as dfjk_get_df_diag,
+ *     diag[mu][nu] = sum_P T_{P,mu nu}^2,
+ * WITHOUT a handle and without a single device allocation, for callers that cannot allocate:
+ * code running inside a framework whose caching allocator already owns the device (a stray
+ * cudaMalloc there fails or fragments the pool), code bound by a "no allocation after start-up"
+ * rule (cudaMalloc / cudaFree synchronise the whole device and would stall a serving or
+ * real-time loop), and processes that have given every free byte of HBM to B itself.  Such
+ * callers cannot use dfjk_create, whose workspace comes from cudaMalloc.
+ *
+ *   naux, nao  as in dfjk_create, with nao <= DFJK_NOALLOC_MAX_NAO (= dfjk_noalloc_max_nao());
+ *              naux is not limited.  A larger nao is DFJK_EINVAL with a message naming the limit.
+ *   B_packed   DEVICE, naux*npair doubles, packed as in dfjk_create, 16-byte aligned, read only.
+ *   diag       DEVICE, nao x nao, OVERWRITTEN, both triangles written.
+ *   stream     cudaStream_t; the call only enqueues two kernels (the J2 stream with every element
+ *              weighted by itself, then the J3 unpack) and returns.
+ *
+ * Scratch: the per-row-group partial triangles that the handle keeps in its workspace live here in
+ * a fixed array of DFJK_NOALLOC_SCRATCH_BYTES inside the library image; every GPU that loads
+ * libdfjk.so holds it until the process exits.  The call uses cudaMalloc, cudaFree or an
+ * allocating library routine nowhere.  Consequences the caller has to know:
+ *   - The FIRST call on each device looks up the array's device address (cudaGetSymbolAddress)
+ *     and the SM count, with that device current; make that first call during start-up, before
+ *     any stream capture begins.  Later calls on the device reuse the cached values.
+ *   - All calls on a device share the one array, which simply keeps what the last call wrote.
+ *     Nothing in it needs to be zero at entry (each call overwrites every partial it later
+ *     reads), so calls of different sizes may follow each other freely -- but two calls whose
+ *     kernels can run at the same time on the GPU (different streams without an event between
+ *     them, or two host threads) RACE on it and give garbage.  Order them on one stream or with
+ *     events.  Handle-based calls are unaffected: they never touch this array.
+ *   - With fewer row groups than the handle path would choose when the array is the limit
+ *     (nao > ~500), the additions happen in another order: results agree with dfjk_get_df_diag to
+ *     rounding (the library's 1e-11 relative Frobenius bar), not necessarily bit for bit.
+ */
+#define DFJK_NOALLOC_SCRATCH_BYTES 8388608   /* 8 MiB = 1048576 doubles */
+#define DFJK_NOALLOC_MAX_NAO       1023      /* 2 * npair = nao (nao + 1) <= 1048576 */
+int dfjk_df_diag_noalloc(int64_t naux, int64_t nao, const double *B_packed, double *diag,
+                         void *stream);
+/* the largest nao dfjk_df_diag_noalloc accepts (DFJK_NOALLOC_MAX_NAO of the loaded library) */
+int64_t dfjk_noalloc_max_nao(void);
+
+/*
  * dfjk_get_jk_u_host -- the unrestricted build (dfjk_get_jk_u) for HOST orbitals and results, with the
  * same copy-in / run / copy-out / synchronise sequence as dfjk_get_jk_host.
  *   C_a_host (nao x nocc_a), C_b_host (nao x nocc_b): HOST;  J_host, K_a_host, K_b_host: HOST nao x nao,

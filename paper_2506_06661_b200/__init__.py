@@ -17,7 +17,7 @@ import os
 import subprocess
 from typing import Optional, Tuple
 
-__all__ = ["build", "lib", "build_b", "device_info", "probe_fp64_peak", "DFJK", "DFJKError", "SYMBOLS", "KERNELS", "LIB_PATH", "HEADER_PATH"]
+__all__ = ["build", "lib", "build_b", "df_diag_noalloc", "noalloc_max_nao", "device_info", "probe_fp64_peak", "DFJK", "DFJKError", "SYMBOLS", "KERNELS", "LIB_PATH", "HEADER_PATH"]
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libdfjk.so")
@@ -32,6 +32,7 @@ SYMBOLS = (
     "dfjk_get_jk_pair", "dfjk_get_jk_dm", "dfjk_get_jk_dms", "dfjk_get_df_diag",
     "dfjk_build_b", "dfjk_scf_rhf", "dfjk_probe_dmma_peak",
     "dfjk_get_jk_u_host", "dfjk_scf_uhf", "dfjk_device_info", "dfjk_scf_timing",
+    "dfjk_df_diag_noalloc", "dfjk_noalloc_max_nao",
 )
 
 # DFJK_KERNEL_* ids of include/dfjk.h
@@ -93,6 +94,10 @@ def lib() -> ctypes.CDLL:
     L.dfjk_build_b.argtypes = [i64, i64, vp, vp, vp, vp]
     L.dfjk_get_df_diag.restype = ci
     L.dfjk_get_df_diag.argtypes = [vp, vp, vp]
+    L.dfjk_df_diag_noalloc.restype = ci
+    L.dfjk_df_diag_noalloc.argtypes = [i64, i64, vp, vp, vp]
+    L.dfjk_noalloc_max_nao.restype = i64
+    L.dfjk_noalloc_max_nao.argtypes = []
     L.dfjk_get_jk_host.restype = ci
     L.dfjk_get_jk_host.argtypes = [vp, vp, i64, vp, vp]
     L.dfjk_get_jk_u_host.restype = ci
@@ -165,6 +170,34 @@ def build_b(M, R_packed, nao: int, stream=None):
         st = (stream or torch.cuda.current_stream(R_packed.device)).cuda_stream
         _check(lib().dfjk_build_b(naux, nao, mp, rp, info.data_ptr(), st), "dfjk_build_b")
     return info
+
+
+def noalloc_max_nao() -> int:
+    """Largest nao ``df_diag_noalloc`` accepts (its scratch is a fixed 8 MiB array in the library)."""
+    return int(lib().dfjk_noalloc_max_nao())
+
+
+def df_diag_noalloc(B_packed, nao: int, out, stream=None):
+    """``out[mu][nu] = sum_P B_P[mu,nu]^2`` (Eq. 7) through ``dfjk_df_diag_noalloc``:
+    no handle and no device allocation anywhere, for callers that cannot allocate -- code living
+    inside another framework's memory pool, code under a no-allocation-after-start-up rule, or a
+    process whose HBM is already full of B.  That is why ``out`` (nao x nao CUDA float64) is the
+    caller's buffer and not created here.  ``nao <= noalloc_max_nao()``; larger sizes raise.
+
+    All calls on a device share one scratch array inside the library: issue them on one stream (or
+    order them with events), never concurrently.  Make the first call on a device during start-up,
+    outside any stream capture (it looks up the array's device address once)."""
+    import torch
+    nao = int(nao)
+    npair = nao * (nao + 1) // 2
+    if B_packed.dim() != 2 or B_packed.shape[1] != npair:
+        raise ValueError(f"B_packed must be [naux][{npair}]")
+    bp = _dev_f64(B_packed, "B_packed")
+    op = _dev_f64(out, "out", nao * nao)
+    with torch.cuda.device(B_packed.device):
+        st = (stream or torch.cuda.current_stream(B_packed.device)).cuda_stream
+        _check(lib().dfjk_df_diag_noalloc(int(B_packed.shape[0]), nao, bp, op, st), "dfjk_df_diag_noalloc")
+    return out
 
 
 class DFJK:

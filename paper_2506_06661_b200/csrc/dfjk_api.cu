@@ -56,6 +56,17 @@ int64_t round_up(int64_t x, int64_t m) { return (x + m - 1) / m * m; }
 
 }  // namespace
 
+/* for the entry points that live in other translation units (df_diag_noalloc.cu): the same
+ * thread-local text dfjk_last_error() returns */
+int dfjk::set_last_error(int code, const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof g_err, fmt, ap);
+    va_end(ap);
+    return code;
+}
+
 #define DFJK_GRAPH_SLOTS 4
 #ifndef DFJK_K2P_MIN_NB
 #define DFJK_K2P_MIN_NB 6   /* K2P needs enough tiles per panel: below 21 lower tiles the split kernel wins */

@@ -139,6 +139,12 @@ void launch_fp64_tile_gemm(const double *A, int64_t lda, const double *Bop, int6
 
 }  // namespace dfjk
 
+/* ---------------------------------------------------------------- error text */
+namespace dfjk {
+/* printf-style: stores the calling thread's dfjk_last_error() text and returns `code` */
+int set_last_error(int code, const char *fmt, ...);
+}  // namespace dfjk
+
 /* ---------------------------------------------------------------- SCF driver (scf_rhf.cu) */
 struct dfjk_handle;
 namespace dfjk {

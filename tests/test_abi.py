@@ -42,6 +42,13 @@ def test_version_and_null_handling(L):
     assert L.dfjk_get_jk_dm(None, None, None, None, None) == -1
     assert L.dfjk_get_jk_dms(None, 1, None, None, None, None) == -1
     assert L.dfjk_get_df_diag(None, None, None) == -1
+    # the allocation-free entry point: argument checks come before any CUDA call
+    assert L.dfjk_noalloc_max_nao() == 1023
+    assert L.dfjk_df_diag_noalloc(4, 4, None, None, None) == -1
+    assert b"NULL" in L.dfjk_last_error()
+    assert L.dfjk_df_diag_noalloc(0, 4, None, None, None) == -1
+    assert L.dfjk_df_diag_noalloc(4, 1024, None, None, None) == -1
+    assert b"1023" in L.dfjk_last_error() and b"scratch" in L.dfjk_last_error()
     assert L.dfjk_scf_rhf(None, None, None, 1, 1, 1e-8, 4, None, None, None, None, None, None, None, None) == -1
     assert b"NULL handle" in L.dfjk_last_error()
     assert L.dfjk_probe_dmma_peak(None) == -1
