@@ -300,8 +300,11 @@ int dfjk_get_d(dfjk_handle *h, double *d_out, void *stream);
  *               items (panel, tile) are dealt dynamically to persistent CTAs and added in panel
  *               order into L2-resident slabs, so that X is read from HBM once instead of ~8 times);
  *               2 (default) = 1 when the X chunk is larger than L2 and there are at least 21
- *               lower tiles (nao > 640), else 0.
- *   "k2_panel_kb"  target size in KB of one k panel of X for "k2_panel" (default 32768)
+ *               lower tiles (nao > 640), else 0.  The full (non-symmetric) product of
+ *               dfjk_get_jk_pair / _dm has nb^2 tiles instead of nb(nb+1)/2 and switches one block
+ *               row earlier: at nb >= 5 (nao > 512, 25 tiles).
+ *   "k2_panel_kb"  target size in KB of one k panel of X for "k2_panel" (default 32768; accepted
+ *               range 64 .. 4194304)
  *   "k2_weighted"  split counts of the "k2_panel" = 0 kernel: 0 = the same for every lower tile; 1 = in
  *               proportion to the tile's cost (diagonal and ragged tiles are cheaper), so that the
  *               CTAs of a single wave run equally long; 2 (default) = 1 when there are no more lower
@@ -338,7 +341,8 @@ int64_t dfjk_launch_count(const dfjk_handle *h);
  * dfjk_kernel_time -- with option "time_kernels" = 1: total device time (ms, CUDA events
  * on the launching stream) and number of launches of kernel `kernel` (DFJK_KERNEL_*)
  * recorded since the option was last set.  Waits for the recorded events (HOST pointers
- * ms_total, count).  At most 16384 launches are recorded.
+ * ms_total, count).  The event ring grows as needed (1024 launches at first, doubling); if it
+ * cannot grow, later launches go unrecorded and this call reports DFJK_ENOMEM.
  */
 int dfjk_kernel_time(dfjk_handle *h, int kernel, double *ms_total, int64_t *count);
 
@@ -366,7 +370,9 @@ int dfjk_probe_dmma_peak(double *tflops);
  * (HOST pointers, any may be NULL), measured with CUDA events on the run's stream: iterations done,
  * total ms inside get_jk / get_jk_u, total ms inside the eigensolver (cuSOLVER Dsygvd, core guess
  * included) and everything else (Fock, density, energy, DIIS error and extrapolation, host solves
- * and read-backs).  DFJK_EINVAL if no SCF has run.  PAPER.md:258-262 (the SCF loop).
+ * and read-backs).  DFJK_EINVAL if there is nothing valid to report: no SCF has run, or the last run
+ * failed or could not create / record one of its events (a run never reports an earlier run's
+ * figures).  PAPER.md:258-262 (the SCF loop).
  */
 int dfjk_scf_timing(const dfjk_handle *h, int64_t *iters, double *get_jk_ms, double *eig_ms, double *other_ms);
 

@@ -32,56 +32,80 @@ def build(force: bool = False) -> str:
     if (not force and os.path.exists(_LIB)
             and os.path.getmtime(_LIB) >= os.path.getmtime(_SRC)):
         return _LIB
-    cmd = ["gcc", "-O3", "-march=x86-64-v3", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC",
-           "-Wall", "-o", _LIB, _SRC, "-lm"]
-    subprocess.run(cmd, check=True)
+    subprocess.run(build_command(_LIB, vector=host_has_avx2()), check=True)
     return _LIB
+
+
+def host_has_avx2() -> bool:
+    """True when /proc/cpuinfo lists avx2 and fma (what -march=x86-64-v3 code needs to run)."""
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.startswith("flags"):
+                    flags = set(line.split(":", 1)[1].split())
+                    return {"avx2", "fma", "bmi2"} <= flags
+    except OSError:
+        pass
+    return False
+
+
+def build_command(out: str, vector: bool) -> list:
+    """The gcc line of the oracle: the AVX2 build (``vector``) or the portable -O2 one a host
+    without AVX2 falls back to.  Same arithmetic either way: no fast-math, no reassociation,
+    -ffp-contract=off (tests/test_oracle_pins.py compares the two builds bit for bit)."""
+    opt = ["-O3", "-march=x86-64-v3"] if vector else ["-O2"]
+    return ["gcc", *opt, "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC", "-Wall", "-o", out, _SRC, "-lm"]
 
 
 def _load():
     global _lib
     if _lib is None:
         build()
-        lib = ctypes.CDLL(_LIB)
-        pp = ctypes.POINTER(ctypes.c_void_p)
-        lib.oracle_num_threads.restype = ctypes.c_int
-        lib.oracle_jk_slab.restype = ctypes.c_int
-        lib.oracle_jk_slab.argtypes = [
-            ctypes.c_int64, ctypes.c_int64, ctypes.c_void_p, ctypes.c_int,
-            pp, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, pp,
-            ctypes.c_void_p]
-        lib.oracle_bruteforce_jk.restype = ctypes.c_int
-        lib.oracle_bruteforce_jk.argtypes = [
-            ctypes.c_int64, ctypes.c_int64, ctypes.c_void_p, ctypes.c_int,
-            pp, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, pp,
-            ctypes.c_void_p]
-        lib.oracle_kv_slab.restype = ctypes.c_int
-        lib.oracle_kv_slab.argtypes = [
-            ctypes.c_int64, ctypes.c_int64, ctypes.c_void_p, ctypes.c_int,
-            pp, ctypes.c_void_p, ctypes.c_int64, ctypes.c_void_p, pp]
-        lib.oracle_jk_dm_slab.restype = ctypes.c_int
-        lib.oracle_jk_dm_slab.argtypes = [
-            ctypes.c_int64, ctypes.c_int64, ctypes.c_void_p, ctypes.c_void_p,
-            ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
-        lib.oracle_jk_pair_slab.restype = ctypes.c_int
-        lib.oracle_jk_pair_slab.argtypes = [
-            ctypes.c_int64, ctypes.c_int64, ctypes.c_void_p, ctypes.c_int64,
-            ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p,
-            ctypes.c_void_p]
-        lib.oracle_bruteforce_jk_dm.restype = ctypes.c_int
-        lib.oracle_bruteforce_jk_dm.argtypes = [
-            ctypes.c_int64, ctypes.c_int64, ctypes.c_void_p, ctypes.c_void_p,
-            ctypes.c_void_p, ctypes.c_void_p]
-        lib.oracle_df_diag_slab.restype = ctypes.c_int
-        lib.oracle_df_diag_slab.argtypes = [ctypes.c_int64, ctypes.c_int64, ctypes.c_void_p,
-                                            ctypes.c_void_p]
-        lib.oracle_cholesky_lower.restype = ctypes.c_int
-        lib.oracle_cholesky_lower.argtypes = [ctypes.c_int64, ctypes.c_void_p, ctypes.c_void_p]
-        lib.oracle_whiten.restype = ctypes.c_int
-        lib.oracle_whiten.argtypes = [ctypes.c_int64, ctypes.c_int64, ctypes.c_void_p,
-                                      ctypes.c_void_p, ctypes.c_void_p]
-        _lib = lib
+        _lib = _open(_LIB)
     return _lib
+
+
+def _open(path: str):
+    """dlopen one build of the oracle and declare its signatures."""
+    lib = ctypes.CDLL(path)
+    pp = ctypes.POINTER(ctypes.c_void_p)
+    lib.oracle_num_threads.restype = ctypes.c_int
+    lib.oracle_jk_slab.restype = ctypes.c_int
+    lib.oracle_jk_slab.argtypes = [
+        ctypes.c_int64, ctypes.c_int64, ctypes.c_void_p, ctypes.c_int,
+        pp, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, pp,
+        ctypes.c_void_p]
+    lib.oracle_bruteforce_jk.restype = ctypes.c_int
+    lib.oracle_bruteforce_jk.argtypes = [
+        ctypes.c_int64, ctypes.c_int64, ctypes.c_void_p, ctypes.c_int,
+        pp, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, pp,
+        ctypes.c_void_p]
+    lib.oracle_kv_slab.restype = ctypes.c_int
+    lib.oracle_kv_slab.argtypes = [
+        ctypes.c_int64, ctypes.c_int64, ctypes.c_void_p, ctypes.c_int,
+        pp, ctypes.c_void_p, ctypes.c_int64, ctypes.c_void_p, pp]
+    lib.oracle_jk_dm_slab.restype = ctypes.c_int
+    lib.oracle_jk_dm_slab.argtypes = [
+        ctypes.c_int64, ctypes.c_int64, ctypes.c_void_p, ctypes.c_void_p,
+        ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
+    lib.oracle_jk_pair_slab.restype = ctypes.c_int
+    lib.oracle_jk_pair_slab.argtypes = [
+        ctypes.c_int64, ctypes.c_int64, ctypes.c_void_p, ctypes.c_int64,
+        ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p,
+        ctypes.c_void_p]
+    lib.oracle_bruteforce_jk_dm.restype = ctypes.c_int
+    lib.oracle_bruteforce_jk_dm.argtypes = [
+        ctypes.c_int64, ctypes.c_int64, ctypes.c_void_p, ctypes.c_void_p,
+        ctypes.c_void_p, ctypes.c_void_p]
+    lib.oracle_df_diag_slab.restype = ctypes.c_int
+    lib.oracle_df_diag_slab.argtypes = [ctypes.c_int64, ctypes.c_int64, ctypes.c_void_p,
+                                        ctypes.c_void_p]
+    lib.oracle_cholesky_lower.restype = ctypes.c_int
+    lib.oracle_cholesky_lower.argtypes = [ctypes.c_int64, ctypes.c_void_p, ctypes.c_void_p]
+    lib.oracle_whiten.restype = ctypes.c_int
+    lib.oracle_whiten.argtypes = [ctypes.c_int64, ctypes.c_int64, ctypes.c_void_p,
+                                  ctypes.c_void_p, ctypes.c_void_p]
+    return lib
 
 
 def num_threads() -> int:

@@ -358,11 +358,13 @@ class DFJK:
         return dict(converged=bool(conv.value), e_hist=list(e_hist[:n_iter.value]), C=C, mo_energy=eps, D=D,
                     timing=self.scf_timing())
 
-    def scf_timing(self) -> dict:
-        """ms per iteration of the last SCF run: get_jk, eigensolver (cuSOLVER Dsygvd), everything else."""
+    def scf_timing(self) -> Optional[dict]:
+        """ms per iteration of the last SCF run: get_jk, eigensolver (cuSOLVER Dsygvd), everything else.
+        None when the library has no valid timing on record (no run yet, or its events failed)."""
         it, a, b, c = ctypes.c_int64(0), ctypes.c_double(0), ctypes.c_double(0), ctypes.c_double(0)
-        _check(lib().dfjk_scf_timing(self._h, ctypes.byref(it), ctypes.byref(a), ctypes.byref(b),
-                                     ctypes.byref(c)), "dfjk_scf_timing")
+        if lib().dfjk_scf_timing(self._h, ctypes.byref(it), ctypes.byref(a), ctypes.byref(b),
+                                 ctypes.byref(c)) != 0:
+            return None
         n = max(it.value, 1)
         return {"iterations": it.value, "get_jk": a.value / n, "eigensolver": b.value / n, "glue": c.value / n}
 

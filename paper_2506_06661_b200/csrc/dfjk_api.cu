@@ -141,7 +141,8 @@ struct dfjk_handle {
     int ev_cap, ev_used;
     bool ev_overflow;    /* a launch went unrecorded (the ring could not grow): kernel_time reports it */
     /* replayed launch sequences of get_jk / get_jk_u (see get_jk_impl) */
-    struct GraphSlot { bool seen; unsigned char key[64]; cudaGraphExec_t exec; int64_t launches; };
+    /* key: the bytes of a GraphKey (defined with get_jk_impl below), copied in and out with memcpy */
+    struct GraphSlot { bool seen; alignas(8) unsigned char key[64]; cudaGraphExec_t exec; int64_t launches; };
     GraphSlot graphs[DFJK_GRAPH_SLOTS];
     int graph_next;
     int64_t opt_graph;
@@ -290,7 +291,7 @@ extern "C" dfjk_handle *dfjk_create(int64_t naux, int64_t nao, const double *B_p
     if (rc == DFJK_OK) rc = alloc_ws(h, &h->Ccat, round_up(nao, 32) * h->ldc_max);
     if (rc == DFJK_OK) rc = alloc_ws(h, &h->Dt, h->npair);
     /* d partials: J1's column chunks, or J1X's blocks at the widest ldc */
-    int64_t dparts = dfjk::j1x_num_blocks(nao, h->ldc_max);
+    int64_t dparts = dfjk::j1x_max_blocks(nao, h->ldc_max);
     if (dparts < h->nchunk) dparts = h->nchunk;
     if (rc == DFJK_OK) rc = alloc_ws(h, &h->d_part, dparts * naux);
     if (rc == DFJK_OK) rc = alloc_ws(h, &h->d, naux);
@@ -344,7 +345,7 @@ extern "C" int dfjk_set_option(dfjk_handle *h, const char *name, int64_t value)
         h->opt_k2_weighted = value; return DFJK_OK;
     }
     if (!strcmp(name, "k2_panel_kb")) {
-        if (value < 64) return fail(DFJK_EINVAL, "k2_panel_kb must be >= 64");
+        if (value < 64 || value > (1 << 22)) return fail(DFJK_EINVAL, "k2_panel_kb must be in [64, 4194304] (KB)");
         h->opt_k2_panel_kb = value; return DFJK_OK;
     }
     return fail(DFJK_EINVAL, "dfjk_set_option: unknown option '%s'", name);
@@ -500,19 +501,16 @@ int get_jk_impl(dfjk_handle *h, int nset, const double *const *C, const int64_t 
         }
     }
     dfjk_handle::GraphSlot *slot = nullptr;
+    bool first_of_shape = false;
     if (use_graph) {
-        for (auto &g : h->graphs)
-            if (g.seen && *reinterpret_cast<const GraphKey *>(g.key) == key) { slot = &g; break; }
-        if (!slot) {
-            /* first call of this shape: remember it (round-robin over the slots), launch plainly */
-            slot = &h->graphs[h->graph_next];
-            h->graph_next = (h->graph_next + 1) % DFJK_GRAPH_SLOTS;
-            if (slot->exec) { cudaGraphExecDestroy(slot->exec); slot->exec = nullptr; }
-            static_assert(sizeof(GraphKey) <= sizeof(slot->key), "GraphSlot::key too small");
-            memcpy(slot->key, &key, sizeof key);
-            slot->seen = true;
-            slot = nullptr;
+        for (auto &g : h->graphs) {
+            if (!g.seen) continue;
+            GraphKey k;
+            static_assert(sizeof(GraphKey) <= sizeof(g.key), "GraphSlot::key too small");
+            memcpy(&k, g.key, sizeof k);
+            if (k == key) { slot = &g; break; }
         }
+        first_of_shape = slot == nullptr;   /* launched plainly; remembered below once it has succeeded */
     }
 
     /* K0: zero-padded concatenation [C_0 | C_1], each set padded to a multiple of 8 columns; it also
@@ -546,6 +544,14 @@ int get_jk_impl(dfjk_handle *h, int nset, const double *const *C, const int64_t 
     }
     if (J) h->have_d = true;
     DFJK_CUDA_TRY(cudaGetLastError());
+    if (first_of_shape) {
+        /* first successful call of this shape: remember it (round-robin over the slots) */
+        dfjk_handle::GraphSlot *ns = &h->graphs[h->graph_next];
+        h->graph_next = (h->graph_next + 1) % DFJK_GRAPH_SLOTS;
+        if (ns->exec) { cudaGraphExecDestroy(ns->exec); ns->exec = nullptr; }
+        memcpy(ns->key, &key, sizeof key);
+        ns->seen = true;
+    }
     return DFJK_OK;
 }
 
@@ -728,7 +734,7 @@ extern "C" int dfjk_scf_timing(const dfjk_handle *h, int64_t *iters, double *get
 {
     g_err[0] = 0;
     if (!h) return fail(DFJK_EINVAL, "dfjk_scf_timing: NULL handle");
-    if (h->scf_iters <= 0) return fail(DFJK_EINVAL, "dfjk_scf_timing: no SCF has run on this handle");
+    if (h->scf_iters <= 0) return fail(DFJK_EINVAL, "dfjk_scf_timing: no timing on record (no SCF has run on this handle, or the last run failed or could not record its events)");
     if (iters) *iters = h->scf_iters;
     if (get_jk_ms) *get_jk_ms = h->scf_get_jk_ms;
     if (eig_ms) *eig_ms = h->scf_eig_ms;

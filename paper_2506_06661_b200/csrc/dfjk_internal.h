@@ -39,6 +39,7 @@ void launch_j1_dot(const double *B, int64_t naux, int64_t npair, const double *D
  * 4): the C block of X column c is Ccat column c + c_shift -- 0 for C C^T densities, the width of C1
  * for the pair form, where d_P = <B_P C1, C2>. */
 int64_t j1x_num_blocks(int64_t nao, int64_t ldc);
+int64_t j1x_max_blocks(int64_t nao, int64_t ldc_max);   /* >= j1x_num_blocks(nao, ldc) for every ldc <= ldc_max */
 void launch_j1x_dot(const double *X4, const double *Ccat4, int64_t nao, int64_t np, int64_t ldx, int64_t ldc,
                     int64_t c_shift, int nset, const int *col0, const int *nocc, const double *w, int64_t P0,
                     int64_t naux, double *d_part, cudaStream_t st);

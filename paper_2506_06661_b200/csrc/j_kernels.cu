@@ -255,18 +255,22 @@ j1_dot_kernel(const double *__restrict__ B, int64_t naux, int64_t npair,
  * u-th 16-byte piece = X_P[mu][col], X_P[mu][col+1] with col = 4 cg + 2 h, u = (cg*nao + mu)*2 + h.
  * A thread takes one unit per tile of 256, keeps the two matching C values (times w) in registers
  * and walks J1X_PB consecutive P with them: every warp load is 512 contiguous bytes.  A CTA covers
- * J1X_TILES tiles; its 256 x PB shares are reduced through shared memory in a fixed order into
+ * `tiles` tiles; its 256 x PB shares are reduced through shared memory in a fixed order into
  * d_part[blockIdx.x][P] (deterministic; J1R adds the blocks). */
 constexpr int J1X_PB = 16;            /* P per CTA */
 constexpr int J1X_PARTS = 256 / J1X_PB;
-constexpr int J1X_TILES = 1;          /* tiles of 256 units per CTA: swept on B200 at cfg 4, PB x TILES = 16 x 8:
-                                         2.10 ms, 16 x 2: 1.50, 8 x 1: 1.41, 16 x 1: 1.29 ms (6.7 TB/s) -- short CTAs,
-                                         many in flight; J1R then adds 425 instead of 53 partials per P */
+/* tiles of 256 units per CTA: swept on B200 at cfg 4, PB x tiles = 16 x 8: 2.10 ms, 16 x 2: 1.50, 8 x 1: 1.41,
+ * 16 x 1: 1.29 ms (6.7 TB/s) -- short CTAs, many in flight; J1R then adds 425 instead of 53 partials per P.
+ * One tile per CTA up to J1X_MAX_BLOCKS blocks (occupied-orbital widths: cfg 4 has 425, cfg 5 1313); wider
+ * column blocks (pair / raw-dm calls up to ldc = 2 nao) give each CTA more tiles, so that d_part -- one
+ * row of naux doubles per block -- stays below J1X_MAX_BLOCKS * naux doubles (82 MB at cfg 4) instead of
+ * nao^2/256 * naux (0.8 GB). */
+constexpr int64_t J1X_MAX_BLOCKS = 2048;
 
 __global__ void __launch_bounds__(256)
 j1x_dot_kernel(const double *__restrict__ X4, const double *__restrict__ Ccat4, int64_t nao, int64_t np,
                int64_t ldx4, int64_t ldc, int64_t c_shift, SetDesc sd, int64_t P0, int64_t naux,
-               double *__restrict__ d_part)
+               int tiles, double *__restrict__ d_part)
 {
     __shared__ double ts[J1X_PB][264];                     /* this thread's share of d_P, P in the CTA's range */
     const int64_t nunit = (ldc / 4) * nao * 2;             /* units that face columns of Ccat */
@@ -275,8 +279,8 @@ j1x_dot_kernel(const double *__restrict__ X4, const double *__restrict__ Ccat4, 
     double t[J1X_PB];
 #pragma unroll
     for (int pp = 0; pp < J1X_PB; ++pp) t[pp] = 0.0;
-    for (int tile = 0; tile < J1X_TILES; ++tile) {
-        const int64_t u = ((int64_t)blockIdx.x * J1X_TILES + tile) * 256 + threadIdx.x;
+    for (int tile = 0; tile < tiles; ++tile) {
+        const int64_t u = ((int64_t)blockIdx.x * tiles + tile) * 256 + threadIdx.x;
         if (u >= nunit) break;
         const int64_t row = u >> 1;                        /* cg*nao + mu */
         const int64_t cg = row / nao, mu = row - cg * nao;
@@ -490,9 +494,23 @@ void launch_j1_dot(const double *B, int64_t naux, int64_t npair, const double *D
                                                                                   d_part);
 }
 
+static int64_t j1x_tiles_per_cta(int64_t nao, int64_t ldc)
+{
+    const int64_t ntile = ((ldc / 4) * nao * 2 + 255) / 256;
+    return ntile <= J1X_MAX_BLOCKS ? 1 : (ntile + J1X_MAX_BLOCKS - 1) / J1X_MAX_BLOCKS;
+}
+
+/* upper bound of j1x_num_blocks over every ldc <= ldc_max (the block count is not monotonic in ldc
+ * once CTAs take several tiles): what dfjk_create sizes d_part for */
+int64_t j1x_max_blocks(int64_t nao, int64_t ldc_max)
+{
+    const int64_t ntile = ((ldc_max / 4) * nao * 2 + 255) / 256;
+    return ntile < J1X_MAX_BLOCKS ? ntile : J1X_MAX_BLOCKS;
+}
+
 int64_t j1x_num_blocks(int64_t nao, int64_t ldc)
 {
-    const int64_t per_cta = 256LL * J1X_TILES;
+    const int64_t per_cta = 256LL * j1x_tiles_per_cta(nao, ldc);
     return ((ldc / 4) * nao * 2 + per_cta - 1) / per_cta;
 }
 
@@ -508,7 +526,8 @@ void launch_j1x_dot(const double *X4, const double *Ccat4, int64_t nao, int64_t 
         sd.w[s] = s < nset ? w[s] : 0.0;
     }
     dim3 grid((unsigned)j1x_num_blocks(nao, ldc), (unsigned)((np + J1X_PB - 1) / J1X_PB));
-    j1x_dot_kernel<<<grid, 256, 0, st>>>(X4, Ccat4, nao, np, ldx / 4, ldc, c_shift, sd, P0, naux, d_part);
+    j1x_dot_kernel<<<grid, 256, 0, st>>>(X4, Ccat4, nao, np, ldx / 4, ldc, c_shift, sd, P0, naux,
+                                         (int)j1x_tiles_per_cta(nao, ldc), d_part);
 }
 
 void launch_j1_reduce(const double *d_part, int64_t nchunk, int64_t naux, double *d, cudaStream_t st)

@@ -248,11 +248,15 @@ bool solve_dense(std::vector<double> &A, std::vector<double> &b, int n)
 }  // namespace
 
 namespace {
-void mark_end(std::vector<cudaEvent_t> &v, cudaStream_t st)
+/* one timing mark: an event created and recorded on the run's stream.  A mark that cannot be made
+ * clears *ok -- the (begin, end) pairing of its vector is then broken, and the run's timing is
+ * reported as invalid instead of as a wrong sum. */
+void mark_event(std::vector<cudaEvent_t> &v, cudaStream_t st, bool *ok)
 {
-    if (v.size() != 1) return;                        /* the opening mark was never recorded */
     cudaEvent_t e = nullptr;
-    if (cudaEventCreate(&e) == cudaSuccess) { cudaEventRecord(e, st); v.push_back(e); }
+    if (cudaEventCreate(&e) != cudaSuccess) { cudaGetLastError(); *ok = false; return; }
+    if (cudaEventRecord(e, st) != cudaSuccess) { cudaGetLastError(); cudaEventDestroy(e); *ok = false; return; }
+    v.push_back(e);
 }
 }  // namespace
 
@@ -292,6 +296,8 @@ int scf_run(dfjk_handle *h, int64_t nao, int nspin, const double *hcore, const d
     std::vector<double> Bmat((size_t)m_max * m_max, 0.0);
     std::vector<int> slot_of;                        /* history, oldest first: ring slot ids */
     std::vector<cudaEvent_t> ev_jk, ev_eig, ev_total; /* timing: pairs (begin, end) */
+    bool timing_ok = true;
+    scf_store_timing(h, 0, 0.0, 0.0, 0.0);             /* a failed run must not report the previous run's timing */
     double e_prev = 0.0;
     *n_iter = 0;
     *converged = 0;
@@ -333,10 +339,7 @@ int scf_run(dfjk_handle *h, int64_t nao, int nspin, const double *hcore, const d
     /* generalised symmetric eigenproblem A C = S C eps; a symmetric row-major matrix is its own
      * column-major image, the eigenvectors come back as columns of the column-major Va */
     {
-        auto mark_eig = [&]() {
-            cudaEvent_t e = nullptr;
-            if (cudaEventCreate(&e) == cudaSuccess) { cudaEventRecord(e, st); ev_eig.push_back(e); }
-        };
+        auto mark_eig = [&]() { mark_event(ev_eig, st, &timing_ok); };
         auto diagonalise = [&](const double *A, int s) -> int {
             if (cudaMemcpyAsync(Va, A, (size_t)n2 * 8, cudaMemcpyDeviceToDevice, st) != cudaSuccess) return 1;
             if (cudaMemcpyAsync(Sb, S, (size_t)n2 * 8, cudaMemcpyDeviceToDevice, st) != cudaSuccess) return 1;
@@ -382,10 +385,7 @@ int scf_run(dfjk_handle *h, int64_t nao, int nspin, const double *hcore, const d
             goto done;
         }
         /* timing (dfjk_scf_timing): event pairs around every get_jk and every Dsygvd */
-        auto mark = [&](std::vector<cudaEvent_t> &v) {
-            cudaEvent_t e = nullptr;
-            if (cudaEventCreate(&e) == cudaSuccess) { cudaEventRecord(e, st); v.push_back(e); }
-        };
+        auto mark = [&](std::vector<cudaEvent_t> &v) { mark_event(v, st, &timing_ok); };
         mark(ev_total);
 
         for (int s = 0; s < nspin; ++s) {                               /* 0. core guess, both spins */
@@ -494,13 +494,15 @@ int scf_run(dfjk_handle *h, int64_t nao, int nspin, const double *hcore, const d
 done:
     {
         /* where the time went: sums over the (begin, end) event pairs; the run has synchronised */
-        mark_end(ev_total, st);
+        if (ev_total.size() == 1) mark_event(ev_total, st, &timing_ok);
         cudaStreamSynchronize(st);
-        auto total = [](std::vector<cudaEvent_t> &v) {
+        auto total = [&timing_ok](std::vector<cudaEvent_t> &v) {
             double t = 0.0;
+            if (v.size() & 1) timing_ok = false;          /* an unmatched begin */
             for (size_t i = 0; i + 1 < v.size(); i += 2) {
                 float ms = 0.f;
                 if (cudaEventElapsedTime(&ms, v[i], v[i + 1]) == cudaSuccess) t += ms;
+                else timing_ok = false;
             }
             for (cudaEvent_t e : v) cudaEventDestroy(e);
             v.clear();
@@ -508,7 +510,7 @@ done:
         };
         const double t_jk = total(ev_jk), t_eig = total(ev_eig), t_all = total(ev_total);
         cudaGetLastError();
-        if (rc == DFJK_OK) scf_store_timing(h, *n_iter, t_jk, t_eig, t_all);
+        if (rc == DFJK_OK && timing_ok) scf_store_timing(h, *n_iter, t_jk, t_eig, t_all);
     }
     if (sol) cs.destroy(sol);
     cudaFree(ws);

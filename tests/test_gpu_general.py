@@ -69,6 +69,26 @@ def test_pair_parity(dfjk, nao, naux, ncol):
     h.close()
 
 
+def test_pair_parity_widest_column_block(dfjk):
+    """ncol = nao = 808: the column block [C1|C2] is 2 nao wide, the widest the handle is sized for.
+    J1X then deals two 256-unit tiles to each CTA (its block count is capped so that the d-partial
+    workspace stays small), with a ragged last CTA; d, J and K against the oracle."""
+    nao, naux, ncol = 808, 5, 808
+    Bp = make_B(nao, naux, 4242)
+    rng = np.random.default_rng(77)
+    C1, C2 = rng.standard_normal((nao, ncol)), rng.standard_normal((nao, ncol))
+    h = dfjk.DFJK(dev(Bp), nao)
+    assert h.workspace_bytes < 3.2e9
+    Jo, Ko, do = oracle.get_jk_pair(Bp, nao, C1, C2)
+    J, K = h.get_jk_pair(dev(C1), dev(C2))
+    d = h.get_d()
+    torch.cuda.synchronize()
+    assert relerr(d.cpu().numpy(), do) <= TOL
+    assert relerr(J.cpu().numpy(), Jo) <= TOL
+    assert relerr(K.cpu().numpy(), Ko) <= TOL
+    h.close()
+
+
 @pytest.mark.parametrize("nao,naux", [(1, 2), (3, 4), (31, 6), (130, 9), (257, 5)])
 def test_dm_parity(dfjk, nao, naux):
     Bp = make_B(nao, naux, 300 + nao)

@@ -305,3 +305,32 @@ def test_k_block_matches_full_K():
         assert relerr(kb.K[s], K[s][np.ix_(rows, rows)]) < 1e-13
         X = Bf[:, rows, :] @ C
         assert relerr(kb.K[s], np.einsum("pai,pbi->ab", X, X)) < 1e-13
+
+
+def test_vectorised_and_portable_builds_agree_bitwise(tmp_path, monkeypatch):
+    """The oracle is normally built -O3 -march=x86-64-v3 (AVX2) and falls back to plain -O2 on a host
+    without AVX2 (oracle.build_command).  Neither build may reassociate a sum or contract an FMA, so
+    d, J, K -- and the general-density and whitening routines -- must come out bit for bit the same."""
+    import subprocess
+    if not oracle.host_has_avx2():
+        pytest.skip("this host cannot run the AVX2 build")
+    libs = {}
+    for name, vector in (("vec", True), ("o2", False)):
+        out = str(tmp_path / f"liboracle_{name}.so")
+        subprocess.run(oracle.build_command(out, vector=vector), check=True)
+        libs[name] = oracle._open(out)
+    nao, naux = 37, 11
+    Bp, Cs = rand_case(nao, naux, (5, 3), seed=99, orthonormal=False)
+    rng = np.random.default_rng(5)
+    dm = rng.standard_normal((nao, nao))
+    M = rng.standard_normal((naux, naux))
+    M = M @ M.T + naux * np.eye(naux)
+    res = {}
+    for name, lib in libs.items():
+        monkeypatch.setattr(oracle, "_lib", lib)
+        J, K, d = oracle.get_jk(Bp, nao, Cs, [1.0, 0.5])
+        Jd, Kd, _ = oracle.get_jk_dm(Bp, nao, dm)
+        L = oracle.cholesky_lower(M)
+        res[name] = [J, *K, d, Jd, Kd, oracle.df_diag(Bp, nao), L, oracle.whiten(L, Bp)]
+    for a, b in zip(res["vec"], res["o2"]):
+        assert np.array_equal(a, b)
