@@ -317,6 +317,9 @@ int dfjk_get_d(dfjk_handle *h, double *d_out, void *stream);
  *               output pointers reach the finishing kernels through device memory).  Small problems
  *               are bound by launch count, not by work.  0 = always launch kernel by kernel.  Not
  *               used while "time_kernels" is on or while `stream` is itself being captured.
+ *   "poison_workspace"  test aid, not a setting: value 1 waits for the device and fills the handle's
+ *               whole workspace with 0xFF bytes (NaN as doubles) once, so that a later call that reads
+ *               workspace it has not written itself produces NaN instead of a plausible number.
  */
 int dfjk_set_option(dfjk_handle *h, const char *name, int64_t value);
 

@@ -132,6 +132,8 @@ struct dfjk_handle {
     /* options */
     int64_t opt_k_chunk, opt_k_splits, opt_j_fused, opt_k2_panel, opt_k2_panel_kb;
     int *k2work;         /* 1 + nsplit_alloc * nb^2 ints: item counter and per-(slab, tile) counters of K2P */
+    struct WsBuf { void *p; size_t bytes; } ws_list[12];   /* every alloc_ws buffer, for "poison_workspace" */
+    int ws_count;
     bool have_d;
     /* instrumentation: launch counter and optional per-kernel CUDA-event timing */
     int64_t launches;
@@ -220,6 +222,8 @@ int alloc_ws(dfjk_handle *h, double **p, int64_t ndoubles)
                     cudaGetErrorString(e));
     }
     h->ws_bytes += ndoubles * 8;
+    if (h->ws_count < (int)(sizeof h->ws_list / sizeof h->ws_list[0]))
+        h->ws_list[h->ws_count++] = {(void *)*p, (size_t)ndoubles * sizeof(double)};
     return DFJK_OK;
 }
 
@@ -306,6 +310,10 @@ extern "C" dfjk_handle *dfjk_create(int64_t naux, int64_t nao, const double *B_p
         h->out_slots = nullptr;
         rc = fail(DFJK_ENOMEM, "dfjk_create: cudaMalloc of the output-pointer slots failed");
     }
+    if (rc == DFJK_OK) {   /* "poison_workspace" covers these two as well */
+        h->ws_list[h->ws_count++] = {(void *)h->k2work, sizeof(int) * (size_t)(1 + h->nsplit_alloc * nb * nb)};
+        h->ws_list[h->ws_count++] = {(void *)h->out_slots, DFJK_OUT_SLOTS * sizeof(double *)};
+    }
     if (rc != DFJK_OK) { free_all(h); delete h; return nullptr; }
     return h;
 }
@@ -347,6 +355,17 @@ extern "C" int dfjk_set_option(dfjk_handle *h, const char *name, int64_t value)
     if (!strcmp(name, "k2_panel_kb")) {
         if (value < 64 || value > (1 << 22)) return fail(DFJK_EINVAL, "k2_panel_kb must be in [64, 4194304] (KB)");
         h->opt_k2_panel_kb = value; return DFJK_OK;
+    }
+    if (!strcmp(name, "poison_workspace")) {
+        /* test aid (tests/test_gpu_guard.py): waits for the device, then fills every workspace buffer
+         * with 0xFF bytes -- NaN as doubles -- so that a kernel that reads workspace no earlier kernel
+         * of the same call has written shows up as NaN in J / K instead of passing by luck */
+        if (value == 0) return DFJK_OK;
+        DFJK_CUDA_TRY(cudaDeviceSynchronize());
+        for (int i = 0; i < h->ws_count; ++i) DFJK_CUDA_TRY(cudaMemset(h->ws_list[i].p, 0xFF, h->ws_list[i].bytes));
+        DFJK_CUDA_TRY(cudaDeviceSynchronize());
+        h->have_d = false;
+        return DFJK_OK;
     }
     return fail(DFJK_EINVAL, "dfjk_set_option: unknown option '%s'", name);
 }

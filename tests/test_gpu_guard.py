@@ -115,6 +115,53 @@ def test_poisoned_surroundings(dfjk, nao, naux, nocc):
     h.close()
 
 
+@pytest.mark.parametrize("nao,naux,na,nb", [(129, 11, 3, 2), (290, 9, 25, 24), (417, 5, 40, 33), (700, 3, 20, 20)])
+def test_poisoned_workspace(dfjk, nao, naux, na, nb):
+    """initcheck of our own: the handle's whole workspace (X and its padding, Kpart slabs, d partials,
+    Jp partials, packed orbitals, K2P counters) is filled with NaN bytes before EVERY call, so a
+    kernel that reads workspace which no earlier kernel of the same call has written cannot pass."""
+    Bp = gi.fill_B_host(gi.custom_config(nao, naux, (na, nb), seed=nao + 7))
+    Ca, Cb = gi.random_orbitals(nao, na, 1), gi.random_orbitals(nao, nb, 2)
+    rng = np.random.default_rng(nao)
+    V = rng.standard_normal((nao, na))
+    dm = rng.standard_normal((nao, nao))
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    Jo, Ko = oracle.get_jk_restricted(Bp, nao, Ca)
+    Ju, Kao, Kbo = oracle.get_jk_unrestricted(Bp, nao, Ca, Cb)
+    Jpo, Kpo, _ = oracle.get_jk_pair(Bp, nao, Ca, V)
+    Jdo, Kdo, _ = oracle.get_jk_dm(Bp, nao, dm)
+    want_diag = oracle.df_diag(Bp, nao)
+    h = dfjk.DFJK(dev(Bp), nao)
+    h.set_option("graph", 0)                  # a replayed graph is the same launch sequence; keep every call plain
+    h.set_option("k2_panel_kb", 64)
+    h.set_option("k_chunk", max(1, naux // 2))
+    ok = lambda got, want: relerr(got.cpu().numpy(), want) <= TOL
+
+    def fresh(call):
+        h.set_option("poison_workspace", 1)
+        out = call()
+        torch.cuda.synchronize()
+        return out
+
+    for k2_panel in (0, 1):
+        h.set_option("k2_panel", k2_panel)
+        for fused in (1, 0):
+            h.set_option("j_fused", fused)
+            J, K = fresh(lambda: h.get_jk(dev(Ca)))
+            assert ok(J, Jo) and ok(K, Ko), (k2_panel, fused)
+            J, Ka, Kb = fresh(lambda: h.get_jk_u(dev(Ca), dev(Cb)))
+            assert ok(J, Ju) and ok(Ka, Kao) and ok(Kb, Kbo), (k2_panel, fused)
+            J, K = fresh(lambda: h.get_jk_pair(dev(Ca), dev(V)))
+            assert ok(J, Jpo) and ok(K, Kpo), (k2_panel, fused)
+        J, K = fresh(lambda: h.get_jk_dm(dev(dm)))
+        assert ok(J, Jdo) and ok(K, Kdo), k2_panel
+        J, _ = fresh(lambda: h.get_jk(dev(Ca), with_k=False))
+        _, K = fresh(lambda: h.get_jk(dev(Ca), with_j=False))
+        assert ok(J, Jo) and ok(K, Ko), k2_panel
+    assert ok(fresh(lambda: h.get_df_diag()), want_diag)
+    h.close()
+
+
 def test_build_b_poisoned_surroundings(dfjk):
     nao, naux = 33, 261                                   # 3 block rows of the blocked Cholesky, ragged
     cfg = gi.custom_config(nao, naux, (1,), seed=5)
