@@ -126,9 +126,36 @@ int dfjk_get_jk_pair(dfjk_handle *h, const double *C1, const double *C2, int64_t
 int dfjk_get_jk_dm(dfjk_handle *h, const double *dm, double *J, double *K, void *stream);
 
 /*
- * dfjk_get_jk_dms -- "an arbitrary number of density matrices":
- *   dms     DEVICE, ndm x nao x nao;  Js, Ks  DEVICE, ndm x nao x nao (either may be NULL).
- * Equivalent to ndm stream-ordered dfjk_get_jk_dm calls.
+ * dfjk_get_jk_pairs -- several factored densities dm_i = C1_i C2_i^T, i < nbatch, from ONE sweep over B
+ * ("an arbitrary number of density matrices"; the batches of Hessian x trial-vector
+ * products of SOSCF).  Per density the results are those of dfjk_get_jk_pair:
+ *     J_i = sum_P B_P <B_P, C1_i C2_i^T>        K_i = sum_P (B_P C1_i)(B_P C2_i)^T
+ * How B is shared: the factors of as many pairs as fit 2 round_up(nao, 8) columns are packed side by side
+ * and half-transformed by ONE K1 launch per X chunk (the packed triangle is read and unpacked once for
+ * all of them -- with few columns per pair K1 is bound by exactly that); each pair's d_P is read off its
+ * columns of X and its product added to K_i chunk by chunk; all J_i of up to 8 densities come out of ONE
+ * axpy pass over B (every loaded element feeds 8 FMAs).  Larger batches are cut into sub-batches of 8.
+ *   C1s, C2s  HOST arrays of nbatch DEVICE pointers, factor i is nao x ncols[i] row-major
+ *   ncols     HOST array of nbatch column counts, 1 <= ncols[i] <= nao (they may differ)
+ *   Js, Ks    HOST arrays of nbatch DEVICE pointers to nao x nao outputs (OVERWRITTEN); either ARRAY may
+ *             be NULL (skip all J / all K), not both; an array that is given has no NULL entry.
+ *             With Ks == NULL (or option "j_fused" = 0) every d_i costs its own dot pass over B; the
+ *             axpy pass is still shared.
+ * With d from the dot pass J_i is bitwise what dfjk_get_jk_pair gives (the shared axpy pass adds in the
+ * same order per density); read off X, d_P is summed over other column blocks than in a single-pair call,
+ * and K_i adds its X chunks in another order: deterministic, a different rounding.  dfjk_get_d is not
+ * updated by batched calls.
+ */
+int dfjk_get_jk_pairs(dfjk_handle *h, int64_t nbatch, const double *const *C1s,
+                      const double *const *C2s, const int64_t *ncols, double *const *Js,
+                      double *const *Ks, void *stream);
+
+/*
+ * dfjk_get_jk_dms -- the same for raw density matrices:
+ *   dms     DEVICE, ndm x nao x nao;  Js, Ks  DEVICE, ndm x nao x nao (either may be NULL, not both).
+ * Results per density as dfjk_get_jk_dm.  The J_i of up to 8 densities share ONE axpy pass over B
+ * (ndm + 1 streaming passes instead of 2 ndm); K_i is built per density as the pair (dm_i, I), which is
+ * bound by its 4 naux nao^3 flop, not by B.
  */
 int dfjk_get_jk_dms(dfjk_handle *h, int64_t ndm, const double *dms, double *Js, double *Ks,
                     void *stream);

@@ -32,7 +32,7 @@ SYMBOLS = (
     "dfjk_get_jk_pair", "dfjk_get_jk_dm", "dfjk_get_jk_dms", "dfjk_get_df_diag",
     "dfjk_build_b", "dfjk_scf_rhf", "dfjk_probe_dmma_peak",
     "dfjk_get_jk_u_host", "dfjk_scf_uhf", "dfjk_device_info", "dfjk_scf_timing",
-    "dfjk_df_diag_noalloc", "dfjk_noalloc_max_nao",
+    "dfjk_df_diag_noalloc", "dfjk_noalloc_max_nao", "dfjk_get_jk_pairs",
 )
 
 # DFJK_KERNEL_* ids of include/dfjk.h
@@ -71,6 +71,8 @@ def lib() -> ctypes.CDLL:
     L.dfjk_get_jk_u.argtypes = [vp, vp, i64, vp, i64, vp, vp, vp, vp]
     L.dfjk_get_jk_pair.restype = ci
     L.dfjk_get_jk_pair.argtypes = [vp, vp, vp, i64, vp, vp, vp]
+    L.dfjk_get_jk_pairs.restype = ci
+    L.dfjk_get_jk_pairs.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp]
     L.dfjk_get_jk_dm.restype = ci
     L.dfjk_get_jk_dm.argtypes = [vp, vp, vp, vp, vp]
     L.dfjk_get_jk_dms.restype = ci
@@ -367,6 +369,29 @@ class DFJK:
             return None
         n = max(it.value, 1)
         return {"iterations": it.value, "get_jk": a.value / n, "eigensolver": b.value / n, "glue": c.value / n}
+
+    def get_jk_pairs(self, C1s, C2s, with_j: bool = True, with_k: bool = True, stream=None):
+        """Several factored densities dm_i = C1_i C2_i^T from one sweep over B (dfjk_get_jk_pairs): one
+        half transform over all factors side by side, one axpy pass for all J_i.  ``C1s`` / ``C2s`` are
+        sequences of nao x ncol_i CUDA float64 tensors.  Returns (list of J_i or None, list of K_i or None)."""
+        import torch
+        n = len(C1s)
+        if n < 1 or len(C2s) != n:
+            raise ValueError("C1s and C2s must be non-empty sequences of the same length")
+        ncols = (ctypes.c_int64 * n)()
+        p1, p2 = (ctypes.c_void_p * n)(), (ctypes.c_void_p * n)()
+        for i, (a, b) in enumerate(zip(C1s, C2s)):
+            if a.dim() != 2 or a.shape[0] != self.nao or tuple(b.shape) != tuple(a.shape):
+                raise ValueError("C1_i and C2_i must both be nao x ncol_i")
+            p1[i], p2[i], ncols[i] = _dev_f64(a, "C1"), _dev_f64(b, "C2"), int(a.shape[1])
+        Js = [self._out(True) for _ in range(n)] if with_j else None
+        Ks = [self._out(True) for _ in range(n)] if with_k else None
+        pj = (ctypes.c_void_p * n)(*[t.data_ptr() for t in Js]) if with_j else None
+        pk = (ctypes.c_void_p * n)(*[t.data_ptr() for t in Ks]) if with_k else None
+        with torch.cuda.device(self.device):
+            st = (stream or torch.cuda.current_stream(self.device)).cuda_stream
+            _check(lib().dfjk_get_jk_pairs(self._h, n, p1, p2, ncols, pj, pk, st), "dfjk_get_jk_pairs")
+        return Js, Ks
 
     def get_df_diag(self, stream=None):
         """diag[mu][nu] = sum_P B_P[mu,nu]^2, the DF term of Eq. 7."""

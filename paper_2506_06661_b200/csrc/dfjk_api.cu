@@ -120,6 +120,7 @@ struct dfjk_handle {
     double *Dt;          /* npair */
     double *d_part;      /* nchunk x naux */
     double *d;           /* naux */
+    double *d_batch;     /* DFJK_MAX_BATCH x naux: d of every density of a batched call */
     double *Jp_part;     /* j2_groups x npair */
     double *X;           /* x_doubles */
     double *Kpart;       /* 2 x nsplit_alloc x nao x nao */
@@ -162,7 +163,7 @@ namespace {
 
 void free_all(dfjk_handle *h)
 {
-    cudaFree(h->Ccat); cudaFree(h->Dt); cudaFree(h->d_part); cudaFree(h->d);
+    cudaFree(h->Ccat); cudaFree(h->Dt); cudaFree(h->d_part); cudaFree(h->d); cudaFree(h->d_batch);
     cudaFree(h->Jp_part); cudaFree(h->X); cudaFree(h->Kpart); cudaFree(h->k2work);
     cudaFree(h->hostC); cudaFree(h->hostJ); cudaFree(h->hostK); cudaFree(h->hostC2); cudaFree(h->hostK2);
     if (h->host_stream) cudaStreamDestroy(h->host_stream);
@@ -299,6 +300,7 @@ extern "C" dfjk_handle *dfjk_create(int64_t naux, int64_t nao, const double *B_p
     if (dparts < h->nchunk) dparts = h->nchunk;
     if (rc == DFJK_OK) rc = alloc_ws(h, &h->d_part, dparts * naux);
     if (rc == DFJK_OK) rc = alloc_ws(h, &h->d, naux);
+    if (rc == DFJK_OK) rc = alloc_ws(h, &h->d_batch, DFJK_MAX_BATCH * naux);
     if (rc == DFJK_OK) rc = alloc_ws(h, &h->Jp_part, h->j2_groups * h->npair);
     if (rc == DFJK_OK) rc = alloc_ws(h, &h->X, h->x_doubles);
     if (rc == DFJK_OK) rc = alloc_ws(h, &h->Kpart, 2LL * h->nsplit_alloc * nao * nao);
@@ -670,18 +672,185 @@ extern "C" int dfjk_get_jk_dm(dfjk_handle *h, const double *dm, double *J, doubl
     return get_jk_general_impl(h, dm, nullptr, h ? h->nao : 1, J, K, (cudaStream_t)stream, "dfjk_get_jk_dm");
 }
 
+namespace {
+
+/* The Coulomb matrices of nb <= DFJK_MAX_BATCH densities whose fitting coefficients d_k[P] already sit in
+ * h->d_batch: ONE pass over B carries all of them (launch_j2_axpy_multi), the partial triangles live in the
+ * X workspace, which is idle at this point of a call.  Falls back to one pass per density only when the X
+ * workspace cannot hold nb x j2_groups partial triangles. */
+int batched_j_from_d(dfjk_handle *h, int nb, double *const *Js, cudaStream_t st)
+{
+    const int64_t nao = h->nao, naux = h->naux, npair = h->npair;
+    const int64_t per = h->j2_groups * npair;
+    if ((int64_t)nb * per <= h->x_doubles) {
+        { Timed t_(h, DFJK_KERNEL_J2, st); dfjk::launch_j2_axpy_multi(h->B, naux, npair, h->d_batch, nb, h->X, h->j2_groups, st); }
+        for (int i = 0; i < nb; ++i) {
+            Timed t_(h, DFJK_KERNEL_J3, st);
+            dfjk::launch_j3_unpack(h->X + i * per, h->j2_groups, npair, nao, Js[i], nullptr, st);
+        }
+    } else {
+        for (int i = 0; i < nb; ++i) {
+            { Timed t_(h, DFJK_KERNEL_J2, st); dfjk::launch_j2_axpy(h->B, naux, npair, h->d_batch + i * naux, h->Jp_part, h->j2_groups, st); }
+            { Timed t_(h, DFJK_KERNEL_J3, st); dfjk::launch_j3_unpack(h->Jp_part, h->j2_groups, npair, nao, Js[i], nullptr, st); }
+        }
+    }
+    return DFJK_OK;
+}
+
+/* d_k = <B_P, dm_k> by a streaming pass over B per density (J0 general -> J1 -> J1R into d_batch[k]) */
+void d_by_pass_over_b(dfjk_handle *h, int k, const double *C1, const double *C2, int64_t ncol, cudaStream_t st)
+{
+    { Timed t_(h, DFJK_KERNEL_J0, st); dfjk::launch_j0_general_dt(C1, C2, ncol, h->nao, h->Dt, st); }
+    { Timed t_(h, DFJK_KERNEL_J1, st); dfjk::launch_j1_dot(h->B, h->naux, h->npair, h->Dt, h->d_part, h->sm_count, st); }
+    { Timed t_(h, DFJK_KERNEL_J1R, st); dfjk::launch_j1_reduce(h->d_part, h->nchunk, h->naux, h->d_batch + (int64_t)k * h->naux, st); }
+}
+
+/* One sub-batch (nb <= DFJK_MAX_BATCH) of dfjk_get_jk_pairs.  K: the factors of as many pairs as fit
+ * ldc_max columns are packed side by side, ONE half transform (K1) per X chunk serves them all; per pair
+ * d_P is read off its columns of X (J1X) and its full product (K2) is added to K_i chunk by chunk.
+ * J: one multi-right-hand-side pass over B for the whole sub-batch. */
+int pairs_subbatch(dfjk_handle *h, int nb, const double *const *C1s, const double *const *C2s,
+                   const int64_t *ncols, double *const *Js, double *const *Ks, cudaStream_t st, const char *who)
+{
+    const int64_t nao = h->nao, naux = h->naux, npair = h->npair;
+    const bool want_j = Js != nullptr, want_k = Ks != nullptr;
+    const bool fused = want_j && want_k && h->opt_j_fused != 0;
+    if (want_j && !fused)
+        for (int i = 0; i < nb; ++i) d_by_pass_over_b(h, i, C1s[i], C2s[i], ncols[i], st);
+    if (want_k) {
+        const int nbk = (int)((nao + 127) / 128);
+        int i0 = 0;
+        while (i0 < nb) {
+            int i1 = i0;
+            int64_t ldc = 0, col1[DFJK_MAX_BATCH], w8[DFJK_MAX_BATCH];
+            while (i1 < nb && ldc + 2 * round_up(ncols[i1], 8) <= h->ldc_max) {
+                w8[i1] = round_up(ncols[i1], 8);
+                col1[i1] = ldc;
+                ldc += 2 * w8[i1];
+                ++i1;
+            }
+            for (int i = i0; i < i1; ++i) {
+                { Timed t_(h, DFJK_KERNEL_K0, st); dfjk::launch_k0_pack_cols(C1s[i], ncols[i], col1[i], w8[i], nao, ldc, h->Ccat, st); }
+                { Timed t_(h, DFJK_KERNEL_K0, st); dfjk::launch_k0_pack_cols(C2s[i], ncols[i], col1[i] + w8[i], w8[i], nao, ldc, h->Ccat, st); }
+            }
+            int64_t pc = h->x_doubles / (nao * ldc);
+            if (h->opt_k_chunk > 0 && h->opt_k_chunk < pc) pc = h->opt_k_chunk;
+            if (pc > naux) pc = naux;
+            if (pc < 1) return fail(DFJK_ENOMEM, "%s: X workspace too small", who);
+            bool panel[DFJK_MAX_BATCH];
+            int nsplit[DFJK_MAX_BATCH], pstages[DFJK_MAX_BATCH];
+            for (int i = i0; i < i1; ++i) {
+                panel[i] = h->opt_k2_panel == 1 ||
+                           (h->opt_k2_panel == 2 && pc * nao * ldc * 8 > h->l2_bytes && nbk >= DFJK_K2P_MIN_NB - 1);
+                nsplit[i] = h->opt_k_splits > 0 ? (int)h->opt_k_splits : choose_splits(nbk * nbk, h->sm_count, h->nsplit_alloc);
+                pstages[i] = 0;
+            }
+            const int64_t nblk = dfjk::j1x_num_blocks(nao, ldc);
+            int chunk = 0;
+            for (int64_t P0 = 0; P0 < naux; P0 += pc, ++chunk) {
+                const int64_t np = (P0 + pc <= naux) ? pc : naux - P0;
+                { Timed t_(h, DFJK_KERNEL_K1, st); DFJK_LAUNCH_TRY(dfjk::launch_k1_half_transform(h->B, naux, nao, npair, P0, np, h->Ccat, ldc, ldc, h->X, st)); }
+                for (int i = i0; i < i1; ++i) {
+                    const int c1 = (int)col1[i], c2 = (int)(col1[i] + w8[i]), nc = (int)ncols[i];
+                    if (fused) {
+                        const double one = 1.0;
+                        { Timed t_(h, DFJK_KERNEL_J1, st);
+                          dfjk::launch_j1x_dot(h->X, h->Ccat, nao, np, ldc, ldc, w8[i], 1, &c1, &nc, &one, P0, naux, h->d_part, st); }
+                        { Timed t_(h, DFJK_KERNEL_J1R, st);
+                          dfjk::launch_j1_reduce_rows(h->d_part, nblk, naux, P0, np, h->d_batch + (int64_t)i * naux, st); }
+                    }
+                    /* every (chunk, pair) product starts its slabs afresh (accumulate = 0) and is summed into
+                     * K_i right away, so the panel plan is made for THIS chunk's row count: a short last
+                     * chunk must not leave slabs unwritten that K3 would then add */
+                    if (panel[i])
+                        dfjk::k2p_plan(nao, np * ((ncols[i] + 3) / 4), nbk * nbk, h->sm_count,
+                                       h->opt_k_splits > 0 ? (int)h->opt_k_splits : h->nsplit_alloc,
+                                       h->opt_k2_panel_kb << 10, &pstages[i], &nsplit[i]);
+                    { Timed t_(h, DFJK_KERNEL_K2, st);
+                      if (panel[i])
+                          DFJK_LAUNCH_TRY(dfjk::launch_k2p_gemm_full(h->X, nao, np, ldc, c1, c2, nc, h->Kpart, pstages[i],
+                                                                     nsplit[i], 0, h->k2work, h->sm_count, st));
+                      else
+                          DFJK_LAUNCH_TRY(dfjk::launch_k2_gemm_full(h->X, nao, np, ldc, c1, c2, nc, h->Kpart, nsplit[i], 0, st)); }
+                    { Timed t_(h, DFJK_KERNEL_K3, st); dfjk::launch_k3_sum(h->Kpart, nsplit[i], nao, Ks[i], st, chunk > 0); }
+                }
+            }
+            i0 = i1;
+        }
+    }
+    if (want_j) {
+        const int rc = batched_j_from_d(h, nb, Js, st);
+        if (rc != DFJK_OK) return rc;
+    }
+    DFJK_CUDA_TRY(cudaGetLastError());
+    return DFJK_OK;
+}
+
+}  // namespace
+
+extern "C" int dfjk_get_jk_pairs(dfjk_handle *h, int64_t nbatch, const double *const *C1s,
+                                 const double *const *C2s, const int64_t *ncols, double *const *Js,
+                                 double *const *Ks, void *stream)
+{
+    const char *who = "dfjk_get_jk_pairs";
+    g_err[0] = 0;
+    if (!h) return fail(DFJK_EINVAL, "%s: NULL handle", who);
+    if (nbatch < 1) return fail(DFJK_EINVAL, "%s: nbatch must be >= 1", who);
+    if (!C1s || !C2s || !ncols) return fail(DFJK_EINVAL, "%s: NULL factor / ncols array", who);
+    if (!Js && !Ks) return fail(DFJK_EINVAL, "%s: no output requested", who);
+    for (int64_t i = 0; i < nbatch; ++i) {
+        if (!C1s[i] || !C2s[i]) return fail(DFJK_EINVAL, "%s: factor pointer %lld is NULL", who, (long long)i);
+        if (ncols[i] < 1 || ncols[i] > h->nao)
+            return fail(DFJK_EINVAL, "%s: ncols[%lld]=%lld outside [1, nao=%lld]", who, (long long)i,
+                        (long long)ncols[i], (long long)h->nao);
+        if ((Js && !Js[i]) || (Ks && !Ks[i]))
+            return fail(DFJK_EINVAL, "%s: output pointer %lld is NULL (pass a NULL array to skip J or K)", who, (long long)i);
+    }
+    int dev = -1;
+    DFJK_CUDA_TRY(cudaGetDevice(&dev));
+    if (dev != h->device) return fail(DFJK_EINVAL, "%s: handle belongs to device %d, current is %d", who, h->device, dev);
+    for (int64_t b0 = 0; b0 < nbatch; b0 += DFJK_MAX_BATCH) {
+        const int nb = (int)(nbatch - b0 < DFJK_MAX_BATCH ? nbatch - b0 : DFJK_MAX_BATCH);
+        const int rc = pairs_subbatch(h, nb, C1s + b0, C2s + b0, ncols + b0, Js ? Js + b0 : nullptr,
+                                      Ks ? Ks + b0 : nullptr, (cudaStream_t)stream, who);
+        if (rc != DFJK_OK) return rc;
+    }
+    return DFJK_OK;
+}
+
 extern "C" int dfjk_get_jk_dms(dfjk_handle *h, int64_t ndm, const double *dms, double *Js, double *Ks,
                                void *stream)
 {
+    const char *who = "dfjk_get_jk_dms";
     g_err[0] = 0;
-    if (!h) return fail(DFJK_EINVAL, "dfjk_get_jk_dms: NULL handle");
-    if (ndm < 1) return fail(DFJK_EINVAL, "dfjk_get_jk_dms: ndm must be >= 1");
+    if (!h) return fail(DFJK_EINVAL, "%s: NULL handle", who);
+    if (ndm < 1) return fail(DFJK_EINVAL, "%s: ndm must be >= 1", who);
+    if (!dms) return fail(DFJK_EINVAL, "%s: density / factor pointer is NULL", who);
+    if (!Js && !Ks) return fail(DFJK_EINVAL, "%s: no output requested", who);
+    int dev = -1;
+    DFJK_CUDA_TRY(cudaGetDevice(&dev));
+    if (dev != h->device) return fail(DFJK_EINVAL, "%s: handle belongs to device %d, current is %d", who, h->device, dev);
+    cudaStream_t st = (cudaStream_t)stream;
     const int64_t n2 = h->nao * h->nao;
-    for (int64_t i = 0; i < ndm; ++i) {
-        const int rc = get_jk_general_impl(h, dms ? dms + i * n2 : nullptr, nullptr, h->nao,
-                                           Js ? Js + i * n2 : nullptr, Ks ? Ks + i * n2 : nullptr,
-                                           (cudaStream_t)stream, "dfjk_get_jk_dms");
-        if (rc != DFJK_OK) return rc;
+    for (int64_t b0 = 0; b0 < ndm; b0 += DFJK_MAX_BATCH) {
+        const int nb = (int)(ndm - b0 < DFJK_MAX_BATCH ? ndm - b0 : DFJK_MAX_BATCH);
+        if (Js) {
+            /* J of the whole sub-batch: a dot pass per density, then ONE axpy pass over B for all of them
+             * (nb + 1 passes instead of 2 nb) */
+            double *Jp[DFJK_MAX_BATCH];
+            for (int i = 0; i < nb; ++i) {
+                d_by_pass_over_b(h, i, dms + (b0 + i) * n2, nullptr, h->nao, st);
+                Jp[i] = Js + (b0 + i) * n2;
+            }
+            const int rc = batched_j_from_d(h, nb, Jp, st);
+            if (rc != DFJK_OK) return rc;
+            DFJK_CUDA_TRY(cudaGetLastError());
+        }
+        if (Ks)   /* K[dm] as the pair (dm, I): 4 naux nao^3 flop each, FP64-bound -- nothing to share but B's unpack */
+            for (int i = 0; i < nb; ++i) {
+                const int rc = get_jk_general_impl(h, dms + (b0 + i) * n2, nullptr, h->nao, nullptr, Ks + (b0 + i) * n2, st, who);
+                if (rc != DFJK_OK) return rc;
+            }
     }
     return DFJK_OK;
 }

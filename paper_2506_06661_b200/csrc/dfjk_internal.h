@@ -112,7 +112,21 @@ cudaError_t launch_k2p_gemm_full(const double *X4, int64_t nao, int64_t np, int6
                                  int accumulate, int *work, int sm_count, cudaStream_t st);
 
 /* K3 general: K[mu][nu] = sum_split Kpart[split][mu][nu] for every (mu, nu). */
-void launch_k3_sum(const double *Kpart, int nsplit, int64_t nao, double *K, cudaStream_t st);
+/* accumulate != 0: K[mu][nu] += the sum (the batched build adds one X chunk after the other) */
+void launch_k3_sum(const double *Kpart, int nsplit, int64_t nao, double *K, cudaStream_t st, int accumulate = 0);
+
+/* ---------------------------------------------------------------- batched densities (dfjk_get_jk_pairs) */
+#define DFJK_MAX_BATCH 8   /* densities per multi-right-hand-side J2 pass / per d_batch workspace */
+/* one factor C (nao x ncol) into columns [col0, col0 + width) of Ccat4 (zero beyond ncol) */
+void launch_k0_pack_cols(const double *C, int64_t ncol, int64_t col0, int64_t width, int64_t nao, int64_t ldc,
+                         double *Ccat, cudaStream_t st);
+/* d_out[P0 + p] = sum_c d_part[c][P0 + p], p < np (J1R for the rows of one X chunk) */
+void launch_j1_reduce_rows(const double *d_part, int64_t nchunk, int64_t naux, int64_t P0, int64_t np,
+                           double *d_out, cudaStream_t st);
+/* J2 for nbatch <= DFJK_MAX_BATCH densities in one pass over B: d[k][P] (pitch naux),
+ * Jp_part[(k*ngroup + g)][pair]; per density bitwise equal to launch_j2_axpy */
+void launch_j2_axpy_multi(const double *B, int64_t naux, int64_t npair, const double *d, int nbatch,
+                          double *Jp_part, int64_t ngroup, cudaStream_t st);
 
 /* K3: K[mu][nu] = K[nu][mu] = sum_split Kpart[split][mu][nu], mu >= nu. */
 void launch_k3_finish(const double *Kpart, int nsplit, int weighted, int64_t nao, double *K, double *const *Kslot,

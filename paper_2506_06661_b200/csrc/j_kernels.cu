@@ -341,6 +341,30 @@ j1_reduce_kernel(const double *__restrict__ d_part, int64_t nchunk, int64_t naux
     }
 }
 
+/* the same sum for the np rows [P0, P0 + np) only, written to d_out[P0 ..]: the batched build
+ * (dfjk_get_jk_pairs) reduces every X chunk's partials at once, into the d vector of one density */
+__global__ void __launch_bounds__(256)
+j1_reduce_rows_kernel(const double *__restrict__ d_part, int64_t nchunk, int64_t naux, int64_t P0, int64_t np,
+                      double *__restrict__ d_out)
+{
+    __shared__ double gs[8][33];
+    const int pl = threadIdx.x & 31, g = threadIdx.x >> 5;
+    const int64_t p = (int64_t)blockIdx.x * 32 + pl;
+    double acc = 0.0;
+    if (p < np) {
+#pragma unroll 8
+        for (int c = g; c < (int)nchunk; c += 8) acc += d_part[(int64_t)c * naux + P0 + p];
+    }
+    gs[g][pl] = acc;
+    __syncthreads();
+    if (g == 0 && p < np) {
+        double v = gs[0][pl];
+#pragma unroll
+        for (int q = 1; q < 8; ++q) v += gs[q][pl];
+        d_out[P0 + p] = v;
+    }
+}
+
 /* ------------------------------------------------------------------ J2 */
 #ifndef DFJK_J2_THREADS
 #define DFJK_J2_THREADS 256
@@ -403,6 +427,71 @@ j2_axpy_kernel(const double *__restrict__ B, int64_t naux, int64_t npair,
     double *out = Jp_part + g * npair;
     if (okx) out[colx] = ax;
     if (oky) out[coly] = ay;
+}
+
+/* J2 for NB densities in ONE pass over B (dfjk_get_jk_pairs / _dms: "an arbitrary number of density
+ * matrices"):  Jp_part[(k*ngroup + g)][pair] = sum_{P in group g} d[k][P] B[P][pair], k < NB.
+ * The stream is J2's (same column ownership, same 128-bit evict-first loads, same row groups); every
+ * loaded element feeds NB FMAs instead of one, so B is read once for the whole batch.  Per density the
+ * additions happen in J2's order: the result is bitwise that of NB single-density passes. */
+template <int NB, int UNROLL>
+__global__ void __launch_bounds__(J2_THREADS)
+j2_axpy_multi_kernel(const double *__restrict__ B, int64_t naux, int64_t npair, const double *__restrict__ d,
+                     double *__restrict__ Jp_part, int64_t ngroup)
+{
+    const int64_t g = blockIdx.y;
+    const int64_t s = (g * npair) & 1;
+    const int64_t vv = (int64_t)blockIdx.x * J2_THREADS + threadIdx.x;
+    const int64_t colx = 2 * vv - s, coly = colx + 1;
+    const bool okx = colx >= 0 && colx < npair;
+    const bool oky = coly < npair;
+    if (!okx && !oky) return;
+    double ax[NB], ay[NB];
+#pragma unroll
+    for (int k = 0; k < NB; ++k) ax[k] = ay[k] = 0.0;
+    if (okx && oky) {
+        const double *bp = B + colx;
+        int64_t P = g;
+        for (; P + (UNROLL - 1) * ngroup < naux; P += UNROLL * ngroup) {
+            double2 b[UNROLL];
+#pragma unroll
+            for (int u = 0; u < UNROLL; ++u) b[u] = ldg_stream2(bp + (P + u * ngroup) * npair);
+#pragma unroll
+            for (int u = 0; u < UNROLL; ++u) {
+#pragma unroll
+                for (int k = 0; k < NB; ++k) {
+                    const double dv = __ldg(d + k * naux + P + u * ngroup);
+                    ax[k] += dv * b[u].x;
+                    ay[k] += dv * b[u].y;
+                }
+            }
+        }
+        for (; P < naux; P += ngroup) {
+            const double2 b = ldg_stream2(bp + P * npair);
+#pragma unroll
+            for (int k = 0; k < NB; ++k) {
+                const double dv = __ldg(d + k * naux + P);
+                ax[k] += dv * b.x;
+                ay[k] += dv * b.y;
+            }
+        }
+    } else {
+        const int64_t col = okx ? colx : coly;
+        for (int64_t P = g; P < naux; P += ngroup) {
+            const double b = ldg_stream1(B + P * npair + col);
+#pragma unroll
+            for (int k = 0; k < NB; ++k) {
+                const double t = __ldg(d + k * naux + P) * b;
+                if (okx) ax[k] += t; else ay[k] += t;
+            }
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < NB; ++k) {
+        double *out = Jp_part + (k * ngroup + g) * npair;
+        if (okx) out[colx] = ax[k];
+        if (oky) out[coly] = ay[k];
+    }
 }
 
 /* ------------------------------------------------------------------ J3 */
@@ -559,6 +648,31 @@ void launch_j2_axpy(const double *B, int64_t naux, int64_t npair, const double *
     else    /* d == NULL: Eq. 7's DF diagonal, sum_P B[P][pair]^2 */
         j2_axpy_kernel<true><<<dim3(nbx, (unsigned)ngroup), J2_THREADS, 0, st>>>(B, naux, npair, nullptr,
                                                                                  Jp_part, ngroup);
+}
+
+void launch_j1_reduce_rows(const double *d_part, int64_t nchunk, int64_t naux, int64_t P0, int64_t np,
+                           double *d_out, cudaStream_t st)
+{
+    j1_reduce_rows_kernel<<<(unsigned)((np + 31) / 32), 256, 0, st>>>(d_part, nchunk, naux, P0, np, d_out);
+}
+
+void launch_j2_axpy_multi(const double *B, int64_t naux, int64_t npair, const double *d, int nbatch,
+                          double *Jp_part, int64_t ngroup, cudaStream_t st)
+{
+    const int64_t nvec = (npair + 1) / 2 + 1;
+    const dim3 grid((unsigned)((nvec + J2_THREADS - 1) / J2_THREADS), (unsigned)ngroup);
+#define DFJK_J2M(NB, U) j2_axpy_multi_kernel<NB, U><<<grid, J2_THREADS, 0, st>>>(B, naux, npair, d, Jp_part, ngroup)
+    switch (nbatch) {
+    case 1: DFJK_J2M(1, 12); break;
+    case 2: DFJK_J2M(2, 12); break;
+    case 3: DFJK_J2M(3, 12); break;
+    case 4: DFJK_J2M(4, 12); break;
+    case 5: DFJK_J2M(5, 8); break;
+    case 6: DFJK_J2M(6, 8); break;
+    case 7: DFJK_J2M(7, 8); break;
+    default: DFJK_J2M(8, 8); break;     /* nbatch <= DFJK_MAX_BATCH = 8, checked by the caller */
+    }
+#undef DFJK_J2M
 }
 
 void launch_j3_unpack(const double *Jp_part, int64_t ngroup, int64_t npair, int64_t nao, double *J,

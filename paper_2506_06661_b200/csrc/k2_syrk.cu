@@ -60,6 +60,19 @@ __global__ void k0_pack_c_kernel(PackDesc pd, int64_t nao, int64_t nao16, int64_
     Ccat4[((mu >> 2) * ldc + c) * 4 + (mu & 3)] = v;
 }
 
+/* One factor into a column range of Ccat4: columns [col0, col0 + width) = C (nao x ncol, zero beyond
+ * ncol and for rows >= nao).  The batched build packs its 2 x nbatch factors one by one. */
+__global__ void k0_pack_cols_kernel(const double *__restrict__ C, int64_t ncol, int64_t col0, int64_t width,
+                                    int64_t nao, int64_t nao16, int64_t ldc, double *__restrict__ Ccat4)
+{
+    const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= nao16 * width) return;
+    const int64_t mu = idx / width;
+    const int64_t j = idx % width;
+    const double v = (mu < nao && j < ncol) ? C[mu * ncol + j] : 0.0;
+    Ccat4[((mu >> 2) * ldc + col0 + j) * 4 + (mu & 3)] = v;
+}
+
 /* ------------------------------------------------------------------ K2 */
 constexpr int K2_T = 128;
 constexpr int K2_KG = 8;                              /* k-groups (of 4) per stage: k = 32 */
@@ -807,11 +820,11 @@ fp64_peak_probe_kernel(int iters, double *__restrict__ sink)
 
 /* general (non-symmetric) finish: K[mu][nu] = sum_split Kpart[split][mu][nu], every entry */
 __global__ void __launch_bounds__(256)
-k3_sum_kernel(const double *__restrict__ Kpart, int nsplit, int64_t n2, double *__restrict__ K)
+k3_sum_kernel(const double *__restrict__ Kpart, int nsplit, int64_t n2, double *__restrict__ K, int accumulate)
 {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n2) return;
-    double v = 0.0;
+    double v = accumulate ? K[i] : 0.0;    /* batched build: K collects one X chunk after the other */
 #pragma unroll 8
     for (int s = 0; s < nsplit; ++s) v += Kpart[(int64_t)s * n2 + i];
     K[i] = v;
@@ -956,10 +969,18 @@ void launch_fp64_peak_probe(int ctas, int iters, double *sink, cudaStream_t st)
     fp64_peak_probe_kernel<<<ctas, 256, 0, st>>>(iters, sink);
 }
 
-void launch_k3_sum(const double *Kpart, int nsplit, int64_t nao, double *K, cudaStream_t st)
+void launch_k3_sum(const double *Kpart, int nsplit, int64_t nao, double *K, cudaStream_t st, int accumulate)
 {
     const int64_t n2 = nao * nao;
-    k3_sum_kernel<<<(unsigned)((n2 + 255) / 256), 256, 0, st>>>(Kpart, nsplit, n2, K);
+    k3_sum_kernel<<<(unsigned)((n2 + 255) / 256), 256, 0, st>>>(Kpart, nsplit, n2, K, accumulate);
+}
+
+void launch_k0_pack_cols(const double *C, int64_t ncol, int64_t col0, int64_t width, int64_t nao, int64_t ldc,
+                         double *Ccat, cudaStream_t st)
+{
+    const int64_t nao16 = (nao + 31) / 32 * 32;
+    const int64_t n = nao16 * width;
+    k0_pack_cols_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(C, ncol, col0, width, nao, nao16, ldc, Ccat);
 }
 
 }  // namespace dfjk

@@ -41,6 +41,8 @@ def test_version_and_null_handling(L):
     assert b"NULL" in L.dfjk_last_error()
     assert L.dfjk_get_jk_dm(None, None, None, None, None) == -1
     assert L.dfjk_get_jk_dms(None, 1, None, None, None, None) == -1
+    assert L.dfjk_get_jk_pairs(None, 1, None, None, None, None, None, None) == -1
+    assert b"NULL handle" in L.dfjk_last_error()
     assert L.dfjk_get_df_diag(None, None, None) == -1
     # the allocation-free entry point: argument checks come before any CUDA call
     assert L.dfjk_noalloc_max_nao() == 1023

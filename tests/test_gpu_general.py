@@ -215,3 +215,76 @@ def test_pair_is_the_orbital_derivative_of_get_jk_on_the_device(dfjk):
     assert relerr(dJ, 4.0 * J1.cpu().numpy()) <= 1e-9
     assert relerr(dK, K1n + K1n.T) <= 1e-9
     h.close()
+
+
+@pytest.mark.parametrize("nao,naux,ncols", [
+    (64, 16, (5,)),                               # nbatch 1
+    (129, 12, (1, 31)),                           # ncol 1 beside a wide one
+    (200, 40, (13, 8, 3)),
+    (150, 11, (150, 4, 150, 9, 20)),              # ncol = nao twice: the batch overflows ldc_max, three K1 sweeps
+    (290, 30, (8, 8, 8, 8, 8, 8, 8, 8)),          # the SOSCF shape: 8 trial vectors of 8 columns, 3 x 3 tiles
+    (300, 7, (3, 130, 7, 7, 1, 2, 64, 9, 11, 5)), # more than DFJK_MAX_BATCH = 8: two sub-batches
+])
+def test_pairs_batch_parity(dfjk, nao, naux, ncols):
+    """dfjk_get_jk_pairs: every density of a batch against the oracle's single-pair result, on both K2
+    kernels, fused and two-pass d, several X chunks, J-only and K-only batches; with d from the dot
+    pass J is bitwise that of the single-pair call (same summation order per density)."""
+    Bp = make_B(nao, naux, 900 + nao)
+    rng = np.random.default_rng(nao + len(ncols))
+    C1s = [rng.standard_normal((nao, c)) for c in ncols]
+    C2s = [rng.standard_normal((nao, c)) for c in ncols]
+    ref = [oracle.get_jk_pair(Bp, nao, a, b) for a, b in zip(C1s, C2s)]
+    d1, d2 = [dev(a) for a in C1s], [dev(b) for b in C2s]
+    h = dfjk.DFJK(dev(Bp), nao)
+    h.set_option("k2_panel_kb", 64)
+    h.set_option("k_chunk", max(1, naux // 3))
+    for fused, k2_panel in ((1, 0), (0, 0), (1, 1)):
+        h.set_option("j_fused", fused)
+        h.set_option("k2_panel", k2_panel)
+        Js, Ks = h.get_jk_pairs(d1, d2)
+        torch.cuda.synchronize()
+        for i, (Jo, Ko, _) in enumerate(ref):
+            assert relerr(Js[i].cpu().numpy(), Jo) <= TOL, (i, fused, k2_panel)
+            assert relerr(Ks[i].cpu().numpy(), Ko) <= TOL, (i, fused, k2_panel)
+        if fused == 0:                      # d from the dot pass over B: the same sums in the same order
+            J1, _ = h.get_jk_pair(d1[-1], d2[-1])
+            torch.cuda.synchronize()
+            assert torch.equal(J1, Js[-1])
+    h.set_option("j_fused", 1)
+    Js, none = h.get_jk_pairs(d1, d2, with_k=False)
+    none2, Ks = h.get_jk_pairs(d1, d2, with_j=False)
+    torch.cuda.synchronize()
+    assert none is None and none2 is None
+    for i, (Jo, Ko, _) in enumerate(ref):
+        assert relerr(Js[i].cpu().numpy(), Jo) <= TOL and relerr(Ks[i].cpu().numpy(), Ko) <= TOL
+    h.close()
+
+
+def test_dms_batch_shares_the_axpy_pass(dfjk):
+    """dfjk_get_jk_dms with 10 raw densities (two sub-batches): J and K per density against the oracle;
+    the J pass count is ndm + 2 streaming kernels per sub-batch instead of 2 per density."""
+    nao, naux, ndm = 130, 9, 10
+    Bp = make_B(nao, naux, 55)
+    dms = np.random.default_rng(8).standard_normal((ndm, nao, nao))
+    h = dfjk.DFJK(dev(Bp), nao)
+    h.set_option("time_kernels", 1)
+    J, K = h.get_jk_dm(dev(dms))
+    torch.cuda.synchronize()
+    assert h.kernel_time("J2")[1] == 2 and h.kernel_time("J1")[1] == ndm
+    for i in range(ndm):
+        Jo, Ko, _ = oracle.get_jk_dm(Bp, nao, dms[i])
+        assert relerr(J[i].cpu().numpy(), Jo) <= TOL and relerr(K[i].cpu().numpy(), Ko) <= TOL
+    h.close()
+
+
+def test_pairs_error_paths(dfjk):
+    nao, naux = 6, 3
+    h = dfjk.DFJK(dev(make_B(nao, naux, 1)), nao)
+    C = dev(np.ones((nao, 2)))
+    with pytest.raises(ValueError):
+        h.get_jk_pairs([C], [C, C])
+    with pytest.raises(ValueError):
+        h.get_jk_pairs([C], [dev(np.ones((nao, 3)))])
+    with pytest.raises(dfjk.DFJKError):
+        h.get_jk_pairs([C], [C], with_j=False, with_k=False)
+    h.close()
