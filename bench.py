@@ -146,6 +146,24 @@ class ClockSampler:
                 "reasons": sorted(reasons)}
 
 
+def oracle_full(cfg, call=0, slab=250):
+    """Time the oracle (as it stands) on ALL rows of the config's B, fed slab by slab (the tensor is up
+    to 96 GB: it is generated, consumed and dropped 250 rows at a time; only the oracle's own time is
+    summed, not the generator's).  Returns seconds, threads."""
+    import oracle
+    Cs = gi.orbitals(cfg, call)
+    warm = oracle.JKAccumulator(cfg.nao, Cs, cfg.weights)
+    warm.add_slab(gi.fill_B_host(cfg, 0, 1))   # touch the code path / page in
+    acc = oracle.JKAccumulator(cfg.nao, Cs, cfg.weights)
+    t = 0.0
+    for P0 in range(0, cfg.naux, slab):
+        Bp = gi.fill_B_host(cfg, P0, min(slab, cfg.naux - P0))
+        t0 = time.perf_counter()
+        acc.add_slab(Bp)
+        t += time.perf_counter() - t0
+    return t, oracle.num_threads()
+
+
 def oracle_sample(cfg, rows, call=0):
     """Time the oracle (as it stands) on `rows` rows of the config's B. Returns seconds, threads."""
     import oracle
@@ -325,9 +343,10 @@ def other_workloads(pkg, wl4, args, dev, local, barrier, peak, hbm, peak_src):
     the section-8f operations at cfg 4 (on the resident B), then BASELINE configs 3, 5, 2, 1 and the
     LRDF shape."""
     import torch
-    out = {}
+    out = {}      # the section-8f operations at cfg 4: run first (B is resident), emitted LAST (see the end)
     W, K = 3, 3
-    cfg = wl4.cfg
+    cc = lambda c: {"sm_mhz": c.get("sm_mhz"), "reasons": c.get("reasons")}   # the driver keeps only the tail of
+    cfg = wl4.cfg                                                             # stdout: every entry stays short
     nao, naux, nocc = cfg.nao, cfg.naux, cfg.nocc[0]
     rng = np.random.default_rng(cfg.seed)
 
@@ -355,18 +374,49 @@ def other_workloads(pkg, wl4, args, dev, local, barrier, peak, hbm, peak_src):
     C2 = torch.from_numpy(rng.standard_normal((nao, nocc))).to(dev)
     ms, clocks = timed(lambda: wl4.h.get_jk_pair(C1, C2))
     fl = flops_j(cfg) + 2.0 * naux * nao ** 2 * (2 * nocc) + 2.0 * naux * nao ** 2 * nocc
-    out["cfg4_pair"] = {"op": f"dfjk_get_jk_pair ncol={nocc}", "ms_per_step": ms, "gflops": fl / ms / 1e6,
-                        "frac_fp64_peak": fl / ms / 1e9 / peak, "clocks": clocks}
+    out["cfg4_pair"] = {"op": f"get_jk_pair ncol={nocc}", "ms": ms, "frac_fp64_peak": fl / ms / 1e9 / peak, **cc(clocks)}
+    # -- section 8f rank 1, batch half: several pairs from one sweep over B against the same pairs one by one
+    for nb, nc in ((8, 8), (4, 32)):
+        A = [torch.from_numpy(rng.standard_normal((nao, nc))).to(dev) for _ in range(nb)]
+        Bf = [torch.from_numpy(rng.standard_normal((nao, nc))).to(dev) for _ in range(nb)]
+        ms_b, clocks = timed(lambda: wl4.h.get_jk_pairs(A, Bf))
+        ms_1, _ = timed(lambda: [wl4.h.get_jk_pair(a, b) for a, b in zip(A, Bf)])
+        wl4.h.set_option("time_kernels", 1)
+        wl4.h.get_jk_pairs(A, Bf)
+        torch.cuda.synchronize()
+        k1_ms, k1_n = wl4.h.kernel_time("K1")
+        j2_ms, j2_n = wl4.h.kernel_time("J2")
+        wl4.h.set_option("time_kernels", 0)
+        k1_fl = 2.0 * naux * nao ** 2 * (2 * nb * ((nc + 7) // 8 * 8))
+        out[f"cfg4_pairs_{nb}x{nc}"] = {"op": f"get_jk_pairs: {nb} pairs of ncol {nc} in one call", "ms": ms_b,
+                                        "ms_one_by_one": ms_1, "ratio": ms_b / ms_1, "k1_ms": k1_ms, "k1_launches": k1_n,
+                                        "k1_frac_fp64_peak": k1_fl / k1_ms / 1e9 / peak if k1_ms > 0 else None,
+                                        "j2_ms": j2_ms, "j2_passes": j2_n, **cc(clocks)}
+        del A, Bf
     # -- section 8f rank 3: Eq. 7's DF diagonal, one pass over B
     ms, clocks = timed(lambda: wl4.h.get_df_diag())
-    out["cfg4_diag"] = {"op": "dfjk_get_df_diag (Eq. 7)", "ms_per_step": ms, "gbs": cfg.b_bytes / ms / 1e6,
-                        "frac_hbm": cfg.b_bytes / ms / 1e6 / hbm, "clocks": clocks}
+    out["cfg4_diag"] = {"op": "get_df_diag (Eq. 7)", "ms": ms, "gbs": cfg.b_bytes / ms / 1e6,
+                        "frac_hbm": cfg.b_bytes / ms / 1e6 / hbm, **cc(clocks)}
     # -- the north_star configuration of the whole step: J by two plain passes over B (j_fused = 0)
     wl4.h.set_option("j_fused", 0)
     ms, clocks = timed(lambda: wl4.step(0))
     wl4.h.set_option("j_fused", 1)
-    out["cfg4_two_pass_j"] = {"op": "dfjk_get_jk with j_fused=0 (J1 dot + J2 axpy: B streamed three times)",
-                              "ms_per_step": ms, "gflops": flops_step(cfg) / ms / 1e6, "clocks": clocks}
+    out["cfg4_two_pass_j"] = {"op": "get_jk, j_fused=0 (J1 dot + J2 axpy)", "ms": ms,
+                              "gflops": flops_step(cfg) / ms / 1e6, **cc(clocks)}
+    # -- section 8f rank 4: the SCF driver, 4 fixed iterations (B scaled so the two-electron term is a
+    #    perturbation; build_b below regenerates B)
+    try:
+        wl4.B.mul_(0.02)
+        hc = torch.from_numpy(gi.core_hamiltonian(cfg)).to(dev)
+        S = torch.from_numpy(gi.overlap(cfg)).to(dev)
+        res = {}
+        ms, clocks = timed(lambda: res.update(wl4.h.scf_rhf(hc, S, nocc, max_iter=4, conv_tol=1e-300)), warm=1, steps=1)
+        tm = res.get("timing") or {}
+        out["cfg4_scf"] = {"op": "scf_rhf, 4 iterations", "ms_per_iteration": ms / 4, "get_jk_ms": tm.get("get_jk"),
+                           "eig_ms": tm.get("eigensolver"), "glue_ms": tm.get("glue"), **cc(clocks)}
+        del hc, S
+    except Exception as e:
+        out["cfg4_scf"] = {"error": repr(e)[:120]}
     # -- section 8f rank 2: building B in place (once: 1 warm-up + 1 timed, ~1 s each)
     Mh = torch.from_numpy(gi.metric(cfg)).pin_memory()
     Md = torch.empty(naux, naux, dtype=torch.float64, device=dev)
@@ -376,10 +426,10 @@ def other_workloads(pkg, wl4, args, dev, local, barrier, peak, hbm, peak_src):
         gi.fill_B_device(cfg, wl4.B)                 # R is overwritten in place: regenerate it
     ms, clocks = timed(lambda: pkg.build_b(Md, wl4.B, nao), prep, warm=1, steps=1)
     fl = float(naux) ** 2 * cfg.npair + float(naux) ** 3 / 3.0
-    out["cfg4_build_b"] = {"op": "dfjk_build_b (Eq. 2-3, in place)", "ms_per_step": ms, "gflops": fl / ms / 1e6,
-                           "frac_fp64_peak": fl / ms / 1e9 / peak, "clocks": clocks}
+    out["cfg4_build_b"] = {"op": "build_b (Eq. 2-3, in place)", "ms": ms, "frac_fp64_peak": fl / ms / 1e9 / peak, **cc(clocks)}
     del Md, Mh, C1, C2
     wl4.close()
+    f_ops, out = out, {}
 
     for cid in (3, 5, 2, 1, 6):
         c = gi.CONFIGS[cid]
@@ -397,16 +447,15 @@ def other_workloads(pkg, wl4, args, dev, local, barrier, peak, hbm, peak_src):
         kt = kernel_breakdown(wl, Wc, min(Kc, 5))
         j, kk = j_and_k_summary(c, kt, peak, hbm, peak_src)
         ms = float(np.mean(step_ms))
-        rec = {"workload": workload_config(c, args)["workload"], "ms_per_step": ms, "steps": Kc, "warmup": Wc,
-               "step_ms": step_ms if Kc <= 5 else [float(np.min(step_ms)), float(np.median(step_ms)), float(np.max(step_ms))],
+        rec = {"shape": f"nao {c.nao} naux {c.naux} nocc {'+'.join(map(str, c.nocc))}", "ms_per_step": ms, "steps": Kc,
                "gflops": flops_step(c) / ms / 1e6, "launches_per_step": launches / Kc,
                "k_frac_fp64_peak": kk["frac_fp64_peak"], "k1_ms": kk["k1_ms"], "k2_ms": kk["k2_ms"],
-               "k1_tflops": kk["k1_tflops"], "k2_tflops": kk["k2_tflops"],
-               "j_ms": j["ms"], "j_gbs": j["gbs"], "clocks": clocks}
+               "j_ms": j["ms"], "j_gbs": j["gbs"], **cc(clocks)}
         if c.b_bytes > (1 << 30):
             rec["j_two_pass_gbs"] = two_pass_j(wl, Wc, 2, hbm)["gbs"]
         out[f"cfg{cid}"] = rec
         wl.close()
+    out.update(f_ops)          # last in the line: they survive in a record that keeps only the tail of stdout
     return out
 
 
@@ -541,8 +590,8 @@ def run_ours(args, cfg):
     if step_fn is not None:
         out["config"]["launch"] = "one CUDA-graph replay per step (+ a device copy of C_occ into the captured input)"
     if world == 1:
-        if args.cpu_baseline_full:
-            rows, (t, threads) = cfg.naux, oracle_sample(cfg, cfg.naux)
+        if args.cpu_baseline_full or (cfg.index == 4 and not args.cpu_baseline_sample):
+            rows, (t, threads) = cfg.naux, oracle_full(cfg)
         else:
             rows, t, threads = size_sample(cfg, 15.0)
         out["cpu_baseline"] = {
@@ -663,7 +712,9 @@ def main():
     ap.add_argument("--no-others", action="store_true",
                     help="skip the short passes over the other configs / section-8f ops after the cfg-4 headline")
     ap.add_argument("--cpu-baseline-full", action="store_true",
-                    help="time the oracle on ALL rows of the config instead of a ~15 s sample (cfg 4: ~90 s)")
+                    help="time the oracle on ALL rows of the config instead of a ~15 s sample (the default at cfg 4: ~40 s)")
+    ap.add_argument("--cpu-baseline-sample", action="store_true",
+                    help="cfg 4: time the oracle on a ~15 s row sample instead of all 5000 rows")
     ap.add_argument("--op", default="get_jk", choices=["get_jk", "build_b", "pair", "dm", "diag", "scf"],
                     help="get_jk (default, the contract line) or one of the section-8f rows")
     args = ap.parse_args()
