@@ -661,6 +661,13 @@ def run_extra(args, cfg):
             flops = flops_j(cfg) + 2.0 * naux * nao ** 2 * (2 * nocc) + 2.0 * naux * nao ** 2 * nocc
             what = f"dfjk_get_jk_pair, ncol={nocc}: J[C1 C2^T] + K = sum_P (B_P C1)(B_P C2)^T"
             run = lambda: h.get_jk_pair(C1, C2)
+        elif args.op == "pairs":
+            nbp, ncp = 8, 8
+            A = [torch.from_numpy(rng.standard_normal((nao, ncp))).to(dev) for _ in range(nbp)]
+            Bf = [torch.from_numpy(rng.standard_normal((nao, ncp))).to(dev) for _ in range(nbp)]
+            flops = nbp * (flops_j(cfg) + 2.0 * naux * nao ** 2 * (2 * ncp) + 2.0 * naux * nao ** 2 * ncp)
+            what = f"dfjk_get_jk_pairs: {nbp} pairs of ncol {ncp} from one sweep over B (one K1 per X chunk, one J2 pass)"
+            run = lambda: h.get_jk_pairs(A, Bf)
         elif args.op == "dm":
             dm = torch.from_numpy(rng.standard_normal((nao, nao))).to(dev)
             flops = flops_j(cfg) + 2.0 * naux * nao ** 3 + 2.0 * naux * nao ** 3
@@ -715,7 +722,7 @@ def main():
                     help="time the oracle on ALL rows of the config instead of a ~15 s sample (the default at cfg 4: ~40 s)")
     ap.add_argument("--cpu-baseline-sample", action="store_true",
                     help="cfg 4: time the oracle on a ~15 s row sample instead of all 5000 rows")
-    ap.add_argument("--op", default="get_jk", choices=["get_jk", "build_b", "pair", "dm", "diag", "scf"],
+    ap.add_argument("--op", default="get_jk", choices=["get_jk", "build_b", "pair", "pairs", "dm", "diag", "scf"],
                     help="get_jk (default, the contract line) or one of the section-8f rows")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
